@@ -1,0 +1,183 @@
+/*
+ * polylab.h -- C ABI of polylab-b200: simplification of sparse multivariate polynomials on one
+ * NVIDIA B200 (sm_100a).  Plain pointers and sizes only; no C++ or torch types.
+ *
+ * Data model (the paper's): a polynomial is a coefficient vector plus an exponent matrix with one
+ * row per monomial -- constructor MPOLY(n,coef,pow), /root/reference/PAPER.md:80 (Table 3) and
+ * PAPER.md:97 (section 3.1).  Exponents are non-negative integers (alpha in N^n).
+ * Variable identity is outside this ABI: operands of a product share nvars and column meaning
+ * (the paper aligns variable spaces BEFORE an operation).
+ *
+ * Operations:
+ *   simplify(p, zeroprec): "merges repeated monomials and removes coefficients below a user-chosen
+ *     tolerance" (Table 4; Table 3).
+ *   product of scalar polynomials (mtimes/times): every term of a times every
+ *     term of b -- coefficient products and exponent sums -- then simplify (the paper's heavy
+ *     workload simplify(p_d^3)).
+ *
+ * Result form (readings A1-A4): monomials strictly ascending in lexicographic order of
+ * the exponent row with variable 0 (column 0) most significant -- the order of the paper's
+ * transcripts PAPER.md:195-201 and PAPER.md:134; no duplicates; a merged monomial is kept iff
+ * |sum| > tol (absolute, applied after merging; NaN sums are dropped); the zero polynomial is
+ * *out_nterms = 0.
+ *
+ * Pointers: DEVICE unless the name or the comment says host.  The library allocates nothing and
+ * frees nothing: inputs are const and never written, outputs and workspace are caller-owned and
+ * must not overlap the inputs or each other.  All work is enqueued on `cuda_stream` (a cudaStream_t
+ * passed as void*, NULL = legacy default stream).  Unless POLYLAB_FLAG_DEVICE_COUNT is set a call
+ * synchronises that stream before returning (to deliver *out_nterms and the status).
+ * Thread-safe for distinct workspaces.  Every function returns a polylab_status; nothing aborts.
+ */
+#ifndef POLYLAB_H
+#define POLYLAB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)
+#endif
+
+#define POLYLAB_VERSION 100          /* 0.1.0 */
+#define POLYLAB_MAX_NVARS 128        /* packed keys hold at most 128 bits (reading A9) */
+#define POLYLAB_MAX_TERMS ((int64_t)1 << 30)   /* exclusive bound on nterms and on na*nb */
+#define POLYLAB_SMALL_WORKSPACE_BYTES 32768    /* workspace of polylab_expand and polylab_pack_keys */
+
+typedef enum {
+    POLYLAB_OK = 0,
+    POLYLAB_ERR_INVALID_ARGUMENT = 1,   /* null pointer with work to do, nvars < 1 or > MAX_NVARS, nterms < 0 or
+                                           >= MAX_TERMS, tol NaN or < 0, unknown exp_type, nvars mismatch */
+    POLYLAB_ERR_KEY_TOO_WIDE = 2,       /* sum over variables of bitlen(max exponent) > 128 */
+    POLYLAB_ERR_EXPONENT_RANGE = 3,     /* an exponent exceeds the caller's max_exp_host bound, or a product's
+                                           exponent sum does not fit exp_type */
+    POLYLAB_ERR_WORKSPACE_TOO_SMALL = 4,
+    POLYLAB_ERR_OUTPUT_TOO_SMALL = 5,   /* survivors > out_capacity: *out_nterms = required size, the first
+                                           out_capacity terms are written */
+    POLYLAB_ERR_CUDA = 6                /* a CUDA runtime call failed (see polylab_last_cuda_error) */
+} polylab_status;
+
+typedef enum { POLYLAB_EXP_U8 = 1, POLYLAB_EXP_U16 = 2, POLYLAB_EXP_U32 = 4 } polylab_exp_type;
+
+enum {
+    POLYLAB_FLAG_DEVICE_COUNT = 1u   /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
+                                        Requires max_exp_host (no bounds read-back).  Data errors are then
+                                        reported only through the device status word, see polylab_opts. */
+};
+
+/* Per-call statistics (HOST, optional): the plan that was chosen and what the pipeline saw. */
+typedef struct polylab_stats {
+    int32_t key_bits;        /* B = sum of field widths                                  */
+    int32_t key_bytes;       /* W = 8 or 16                                              */
+    int32_t sort_passes;     /* P radix passes executed                                  */
+    int32_t digit_bits[16];  /* width of each pass's digit, least significant first      */
+    int64_t sort_terms;      /* N = terms that entered the sort (na*nb for a product)    */
+    int64_t distinct;        /* U = distinct monomials before pruning (-1 with DEVICE_COUNT) */
+    int64_t survivors;       /* U' (-1 with DEVICE_COUNT)                                */
+    int32_t kernel_launches; /* kernels of this library launched by the call             */
+    int32_t reserved;
+} polylab_stats;
+
+/* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */
+typedef struct polylab_opts {
+    int32_t exp_type;             /* polylab_exp_type of exps and out_exps; 0 = POLYLAB_EXP_U32          */
+    uint32_t flags;               /* POLYLAB_FLAG_*                                                      */
+    int64_t term_stride;          /* element (t,v) of an exponent matrix is at index                     */
+    int64_t var_stride;           /*   t*term_stride + v*var_stride (in elements); both 0 = row-major    */
+                                  /*   (nvars,1); MATLAB's column-major pow is (1,nterms).  Applies to   */
+                                  /*   inputs; outputs are always row-major [out_capacity x nvars].      */
+    const uint32_t* max_exp_host; /* HOST, nvars entries, optional: upper bounds on the exponents of     */
+                                  /*   each variable (for a product: of EACH operand).  Skips the bounds */
+                                  /*   kernel and its read-back; violations -> POLYLAB_ERR_EXPONENT_RANGE */
+    int32_t* status_device;       /* DEVICE, optional: receives the polylab_status of data-dependent      */
+                                  /*   checks (used with POLYLAB_FLAG_DEVICE_COUNT)                      */
+    polylab_stats* stats;         /* HOST, optional                                                      */
+} polylab_opts;
+
+/* A read-only view of a polynomial: coef[nterms], exps[nterms x nvars] (strides from polylab_opts). */
+typedef struct polylab_poly {
+    const double* coef;
+    const void* exps;
+    int64_t nterms;
+    int32_t nvars;
+} polylab_poly;
+
+/* Workspace sizes (bytes, worst case over all key layouts) for the device-pointer entry points. */
+size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts);
+size_t polylab_mul_simplify_workspace_bytes(int64_t na, int64_t nb, int32_t nvars, const polylab_opts* opts);
+
+/*
+ * simplify.  coef[nterms], exps[nterms x nvars] DEVICE inputs (may be unsorted, contain
+ * duplicates, zeros, cancelling pairs).  Outputs: out_coef[out_capacity], out_exps[out_capacity x nvars]
+ * (row-major, exp_type) DEVICE; *out_nterms HOST (DEVICE with POLYLAB_FLAG_DEVICE_COUNT) = number of
+ * surviving monomials U'.  out_capacity = nterms always suffices.  nterms == 0 is valid (0 terms).
+ * Steps: bounds -> pack exponent rows into 64/128-bit keys -> LSD radix sort of (key, coef) -> segmented
+ * sum of equal keys -> prune |s| <= tol -> unpack survivors.
+ */
+int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
+                     const polylab_opts* opts,
+                     double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * simplify(a*b): forms all a->nterms * b->nterms products -- coefficient
+ * fl(ca_i*cb_j) (one IEEE multiplication, never fused with the later sums) and exponent row a_i + b_j --
+ * then merges them as polylab_simplify does.  out_capacity = na*nb always suffices.
+ */
+int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol,
+                         const polylab_opts* opts,
+                         double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * The raw product a*b without merging (reading A10): out_coef[na*nb], out_exps[na*nb x nvars] row-major,
+ * term (i,j) at index i*nb + j.  workspace: POLYLAB_SMALL_WORKSPACE_BYTES.  Exponent sums that do not fit
+ * exp_type -> POLYLAB_ERR_EXPONENT_RANGE (the call synchronises to report it).
+ */
+int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts,
+                   double* out_coef, void* out_exps, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Step S1 alone, exposed for stage-level parity tests: packs each exponent row into a 128-bit key
+ * written as two uint64 (hi, lo) to out_keys[2*nterms]; unsigned order of (hi,lo) = lexicographic order
+ * of rows.  Field widths come from max_exp_host when given, else from the data.  key_bits_host (HOST,
+ * optional) receives B.  workspace: POLYLAB_SMALL_WORKSPACE_BYTES.  Synchronises.
+ */
+int polylab_pack_keys(const void* exps, int64_t nterms, int32_t nvars, const polylab_opts* opts,
+                      uint64_t* out_keys, int32_t* key_bits_host, void* workspace, size_t workspace_bytes,
+                      void* cuda_stream);
+
+/*
+ * The same two operations with HOST input and output buffers (pageable or pinned): copies the inputs
+ * into `device_workspace`, runs the device path, copies the result back, synchronises.  Workspace
+ * size from the *_host_workspace_bytes queries (inputs + outputs + the device path's workspace).
+ * opts->max_exp_host still applies; strides must be row-major here.
+ */
+size_t polylab_simplify_host_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts);
+size_t polylab_mul_simplify_host_workspace_bytes(int64_t na, int64_t nb, int32_t nvars, const polylab_opts* opts);
+int polylab_simplify_host(const double* coef_host, const void* exps_host, int64_t nterms, int32_t nvars,
+                          double tol, const polylab_opts* opts,
+                          double* out_coef_host, void* out_exps_host, int64_t out_capacity,
+                          int64_t* out_nterms_host,
+                          void* device_workspace, size_t workspace_bytes, void* cuda_stream);
+int polylab_mul_simplify_host(const polylab_poly* a_host, const polylab_poly* b_host, double tol,
+                              const polylab_opts* opts,
+                              double* out_coef_host, void* out_exps_host, int64_t out_capacity,
+                              int64_t* out_nterms_host,
+                              void* device_workspace, size_t workspace_bytes, void* cuda_stream);
+
+const char* polylab_status_string(int status);
+const char* polylab_last_cuda_error(void);   /* text of the last CUDA failure seen by this thread */
+int polylab_version(void);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POLYLAB_H */

@@ -1,0 +1,546 @@
+// api.cu -- the C ABI of include/polylab.h: argument checks, the key-layout plan, workspace carving and
+// the launch sequence  S0 bounds -> S1 pack -> (X1 expand) -> S2 radix passes -> S3 reduce -> S4/S5.
+// No step of the path runs on the host; the host only sizes and launches.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "kernels.h"
+
+namespace polylab {
+
+static thread_local char g_cuda_error[256] = "";
+
+static bool cuda_failed(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return false;
+    snprintf(g_cuda_error, sizeof g_cuda_error, "%s: %s", what, cudaGetErrorString(e));
+    return true;
+}
+#define PL_CUDA(call)                                            \
+    do {                                                         \
+        if (cuda_failed((call), #call)) return POLYLAB_ERR_CUDA; \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline int bitlen(uint64_t x) { int b = 0; while (x) { ++b; x >>= 1; } return b; }
+static inline uint32_t exp_max_of(int exp_bytes) { return exp_bytes == 1 ? 0xffu : exp_bytes == 2 ? 0xffffu : 0xffffffffu; }
+
+struct Opts {
+    int exp_bytes;
+    uint32_t flags;
+    int64_t term_stride, var_stride;
+    const uint32_t* max_exp_host;
+    int32_t* status_device;
+    polylab_stats* stats;
+};
+
+static int parse_opts(const polylab_opts* o, int nvars, Opts* out)
+{
+    Opts r;
+    r.exp_bytes = 4; r.flags = 0; r.term_stride = nvars; r.var_stride = 1;
+    r.max_exp_host = nullptr; r.status_device = nullptr; r.stats = nullptr;
+    if (o) {
+        if (o->exp_type != 0) {
+            if (o->exp_type != POLYLAB_EXP_U8 && o->exp_type != POLYLAB_EXP_U16 && o->exp_type != POLYLAB_EXP_U32)
+                return POLYLAB_ERR_INVALID_ARGUMENT;
+            r.exp_bytes = o->exp_type;
+        }
+        r.flags = o->flags;
+        if (o->term_stride != 0 || o->var_stride != 0) { r.term_stride = o->term_stride; r.var_stride = o->var_stride; }
+        if (r.term_stride < 0 || r.var_stride < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+        r.max_exp_host = o->max_exp_host;
+        r.status_device = o->status_device;
+        r.stats = o->stats;
+    }
+    if ((r.flags & POLYLAB_FLAG_DEVICE_COUNT) && !r.max_exp_host) return POLYLAB_ERR_INVALID_ARGUMENT;
+    *out = r;
+    return POLYLAB_OK;
+}
+
+static ExpView make_view(const void* base, const Opts& o, int nvars)
+{
+    ExpView v;
+    v.base = base;
+    v.term_stride = o.term_stride;
+    v.var_stride = o.var_stride;
+    v.exp_bytes = o.exp_bytes;
+    v.row_major_contiguous = (o.term_stride == nvars && o.var_stride == 1 && ((uintptr_t)base % 16) == 0) ? 1 : 0;
+    return v;
+}
+
+// Key layout from the per-variable maxima m_v of the rows that will be SORTED (for a product: max_a + max_b)
+// and the bounds that INPUT rows must respect.  Variable 0 gets the most significant field (reading A1).
+static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* plan)
+{
+    memset(plan, 0, sizeof *plan);
+    plan->nvars = nvars;
+    int bits = 0;
+    for (int v = nvars - 1; v >= 0; --v) {
+        const int w = bitlen(m[v]);
+        if (w > 32) return POLYLAB_ERR_EXPONENT_RANGE;
+        if (bits + w > 128) return POLYLAB_ERR_KEY_TOO_WIDE;
+        plan->shift[v] = (uint8_t)(w ? bits : 0);
+        plan->width[v] = (uint8_t)w;
+        plan->bound[v] = bound[v];
+        bits += w;
+    }
+    plan->key_bits = bits;
+    plan->key_bytes = bits <= 64 ? 8 : 16;
+    const int P = (bits + kRadixBits - 1) / kRadixBits;
+    plan->npasses = P;
+    int pos = 0;
+    for (int p = 0; p < P; ++p) {            // balanced digit widths: B = sum of P digits of floor/ceil(B/P) bits
+        const int w = bits / P + (p < bits % P ? 1 : 0);
+        plan->digit_pos[p] = (uint8_t)pos;
+        plan->digit_bits[p] = (uint8_t)w;
+        pos += w;
+    }
+    return POLYLAB_OK;
+}
+
+// ------------------------------------------------------------------------------ workspace carving
+
+struct Layout {
+    size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, zero_end;
+    size_t keys[2], coefs[2], ka, kb, total;
+};
+
+static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
+{
+    Layout L;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t sort_tiles = (size_t)((n + sort_tile(key_bytes) - 1) / sort_tile(key_bytes));
+    const size_t red_tiles = (size_t)((n + kReduceTile - 1) / kReduceTile);
+    const size_t prune_tiles = (size_t)((n + kPruneTile - 1) / kPruneTile);
+    L.control = take(sizeof(Control));
+    L.sort_state = take(sort_tiles * kRadix * sizeof(uint32_t));
+    L.red_state = take(red_tiles * sizeof(uint32_t));
+    L.prune_state = take(prune_tiles * sizeof(uint32_t));
+    L.zero_end = off;                                   // everything before this is zeroed per call
+    L.red_heads = take(red_tiles * sizeof(uint32_t));
+    L.red_hb = take(red_tiles * sizeof(uint32_t));
+    L.red_frag = take(red_tiles * sizeof(double));
+    L.red_cont = take(red_tiles);
+    for (int i = 0; i < 2; ++i) L.keys[i] = take((size_t)n * key_bytes);
+    for (int i = 0; i < 2; ++i) L.coefs[i] = take((size_t)n * sizeof(double));
+    L.ka = take((size_t)na * key_bytes);
+    L.kb = take((size_t)nb * key_bytes);
+    L.total = off;
+    return L;
+}
+
+static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb)
+{
+    const size_t a = make_layout(n, 8, na, nb).total, b = make_layout(n, 16, na, nb).total;
+    return (a > b ? a : b) + 256;                       // + slack to align the caller's base pointer
+}
+
+static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
+{
+    if (!st) return;
+    memset(st, 0, sizeof *st);
+    st->key_bits = plan.key_bits;
+    st->key_bytes = plan.key_bytes;
+    st->sort_passes = plan.npasses;
+    for (int p = 0; p < plan.npasses; ++p) st->digit_bits[p] = plan.digit_bits[p];
+    st->sort_terms = n;
+    st->distinct = -1;
+    st->survivors = -1;
+}
+
+// ----------------------------------------------------------------------- shared tail of both paths
+
+// keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
+static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
+                            double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
+                            int64_t* out_nterms, int* launches, cudaStream_t stream)
+{
+    Control* ctl = (Control*)(ws + L.control);
+    void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
+    double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
+    const int P = plan.npasses;
+    for (int p = 0; p < P; ++p) {
+        const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
+        *launches += launch_sort_pass(plan, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1], cbuf[(p + 1) & 1],
+                                      (uint32_t*)(ws + L.sort_state), ctl, stream);
+    }
+    const void* skeys = kbuf[P & 1];
+    const double* scoef = (P == 0) ? coef0 : cbuf[P & 1];
+    void* ukeys = kbuf[(P + 1) & 1];
+    double* usums = cbuf[(P + 1) & 1];
+    ReduceScratch sc;
+    sc.tile_state = (uint32_t*)(ws + L.red_state);
+    sc.tile_heads = (uint32_t*)(ws + L.red_heads);
+    sc.tile_hb = (uint32_t*)(ws + L.red_hb);
+    sc.tile_frag = (double*)(ws + L.red_frag);
+    sc.tile_cont = (uint8_t*)(ws + L.red_cont);
+    *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
+    const bool dev_count = (o.flags & POLYLAB_FLAG_DEVICE_COUNT) != 0;
+    *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
+                                     (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+    PL_CUDA(cudaGetLastError());
+    if (o.stats) o.stats->kernel_launches = *launches;
+    if (dev_count) {
+        if (o.status_device)
+            PL_CUDA(cudaMemcpyAsync(o.status_device, &ctl->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+        return POLYLAB_OK;
+    }
+    struct { int32_t status; uint32_t distinct, survivors; } res;
+    PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; }
+    if (res.status != POLYLAB_OK) return res.status;
+    *out_nterms = (int64_t)res.survivors;
+    return (int64_t)res.survivors > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
+}
+
+static int deliver_zero(const Opts& o, int64_t* out_nterms, cudaStream_t stream)
+{
+    if (o.flags & POLYLAB_FLAG_DEVICE_COUNT) {
+        PL_CUDA(cudaMemsetAsync(out_nterms, 0, sizeof(int64_t), stream));
+        if (o.status_device) PL_CUDA(cudaMemsetAsync(o.status_device, 0, sizeof(int32_t), stream));
+    } else *out_nterms = 0;
+    if (o.stats) { memset(o.stats, 0, sizeof *o.stats); }
+    return POLYLAB_OK;
+}
+
+static unsigned char* align_ptr(void* p) { return (unsigned char*)(((uintptr_t)p + 255) / 256 * 256); }
+
+}  // namespace polylab
+
+using namespace polylab;
+
+// =============================================================================== entry points
+
+extern "C" {
+
+size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
+{
+    (void)nvars; (void)opts;
+    if (nterms < 0) return 0;
+    return worst_layout_bytes(nterms, 0, 0);
+}
+
+size_t polylab_mul_simplify_workspace_bytes(int64_t na, int64_t nb, int32_t nvars, const polylab_opts* opts)
+{
+    (void)nvars; (void)opts;
+    if (na < 0 || nb < 0) return 0;
+    if (na > 0 && nb > 0 && na >= POLYLAB_MAX_TERMS / nb + 1) return 0;
+    return worst_layout_bytes(na * nb, na, nb);
+}
+
+int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
+                     const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                     int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || nterms < 0 || nterms >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (!(tol >= 0.0) || isinf(tol) || !out_nterms || out_capacity < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    if (nterms == 0) return deliver_zero(o, out_nterms, stream);
+    if (!coef || !exps || !workspace || (out_capacity > 0 && (!out_coef || !out_exps))) return POLYLAB_ERR_INVALID_ARGUMENT;
+
+    unsigned char* ws = align_ptr(workspace);
+    const size_t avail = workspace_bytes >= (size_t)(ws - (unsigned char*)workspace) ? workspace_bytes - (ws - (unsigned char*)workspace) : 0;
+    if (avail < sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    int launches = 0;
+    const ExpView ev = make_view(exps, o, nvars);
+    Control* ctl = (Control*)ws;             // Layout::control is offset 0 for every layout
+
+    // ---- S0: per-variable maxima (from the caller, or from the data with one read-back)
+    uint64_t m[kMaxVars];
+    uint32_t bound[kMaxVars];
+    if (o.max_exp_host) {
+        for (int v = 0; v < nvars; ++v) { m[v] = o.max_exp_host[v]; bound[v] = o.max_exp_host[v]; }
+    } else {
+        PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
+        launches += launch_bounds(ev, nterms, nvars, ctl, 0, stream);
+        uint32_t mh[kMaxVars];
+        PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp[0], sizeof(uint32_t) * nvars, cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        for (int v = 0; v < nvars; ++v) { m[v] = mh[v]; bound[v] = mh[v]; }
+    }
+    Plan plan;
+    rc = make_plan(nvars, m, bound, &plan);
+    if (rc != POLYLAB_OK) return rc;
+    fill_stats(o.stats, plan, nterms);
+
+    const Layout L = make_layout(nterms, plan.key_bytes, 0, 0);
+    if (avail < L.total) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
+
+    // ---- S1 (+ histogram of the first digit), then the shared tail
+    launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0, stream);
+    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, stream);
+}
+
+int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
+                         double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (!a || !b || a->nvars != b->nvars) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int nvars = a->nvars;
+    const int64_t na = a->nterms, nb = b->nterms;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || na < 0 || nb < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (na > 0 && nb > 0 && na > (POLYLAB_MAX_TERMS - 1) / nb) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (!(tol >= 0.0) || isinf(tol) || !out_nterms || out_capacity < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    const int64_t n = na * nb;
+    if (n == 0) return deliver_zero(o, out_nterms, stream);
+    if (!a->coef || !a->exps || !b->coef || !b->exps || !workspace || (out_capacity > 0 && (!out_coef || !out_exps)))
+        return POLYLAB_ERR_INVALID_ARGUMENT;
+
+    unsigned char* ws = align_ptr(workspace);
+    const size_t avail = workspace_bytes >= (size_t)(ws - (unsigned char*)workspace) ? workspace_bytes - (ws - (unsigned char*)workspace) : 0;
+    if (avail < sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    int launches = 0;
+    Opts oa = o, ob = o;
+    if (o.term_stride == nvars && o.var_stride == 1) { /* row-major: same strides for both operands */ }
+    const ExpView eva = make_view(a->exps, oa, nvars), evb = make_view(b->exps, ob, nvars);
+    Control* ctl = (Control*)ws;
+
+    // ---- S0 on both operands; the sorted rows are sums, so fields are sized for max_a + max_b
+    uint64_t m[kMaxVars];
+    uint32_t ba[kMaxVars], bb[kMaxVars];
+    const uint32_t emax = exp_max_of(o.exp_bytes);
+    if (o.max_exp_host) {
+        for (int v = 0; v < nvars; ++v) { ba[v] = bb[v] = o.max_exp_host[v]; m[v] = 2ull * o.max_exp_host[v]; }
+    } else {
+        PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
+        launches += launch_bounds(eva, na, nvars, ctl, 0, stream);
+        launches += launch_bounds(evb, nb, nvars, ctl, 1, stream);
+        uint32_t mh[2][kMaxVars];
+        PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp, sizeof mh, cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        for (int v = 0; v < nvars; ++v) {
+            ba[v] = mh[0][v]; bb[v] = mh[1][v];
+            m[v] = (uint64_t)mh[0][v] + mh[1][v];
+            if (m[v] > emax) return POLYLAB_ERR_EXPONENT_RANGE;       // the sum must fit exp_type (reading A8)
+        }
+    }
+    Plan plan_a, plan_b;
+    rc = make_plan(nvars, m, ba, &plan_a);
+    if (rc != POLYLAB_OK) return rc;
+    make_plan(nvars, m, bb, &plan_b);
+    fill_stats(o.stats, plan_a, n);
+
+    const Layout L = make_layout(n, plan_a.key_bytes, na, nb);
+    if (avail < L.total) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
+
+    // ---- S1 on the operands, X1 on packed keys (+ histogram of the first digit), then the shared tail
+    launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, false, stream);
+    launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, false, stream);
+    launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
+                                     (double*)(ws + L.coefs[0]), ctl, stream);
+    return sort_reduce_emit(plan_a, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
+                            out_nterms, &launches, stream);
+}
+
+int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts, double* out_coef,
+                   void* out_exps, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (!a || !b || a->nvars != b->nvars) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int nvars = a->nvars;
+    const int64_t na = a->nterms, nb = b->nterms;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || na < 0 || nb < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (na > 0 && nb > 0 && na > (POLYLAB_MAX_TERMS - 1) / nb) return POLYLAB_ERR_INVALID_ARGUMENT;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    if (na * nb == 0) return POLYLAB_OK;
+    if (!a->coef || !a->exps || !b->coef || !b->exps || !out_coef || !out_exps || !workspace) return POLYLAB_ERR_INVALID_ARGUMENT;
+    unsigned char* ws = align_ptr(workspace);
+    if (workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    Control* ctl = (Control*)ws;
+    PL_CUDA(cudaMemsetAsync(&ctl->status, 0, sizeof(int32_t), stream));
+    launch_expand_raw(make_view(a->exps, o, nvars), a->coef, na, make_view(b->exps, o, nvars), b->coef, nb, nvars, out_coef,
+                      out_exps, ctl, stream);
+    PL_CUDA(cudaGetLastError());
+    int32_t status = 0;
+    PL_CUDA(cudaMemcpyAsync(&status, &ctl->status, sizeof status, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    return status;
+}
+
+int polylab_pack_keys(const void* exps, int64_t nterms, int32_t nvars, const polylab_opts* opts, uint64_t* out_keys,
+                      int32_t* key_bits_host, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || nterms < 0 || nterms >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    if (nterms == 0) { if (key_bits_host) *key_bits_host = 0; return POLYLAB_OK; }
+    if (!exps || !out_keys || !workspace) return POLYLAB_ERR_INVALID_ARGUMENT;
+    unsigned char* ws = align_ptr(workspace);
+    if (workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    Control* ctl = (Control*)ws;
+    const ExpView ev = make_view(exps, o, nvars);
+    PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
+    uint64_t m[kMaxVars];
+    uint32_t bound[kMaxVars];
+    if (o.max_exp_host) {
+        for (int v = 0; v < nvars; ++v) { m[v] = o.max_exp_host[v]; bound[v] = o.max_exp_host[v]; }
+    } else {
+        launch_bounds(ev, nterms, nvars, ctl, 0, stream);
+        uint32_t mh[kMaxVars];
+        PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp[0], sizeof(uint32_t) * nvars, cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        for (int v = 0; v < nvars; ++v) { m[v] = mh[v]; bound[v] = mh[v]; }
+    }
+    Plan plan;
+    rc = make_plan(nvars, m, bound, &plan);
+    if (rc != POLYLAB_OK) return rc;
+    if (key_bits_host) *key_bits_host = plan.key_bits;
+    launch_pack_hilo(ev, nterms, plan, out_keys, ctl, stream);
+    PL_CUDA(cudaGetLastError());
+    int32_t status = 0;
+    PL_CUDA(cudaMemcpyAsync(&status, &ctl->status, sizeof status, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    return status;
+}
+
+// ------------------------------------------------------------------- host-buffer entry points
+
+struct HostLayout { size_t coef, exps, out_coef, out_exps, inner, total; };
+
+static HostLayout host_layout(int64_t n_in_terms, int64_t n_sort, int nvars, int exp_bytes, size_t inner_bytes)
+{
+    HostLayout H;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
+    H.coef = take((size_t)n_in_terms * sizeof(double));
+    H.exps = take((size_t)n_in_terms * nvars * exp_bytes);
+    H.out_coef = take((size_t)n_sort * sizeof(double));
+    H.out_exps = take((size_t)n_sort * nvars * exp_bytes);
+    H.inner = take(inner_bytes);
+    H.total = off + 256;
+    return H;
+}
+
+static int opts_exp_bytes(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
+
+size_t polylab_simplify_host_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
+{
+    if (nterms < 0 || nvars < 1) return 0;
+    return host_layout(nterms, nterms, nvars, opts_exp_bytes(opts), polylab_simplify_workspace_bytes(nterms, nvars, opts)).total;
+}
+
+size_t polylab_mul_simplify_host_workspace_bytes(int64_t na, int64_t nb, int32_t nvars, const polylab_opts* opts)
+{
+    if (na < 0 || nb < 0 || nvars < 1) return 0;
+    return host_layout(na + nb + 64, na * nb, nvars, opts_exp_bytes(opts), polylab_mul_simplify_workspace_bytes(na, nb, nvars, opts)).total;
+}
+
+static int host_opts_ok(const polylab_opts* opts, int nvars)
+{
+    if (!opts) return 1;
+    if (opts->flags & POLYLAB_FLAG_DEVICE_COUNT) return 0;
+    if ((opts->term_stride != 0 || opts->var_stride != 0) && !(opts->term_stride == nvars && opts->var_stride == 1)) return 0;
+    return 1;
+}
+
+int polylab_simplify_host(const double* coef_host, const void* exps_host, int64_t nterms, int32_t nvars, double tol,
+                          const polylab_opts* opts, double* out_coef_host, void* out_exps_host, int64_t out_capacity,
+                          int64_t* out_nterms_host, void* device_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || nterms < 0 || nterms >= POLYLAB_MAX_TERMS || !out_nterms_host || out_capacity < 0)
+        return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (!host_opts_ok(opts, nvars)) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (nterms == 0) { *out_nterms_host = 0; return (tol >= 0.0) ? POLYLAB_OK : POLYLAB_ERR_INVALID_ARGUMENT; }
+    if (!coef_host || !exps_host || !device_workspace) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int es = opts_exp_bytes(opts);
+    const size_t inner = polylab_simplify_workspace_bytes(nterms, nvars, opts);
+    const HostLayout H = host_layout(nterms, nterms, nvars, es, inner);
+    unsigned char* ws = align_ptr(device_workspace);
+    if (workspace_bytes < (size_t)(ws - (unsigned char*)device_workspace) + H.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    PL_CUDA(cudaMemcpyAsync(ws + H.coef, coef_host, (size_t)nterms * sizeof(double), cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(ws + H.exps, exps_host, (size_t)nterms * nvars * es, cudaMemcpyHostToDevice, stream));
+    int64_t count = 0;
+    const int rc = polylab_simplify((const double*)(ws + H.coef), ws + H.exps, nterms, nvars, tol, opts, (double*)(ws + H.out_coef),
+                                    ws + H.out_exps, nterms, &count, ws + H.inner, inner, cuda_stream);
+    if (rc != POLYLAB_OK) return rc;
+    *out_nterms_host = count;
+    const int64_t ncopy = count < out_capacity ? count : out_capacity;
+    if (ncopy > 0) {
+        if (!out_coef_host || !out_exps_host) return POLYLAB_ERR_INVALID_ARGUMENT;
+        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaMemcpyAsync(out_exps_host, ws + H.out_exps, (size_t)ncopy * nvars * es, cudaMemcpyDeviceToHost, stream));
+    }
+    PL_CUDA(cudaStreamSynchronize(stream));
+    return count > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
+}
+
+int polylab_mul_simplify_host(const polylab_poly* a_host, const polylab_poly* b_host, double tol, const polylab_opts* opts,
+                              double* out_coef_host, void* out_exps_host, int64_t out_capacity, int64_t* out_nterms_host,
+                              void* device_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (!a_host || !b_host || a_host->nvars != b_host->nvars || !out_nterms_host || out_capacity < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int nvars = a_host->nvars;
+    const int64_t na = a_host->nterms, nb = b_host->nterms;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || na < 0 || nb < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (na > 0 && nb > 0 && na > (POLYLAB_MAX_TERMS - 1) / nb) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (!host_opts_ok(opts, nvars)) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int64_t n = na * nb;
+    if (n == 0) { *out_nterms_host = 0; return (tol >= 0.0) ? POLYLAB_OK : POLYLAB_ERR_INVALID_ARGUMENT; }
+    if (!a_host->coef || !a_host->exps || !b_host->coef || !b_host->exps || !device_workspace) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int es = opts_exp_bytes(opts);
+    const size_t inner = polylab_mul_simplify_workspace_bytes(na, nb, nvars, opts);
+    const HostLayout H = host_layout(na + nb + 64, n, nvars, es, inner);
+    unsigned char* ws = align_ptr(device_workspace);
+    if (workspace_bytes < (size_t)(ws - (unsigned char*)device_workspace) + H.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    // operand b sits behind operand a in the input slices, each 32-term aligned
+    const int64_t nb_off = (na + 31) / 32 * 32;
+    double* dca = (double*)(ws + H.coef);
+    double* dcb = dca + nb_off;
+    unsigned char* dea = ws + H.exps;
+    unsigned char* deb = dea + (size_t)nb_off * nvars * es;
+    PL_CUDA(cudaMemcpyAsync(dca, a_host->coef, (size_t)na * sizeof(double), cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(dcb, b_host->coef, (size_t)nb * sizeof(double), cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(dea, a_host->exps, (size_t)na * nvars * es, cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(deb, b_host->exps, (size_t)nb * nvars * es, cudaMemcpyHostToDevice, stream));
+    polylab_poly da = {dca, dea, na, nvars}, db = {dcb, deb, nb, nvars};
+    int64_t count = 0;
+    const int rc = polylab_mul_simplify(&da, &db, tol, opts, (double*)(ws + H.out_coef), ws + H.out_exps, n, &count, ws + H.inner,
+                                        inner, cuda_stream);
+    if (rc != POLYLAB_OK) return rc;
+    *out_nterms_host = count;
+    const int64_t ncopy = count < out_capacity ? count : out_capacity;
+    if (ncopy > 0) {
+        if (!out_coef_host || !out_exps_host) return POLYLAB_ERR_INVALID_ARGUMENT;
+        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaMemcpyAsync(out_exps_host, ws + H.out_exps, (size_t)ncopy * nvars * es, cudaMemcpyDeviceToHost, stream));
+    }
+    PL_CUDA(cudaStreamSynchronize(stream));
+    return count > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
+}
+
+const char* polylab_status_string(int status)
+{
+    switch (status) {
+    case POLYLAB_OK: return "ok";
+    case POLYLAB_ERR_INVALID_ARGUMENT: return "invalid argument";
+    case POLYLAB_ERR_KEY_TOO_WIDE: return "packed key wider than 128 bits";
+    case POLYLAB_ERR_EXPONENT_RANGE: return "exponent out of range";
+    case POLYLAB_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case POLYLAB_ERR_OUTPUT_TOO_SMALL: return "output capacity too small";
+    case POLYLAB_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+    }
+}
+
+const char* polylab_last_cuda_error(void) { return g_cuda_error; }
+int polylab_version(void) { return POLYLAB_VERSION; }
+
+}  // extern "C"

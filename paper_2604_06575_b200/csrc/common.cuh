@@ -1,0 +1,236 @@
+// common.cuh -- shared device/host definitions of the polylab-b200 CUDA path (sm_100a).
+//
+// Nothing here is shared with oracle/: the oracle never packs keys.  The key layout follows
+// variable 0 occupies the most significant field, fields are right-aligned to
+// bit 0, field v is w_v = bitlen(m_v) bits wide (0 bits when the variable is identically zero), so
+// that unsigned order of keys = ascending lexicographic order of exponent rows (reading A1, the
+// order of the paper's transcripts PAPER.md:195-201).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/polylab.h"
+
+namespace polylab {
+
+constexpr int kMaxVars = POLYLAB_MAX_NVARS;
+constexpr int kMaxPasses = 16;          // 128 bits / 8-bit digits
+constexpr int kRadixBits = 8;           // widest digit
+constexpr int kRadix = 1 << kRadixBits; // bins per pass
+constexpr unsigned kFullMask = 0xffffffffu;
+
+// ------------------------------------------------------------------------------------ keys
+
+// 128-bit key, 16-byte aligned so that one key is one vector load/store.
+struct __align__(16) Key128 {
+    uint64_t hi, lo;     // memory order (hi, lo): the layout polylab_pack_keys exposes
+};
+
+__host__ __device__ inline bool key_eq(uint64_t a, uint64_t b) { return a == b; }
+__host__ __device__ inline bool key_eq(const Key128& a, const Key128& b) { return a.lo == b.lo && a.hi == b.hi; }
+
+// `bits` (<= 8) bits of the key starting at bit `pos` (0 = least significant)
+__device__ __forceinline__ uint32_t key_digit(uint64_t k, int pos, uint32_t mask) { return (uint32_t)(k >> pos) & mask; }
+__device__ __forceinline__ uint32_t key_digit(const Key128& k, int pos, uint32_t mask)
+{
+    uint64_t w;
+    if (pos >= 64) w = k.hi >> (pos - 64);
+    else if (pos == 0) w = k.lo;
+    else w = (k.lo >> pos) | (k.hi << (64 - pos));
+    return (uint32_t)w & mask;
+}
+
+__device__ __forceinline__ uint64_t key_add(uint64_t a, uint64_t b) { return a + b; }
+__device__ __forceinline__ Key128 key_add(const Key128& a, const Key128& b)
+{
+    Key128 r;
+    r.lo = a.lo + b.lo;
+    r.hi = a.hi + b.hi + (r.lo < a.lo ? 1ull : 0ull);   // fields never carry into each other, words may
+    return r;
+}
+
+template <typename K> __device__ __forceinline__ K key_max();
+template <> __device__ __forceinline__ uint64_t key_max<uint64_t>() { return ~0ull; }
+template <> __device__ __forceinline__ Key128 key_max<Key128>() { Key128 k; k.lo = ~0ull; k.hi = ~0ull; return k; }
+
+// OR `e << shift` into a key (shift + width <= key bits by construction of the plan)
+__device__ __forceinline__ void key_or_field(uint64_t& k, uint32_t e, int shift) { k |= (uint64_t)e << shift; }
+__device__ __forceinline__ void key_or_field(Key128& k, uint32_t e, int shift)
+{
+    if (shift >= 64) k.hi |= (uint64_t)e << (shift - 64);
+    else {
+        k.lo |= (uint64_t)e << shift;
+        if (shift > 32) k.hi |= (uint64_t)e >> (64 - shift);   // e has 32 bits: spills iff shift > 32
+    }
+}
+__device__ __forceinline__ uint32_t key_get_field(uint64_t k, int shift, int width)
+{
+    return width == 0 ? 0u : (uint32_t)((k >> shift) & ((width == 32) ? 0xffffffffull : ((1ull << width) - 1)));
+}
+__device__ __forceinline__ uint32_t key_get_field(const Key128& k, int shift, int width)
+{
+    if (width == 0) return 0u;
+    uint64_t w;
+    if (shift >= 64) w = k.hi >> (shift - 64);
+    else if (shift == 0) w = k.lo;
+    else w = (k.lo >> shift) | (k.hi << (64 - shift));
+    return (uint32_t)(w & ((width == 32) ? 0xffffffffull : ((1ull << width) - 1)));
+}
+__device__ __forceinline__ void key_zero(uint64_t& k) { k = 0; }
+__device__ __forceinline__ void key_zero(Key128& k) { k.lo = 0; k.hi = 0; }
+
+// ------------------------------------------------------------------------------------ plan
+
+// Key layout and pass table, computed on the host from the per-variable maxima (step S0) and passed
+// to kernels by value.
+struct Plan {
+    int32_t nvars;
+    int32_t key_bits;                  // B
+    int32_t key_bytes;                 // W: 8 or 16
+    int32_t npasses;                   // P
+    uint8_t shift[kMaxVars];           // bit position of field v
+    uint8_t width[kMaxVars];           // w_v
+    uint32_t bound[kMaxVars];          // largest exponent an INPUT row may hold in variable v
+    uint8_t digit_pos[kMaxPasses];     // bit position of pass p's digit
+    uint8_t digit_bits[kMaxPasses];    // its width (<= kRadixBits)
+};
+
+// How an exponent matrix is addressed: element (t,v) at base[t*term_stride + v*var_stride].
+struct ExpView {
+    const void* base;
+    int64_t term_stride;
+    int64_t var_stride;
+    int32_t exp_bytes;                 // 1, 2 or 4
+    int32_t row_major_contiguous;      // term_stride == nvars && var_stride == 1 && base 16-byte aligned
+};
+
+__device__ __forceinline__ uint32_t load_exp(const void* base, int exp_bytes, int64_t idx)
+{
+    if (exp_bytes == 1) return ((const uint8_t*)base)[idx];
+    if (exp_bytes == 2) return ((const uint16_t*)base)[idx];
+    return ((const uint32_t*)base)[idx];
+}
+__device__ __forceinline__ void store_exp(void* base, int exp_bytes, int64_t idx, uint32_t e)
+{
+    if (exp_bytes == 1) ((uint8_t*)base)[idx] = (uint8_t)e;
+    else if (exp_bytes == 2) ((uint16_t*)base)[idx] = (uint16_t)e;
+    else ((uint32_t*)base)[idx] = e;
+}
+
+// --------------------------------------------------------------------------- control block
+
+// Small device-side state at the head of the workspace, zeroed at the start of every call.
+struct Control {
+    uint32_t hist[kMaxPasses + 1][kRadix];   // digit histograms, one per pass (filled one pass ahead)
+    uint32_t ticket[kMaxPasses + 4];         // dynamic tile ids: sort passes, then reduce, then prune
+    uint32_t max_exp[2][kMaxVars];           // S0 results (operand a, operand b)
+    int32_t status;                          // polylab_status of data-dependent checks
+    uint32_t distinct;                       // U
+    uint32_t survivors;                      // U'
+    uint32_t pad;
+};
+
+constexpr int kTicketReduce = kMaxPasses;
+constexpr int kTicketPrune = kMaxPasses + 1;
+
+// ------------------------------------------------------------------------- warp/block helpers
+
+__device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ unsigned lanemask_lt() { return (1u << (threadIdx.x & 31u)) - 1u; }
+
+// lanes of the warp that are `valid` and hold the same digit d (< 256) as the calling lane
+__device__ __forceinline__ unsigned match_digit(uint32_t d, bool valid)
+{
+    unsigned mask = __ballot_sync(kFullMask, valid);
+#pragma unroll
+    for (int b = 0; b < kRadixBits; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const unsigned m = __ballot_sync(kFullMask, bit);
+        mask &= bit ? m : ~m;
+    }
+    return mask;
+}
+
+// volatile accesses for the decoupled look-back words (value and flag share one 32-bit word)
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v)
+{
+    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Exclusive scan of one uint32 per thread over a block of THREADS (multiple of 32, <= 1024).
+// `warp_scratch` holds THREADS/32 + 1 words of shared memory; returns the exclusive prefix and
+// stores the block total in *total.  Contains two __syncthreads().
+template <int THREADS>
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* warp_scratch, uint32_t* total)
+{
+    constexpr int NW = THREADS / 32;
+    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t incl = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(kFullMask, incl, o);
+        if (lane >= (unsigned)o) incl += y;
+    }
+    if (lane == 31) warp_scratch[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = lane < NW ? warp_scratch[lane] : 0u;
+        uint32_t wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(kFullMask, wi, o);
+            if (lane >= (unsigned)o) wi += y;
+        }
+        if (lane < NW) warp_scratch[lane] = wi - w;      // exclusive warp offsets
+        if (lane == NW - 1) warp_scratch[NW] = wi;       // block total
+    }
+    __syncthreads();
+    *total = warp_scratch[NW];
+    return warp_scratch[warp] + incl - x;
+}
+
+// Decoupled look-back over single-word tile states: word = (value << 2) | flag.
+constexpr uint32_t kFlagInvalid = 0, kFlagPartial = 1, kFlagInclusive = 2;
+
+// Called by ONE warp of the block.  Publishes `count` for tile `tile`, walks back over the
+// predecessors (32 at a time) and returns the sum of the counts of tiles < tile (valid in all lanes).
+// state[] must be zero before the kernel; tiles are handed out by an atomic ticket so every
+// predecessor is resident and makes progress.
+__device__ __forceinline__ uint32_t warp_lookback_u32(uint32_t* state, uint32_t tile, uint32_t count)
+{
+    const unsigned lane = lane_id();
+    if (tile == 0) {
+        if (lane == 0) st_volatile_u32(&state[0], (count << 2) | kFlagInclusive);
+        return 0u;
+    }
+    if (lane == 0) st_volatile_u32(&state[tile], (count << 2) | kFlagPartial);
+    uint32_t excl = 0;
+    int64_t base = (int64_t)tile - 1;                  // lane l looks at tile base - l
+    while (true) {
+        const int64_t t = base - lane;
+        uint32_t w = kFlagInclusive;                   // tiles before 0: inclusive, value 0
+        if (t >= 0) {
+            do { w = ld_volatile_u32(&state[t]); } while ((w & 3u) == kFlagInvalid);
+        }
+        const unsigned incl_mask = __ballot_sync(kFullMask, (w & 3u) == kFlagInclusive);
+        // lanes up to and including the nearest inclusive one contribute
+        const int stop = incl_mask ? (__ffs(incl_mask) - 1) : 31;
+        uint32_t v = (lane <= (unsigned)stop) ? (w >> 2) : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFullMask, v, o);
+        excl += v;
+        if (incl_mask) break;
+        base -= 32;
+    }
+    if (lane == 0) st_volatile_u32(&state[tile], ((excl + count) << 2) | kFlagInclusive);
+    return excl;
+}
+
+}  // namespace polylab

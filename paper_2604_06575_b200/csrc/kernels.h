@@ -1,0 +1,68 @@
+// kernels.h -- host-side launchers of the polylab-b200 kernels (internal; the public ABI is
+// include/polylab.h).  Every launcher enqueues on `stream`, returns the number of kernels it
+// launched, and never synchronises.  Step names S0..S5, X1 are those of DESIGN.md.
+#pragma once
+
+#include "common.cuh"
+
+namespace polylab {
+
+// Tile sizes of the streaming kernels (records per thread block); also used by the workspace query.
+constexpr int kSortThreads = 256;
+constexpr int kSortItems64 = 16;    // 4096-record tiles of (u64 key, f64 coef)
+constexpr int kSortItems128 = 12;   // 3072-record tiles of (u128 key, f64 coef)
+constexpr int kReduceThreads = 256;
+constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from shared memory
+constexpr int kPruneThreads = 256;
+constexpr int kPruneItems = 8;
+
+inline int sort_tile(int key_bytes) { return kSortThreads * (key_bytes == 8 ? kSortItems64 : kSortItems128); }
+constexpr int kReduceTile = kReduceThreads * kReduceItems;
+constexpr int kPruneTile = kPruneThreads * kPruneItems;
+
+// S0: per-variable maxima of an exponent matrix into ctl->max_exp[which][v] (atomicMax).
+int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream);
+
+// S1: pack rows into keys (key_bytes from the plan), check e <= plan.bound (-> ctl->status), and, when
+// hist0 is true, accumulate the histogram of pass 0's digit into ctl->hist[0].
+int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, bool hist0,
+                cudaStream_t stream);
+
+// S1 for the test entry point: always writes (hi, lo) pairs.
+int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
+                     cudaStream_t stream);
+
+// X1: all products of packed operands: key = ka_i + kb_j, coef = fl(ca_i * cb_j); N = na*nb pairs written
+// to keys/coefs (emission order: i*nb + j); histogram of pass 0's digit into ctl->hist[0].
+int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
+                         const Plan& plan, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
+
+// Raw product without keys (polylab_expand): rows a_i + b_j, coefficients fl(ca_i*cb_j).
+int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const ExpView& eb, const double* cb, int64_t nb,
+                      int nvars, double* out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream);
+
+// S2: one stable LSD radix pass (digit `pass` of the plan) of n (key, coef) pairs from (keys_in, coef_in)
+// to (keys_out, coef_out).  tile_state: ceil(n/tile) * 256 words, zero before the FIRST pass of a call and
+// reused by every later pass (flag parity alternates).  Also accumulates the next pass's histogram.
+int launch_sort_pass(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in, void* keys_out,
+                     double* coef_out, uint32_t* tile_state, Control* ctl, cudaStream_t stream);
+
+// S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U.
+// Scratch: tile_state/tile_heads/tile_hb [ntiles] uint32 (zeroed), tile_frag [ntiles] double, tile_cont [ntiles] uint8.
+struct ReduceScratch {
+    uint32_t* tile_state;
+    uint32_t* tile_heads;
+    uint32_t* tile_hb;
+    double* tile_frag;
+    uint8_t* tile_cont;
+};
+int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coefs, void* ukeys, double* usums,
+                  const ReduceScratch& sc, Control* ctl, cudaStream_t stream);
+
+// S4+S5: keep |s| > tol, order-preserving compaction, unpack into out_coef/out_exps (row-major, exp_bytes);
+// ctl->survivors = U'.  max_units bounds U (grid sizing); tile_state: ceil(max_units/kPruneTile) words, zeroed.
+int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
+                        double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
+                        Control* ctl, int64_t* out_count_device, cudaStream_t stream);
+
+}  // namespace polylab

@@ -1,0 +1,263 @@
+// pack.cu -- steps S0 (bounds), S1 (pack exponent rows into keys) and X1 (term-product expansion).
+//
+// S1: key_t = sum_v e_{t,v} << shift_v with variable 0 in the most significant field (
+// the row order it must reproduce is the paper's transcript order).
+// X1: all na*nb products of two polynomials -- coefficient products and exponent sums (mtimes/times,
+// PAPER.md:117-118); on packed keys the exponent sum of every variable is ONE integer addition because
+// the plan sizes each field for max_a + max_b (no carry between fields).
+#include "kernels.h"
+
+namespace polylab {
+
+// ----------------------------------------------------------------------------------------------- S0
+
+// Thread tid of the first VT = (THREADS / nvars) * nvars threads always meets variable tid % nvars, so
+// the running maximum lives in a register; one shared and one global atomicMax per variable per block.
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS) bounds_kernel(ExpView ev, int64_t nterms, int nvars, uint32_t* gmax)
+{
+    __shared__ uint32_t smax[kMaxVars];
+    const int tid = threadIdx.x;
+    if (tid < nvars) smax[tid] = 0u;
+    __syncthreads();
+    const int rows_per_iter = THREADS / nvars;
+    if (tid < rows_per_iter * nvars) {
+        const int v = tid % nvars, r = tid / nvars;
+        const int64_t step = (int64_t)gridDim.x * rows_per_iter;
+        uint32_t m = 0u;
+        const int64_t voff = (int64_t)v * ev.var_stride;
+#pragma unroll 8
+        for (int64_t t = (int64_t)blockIdx.x * rows_per_iter + r; t < nterms; t += step)
+            m = max(m, load_exp(ev.base, ev.exp_bytes, t * ev.term_stride + voff));
+        if (m) atomicMax(&smax[v], m);
+    }
+    __syncthreads();
+    if (tid < nvars && smax[tid]) atomicMax(&gmax[tid], smax[tid]);
+}
+
+int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream)
+{
+    if (nterms <= 0) return 0;
+    constexpr int T = 256;
+    const int rows_per_iter = T / nvars;
+    int64_t blocks = (nterms + (int64_t)rows_per_iter * 16 - 1) / ((int64_t)rows_per_iter * 16);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    bounds_kernel<T><<<(unsigned)blocks, T, 0, stream>>>(ev, nterms, nvars, ctl->max_exp[which]);
+    return 1;
+}
+
+// ----------------------------------------------------------------------------------------------- S1
+
+// digit-0 histogram of a block: shared atomics, flushed with one global reduction per non-empty bin
+struct BlockHist {
+    uint32_t* sh;
+    __device__ void init(uint32_t* s) { sh = s; for (int b = threadIdx.x; b < kRadix; b += blockDim.x) sh[b] = 0u; }
+    __device__ void add(uint32_t d) { atomicAdd(&sh[d], 1u); }
+    __device__ void flush(uint32_t* g)
+    {
+        for (int b = threadIdx.x; b < kRadix; b += blockDim.x)
+            if (sh[b]) atomicAdd(&g[b], sh[b]);
+    }
+};
+
+template <typename K>
+__device__ __forceinline__ void pack_field(K& key, uint32_t e, int v, const Plan& plan, bool& bad)
+{
+    bad |= e > plan.bound[v];
+    key_or_field(key, e, plan.shift[v]);     // width 0 => bound 0 => e must be 0: nothing is OR-ed
+}
+
+// Rows contiguous in memory (row-major, 16-byte aligned base): each thread reads its row with the widest
+// word WB (bytes) that divides the row size; ES = bytes per exponent.
+template <typename K, int ES, int WB>
+__global__ void __launch_bounds__(256) pack_rows_kernel(const uint8_t* __restrict__ base, int64_t nterms,
+                                                        const __grid_constant__ Plan plan, K* __restrict__ keys,
+                                                        Control* ctl, int hist0)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    if (hist0) { bh.init(sh); __syncthreads(); }
+    const int rb = plan.nvars * ES;
+    const int dpos = plan.digit_pos[0];
+    const uint32_t dmask = (1u << plan.digit_bits[0]) - 1u;
+    bool bad = false;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nterms; t += (int64_t)gridDim.x * blockDim.x) {
+        const uint8_t* row = base + t * rb;
+        K key;
+        key_zero(key);
+        for (int c = 0; c < rb; c += WB) {
+            uint32_t w[WB >= 4 ? WB / 4 : 1];
+            if (WB == 16) {
+                const uint4 q = __ldg((const uint4*)(row + c));
+                w[0] = q.x; w[WB >= 16 ? 1 : 0] = q.y; w[WB >= 16 ? 2 : 0] = q.z; w[WB >= 16 ? 3 : 0] = q.w;
+            } else if (WB == 4) w[0] = __ldg((const uint32_t*)(row + c));
+            else if (WB == 2) w[0] = __ldg((const uint16_t*)(row + c));
+            else w[0] = __ldg(row + c);
+            const int v0 = c / ES;
+#pragma unroll
+            for (int k = 0; k < WB / ES; ++k) {
+                uint32_t e;
+                if (ES == 4) e = w[k];
+                else if (ES == 2) e = (w[k / 2] >> (16 * (k % 2))) & 0xffffu;
+                else e = (w[k / 4] >> (8 * (k % 4))) & 0xffu;
+                pack_field(key, e, v0 + k, plan, bad);
+            }
+        }
+        keys[t] = key;
+        if (hist0) bh.add(key_digit(key, dpos, dmask));
+    }
+    if (bad) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+    if (hist0) { __syncthreads(); bh.flush(ctl->hist[0]); }
+}
+
+// Any strides / alignment: one element load per variable.
+template <typename K>
+__global__ void __launch_bounds__(256) pack_strided_kernel(ExpView ev, int64_t nterms, const __grid_constant__ Plan plan,
+                                                           K* __restrict__ keys, Control* ctl, int hist0)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    if (hist0) { bh.init(sh); __syncthreads(); }
+    const int dpos = plan.digit_pos[0];
+    const uint32_t dmask = (1u << plan.digit_bits[0]) - 1u;
+    bool bad = false;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nterms; t += (int64_t)gridDim.x * blockDim.x) {
+        K key;
+        key_zero(key);
+        for (int v = 0; v < plan.nvars; ++v)
+            pack_field(key, load_exp(ev.base, ev.exp_bytes, t * ev.term_stride + (int64_t)v * ev.var_stride), v, plan, bad);
+        keys[t] = key;
+        if (hist0) bh.add(key_digit(key, dpos, dmask));
+    }
+    if (bad) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+    if (hist0) { __syncthreads(); bh.flush(ctl->hist[0]); }
+}
+
+template <typename K, int ES>
+static void launch_pack_rows_es(int wb, unsigned blocks, const ExpView& ev, int64_t nterms, const Plan& plan, K* keys,
+                                Control* ctl, int hist0, cudaStream_t stream)
+{
+    const uint8_t* base = (const uint8_t*)ev.base;
+    if (wb == 16) pack_rows_kernel<K, ES, 16><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
+    else if (wb == 4) pack_rows_kernel<K, ES, 4><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
+    else if (ES <= 2 && wb == 2) pack_rows_kernel<K, ES, (ES <= 2 ? 2 : 4)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
+    else pack_rows_kernel<K, ES, (ES == 1 ? 1 : ES)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
+}
+
+template <typename K>
+static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K* keys, Control* ctl, bool hist0,
+                         cudaStream_t stream)
+{
+    if (nterms <= 0) return 0;
+    int64_t blocks = (nterms + 256 * 4 - 1) / (256 * 4);       // >= 4 rows per thread once the grid saturates
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    if (blocks < 1) blocks = 1;
+    if (ev.row_major_contiguous) {
+        const int rb = plan.nvars * ev.exp_bytes;
+        const int wb = (rb % 16 == 0) ? 16 : (rb % 4 == 0) ? 4 : (rb % 2 == 0) ? 2 : 1;
+        if (ev.exp_bytes == 1) launch_pack_rows_es<K, 1>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
+        else if (ev.exp_bytes == 2) launch_pack_rows_es<K, 2>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
+        else launch_pack_rows_es<K, 4>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
+    } else {
+        pack_strided_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(ev, nterms, plan, keys, ctl, hist0 ? 1 : 0);
+    }
+    return 1;
+}
+
+int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, bool hist0,
+                cudaStream_t stream)
+{
+    if (plan.key_bytes == 8) return launch_pack_t<uint64_t>(ev, nterms, plan, (uint64_t*)keys, ctl, hist0, stream);
+    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)keys, ctl, hist0, stream);
+}
+
+int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
+                     cudaStream_t stream)
+{
+    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)out_hilo, ctl, false, stream);   // Key128 is (hi, lo)
+}
+
+// ----------------------------------------------------------------------------------------------- X1
+
+template <typename K>
+__global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict__ ka, const double* __restrict__ ca,
+                                                            uint32_t na, const K* __restrict__ kb,
+                                                            const double* __restrict__ cb, uint32_t nb,
+                                                            K* __restrict__ keys, double* __restrict__ coefs, int dpos,
+                                                            uint32_t dmask, Control* ctl)
+{
+    constexpr int ITEMS = 4;
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    bh.init(sh);
+    __syncthreads();
+    const uint32_t n = na * nb;                                   // < 2^30, checked on the host
+    const uint32_t q0 = blockIdx.x * (256u * ITEMS) + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        const uint32_t q = q0 + k * 256u;
+        if (q < n) {
+            const uint32_t i = q / nb, j = q - i * nb;
+            const K key = key_add(ka[i], kb[j]);
+            keys[q] = key;
+            coefs[q] = __dmul_rn(ca[i], cb[j]);                   // one IEEE multiplication, never contracted
+            bh.add(key_digit(key, dpos, dmask));
+        }
+    }
+    __syncthreads();
+    bh.flush(ctl->hist[0]);
+}
+
+int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
+                         const Plan& plan, void* keys, double* coefs, Control* ctl, cudaStream_t stream)
+{
+    const int64_t n = na * nb;
+    if (n <= 0) return 0;
+    const unsigned blocks = (unsigned)((n + 1023) / 1024);
+    const int dpos = plan.npasses ? plan.digit_pos[0] : 0;
+    const uint32_t dmask = plan.npasses ? (1u << plan.digit_bits[0]) - 1u : 0u;
+    if (plan.key_bytes == 8)
+        expand_packed_kernel<uint64_t><<<blocks, 256, 0, stream>>>((const uint64_t*)ka, ca, (uint32_t)na, (const uint64_t*)kb,
+                                                                   cb, (uint32_t)nb, (uint64_t*)keys, coefs, dpos, dmask, ctl);
+    else
+        expand_packed_kernel<Key128><<<blocks, 256, 0, stream>>>((const Key128*)ka, ca, (uint32_t)na, (const Key128*)kb, cb,
+                                                                 (uint32_t)nb, (Key128*)keys, coefs, dpos, dmask, ctl);
+    return 1;
+}
+
+// Raw product in (coef, exps) form, no keys: polylab_expand (reading A10).
+__global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, const double* __restrict__ ca, uint32_t na,
+                                                         ExpView eb, const double* __restrict__ cb, uint32_t nb,
+                                                         int nvars, double* __restrict__ out_coef, void* out_exps,
+                                                         int32_t* status)
+{
+    const uint32_t n = na * nb;
+    const uint32_t emax = ea.exp_bytes == 1 ? 0xffu : ea.exp_bytes == 2 ? 0xffffu : 0xffffffffu;
+    bool bad = false;
+    for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += gridDim.x * blockDim.x) {
+        const uint32_t i = q / nb, j = q - i * nb;
+        out_coef[q] = __dmul_rn(ca[i], cb[j]);
+        for (int v = 0; v < nvars; ++v) {
+            const uint32_t x = load_exp(ea.base, ea.exp_bytes, (int64_t)i * ea.term_stride + (int64_t)v * ea.var_stride);
+            const uint32_t y = load_exp(eb.base, eb.exp_bytes, (int64_t)j * eb.term_stride + (int64_t)v * eb.var_stride);
+            const uint32_t s = x + y;
+            bad |= (s < x) || (s > emax);
+            store_exp(out_exps, ea.exp_bytes, (int64_t)q * nvars + v, s);
+        }
+    }
+    if (bad) atomicMax(status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+}
+
+int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const ExpView& eb, const double* cb, int64_t nb,
+                      int nvars, double* out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream)
+{
+    const int64_t n = na * nb;
+    if (n <= 0) return 0;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    expand_raw_kernel<<<(unsigned)blocks, 256, 0, stream>>>(ea, ca, (uint32_t)na, eb, cb, (uint32_t)nb, nvars, out_coef,
+                                                            out_exps, &ctl_status->status);
+    return 1;
+}
+
+}  // namespace polylab
