@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the simplify hot path on synthetic polynomials (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--nterms N] [--impl reference]
+
+One "step" is one pass of the whole hot path (bounds -> pack -> radix sort -> segmented sum -> prune ->
+unpack; plus the term-product expansion for the mul configs) over one synthetic input.  Default workload:
+BASELINE.json config 5 (2e8 terms, 16 variables, 128-bit keys), the largest config and the one the
+north_star's roofline target is quoted on.  Prints ONE JSON line (rank 0).
+
+  value     input terms/s, whole job, inputs resident in HBM, CUDA events around K calls of the C ABI
+  e2e       the same metric through polylab_simplify_host: pinned host buffers, H2D and D2H inside the call
+  roofline  the radix-sort pass kernel (dominant): algorithmic bytes 2*N*(W+8) per launch / mean launch time,
+            timed live with the library's CUDA events on the call's stream (POLYLAB_FLAG_TIMING)
+  cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same recipe (rank 0, N=1 only)
+
+--impl reference times the oracle alone (there is no reference implementation to install: the paper's
+code is unpublished).  Multi-GPU (--gpus N under torchrun): the path does not
+need a collective -- each rank simplifies its own polynomial of the same shape (weak scaling, replicas).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "simplified input terms/sec (fp64)"
+UNIT = "terms/s"
+NOMINAL_HBM_GBS = 8000.0          # the north_star's "~8 TB/s"; the roofline peak is the measured copy bandwidth
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def workload(config: int, nterms, seed_offset: int = 0):
+    """(kind, polys, tol, description, n_sort_terms) for BASELINE.json config `config`."""
+    from paper_2604_06575_b200 import workloads as W
+    if config == 1:
+        p, tol = W.config1(nterms or 100_000, seed_offset)
+        return "simplify", (p,), tol, f"config1: simplify {p.nterms} terms, nvars=4, exps U{{0..3}}, coef U[-1,1], tol=0", p.nterms
+    if config == 2:
+        a, b, tol = W.config2(nterms or 2000, seed_offset)
+        return "mul", (a, b), tol, f"config2: mul+simplify {a.nterms}x{b.nterms} terms, nvars=6, exps U{{0..3}}, coef N(0,1)", a.nterms * b.nterms
+    if config == 3:
+        p, tol = W.config3(nterms or 10_000_000, seed_offset)
+        return "simplify", (p,), tol, f"config3: simplify {p.nterms} terms, nvars=10, 3 nonzero vars with exps U{{1..4}}, coef N(0,1)", p.nterms
+    if config == 4:
+        p, tol = W.config4(seed_offset=seed_offset)
+        return "cubic", (p,), tol, "config4: p*p*p, p 200 terms over 20 vars (variant B: 4e4 + 8e6 product terms)", 40_000 + 8_000_000
+    if config == 5:
+        p, tol = W.config5(nterms or 200_000_000, seed_offset)
+        return "simplify", (p,), tol, (f"config5: simplify {p.nterms} terms, nvars=16, exps U{{0..255}} (128-bit keys), pool of "
+                                       f"{p.nterms // 10} monomials x10, half cancelling, tol=1e-14"), p.nterms
+    raise SystemExit(f"unknown config {config}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, r[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(kind, polys, tol):
+    from oracle import oracle
+    t0 = time.perf_counter()
+    if kind == "simplify":
+        oracle.simplify(polys[0].coef, polys[0].exps, tol)
+    elif kind == "mul":
+        oracle.mul_simplify(polys[0].coef, polys[0].exps, polys[1].coef, polys[1].exps, tol)
+    else:
+        p = polys[0]
+        c, e = oracle.mul_simplify(p.coef, p.exps, p.coef, p.exps, tol).pruned
+        oracle.mul_simplify(c, e, p.coef, p.exps.astype(np.uint32), tol)
+    return time.perf_counter() - t0
+
+
+def oracle_sample(config: int, budget_s: float):
+    """A bounded sample of the workload for the CPU oracle: same recipe, fewer terms (about budget_s of CPU work)."""
+    if config in (1, 2, 4):
+        return workload(config, None)                   # the oracle finishes these in seconds
+    probe_n = 1_000_000
+    kind, polys, tol, _, n = workload(config, probe_n)
+    rate = n / time_oracle(kind, polys, tol)
+    full = 10_000_000 if config == 3 else 200_000_000
+    n_s = int(min(full, max(probe_n, rate * budget_s)) // 20 * 20)
+    return workload(config, n_s)
+
+
+def run_reference(args):
+    """The oracle as the reference arm (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle
+    oracle.build()
+    total = max(args.steps + args.warmup, 1)
+    kind, polys, tol, desc, n = oracle_sample(args.config, budget_s=min(20.0, 150.0 / total))
+    for _ in range(args.warmup):
+        time_oracle(kind, polys, tol)
+    t = [time_oracle(kind, polys, tol) for _ in range(args.steps)]
+    sec = sum(t) / len(t)
+    v = n / sec
+    sample = f"{desc} (bounded sample of the bench workload, same recipe)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--nterms", type=int, default=None, help="override the config's term count (debugging)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2604_06575_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    B.lib()                                             # fail loudly if libpolylab.so is missing
+    steps, warmup = max(args.steps, 1), max(args.warmup, 3)
+
+    kind, polys, tol, desc, n_sort = workload(args.config, args.nterms, seed_offset=rank)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dpolys = [(dev(p.coef), dev(p.exps)) for p in polys]
+    ws = B.Workspace(torch.device("cuda", local_rank))
+    stats_log = []
+
+    def step_device():
+        if kind == "simplify":
+            c, e, st = B.simplify(*dpolys[0], tol, workspace=ws, out=outbuf, return_stats=True, timing=True)
+            stats_log.append(st)
+            return c.shape[0]
+        if kind == "mul":
+            c, e, st = B.mul_simplify(*dpolys[0], *dpolys[1], tol, workspace=ws, return_stats=True, timing=True)
+            stats_log.append(st)
+            return c.shape[0]
+        pc, pe = dpolys[0]
+        rc, re_ = B.expand(pc, pe, pc, pe)
+        c, e, st = B.mul_simplify(rc, re_, pc, pe, tol, workspace=ws, return_stats=True, timing=True)
+        stats_log.append(st)
+        return c.shape[0]
+
+    outbuf = None
+    if kind == "simplify":
+        n0, nv = dpolys[0][1].shape
+        outbuf = (torch.empty(n0, dtype=torch.float64, device="cuda"), torch.empty((n0, nv), dtype=dpolys[0][1].dtype, device="cuda"))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        n_out = step_device()
+    stats_log.clear()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(steps):
+        n_out = step_device()
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / steps
+    value = n_sort * world / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel: one radix pass moves 2*N*(W+8) algorithmic bytes
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured copy bandwidth (MEASURED_PEAKS.json)"
+    else:
+        peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    st = stats_log[-1]
+    P, Wb = st.sort_passes, st.key_bytes
+    sort_ms = statistics.mean(s.stage_ms["sort"] for s in stats_log)
+    pass_ms = sort_ms / P if P else float("nan")
+    pass_bytes = 2.0 * st.sort_terms * (Wb + 8)
+    achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if P else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"config{args.config}", {}).get("sort_pass_dram_bytes_per_launch")
+    stage_ms = {k: statistics.mean(s.stage_ms[k] for s in stats_log) for k in B.STAGES}
+    sr_ms = stage_ms["sort"] + stage_ms["reduce"]
+    sr_bytes = P * pass_bytes + st.sort_terms * (Wb + 8) + st.distinct * (Wb + 8)
+    roofline = {"bound": "hbm", "kernel": "sort_pass_kernel (one LSD radix pass, 8-bit digit)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": pass_bytes, "launch_ms": pass_ms, "launches_per_step": P,
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "sort_plus_reduce": {"ms": sr_ms, "algorithmic_bytes": sr_bytes, "GBps": sr_bytes / (sr_ms * 1e-3) / 1e9,
+                                     "frac": sr_bytes / (sr_ms * 1e-3) / 1e9 / peak},
+                "stage_ms": stage_ms}
+
+    # ---- end to end: host buffers, copies inside the C call
+    e2e = None
+    if not args.no_e2e and kind in ("simplify", "mul"):
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hp = [(pin(p.coef), pin(p.exps)) for p in polys]
+        h2d = sum(c.numel() * 8 + e.numel() * e.element_size() for c, e in hp)
+        if kind == "simplify":
+            n0, nv = hp[0][1].shape
+            hout = (torch.empty(n0, dtype=torch.float64).pin_memory(), torch.empty((n0, nv), dtype=hp[0][1].dtype).pin_memory())
+            call = lambda: B.simplify_host(hp[0][0], hp[0][1], tol, out=hout, workspace=ws, device=torch.device("cuda", local_rank))
+        else:
+            call = lambda: B.mul_simplify_host(hp[0][0], hp[0][1], hp[1][0], hp[1][1], tol, workspace=ws,
+                                               device=torch.device("cuda", local_rank))
+        c, e = call()[:2]                               # warm-up (also sizes the workspace)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k2 = max(1, min(steps, 5))
+        e0.record()
+        for _ in range(k2):
+            c, e = call()[:2]
+        e1.record()
+        barrier()
+        ms2 = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms2], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms2 = float(t.item())
+        esize = e.element_size() if isinstance(e, torch.Tensor) else e.dtype.itemsize
+        d2h = int(c.shape[0]) * (8 + int(e.shape[1]) * esize)
+        e2e = {"value": n_sort * world / (ms2 / k2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h) + 8, "steps": k2, "ms_per_step": ms2 / k2}
+        del hp
+
+    # ---- CPU oracle on a bounded sample (rank 0, N=1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        k_s, p_s, tol_s, desc_s, n_s = oracle_sample(args.config, budget_s=15.0)
+        sec = time_oracle(k_s, p_s, tol_s)
+        cpu = {"value": n_s / sec, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": sec,
+               "sample": f"{desc_s} (bounded sample, same recipe as the bench workload)",
+               "host_cpus": os.cpu_count()}
+
+    if rank == 0:
+        launches = sum(s.kernel_launches for s in stats_log) + (steps if kind == "cubic" else 0)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": desc, "sort_terms_per_step": n_sort, "distinct": st.distinct, "survivors": int(n_out),
+                       "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "digit_bits": st.digit_bits,
+                       "parallelism": f"replicas x{world} (no collective on the path)",
+                       "l2": "inputs and workspace are far larger than the 126 MB L2" if n_sort * (Wb + 8) > 4e8 else
+                             "working set fits L2 (no flush between steps; launch-latency bound)"},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        }))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

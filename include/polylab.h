@@ -63,10 +63,16 @@ typedef enum {
 typedef enum { POLYLAB_EXP_U8 = 1, POLYLAB_EXP_U16 = 2, POLYLAB_EXP_U32 = 4 } polylab_exp_type;
 
 enum {
-    POLYLAB_FLAG_DEVICE_COUNT = 1u   /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
+    POLYLAB_FLAG_DEVICE_COUNT = 1u,  /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
                                         Requires max_exp_host (no bounds read-back).  Data errors are then
                                         reported only through the device status word, see polylab_opts. */
+    POLYLAB_FLAG_TIMING = 2u         /* record CUDA events between the steps and fill stats->stage_ms
+                                        (needs stats; ignored with POLYLAB_FLAG_DEVICE_COUNT) */
 };
+
+/* indices into polylab_stats.stage_ms */
+enum { POLYLAB_STAGE_BOUNDS = 0, POLYLAB_STAGE_PACK = 1, POLYLAB_STAGE_SORT = 2, POLYLAB_STAGE_REDUCE = 3,
+       POLYLAB_STAGE_PRUNE = 4, POLYLAB_STAGE_COUNT = 5 };
 
 /* Per-call statistics (HOST, optional): the plan that was chosen and what the pipeline saw. */
 typedef struct polylab_stats {
@@ -79,6 +85,8 @@ typedef struct polylab_stats {
     int64_t survivors;       /* U' (-1 with DEVICE_COUNT)                                */
     int32_t kernel_launches; /* kernels of this library launched by the call             */
     int32_t reserved;
+    float stage_ms[8];       /* with POLYLAB_FLAG_TIMING: device time of S0 (incl. read-back), S1 (+X1),
+                                S2 (all passes), S3, S4+S5; CUDA events on the call's stream  */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

@@ -150,12 +150,42 @@ static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
     st->survivors = -1;
 }
 
+// ------------------------------------------------------------------------------- stage timing
+
+// Optional CUDA events between the steps (POLYLAB_FLAG_TIMING): recorded on the call's stream, read after
+// the call's final synchronisation.  Events are created once per host thread.
+struct Timing {
+    bool on = false;
+    cudaStream_t stream = nullptr;
+    cudaEvent_t ev[POLYLAB_STAGE_COUNT + 1];
+    void begin(bool enable, cudaStream_t s)
+    {
+        static thread_local cudaEvent_t pool[POLYLAB_STAGE_COUNT + 1];
+        static thread_local bool made = false;
+        on = enable;
+        stream = s;
+        if (!on) return;
+        if (!made) {
+            for (auto& e : pool) cudaEventCreate(&e);
+            made = true;
+        }
+        for (int i = 0; i <= POLYLAB_STAGE_COUNT; ++i) ev[i] = pool[i];
+        cudaEventRecord(ev[0], stream);
+    }
+    void mark(int stage) { if (on) cudaEventRecord(ev[stage + 1], stream); }     // end of `stage`
+    void finish(polylab_stats* st)
+    {
+        if (!on || !st) return;
+        for (int i = 0; i < POLYLAB_STAGE_COUNT; ++i) cudaEventElapsedTime(&st->stage_ms[i], ev[i], ev[i + 1]);
+    }
+};
+
 // ----------------------------------------------------------------------- shared tail of both paths
 
 // keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
 static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
-                            int64_t* out_nterms, int* launches, cudaStream_t stream)
+                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream)
 {
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
@@ -166,6 +196,7 @@ static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, cons
         *launches += launch_sort_pass(plan, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1], cbuf[(p + 1) & 1],
                                       (uint32_t*)(ws + L.sort_state), ctl, stream);
     }
+    tm.mark(POLYLAB_STAGE_SORT);
     const void* skeys = kbuf[P & 1];
     const double* scoef = (P == 0) ? coef0 : cbuf[P & 1];
     void* ukeys = kbuf[(P + 1) & 1];
@@ -177,9 +208,11 @@ static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, cons
     sc.tile_frag = (double*)(ws + L.red_frag);
     sc.tile_cont = (uint8_t*)(ws + L.red_cont);
     *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
+    tm.mark(POLYLAB_STAGE_REDUCE);
     const bool dev_count = (o.flags & POLYLAB_FLAG_DEVICE_COUNT) != 0;
     *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
                                      (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+    tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
     if (o.stats) o.stats->kernel_launches = *launches;
     if (dev_count) {
@@ -190,6 +223,7 @@ static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, cons
     struct { int32_t status; uint32_t distinct, survivors; } res;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));
+    tm.finish(o.stats);
     if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; }
     if (res.status != POLYLAB_OK) return res.status;
     *out_nterms = (int64_t)res.survivors;
@@ -250,6 +284,8 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
     int launches = 0;
     const ExpView ev = make_view(exps, o, nvars);
     Control* ctl = (Control*)ws;             // Layout::control is offset 0 for every layout
+    Timing tm;
+    tm.begin((o.flags & POLYLAB_FLAG_TIMING) && o.stats && !(o.flags & POLYLAB_FLAG_DEVICE_COUNT), stream);
 
     // ---- S0: per-variable maxima (from the caller, or from the data with one read-back)
     uint64_t m[kMaxVars];
@@ -264,6 +300,7 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
         PL_CUDA(cudaStreamSynchronize(stream));
         for (int v = 0; v < nvars; ++v) { m[v] = mh[v]; bound[v] = mh[v]; }
     }
+    tm.mark(POLYLAB_STAGE_BOUNDS);
     Plan plan;
     rc = make_plan(nvars, m, bound, &plan);
     if (rc != POLYLAB_OK) return rc;
@@ -275,7 +312,8 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
 
     // ---- S1 (+ histogram of the first digit), then the shared tail
     launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0, stream);
-    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, stream);
+    tm.mark(POLYLAB_STAGE_PACK);
+    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream);
 }
 
 int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
@@ -301,10 +339,10 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
     const size_t avail = workspace_bytes >= (size_t)(ws - (unsigned char*)workspace) ? workspace_bytes - (ws - (unsigned char*)workspace) : 0;
     if (avail < sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     int launches = 0;
-    Opts oa = o, ob = o;
-    if (o.term_stride == nvars && o.var_stride == 1) { /* row-major: same strides for both operands */ }
-    const ExpView eva = make_view(a->exps, oa, nvars), evb = make_view(b->exps, ob, nvars);
+    const ExpView eva = make_view(a->exps, o, nvars), evb = make_view(b->exps, o, nvars);
     Control* ctl = (Control*)ws;
+    Timing tm;
+    tm.begin((o.flags & POLYLAB_FLAG_TIMING) && o.stats && !(o.flags & POLYLAB_FLAG_DEVICE_COUNT), stream);
 
     // ---- S0 on both operands; the sorted rows are sums, so fields are sized for max_a + max_b
     uint64_t m[kMaxVars];
@@ -325,6 +363,7 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
             if (m[v] > emax) return POLYLAB_ERR_EXPONENT_RANGE;       // the sum must fit exp_type (reading A8)
         }
     }
+    tm.mark(POLYLAB_STAGE_BOUNDS);
     Plan plan_a, plan_b;
     rc = make_plan(nvars, m, ba, &plan_a);
     if (rc != POLYLAB_OK) return rc;
@@ -340,8 +379,9 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
     launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, false, stream);
     launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
                                      (double*)(ws + L.coefs[0]), ctl, stream);
+    tm.mark(POLYLAB_STAGE_PACK);
     return sort_reduce_emit(plan_a, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                            out_nterms, &launches, stream);
+                            out_nterms, &launches, tm, stream);
 }
 
 int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts, double* out_coef,

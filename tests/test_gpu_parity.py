@@ -173,7 +173,7 @@ def test_config4_cubic_both_variants():
     rc, re_ = B.expand(dev(p.coef), dev(p.exps), dev(p.coef), dev(p.exps))
     assert rc.shape[0] == 40_000
     cb, eb, st = B.mul_simplify(rc, re_, dev(p.coef), dev(p.exps), tol, return_stats=True)
-    assert st.sort_terms == 8_000_000 and st.key_bits == 60
+    assert st.sort_terms == 8_000_000 and 40 <= st.key_bits <= 60 and st.key_bytes == 8
     cb, eb = cb.cpu().numpy(), eb.cpu().numpy()
     assert eb.tolist() == ea.tolist()
     # A vs B differ only in summation order
