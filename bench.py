@@ -143,7 +143,7 @@ def run_reference(args):
     from oracle import oracle
     oracle.build()
     total = max(args.steps + args.warmup, 1)
-    kind, polys, tol, desc, n = oracle_sample(args.config, budget_s=min(20.0, 150.0 / total))
+    kind, polys, tol, desc, n = oracle_sample(args.config, budget_s=min(8.0, 60.0 / total))
     for _ in range(args.warmup):
         time_oracle(kind, polys, tol)
     t = [time_oracle(kind, polys, tol) for _ in range(args.steps)]
@@ -305,7 +305,7 @@ def main():
     # ---- CPU oracle on a bounded sample (rank 0, N=1)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        k_s, p_s, tol_s, desc_s, n_s = oracle_sample(args.config, budget_s=15.0)
+        k_s, p_s, tol_s, desc_s, n_s = oracle_sample(args.config, budget_s=8.0)   # the probe overestimates the rate
         sec = time_oracle(k_s, p_s, tol_s)
         cpu = {"value": n_s / sec, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": sec,
                "sample": f"{desc_s} (bounded sample, same recipe as the bench workload)",
