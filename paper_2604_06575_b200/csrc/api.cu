@@ -87,15 +87,22 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
     }
     plan->key_bits = bits;
     plan->key_bytes = bits <= 64 ? 8 : 16;
-    const int P = (bits + kRadixBits - 1) / kRadixBits;
-    plan->npasses = P;
-    int pos = 0;
-    for (int p = 0; p < P; ++p) {            // balanced digit widths: B = sum of P digits of floor/ceil(B/P) bits
-        const int w = bits / P + (p < bits % P ? 1 : 0);
-        plan->digit_pos[p] = (uint8_t)pos;
-        plan->digit_bits[p] = (uint8_t)w;
-        pos += w;
+    // Digits: each 32-bit word of the key is split into ceil(bits_in_word / 8) digits of balanced width, so no digit
+    // straddles a word (one shift + mask per digit) and the pass count is still ceil(B / 8).
+    int P = 0;
+    for (int w = 0; w * 32 < bits; ++w) {
+        const int nb = bits - w * 32 < 32 ? bits - w * 32 : 32;
+        const int pw = (nb + kRadixBits - 1) / kRadixBits;
+        int pos = w * 32;
+        for (int p = 0; p < pw; ++p) {
+            const int dw = nb / pw + (p < nb % pw ? 1 : 0);
+            plan->digit_pos[P] = (uint8_t)pos;
+            plan->digit_bits[P] = (uint8_t)dw;
+            pos += dw;
+            ++P;
+        }
     }
+    plan->npasses = P;
     return POLYLAB_OK;
 }
 

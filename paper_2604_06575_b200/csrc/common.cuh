@@ -30,16 +30,22 @@ struct __align__(16) Key128 {
 __host__ __device__ inline bool key_eq(uint64_t a, uint64_t b) { return a == b; }
 __host__ __device__ inline bool key_eq(const Key128& a, const Key128& b) { return a.lo == b.lo && a.hi == b.hi; }
 
-// `bits` (<= 8) bits of the key starting at bit `pos` (0 = least significant)
-__device__ __forceinline__ uint32_t key_digit(uint64_t k, int pos, uint32_t mask) { return (uint32_t)(k >> pos) & mask; }
-__device__ __forceinline__ uint32_t key_digit(const Key128& k, int pos, uint32_t mask)
+// 32-bit word `wi` of a key (0 = least significant).  wi is uniform across a kernel: the selects cost 1-3 instructions.
+__device__ __forceinline__ uint32_t key_word(uint64_t k, int wi) { return wi ? (uint32_t)(k >> 32) : (uint32_t)k; }
+__device__ __forceinline__ uint32_t key_word(const Key128& k, int wi)
 {
-    uint64_t w;
-    if (pos >= 64) w = k.hi >> (pos - 64);
-    else if (pos == 0) w = k.lo;
-    else w = (k.lo >> pos) | (k.hi << (64 - pos));
-    return (uint32_t)w & mask;
+    const uint64_t h = (wi & 2) ? k.hi : k.lo;
+    return (wi & 1) ? (uint32_t)(h >> 32) : (uint32_t)h;
 }
+// byte offset of word `wi` inside the key as stored in memory (Key128 is stored (hi, lo))
+template <typename K> __host__ __device__ inline int key_word_byte_offset(int wi);
+template <> __host__ __device__ inline int key_word_byte_offset<uint64_t>(int wi) { return wi * 4; }
+template <> __host__ __device__ inline int key_word_byte_offset<Key128>(int wi) { return (wi ^ 2) * 4; }
+
+// The digit of `mask`'s width at bit `pos` (0 = least significant).  The plan never lets a digit straddle a
+// 32-bit word (make_plan), so a digit is one shift and one mask of one word.
+template <typename K>
+__device__ __forceinline__ uint32_t key_digit(const K& k, int pos, uint32_t mask) { return (key_word(k, pos >> 5) >> (pos & 31)) & mask; }
 
 __device__ __forceinline__ uint64_t key_add(uint64_t a, uint64_t b) { return a + b; }
 __device__ __forceinline__ Key128 key_add(const Key128& a, const Key128& b)

@@ -35,10 +35,75 @@ __global__ void __launch_bounds__(THREADS) bounds_kernel(ExpView ev, int64_t nte
     if (tid < nvars && smax[tid]) atomicMax(&gmax[tid], smax[tid]);
 }
 
+// Contiguous row-major rows (16-byte aligned base): the matrix is read as a stream of 16-byte words.  The grid's
+// sweep (gridDim * THREADS * 16 bytes) is a multiple of the row size, so byte lane i of a thread's word always
+// holds the same variable and the running maximum is a lane-wise SIMD max (4 x u8 / 2 x u16 / 1 x u32 per
+// 32-bit register).  One shared atomicMax per lane per thread at the end, one global per variable per block.
+template <int THREADS, int ES>
+__global__ void __launch_bounds__(THREADS) bounds_stream_kernel(const uint4* __restrict__ base, int64_t nbytes, int nvars,
+                                                                uint32_t* gmax)
+{
+    __shared__ uint32_t smax[kMaxVars];
+    const int tid = threadIdx.x;
+    if (tid < nvars) smax[tid] = 0u;
+    __syncthreads();
+    const int64_t nwords = nbytes >> 4;                       // full 16-byte words; the tail is handled below
+    const int64_t stride = (int64_t)gridDim.x * THREADS;
+    const int64_t w0 = (int64_t)blockIdx.x * THREADS + tid;
+    uint32_t m[4] = {0u, 0u, 0u, 0u};
+    auto acc = [&](const uint4& q) {
+        if (ES == 1) { m[0] = __vmaxu4(m[0], q.x); m[1] = __vmaxu4(m[1], q.y); m[2] = __vmaxu4(m[2], q.z); m[3] = __vmaxu4(m[3], q.w); }
+        else if (ES == 2) { m[0] = __vmaxu2(m[0], q.x); m[1] = __vmaxu2(m[1], q.y); m[2] = __vmaxu2(m[2], q.z); m[3] = __vmaxu2(m[3], q.w); }
+        else { m[0] = max(m[0], q.x); m[1] = max(m[1], q.y); m[2] = max(m[2], q.z); m[3] = max(m[3], q.w); }
+    };
+    int64_t w = w0;
+    for (; w + 3 * stride < nwords; w += 4 * stride) {        // four independent 16-byte loads in flight
+        const uint4 q0 = __ldg(base + w), q1 = __ldg(base + w + stride), q2 = __ldg(base + w + 2 * stride),
+                    q3 = __ldg(base + w + 3 * stride);
+        acc(q0); acc(q1); acc(q2); acc(q3);
+    }
+    for (; w < nwords; w += stride) acc(__ldg(base + w));
+    // lane i of this thread's words is element (w0 * 16 / ES + i) of the stream, i.e. variable (that) % nvars
+    const int64_t e0 = w0 * (16 / ES);
+#pragma unroll
+    for (int i = 0; i < 16 / ES; ++i) {
+        uint32_t x;
+        if (ES == 1) x = (m[i / 4] >> (8 * (i % 4))) & 0xffu;
+        else if (ES == 2) x = (m[i / 2] >> (16 * (i % 2))) & 0xffffu;
+        else x = m[i];
+        if (x) atomicMax(&smax[(int)((e0 + i) % nvars)], x);
+    }
+    // tail: the last nbytes % 16 bytes, element by element
+    if (blockIdx.x == 0) {
+        const int64_t ne = nbytes / ES;
+        for (int64_t e = nwords * (16 / ES) + tid; e < ne; e += THREADS) {
+            const uint32_t x = load_exp(base, ES, e);
+            if (x) atomicMax(&smax[(int)(e % nvars)], x);
+        }
+    }
+    __syncthreads();
+    if (tid < nvars && smax[tid]) atomicMax(&gmax[tid], smax[tid]);
+}
+
 int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream)
 {
     if (nterms <= 0) return 0;
     constexpr int T = 256;
+    if (ev.row_major_contiguous) {
+        // grid = k * (row bytes): the sweep of gridDim * T * 16 bytes is then a whole number of rows
+        const int rb = nvars * ev.exp_bytes;
+        const int64_t nbytes = nterms * rb;
+        int64_t k = (nbytes / 16 + (int64_t)T * 8 - 1) / ((int64_t)T * 8) / rb;      // ~8 words per thread
+        const int64_t kmax = (148 * 16 + rb - 1) / rb;
+        if (k > kmax) k = kmax;
+        if (k < 1) k = 1;
+        const unsigned blocks = (unsigned)(k * rb);
+        const uint4* base = (const uint4*)ev.base;
+        if (ev.exp_bytes == 1) bounds_stream_kernel<T, 1><<<blocks, T, 0, stream>>>(base, nbytes, nvars, ctl->max_exp[which]);
+        else if (ev.exp_bytes == 2) bounds_stream_kernel<T, 2><<<blocks, T, 0, stream>>>(base, nbytes, nvars, ctl->max_exp[which]);
+        else bounds_stream_kernel<T, 4><<<blocks, T, 0, stream>>>(base, nbytes, nvars, ctl->max_exp[which]);
+        return 1;
+    }
     const int rows_per_iter = T / nvars;
     int64_t blocks = (nterms + (int64_t)rows_per_iter * 16 - 1) / ((int64_t)rows_per_iter * 16);
     if (blocks > 148 * 16) blocks = 148 * 16;

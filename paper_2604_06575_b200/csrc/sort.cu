@@ -6,6 +6,11 @@
 // then scatters keys and coefficients through shared memory so that global stores are contiguous per bin.
 // The histogram of the NEXT pass's digit is accumulated on the way (keys are in registers anyway), so no
 // pass ever re-reads the keys just to count.  Coefficients are opaque 64-bit payloads here.
+//
+// The kernel is issue-bound before it is DRAM-bound (profiles/r1a_baseline.md), so the body is written for
+// few instructions per record: digits never straddle a 32-bit key word (one select, one shift, one mask),
+// full tiles run a copy of the body without bounds checks, and the second warp match (for the next digit's
+// histogram) is compiled out of passes that do not need it.
 #include "kernels.h"
 
 namespace polylab {
@@ -15,35 +20,59 @@ struct SortSmem {
     static constexpr int TILE = THREADS * ITEMS;
     static constexpr int NW = THREADS / 32;
     static constexpr size_t stage_bytes = (size_t)TILE * sizeof(K);
-    static constexpr size_t bytes = stage_bytes + (size_t)(2 * NW * kRadix + 2 * kRadix + NW + 4) * sizeof(uint32_t);
+    // per-warp histograms of this digit, the block's histogram of the next digit, bin starts, deltas, scan scratch
+    static constexpr size_t bytes() { return stage_bytes + (size_t)(NW * kRadix + 3 * kRadix + NW + 4) * sizeof(uint32_t); }
 };
 
-template <typename K, int THREADS, int ITEMS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
-sort_pass_kernel(const K* __restrict__ keys_in, const double* __restrict__ coef_in, K* __restrict__ keys_out,
-                 double* __restrict__ coef_out, uint32_t n, int dpos, uint32_t dmask, int npos, uint32_t nmask,
-                 int has_next, uint32_t* tile_state, uint32_t flag_partial, uint32_t flag_inclusive,
-                 const uint32_t* __restrict__ hist_this, uint32_t* hist_next, uint32_t* ticket)
+struct PassArgs {
+    const void* keys_in;
+    const double* coef_in;
+    void* keys_out;
+    double* coef_out;
+    uint32_t n;
+    int dword, dshift;          // this pass's digit: 32-bit word of the key, shift inside it
+    uint32_t dmask;
+    int nword, nshift;          // the next pass's digit (kernels with NEXT)
+    uint32_t nmask;
+    uint32_t* tile_state;
+    uint32_t flag_partial, flag_inclusive;
+    const uint32_t* hist_this;
+    uint32_t* hist_next;
+    uint32_t* ticket;
+};
+
+// lanes of the warp holding the same digit d (< 256) as the calling lane; all 32 lanes participate
+__device__ __forceinline__ unsigned match_digit_all(uint32_t d)
 {
-    static_assert(THREADS == kRadix, "one thread per bin");
+    unsigned mask = kFullMask;
+#pragma unroll
+    for (int b = 0; b < kRadixBits; ++b) {
+        const unsigned x = 0u - ((d >> b) & 1u);            // all ones iff bit b of d is set
+        const unsigned m = __ballot_sync(kFullMask, x != 0u);
+        mask &= ~(m ^ x);                                   // keep the lanes whose bit b equals ours
+    }
+    return mask;
+}
+
+template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL>
+__device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char* smem_raw, uint32_t tile, uint32_t tile_base,
+                                               uint32_t tile_n)
+{
     using S = SortSmem<K, THREADS, ITEMS>;
-    constexpr int TILE = S::TILE, NW = S::NW;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = S::NW;
     K* stage = (K*)smem_raw;
     double* stage_c = (double*)smem_raw;
     uint32_t* whist = (uint32_t*)(smem_raw + S::stage_bytes);      // [NW][256] this pass's digit, per warp
-    uint32_t* whist2 = whist + NW * kRadix;                        // [NW][256] next pass's digit, per warp
-    uint32_t* sm_bin_start = whist2 + NW * kRadix;                 // [256]
+    uint32_t* bhist2 = whist + NW * kRadix;                        // [256] next pass's digit, whole block (NEXT only)
+    uint32_t* sm_bin_start = bhist2 + kRadix;                      // [256]
     uint32_t* sm_delta = sm_bin_start + kRadix;                    // [256]
     uint32_t* scratch = sm_delta + kRadix;                         // [NW + 1], then the tile id
 
+    const K* __restrict__ keys_in = (const K*)a.keys_in;
+    const double* __restrict__ coef_in = a.coef_in;
+    K* __restrict__ keys_out = (K*)a.keys_out;
+    double* __restrict__ coef_out = a.coef_out;
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    if (tid == 0) scratch[NW + 2] = atomicAdd(ticket, 1u);
-    for (int i = tid; i < 2 * NW * kRadix; i += THREADS) whist[i] = 0u;
-    __syncthreads();
-    const uint32_t tile = scratch[NW + 2];
-    const uint32_t tile_base = tile * (uint32_t)TILE;
-    const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
 
     // ---- load keys: warp w owns records [w*32*ITEMS, (w+1)*32*ITEMS) of the tile, item j of lane l is j*32+l
     const uint32_t chunk = warp * 32u * ITEMS + lane;
@@ -51,32 +80,36 @@ sort_pass_kernel(const K* __restrict__ keys_in, const double* __restrict__ coef_
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
-        key[j] = (li < tile_n) ? keys_in[tile_base + li] : key_max<K>();
+        if (FULL || li < tile_n) key[j] = keys_in[tile_base + li];
+        else key[j] = key_max<K>();
     }
+#define POLYLAB_DIGIT(j) ((key_word(key[j], a.dword) >> a.dshift) & a.dmask)
 
     // ---- rank within the warp, in record order (stable)
     uint32_t* my_hist = whist + warp * kRadix;
-    uint32_t* my_hist2 = whist2 + warp * kRadix;
     const unsigned lt = lanemask_lt();
     uint32_t pos[ITEMS];
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
-        const bool valid = (chunk + j * 32u) < tile_n;
-        const uint32_t d = key_digit(key[j], dpos, dmask);
-        const unsigned m = match_digit(d, valid);
-        const uint32_t prev = my_hist[d];
-        uint32_t d2 = 0, prev2 = 0;
-        unsigned m2 = 0;
-        if (has_next) {
-            d2 = key_digit(key[j], npos, nmask);
-            m2 = match_digit(d2, valid);
-            prev2 = my_hist2[d2];
+        const uint32_t dj = POLYLAB_DIGIT(j);
+        unsigned m = match_digit_all(dj);
+        bool valid = true;
+        if (!FULL) {
+            valid = (chunk + j * 32u) < tile_n;
+            m &= __ballot_sync(kFullMask, valid);
         }
+        const uint32_t prev = my_hist[dj];
         __syncwarp();
-        if (valid && (m & lt) == 0u) my_hist[d] = prev + __popc(m);
-        if (has_next && valid && (m2 & lt) == 0u) my_hist2[d2] = prev2 + __popc(m2);
+        if (valid && (m & lt) == 0u) my_hist[dj] = prev + __popc(m);
         __syncwarp();
         pos[j] = prev + __popc(m & lt);
+    }
+    if (NEXT) {
+        // histogram of the next pass's digit: plain shared-memory atomics (no order needed; Blackwell's ATOMS
+        // absorbs same-address lanes, measured 2.7 SM-cycles per warp-op uniform or skewed vs 22 for a warp match)
+#pragma unroll
+        for (int j = 0; j < ITEMS; ++j)
+            if (FULL || (chunk + j * 32u) < tile_n) atomicAdd(&bhist2[(key_word(key[j], a.nword) >> a.nshift) & a.nmask], 1u);
     }
     __syncthreads();
 
@@ -89,34 +122,33 @@ sort_pass_kernel(const K* __restrict__ keys_in, const double* __restrict__ coef_
         whist[w * kRadix + b] = count;
         count += c;
     }
-    uint32_t* my_state = tile_state + (size_t)tile * kRadix + b;
-    st_volatile_u32(my_state, (count << 2) | (tile == 0 ? flag_inclusive : flag_partial));
-    if (has_next) {
-        uint32_t c2 = 0;
-#pragma unroll
-        for (int w = 0; w < NW; ++w) c2 += whist2[w * kRadix + b];
-        if (c2) atomicAdd(&hist_next[b], c2);
+    uint32_t* my_state = a.tile_state + (size_t)tile * kRadix + b;
+    st_volatile_u32(my_state, (count << 2) | (tile == 0 ? a.flag_inclusive : a.flag_partial));
+    if (NEXT) {
+        const uint32_t c2 = bhist2[b];
+        if (c2) atomicAdd(&a.hist_next[b], c2);
     }
     uint32_t total;
     const uint32_t bin_start = block_exclusive_scan<THREADS>(count, scratch, &total);
     sm_bin_start[b] = bin_start;
-    const uint32_t gbase = block_exclusive_scan<THREADS>(hist_this[b], scratch, &total);   // syncs: sm_bin_start visible
+    const uint32_t gbase = block_exclusive_scan<THREADS>(a.hist_this[b], scratch, &total);   // syncs: sm_bin_start visible
 
     // ---- scatter keys into shared memory at their position in the sorted tile
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
-        if ((chunk + j * 32u) < tile_n) {
-            const uint32_t d = key_digit(key[j], dpos, dmask);
-            pos[j] += sm_bin_start[d] + my_hist[d];
+        if (FULL || (chunk + j * 32u) < tile_n) {
+            const uint32_t dj = POLYLAB_DIGIT(j);
+            pos[j] += sm_bin_start[dj] + my_hist[dj];
             stage[pos[j]] = key[j];
         }
     }
+#undef POLYLAB_DIGIT
     // coefficients: issue the loads now, they land while the look-back runs
     double c[ITEMS];
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
-        c[j] = (li < tile_n) ? coef_in[tile_base + li] : 0.0;
+        c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
     }
 
     // ---- decoupled look-back: number of records with digit b in all earlier tiles
@@ -126,35 +158,71 @@ sort_pass_kernel(const K* __restrict__ keys_in, const double* __restrict__ coef_
         while (true) {
             const uint32_t w = ld_volatile_u32(p);
             const uint32_t f = w & 3u;
-            if (f == flag_inclusive) { excl += w >> 2; break; }
-            if (f == flag_partial) { excl += w >> 2; p -= kRadix; }
+            if (f == a.flag_inclusive) { excl += w >> 2; break; }
+            if (f == a.flag_partial) { excl += w >> 2; p -= kRadix; }
         }
-        st_volatile_u32(my_state, ((excl + count) << 2) | flag_inclusive);
+        st_volatile_u32(my_state, ((excl + count) << 2) | a.flag_inclusive);
     }
     sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
     __syncthreads();
 
-    // ---- write keys: slot s of the sorted tile, contiguous per bin
+    // ---- write keys: slot s of the sorted tile, contiguous per bin (only the digit's word is re-read for the bin)
+    const uint32_t* stage_w = (const uint32_t*)(smem_raw + key_word_byte_offset<K>(a.dword));
+    constexpr int KW = sizeof(K) / 4;
     uint32_t dst[ITEMS];
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if (s < tile_n) {
+        if (FULL || s < tile_n) {
             const K kk = stage[s];
-            dst[k] = s + sm_delta[key_digit(kk, dpos, dmask)];
+            dst[k] = s + sm_delta[(stage_w[s * KW] >> a.dshift) & a.dmask];
             keys_out[dst[k]] = kk;
         }
     }
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j)
-        if ((chunk + j * 32u) < tile_n) stage_c[pos[j]] = c[j];
+        if (FULL || (chunk + j * 32u) < tile_n) stage_c[pos[j]] = c[j];
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if (s < tile_n) coef_out[dst[k]] = stage_c[s];
+        if (FULL || s < tile_n) coef_out[dst[k]] = stage_c[s];
     }
+}
+
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT>
+__global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_constant__ PassArgs a)
+{
+    static_assert(THREADS == kRadix, "one thread per bin");
+    using S = SortSmem<K, THREADS, ITEMS>;
+    constexpr int TILE = S::TILE, NW = S::NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* whist = (uint32_t*)(smem_raw + S::stage_bytes);
+    uint32_t* scratch = whist + NW * kRadix + 3 * kRadix;
+
+    const unsigned tid = threadIdx.x;
+    if (tid == 0) scratch[NW + 2] = atomicAdd(a.ticket, 1u);
+    for (int i = tid; i < (NW + 1) * kRadix; i += THREADS) whist[i] = 0u;
+    __syncthreads();
+    const uint32_t tile = scratch[NW + 2];
+    const uint32_t tile_base = tile * (uint32_t)TILE;
+    const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true>(a, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false>(a, smem_raw, tile, tile_base, tile_n);
+}
+
+template <typename K, int ITEMS, int MINB, bool NEXT>
+static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t stream)
+{
+    using S = SortSmem<K, kSortThreads, ITEMS>;
+    auto kern = sort_pass_kernel<K, kSortThreads, ITEMS, MINB, NEXT>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
+        attr_set = true;
+    }
+    kern<<<tiles, kSortThreads, S::bytes(), stream>>>(a);
 }
 
 template <typename K, int ITEMS, int MINB>
@@ -162,21 +230,21 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int64_t n, const void*
                               void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, cudaStream_t stream)
 {
     using S = SortSmem<K, kSortThreads, ITEMS>;
-    auto kern = sort_pass_kernel<K, kSortThreads, ITEMS, MINB>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes);
-        attr_set = true;
-    }
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
-    const int has_next = pass + 1 < plan.npasses;
-    const int npos = has_next ? plan.digit_pos[pass + 1] : 0;
-    const uint32_t nmask = has_next ? (1u << plan.digit_bits[pass + 1]) - 1u : 0u;
-    const uint32_t fp = (pass & 1) ? 3u : 1u, fi = (pass & 1) ? 0u : 2u;     // flag parity: no re-zeroing between passes
-    kern<<<tiles, kSortThreads, S::bytes, stream>>>((const K*)keys_in, coef_in, (K*)keys_out, coef_out, (uint32_t)n,
-                                                    plan.digit_pos[pass], (1u << plan.digit_bits[pass]) - 1u, npos, nmask,
-                                                    has_next, tile_state, fp, fi, ctl->hist[pass], ctl->hist[pass + 1],
-                                                    &ctl->ticket[pass]);
+    const bool has_next = pass + 1 < plan.npasses;
+    PassArgs a;
+    a.keys_in = keys_in; a.coef_in = coef_in; a.keys_out = keys_out; a.coef_out = coef_out;
+    a.n = (uint32_t)n;
+    a.dword = plan.digit_pos[pass] >> 5; a.dshift = plan.digit_pos[pass] & 31; a.dmask = (1u << plan.digit_bits[pass]) - 1u;
+    a.nword = has_next ? plan.digit_pos[pass + 1] >> 5 : 0;
+    a.nshift = has_next ? plan.digit_pos[pass + 1] & 31 : 0;
+    a.nmask = has_next ? (1u << plan.digit_bits[pass + 1]) - 1u : 0u;
+    a.tile_state = tile_state;
+    a.flag_partial = (pass & 1) ? 3u : 1u;                 // flag parity: no re-zeroing between passes
+    a.flag_inclusive = (pass & 1) ? 0u : 2u;
+    a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[pass + 1]; a.ticket = &ctl->ticket[pass];
+    if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true>(a, tiles, stream);
+    else launch_sort_pass_k<K, ITEMS, MINB, false>(a, tiles, stream);
     return 1;
 }
 
