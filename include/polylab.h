@@ -57,7 +57,8 @@ typedef enum {
     POLYLAB_ERR_WORKSPACE_TOO_SMALL = 4,
     POLYLAB_ERR_OUTPUT_TOO_SMALL = 5,   /* survivors > out_capacity: *out_nterms = required size, the first
                                            out_capacity terms are written */
-    POLYLAB_ERR_CUDA = 6                /* a CUDA runtime call failed (see polylab_last_cuda_error) */
+    POLYLAB_ERR_CUDA = 6,               /* a CUDA runtime call failed (see polylab_last_cuda_error) */
+    POLYLAB_ERR_INTERNAL = 7            /* the sorted-order self-check failed even with the ballot-ranking kernel */
 } polylab_status;
 
 typedef enum { POLYLAB_EXP_U8 = 1, POLYLAB_EXP_U16 = 2, POLYLAB_EXP_U32 = 4 } polylab_exp_type;
@@ -66,8 +67,18 @@ enum {
     POLYLAB_FLAG_DEVICE_COUNT = 1u,  /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
                                         Requires max_exp_host (no bounds read-back).  Data errors are then
                                         reported only through the device status word, see polylab_opts. */
-    POLYLAB_FLAG_TIMING = 2u         /* record CUDA events between the steps and fill stats->stage_ms
+    POLYLAB_FLAG_TIMING = 2u,        /* record CUDA events between the steps and fill stats->stage_ms
                                         (needs stats; ignored with POLYLAB_FLAG_DEVICE_COUNT) */
+    POLYLAB_FLAG_SAFE_RANK = 4u,     /* rank records inside a radix pass by warp ballot matching (stable by
+                                        construction) instead of one shared-memory atomic per record.  The
+                                        atomic kernel is stable only because sm_100a returns the old values of
+                                        one warp instruction's same-address atomics in lane order (measured, not
+                                        documented); therefore the default path verifies the sorted order in the
+                                        segmented-sum step and re-runs the call with this flag if the check
+                                        fails (stats->rank_fallback = 1).  Implied by POLYLAB_FLAG_DEVICE_COUNT,
+                                        which cannot read the check back. */
+    POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
+                                        (reversed lane order) so that tests can exercise detection and fallback */
 };
 
 /* indices into polylab_stats.stage_ms */
@@ -83,8 +94,8 @@ typedef struct polylab_stats {
     int64_t sort_terms;      /* N = terms that entered the sort (na*nb for a product)    */
     int64_t distinct;        /* U = distinct monomials before pruning (-1 with DEVICE_COUNT) */
     int64_t survivors;       /* U' (-1 with DEVICE_COUNT)                                */
-    int32_t kernel_launches; /* kernels of this library launched by the call             */
-    int32_t reserved;
+    int32_t kernel_launches; /* kernels of this library launched by the call (both attempts after a fallback) */
+    int32_t rank_fallback;   /* 1 if the sorted-order check failed and the call re-ran with SAFE_RANK */
     float stage_ms[8];       /* with POLYLAB_FLAG_TIMING: device time of S0 (incl. read-back), S1 (+X1),
                                 S2 (all passes), S3, S4+S5; CUDA events on the call's stream  */
 } polylab_stats;

@@ -21,9 +21,12 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpolylab.so")
 
-OK, ERR_INVALID_ARGUMENT, ERR_KEY_TOO_WIDE, ERR_EXPONENT_RANGE, ERR_WORKSPACE_TOO_SMALL, ERR_OUTPUT_TOO_SMALL, ERR_CUDA = range(7)
+(OK, ERR_INVALID_ARGUMENT, ERR_KEY_TOO_WIDE, ERR_EXPONENT_RANGE, ERR_WORKSPACE_TOO_SMALL, ERR_OUTPUT_TOO_SMALL, ERR_CUDA,
+ ERR_INTERNAL) = range(8)
 FLAG_DEVICE_COUNT = 1
 FLAG_TIMING = 2
+FLAG_SAFE_RANK = 4
+FLAG_DEBUG_UNSTABLE = 0x40000000
 STAGES = ("bounds", "pack", "sort", "reduce", "prune")
 MAX_NVARS = 128
 MAX_TERMS = 1 << 30
@@ -39,7 +42,7 @@ class PolylabError(RuntimeError):
 class _Stats(ctypes.Structure):
     _fields_ = [("key_bits", ctypes.c_int32), ("key_bytes", ctypes.c_int32), ("sort_passes", ctypes.c_int32),
                 ("digit_bits", ctypes.c_int32 * 16), ("sort_terms", ctypes.c_int64), ("distinct", ctypes.c_int64),
-                ("survivors", ctypes.c_int64), ("kernel_launches", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("survivors", ctypes.c_int64), ("kernel_launches", ctypes.c_int32), ("rank_fallback", ctypes.c_int32),
                 ("stage_ms", ctypes.c_float * 8)]
 
 
@@ -64,6 +67,7 @@ class Stats:
     survivors: int
     kernel_launches: int
     stage_ms: dict
+    rank_fallback: int = 0
 
 
 _lib = None
@@ -170,7 +174,8 @@ def _make_opts(exp_bytes: int, max_exp, flags: int = 0, strides=None, status_dev
 
 def _stats(st: _Stats) -> Stats:
     return Stats(st.key_bits, st.key_bytes, st.sort_passes, list(st.digit_bits)[:st.sort_passes], st.sort_terms,
-                 st.distinct, st.survivors, st.kernel_launches, {k: float(st.stage_ms[i]) for i, k in enumerate(STAGES)})
+                 st.distinct, st.survivors, st.kernel_launches, {k: float(st.stage_ms[i]) for i, k in enumerate(STAGES)},
+                 rank_fallback=st.rank_fallback)
 
 
 def _dev_poly(coef: torch.Tensor, exps: torch.Tensor, strides=None):
@@ -200,14 +205,15 @@ def mul_simplify_workspace_bytes(na: int, nb: int, nvars: int) -> int:
 
 def simplify(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_exp: Optional[Sequence[int]] = None,
              out_capacity: Optional[int] = None, workspace: Optional[Workspace] = None, stream=None,
-             out: Optional[tuple] = None, return_stats: bool = False, timing: bool = False):
-    """polylab_simplify on device tensors: returns (coef[U'], exps[U', nvars]) views of the output buffers."""
+             out: Optional[tuple] = None, return_stats: bool = False, timing: bool = False, flags: int = 0):
+    """polylab_simplify on device tensors: returns (coef[U'], exps[U', nvars]) views of the output buffers.
+    `flags`: extra POLYLAB_FLAG_* bits (FLAG_SAFE_RANK, FLAG_DEBUG_UNSTABLE)."""
     coef, exps, strides = _dev_poly(coef, exps)
     n, nvars = int(exps.shape[0]), int(exps.shape[1])
     eb = _EXP_TYPE[exps.dtype]
     cap = n if out_capacity is None else int(out_capacity)
     keep = []
-    o, st = _make_opts(eb, max_exp, flags=FLAG_TIMING if timing else 0, strides=strides, keep=keep)
+    o, st = _make_opts(eb, max_exp, flags=(FLAG_TIMING if timing else 0) | flags, strides=strides, keep=keep)
     if out is None:
         out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
         out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
@@ -244,7 +250,8 @@ def simplify_async(coef: torch.Tensor, exps: torch.Tensor, tol: float, max_exp: 
 
 def mul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tensor, b_exps: torch.Tensor, tol: float = 0.0, *,
                  max_exp: Optional[Sequence[int]] = None, out_capacity: Optional[int] = None,
-                 workspace: Optional[Workspace] = None, stream=None, return_stats: bool = False, timing: bool = False):
+                 workspace: Optional[Workspace] = None, stream=None, return_stats: bool = False, timing: bool = False,
+                 flags: int = 0):
     """polylab_mul_simplify on device tensors: simplify(a*b)."""
     a_coef, a_exps, sa = _dev_poly(a_coef, a_exps)
     b_coef, b_exps, sb = _dev_poly(b_coef, b_exps)
@@ -258,7 +265,7 @@ def mul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tenso
         raise PolylabError(ERR_INVALID_ARGUMENT, "na*nb must be < 2^30")
     cap = n if out_capacity is None else int(out_capacity)
     keep = []
-    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], max_exp, flags=FLAG_TIMING if timing else 0, keep=keep)
+    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], max_exp, flags=(FLAG_TIMING if timing else 0) | flags, keep=keep)
     out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=a_coef.device)
     out_exps = torch.empty((max(cap, 1), nvars), dtype=a_exps.dtype, device=a_coef.device)
     wsb = mul_simplify_workspace_bytes(na, nb, nvars)

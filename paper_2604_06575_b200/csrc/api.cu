@@ -11,6 +11,9 @@ namespace polylab {
 
 static thread_local char g_cuda_error[256] = "";
 
+// internal return value of one attempt: the sorted-order check failed with the atomic-ranking kernel -> re-run safely
+constexpr int kRetrySafeRank = -1000;
+
 static bool cuda_failed(cudaError_t e, const char* what)
 {
     if (e == cudaSuccess) return false;
@@ -147,7 +150,10 @@ static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb)
 static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
 {
     if (!st) return;
+    const int32_t launches = st->kernel_launches, fallback = st->rank_fallback;
     memset(st, 0, sizeof *st);
+    st->kernel_launches = launches;
+    st->rank_fallback = fallback;
     st->key_bits = plan.key_bits;
     st->key_bytes = plan.key_bytes;
     st->sort_passes = plan.npasses;
@@ -192,7 +198,7 @@ struct Timing {
 // keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
 static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
-                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream)
+                            int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream)
 {
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
@@ -201,7 +207,8 @@ static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, cons
     for (int p = 0; p < P; ++p) {
         const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
         *launches += launch_sort_pass(plan, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1], cbuf[(p + 1) & 1],
-                                      (uint32_t*)(ws + L.sort_state), ctl, stream);
+                                      (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
+                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
     }
     tm.mark(POLYLAB_STAGE_SORT);
     const void* skeys = kbuf[P & 1];
@@ -221,15 +228,16 @@ static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, cons
                                      (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
-    if (o.stats) o.stats->kernel_launches = *launches;
+    if (o.stats) o.stats->kernel_launches += *launches;
     if (dev_count) {
         if (o.status_device)
             PL_CUDA(cudaMemcpyAsync(o.status_device, &ctl->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
         return POLYLAB_OK;
     }
-    struct { int32_t status; uint32_t distinct, survivors; } res;
+    struct { int32_t status; uint32_t distinct, survivors, unsorted; } res;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));
+    if (res.unsorted) return safe_rank ? (int)POLYLAB_ERR_INTERNAL : kRetrySafeRank;
     tm.finish(o.stats);
     if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; }
     if (res.status != POLYLAB_OK) return res.status;
@@ -272,9 +280,9 @@ size_t polylab_mul_simplify_workspace_bytes(int64_t na, int64_t nb, int32_t nvar
     return worst_layout_bytes(na * nb, na, nb);
 }
 
-int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
-                     const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
-                     int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream)
+static int simplify_once(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
+                         const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                         int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream, bool safe_rank)
 {
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || nterms < 0 || nterms >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
@@ -320,12 +328,33 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
     // ---- S1 (+ histogram of the first digit), then the shared tail
     launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0, stream);
     tm.mark(POLYLAB_STAGE_PACK);
-    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream);
+    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
+                            safe_rank, stream);
 }
 
-int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
-                         double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
-                         void* workspace, size_t workspace_bytes, void* cuda_stream)
+static bool wants_safe_rank(const polylab_opts* opts)
+{
+    return opts && (opts->flags & (POLYLAB_FLAG_SAFE_RANK | POLYLAB_FLAG_DEVICE_COUNT)) != 0;
+}
+
+int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
+                     const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                     int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; }
+    int rc = simplify_once(coef, exps, nterms, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
+                           workspace_bytes, cuda_stream, wants_safe_rank(opts));
+    if (rc == kRetrySafeRank) {
+        if (opts && opts->stats) opts->stats->rank_fallback = 1;
+        rc = simplify_once(coef, exps, nterms, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
+                           workspace_bytes, cuda_stream, true);
+    }
+    return rc;
+}
+
+static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
+                             double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream, bool safe_rank)
 {
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (!a || !b || a->nvars != b->nvars) return POLYLAB_ERR_INVALID_ARGUMENT;
@@ -388,7 +417,22 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
                                      (double*)(ws + L.coefs[0]), ctl, stream);
     tm.mark(POLYLAB_STAGE_PACK);
     return sort_reduce_emit(plan_a, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                            out_nterms, &launches, tm, stream);
+                            out_nterms, &launches, tm, safe_rank, stream);
+}
+
+int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
+                         double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; }
+    int rc = mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
+                               cuda_stream, wants_safe_rank(opts));
+    if (rc == kRetrySafeRank) {
+        if (opts && opts->stats) opts->stats->rank_fallback = 1;
+        rc = mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
+                               cuda_stream, true);
+    }
+    return rc;
 }
 
 int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts, double* out_coef,
@@ -583,6 +627,7 @@ const char* polylab_status_string(int status)
     case POLYLAB_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case POLYLAB_ERR_OUTPUT_TOO_SMALL: return "output capacity too small";
     case POLYLAB_ERR_CUDA: return "CUDA error";
+    case POLYLAB_ERR_INTERNAL: return "internal error: sorted-order self-check failed";
     default: return "unknown status";
     }
 }

@@ -29,6 +29,8 @@ struct __align__(16) Key128 {
 
 __host__ __device__ inline bool key_eq(uint64_t a, uint64_t b) { return a == b; }
 __host__ __device__ inline bool key_eq(const Key128& a, const Key128& b) { return a.lo == b.lo && a.hi == b.hi; }
+__host__ __device__ inline bool key_lt(uint64_t a, uint64_t b) { return a < b; }
+__host__ __device__ inline bool key_lt(const Key128& a, const Key128& b) { return a.hi < b.hi || (a.hi == b.hi && a.lo < b.lo); }
 
 // 32-bit word `wi` of a key (0 = least significant).  wi is uniform across a kernel: the selects cost 1-3 instructions.
 __device__ __forceinline__ uint32_t key_word(uint64_t k, int wi) { return wi ? (uint32_t)(k >> 32) : (uint32_t)k; }
@@ -134,7 +136,7 @@ struct Control {
     int32_t status;                          // polylab_status of data-dependent checks
     uint32_t distinct;                       // U
     uint32_t survivors;                      // U'
-    uint32_t pad;
+    uint32_t unsorted;                       // S3 saw a key smaller than its predecessor (the sort was not stable)
 };
 
 constexpr int kTicketReduce = kMaxPasses;

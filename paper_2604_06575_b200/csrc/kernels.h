@@ -44,10 +44,14 @@ int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const Exp
 // S2: one stable LSD radix pass (digit `pass` of the plan) of n (key, coef) pairs from (keys_in, coef_in)
 // to (keys_out, coef_out).  tile_state: ceil(n/tile) * 256 words, zero before the FIRST pass of a call and
 // reused by every later pass (flag parity alternates).  Also accumulates the next pass's histogram.
+// safe_rank: ballot-matching ranking (stable by construction); otherwise one shared atomic per record (see sort.cu).
+// debug_unstable: test hook, reverses the lane order of the atomic kernel.
 int launch_sort_pass(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in, void* keys_out,
-                     double* coef_out, uint32_t* tile_state, Control* ctl, cudaStream_t stream);
+                     double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank, bool debug_unstable,
+                     cudaStream_t stream);
 
-// S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U.
+// S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U; sets ctl->unsorted
+// when a key is smaller than its predecessor.
 // Scratch: tile_state/tile_heads/tile_hb [ntiles] uint32 (zeroed), tile_frag [ntiles] double, tile_cont [ntiles] uint8.
 struct ReduceScratch {
     uint32_t* tile_state;

@@ -70,6 +70,7 @@ reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint
     // ---- phase 1: heads, sum before the first head, sum after the last head
     uint32_t nh = 0;
     double acc = 0.0;
+    bool descending = false;                         // a key below its predecessor: the sort failed (see sort.cu)
     {
         K kp = kprev0;
         bool hp = has_prev;
@@ -78,6 +79,7 @@ reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint
             if (first + j < tile_n) {
                 const K kk = skeys[first + j];
                 const bool head = !hp || !key_eq(kk, kp);
+                descending |= hp && key_lt(kk, kp);
                 if (head) { ++nh; acc = scoef[first + j]; }
                 else acc = __dadd_rn(acc, scoef[first + j]);
                 kp = kk;
@@ -85,6 +87,7 @@ reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint
             }
         }
     }
+    if (descending) ctl->unsorted = 1u;
     uint32_t H;
     const uint32_t hb = block_exclusive_scan<THREADS>(nh, scratch, &H);
 

@@ -39,6 +39,7 @@ struct PassArgs {
     const uint32_t* hist_this;
     uint32_t* hist_next;
     uint32_t* ticket;
+    int reverse_lanes;          // POLYLAB_FLAG_DEBUG_UNSTABLE: the atomic kernel maps lane l to record 31 - l
 };
 
 // lanes of the warp holding the same digit d (< 256) as the calling lane; all 32 lanes participate
@@ -54,7 +55,12 @@ __device__ __forceinline__ unsigned match_digit_all(uint32_t d)
     return mask;
 }
 
-template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL>
+// RANK_ATOMIC: rank a record among the warp's records of the same digit with ONE shared-memory atomic (the old
+// value of the warp's counter).  Lanes of one warp instruction that hit the same counter receive their old
+// values in ascending lane order on sm_100a (measured, profiles/r1b_shared_atomics.md; not documented), which
+// is what makes the pass stable; the reduce step verifies the sorted order and the call falls back to the
+// ballot-matching kernel (RANK_ATOMIC = false) if it ever does not hold.
+template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC>
 __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char* smem_raw, uint32_t tile, uint32_t tile_base,
                                                uint32_t tile_n)
 {
@@ -75,7 +81,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char*
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 
     // ---- load keys: warp w owns records [w*32*ITEMS, (w+1)*32*ITEMS) of the tile, item j of lane l is j*32+l
-    const uint32_t chunk = warp * 32u * ITEMS + lane;
+    const uint32_t chunk = warp * 32u * ITEMS + ((RANK_ATOMIC && a.reverse_lanes) ? 31u - lane : lane);
     K key[ITEMS];
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
@@ -87,22 +93,31 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char*
 
     // ---- rank within the warp, in record order (stable)
     uint32_t* my_hist = whist + warp * kRadix;
-    const unsigned lt = lanemask_lt();
     uint32_t pos[ITEMS];
+    if (RANK_ATOMIC) {
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-        const uint32_t dj = POLYLAB_DIGIT(j);
-        unsigned m = match_digit_all(dj);
-        bool valid = true;
-        if (!FULL) {
-            valid = (chunk + j * 32u) < tile_n;
-            m &= __ballot_sync(kFullMask, valid);
+        for (int j = 0; j < ITEMS; ++j) {
+            pos[j] = 0u;
+            if (FULL || (chunk + j * 32u) < tile_n) pos[j] = atomicAdd(&my_hist[POLYLAB_DIGIT(j)], 1u);
+            __syncwarp();                                   // item j's atomics are performed before item j+1's
         }
-        const uint32_t prev = my_hist[dj];
-        __syncwarp();
-        if (valid && (m & lt) == 0u) my_hist[dj] = prev + __popc(m);
-        __syncwarp();
-        pos[j] = prev + __popc(m & lt);
+    } else {
+        const unsigned lt = lanemask_lt();
+#pragma unroll
+        for (int j = 0; j < ITEMS; ++j) {
+            const uint32_t dj = POLYLAB_DIGIT(j);
+            unsigned m = match_digit_all(dj);
+            bool valid = true;
+            if (!FULL) {
+                valid = (chunk + j * 32u) < tile_n;
+                m &= __ballot_sync(kFullMask, valid);
+            }
+            const uint32_t prev = my_hist[dj];
+            __syncwarp();
+            if (valid && (m & lt) == 0u) my_hist[dj] = prev + __popc(m);
+            __syncwarp();
+            pos[j] = prev + __popc(m & lt);
+        }
     }
     if (NEXT) {
         // histogram of the next pass's digit: plain shared-memory atomics (no order needed; Blackwell's ATOMS
@@ -151,31 +166,43 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char*
         c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
     }
 
-    // ---- decoupled look-back: number of records with digit b in all earlier tiles
+    // ---- decoupled look-back: number of records with digit b in all earlier tiles.  The walk over the predecessors
+    // is the longest stall of the kernel when done one dependent load at a time (profiles/r1b), so LB states are
+    // fetched per round trip and consumed in order up to the first inclusive one (or the first not yet published).
     uint32_t excl = 0;
     if (tile > 0) {
-        const uint32_t* p = my_state - kRadix;
-        while (true) {
-            const uint32_t w = ld_volatile_u32(p);
-            const uint32_t f = w & 3u;
-            if (f == a.flag_inclusive) { excl += w >> 2; break; }
-            if (f == a.flag_partial) { excl += w >> 2; p -= kRadix; }
+        constexpr int LB = 8;
+        int64_t t = (int64_t)tile - 1;                       // nearest predecessor not consumed yet
+        bool done = false;
+        while (!done) {
+            uint32_t w[LB];
+#pragma unroll
+            for (int i = 0; i < LB; ++i)
+                w[i] = (t - i >= 0) ? ld_volatile_u32(a.tile_state + (size_t)(t - i) * kRadix + b) : a.flag_inclusive;
+            int used = 0;
+            bool open = true;                                // still consuming this window
+#pragma unroll
+            for (int i = 0; i < LB; ++i) {
+                const uint32_t f = w[i] & 3u;
+                if (open && f == a.flag_inclusive) { excl += w[i] >> 2; done = true; open = false; }
+                else if (open && f == a.flag_partial) { excl += w[i] >> 2; ++used; }
+                else open = false;                           // not published yet: poll again from here
+            }
+            t -= used;
         }
         st_volatile_u32(my_state, ((excl + count) << 2) | a.flag_inclusive);
     }
     sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
     __syncthreads();
 
-    // ---- write keys: slot s of the sorted tile, contiguous per bin (only the digit's word is re-read for the bin)
-    const uint32_t* stage_w = (const uint32_t*)(smem_raw + key_word_byte_offset<K>(a.dword));
-    constexpr int KW = sizeof(K) / 4;
+    // ---- write keys: slot s of the sorted tile, contiguous per bin
     uint32_t dst[ITEMS];
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
         if (FULL || s < tile_n) {
             const K kk = stage[s];
-            dst[k] = s + sm_delta[(stage_w[s * KW] >> a.dshift) & a.dmask];
+            dst[k] = s + sm_delta[(key_word(kk, a.dword) >> a.dshift) & a.dmask];
             keys_out[dst[k]] = kk;
         }
     }
@@ -191,7 +218,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char*
     }
 }
 
-template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT>
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
 __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_constant__ PassArgs a)
 {
     static_assert(THREADS == kRadix, "one thread per bin");
@@ -208,15 +235,15 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_c
     const uint32_t tile = scratch[NW + 2];
     const uint32_t tile_base = tile * (uint32_t)TILE;
     const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
-    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true>(a, smem_raw, tile, tile_base, tile_n);
-    else sort_tile_body<K, THREADS, ITEMS, NEXT, false>(a, smem_raw, tile, tile_base, tile_n);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, RANK_ATOMIC>(a, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, RANK_ATOMIC>(a, smem_raw, tile, tile_base, tile_n);
 }
 
-template <typename K, int ITEMS, int MINB, bool NEXT>
+template <typename K, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
 static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t stream)
 {
     using S = SortSmem<K, kSortThreads, ITEMS>;
-    auto kern = sort_pass_kernel<K, kSortThreads, ITEMS, MINB, NEXT>;
+    auto kern = sort_pass_kernel<K, kSortThreads, ITEMS, MINB, NEXT, RANK_ATOMIC>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
@@ -227,7 +254,8 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 
 template <typename K, int ITEMS, int MINB>
 static int launch_sort_pass_t(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in,
-                              void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, cudaStream_t stream)
+                              void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
+                              bool debug_unstable, cudaStream_t stream)
 {
     using S = SortSmem<K, kSortThreads, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
@@ -243,20 +271,27 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int64_t n, const void*
     a.flag_partial = (pass & 1) ? 3u : 1u;                 // flag parity: no re-zeroing between passes
     a.flag_inclusive = (pass & 1) ? 0u : 2u;
     a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[pass + 1]; a.ticket = &ctl->ticket[pass];
-    if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true>(a, tiles, stream);
-    else launch_sort_pass_k<K, ITEMS, MINB, false>(a, tiles, stream);
+    a.reverse_lanes = debug_unstable ? 1 : 0;
+    if (safe_rank) {
+        if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, false>(a, tiles, stream);
+        else launch_sort_pass_k<K, ITEMS, MINB, false, false>(a, tiles, stream);
+    } else {
+        if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, true>(a, tiles, stream);
+        else launch_sort_pass_k<K, ITEMS, MINB, false, true>(a, tiles, stream);
+    }
     return 1;
 }
 
 int launch_sort_pass(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in, void* keys_out,
-                     double* coef_out, uint32_t* tile_state, Control* ctl, cudaStream_t stream)
+                     double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank, bool debug_unstable,
+                     cudaStream_t stream)
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, n, keys_in, coef_in, keys_out, coef_out, tile_state,
-                                                             ctl, stream);
+                                                             ctl, safe_rank, debug_unstable, stream);
     return launch_sort_pass_t<Key128, kSortItems128, 3>(plan, pass, n, keys_in, coef_in, keys_out, coef_out, tile_state, ctl,
-                                                        stream);
+                                                        safe_rank, debug_unstable, stream);
 }
 
 }  // namespace polylab

@@ -410,3 +410,39 @@ def test_async_device_count():
     k = int(cnt.item())
     assert int(status.item()) == 0 and k == 256
     assert_parity(oracle.simplify(p.coef, p.exps, tol), oc[:k].cpu().numpy(), oe[:k].cpu().numpy())
+
+
+# ------------------------------------------------------------------------------- ranking kernels
+
+@pytest.mark.parametrize("cfg", ["c3", "c5", "c2"])
+def test_safe_rank_kernel_matches_default(cfg):
+    """The ballot-matching radix pass (POLYLAB_FLAG_SAFE_RANK) and the default atomic-ranking pass are both stable:
+    same monomials, bit-identical sums (the summation tree is the same when the sorted order is the same)."""
+    if cfg == "c2":
+        a, b, tol = W.config2(300)
+        r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True)
+        r1 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_SAFE_RANK)
+        res = oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol)
+    else:
+        p, tol = (W.config3(300_000) if cfg == "c3" else W.config5(300_000))
+        r0 = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True)
+        r1 = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=B.FLAG_SAFE_RANK)
+        res = oracle.simplify(p.coef, p.exps, tol)
+    assert r0[2].rank_fallback == 0 and r1[2].rank_fallback == 0
+    c0, e0, c1, e1 = r0[0].cpu().numpy(), r0[1].cpu().numpy(), r1[0].cpu().numpy(), r1[1].cpu().numpy()
+    assert_parity(res, c0, e0)
+    assert (e0 == e1).all() and (c0.view(np.uint64) == c1.view(np.uint64)).all()
+
+
+def test_unstable_rank_is_detected_and_falls_back():
+    """POLYLAB_FLAG_DEBUG_UNSTABLE reverses the lane order of the atomic-ranking pass, which breaks LSD stability;
+    the segmented-sum step must see the unsorted keys and the call must re-run with the ballot kernel."""
+    p, tol = W.config5(300_000)
+    c, e, st = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=B.FLAG_DEBUG_UNSTABLE)
+    assert st.rank_fallback == 1
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c.cpu().numpy(), e.cpu().numpy())
+    a, b, tol = W.config2(300)
+    c, e, st = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True,
+                              flags=B.FLAG_DEBUG_UNSTABLE)
+    assert st.rank_fallback == 1
+    assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol), c.cpu().numpy(), e.cpu().numpy())
