@@ -77,9 +77,21 @@ enum {
                                         segmented-sum step and re-runs the call with this flag if the check
                                         fails (stats->rank_fallback = 1).  Implied by POLYLAB_FLAG_DEVICE_COUNT,
                                         which cannot read the check back. */
+    POLYLAB_FLAG_NO_BUCKET = 8u,     /* never take the bucket path: always sort with ceil(B/8) LSD passes.  By default a
+                                        call with >= 2^20 terms and >= 4 digits first partitions the pairs on their
+                                        most significant digit(s) and, if those spread the keys evenly enough for every
+                                        bucket to fit shared memory, finishes sort + sum + prune + unpack on chip
+                                        (stats->prefix_passes > 0); otherwise (stats->bucket_fallback = 1) it runs the
+                                        LSD passes.  Both paths give the same result up to summation order.  Not
+                                        taken with POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
+    POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
+                                        skew pre-check), so that small tests reach it and its overflow fallback */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
                                         (reversed lane order) so that tests can exercise detection and fallback */
 };
+/* test hook: bits 8..11 of flags, when non-zero, override how many low digits the bucket path's first local sort
+   attempt uses (default 3); 1 makes most tiles fail the order check and re-sort on every digit */
+#define POLYLAB_FLAG_DEBUG_NFAST_SHIFT 8
 
 /* indices into polylab_stats.stage_ms */
 enum { POLYLAB_STAGE_BOUNDS = 0, POLYLAB_STAGE_PACK = 1, POLYLAB_STAGE_SORT = 2, POLYLAB_STAGE_REDUCE = 3,
@@ -90,14 +102,20 @@ typedef struct polylab_stats {
     int32_t key_bits;        /* B = sum of field widths                                  */
     int32_t key_bytes;       /* W = 8 or 16                                              */
     int32_t sort_passes;     /* P radix passes executed                                  */
-    int32_t digit_bits[16];  /* width of each pass's digit, least significant first      */
+    int32_t digit_bits[16];  /* width of each digit of the key, least significant first   */
     int64_t sort_terms;      /* N = terms that entered the sort (na*nb for a product)    */
     int64_t distinct;        /* U = distinct monomials before pruning (-1 with DEVICE_COUNT) */
     int64_t survivors;       /* U' (-1 with DEVICE_COUNT)                                */
     int32_t kernel_launches; /* kernels of this library launched by the call (both attempts after a fallback) */
     int32_t rank_fallback;   /* 1 if the sorted-order check failed and the call re-ran with SAFE_RANK */
     float stage_ms[8];       /* with POLYLAB_FLAG_TIMING: device time of S0 (incl. read-back), S1 (+X1),
-                                S2 (all passes), S3, S4+S5; CUDA events on the call's stream  */
+                                S2 (all passes), S3, S4+S5; CUDA events on the call's stream.  On the bucket
+                                path S2 = the prefix passes and S3 = the fused finish (local sort + S3 + S4 + S5) */
+    int32_t prefix_passes;   /* > 0: the bucket path ran with this many prefix passes (then sort_passes == prefix_passes) */
+    int32_t bucket_fallback; /* 1 if the bucket path was planned and abandoned (skewed digit histogram or a bucket
+                                too long for a tile); the result then comes from the LSD path */
+    int32_t refinish_tiles;  /* bucket path: tiles whose fast local sort failed the order check and re-sorted fully */
+    int32_t plan_digits;     /* ceil(B/8): digits of the key layout = entries of digit_bits = LSD passes the plan needs */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

@@ -26,7 +26,10 @@ LIB_PATH = os.path.join(_HERE, "libpolylab.so")
 FLAG_DEVICE_COUNT = 1
 FLAG_TIMING = 2
 FLAG_SAFE_RANK = 4
+FLAG_NO_BUCKET = 8
+FLAG_DEBUG_FORCE_BUCKET = 0x20000000
 FLAG_DEBUG_UNSTABLE = 0x40000000
+FLAG_DEBUG_NFAST_SHIFT = 8
 STAGES = ("bounds", "pack", "sort", "reduce", "prune")
 MAX_NVARS = 128
 MAX_TERMS = 1 << 30
@@ -43,7 +46,8 @@ class _Stats(ctypes.Structure):
     _fields_ = [("key_bits", ctypes.c_int32), ("key_bytes", ctypes.c_int32), ("sort_passes", ctypes.c_int32),
                 ("digit_bits", ctypes.c_int32 * 16), ("sort_terms", ctypes.c_int64), ("distinct", ctypes.c_int64),
                 ("survivors", ctypes.c_int64), ("kernel_launches", ctypes.c_int32), ("rank_fallback", ctypes.c_int32),
-                ("stage_ms", ctypes.c_float * 8)]
+                ("stage_ms", ctypes.c_float * 8), ("prefix_passes", ctypes.c_int32), ("bucket_fallback", ctypes.c_int32),
+                ("refinish_tiles", ctypes.c_int32), ("plan_digits", ctypes.c_int32)]
 
 
 class _Opts(ctypes.Structure):
@@ -68,6 +72,9 @@ class Stats:
     kernel_launches: int
     stage_ms: dict
     rank_fallback: int = 0
+    prefix_passes: int = 0
+    bucket_fallback: int = 0
+    refinish_tiles: int = 0
 
 
 _lib = None
@@ -173,9 +180,10 @@ def _make_opts(exp_bytes: int, max_exp, flags: int = 0, strides=None, status_dev
 
 
 def _stats(st: _Stats) -> Stats:
-    return Stats(st.key_bits, st.key_bytes, st.sort_passes, list(st.digit_bits)[:st.sort_passes], st.sort_terms,
+    return Stats(st.key_bits, st.key_bytes, st.sort_passes, list(st.digit_bits)[:st.plan_digits], st.sort_terms,
                  st.distinct, st.survivors, st.kernel_launches, {k: float(st.stage_ms[i]) for i, k in enumerate(STAGES)},
-                 rank_fallback=st.rank_fallback)
+                 rank_fallback=st.rank_fallback, prefix_passes=st.prefix_passes, bucket_fallback=st.bucket_fallback,
+                 refinish_tiles=st.refinish_tiles)
 
 
 def _dev_poly(coef: torch.Tensor, exps: torch.Tensor, strides=None):

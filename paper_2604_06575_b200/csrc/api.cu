@@ -11,8 +11,15 @@ namespace polylab {
 
 static thread_local char g_cuda_error[256] = "";
 
-// internal return value of one attempt: the sorted-order check failed with the atomic-ranking kernel -> re-run safely
+// internal return values of one attempt: the sorted-order check failed with the atomic-ranking kernels -> re-run with
+// ballot ranking on the LSD path; a bucket of the bucket path was too long -> re-run on the LSD path
 constexpr int kRetrySafeRank = -1000;
+constexpr int kRetryNoBucket = -1001;
+
+struct Attempt {
+    bool safe_rank;        // ballot-matching radix passes, LSD path only
+    bool allow_bucket;     // may take the bucket path (finish.cu)
+};
 
 static bool cuda_failed(cudaError_t e, const char* what)
 {
@@ -112,7 +119,7 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 // ------------------------------------------------------------------------------ workspace carving
 
 struct Layout {
-    size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, zero_end;
+    size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, zero_end;
     size_t keys[2], coefs[2], ka, kb, total;
 };
 
@@ -128,7 +135,10 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.sort_state = take(sort_tiles * kRadix * sizeof(uint32_t));
     L.red_state = take(red_tiles * sizeof(uint32_t));
     L.prune_state = take(prune_tiles * sizeof(uint32_t));
+    const size_t fin_tiles = (size_t)((n + kFinMinTile - 1) / kFinMinTile);
+    L.fin_state = take(fin_tiles * sizeof(uint32_t));
     L.zero_end = off;                                   // everything before this is zeroed per call
+    L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.red_heads = take(red_tiles * sizeof(uint32_t));
     L.red_hb = take(red_tiles * sizeof(uint32_t));
     L.red_frag = take(red_tiles * sizeof(double));
@@ -150,13 +160,15 @@ static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb)
 static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
 {
     if (!st) return;
-    const int32_t launches = st->kernel_launches, fallback = st->rank_fallback;
+    const int32_t launches = st->kernel_launches, fallback = st->rank_fallback, bfall = st->bucket_fallback;
     memset(st, 0, sizeof *st);
     st->kernel_launches = launches;
     st->rank_fallback = fallback;
+    st->bucket_fallback = bfall;
     st->key_bits = plan.key_bits;
     st->key_bytes = plan.key_bytes;
     st->sort_passes = plan.npasses;
+    st->plan_digits = plan.npasses;
     for (int p = 0; p < plan.npasses; ++p) st->digit_bits[p] = plan.digit_bits[p];
     st->sort_terms = n;
     st->distinct = -1;
@@ -193,21 +205,121 @@ struct Timing {
     }
 };
 
+// ------------------------------------------------------------------------------- bucket path plan
+
+// How many of the most significant plan digits to partition on before finishing in shared memory (0 = LSD path).
+// The buckets must average at most one finish tile; the path pays only when it replaces at least three LSD passes.
+static int choose_prefix_passes(const Plan& plan, int64_t n, const Opts& o, const Attempt& at)
+{
+    const bool force = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET) != 0;
+    if (!at.allow_bucket || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_BUCKET | POLYLAB_FLAG_DEVICE_COUNT))) return 0;
+    const int P = plan.npasses;
+    if (P < 1 || (!force && (P < 4 || n < (1 << 20)))) return 0;
+    for (int k = 1; k <= P; ++k) {
+        const int T = plan.key_bits - plan.digit_pos[P - k];
+        if (T >= 40 || (n >> T) < kFinCap - 3584) return (force || P - k >= 3) ? k : 0;
+    }
+    return 0;
+}
+
+// Room a finish tile leaves for its longest bucket: twice the mean bucket N / 2^T (duplicated monomials make bucket
+// sizes much wider than Poisson), within [512, kFinCap - kFinMinTile]; the tile covers the other kFinCap - room positions.
+static int bucket_room(const Plan& plan, int k, int64_t n)
+{
+    const int T = plan.key_bits - plan.digit_pos[plan.npasses - k];
+    const int64_t mean = T >= 40 ? 0 : (n >> T);
+    int64_t room = 2 * mean;
+    if (room < 512) room = 512;
+    if (room > kFinCap - kFinMinTile) room = kFinCap - kFinMinTile;
+    return (int)room;
+}
+
+static int fast_digits(const Opts& o)
+{
+    const int dbg = (int)((o.flags >> POLYLAB_FLAG_DEBUG_NFAST_SHIFT) & 0xfu);
+    return dbg ? dbg : 3;          // 24 bits below the prefix separate the distinct keys of a bucket with high probability
+}
+
+// After S1/X1 accumulated the histogram of the first prefix digit: do its bins predict buckets that fit a tile?
+// (A necessary test only; tile_bounds_kernel has the last word.)  On rejection the LSD path needs digit 0's histogram.
+static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* ws, const Layout& L, const Opts& o,
+                           int* launches, cudaStream_t stream)
+{
+    if (*k == 0 || (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET)) return POLYLAB_OK;
+    Control* ctl = (Control*)(ws + L.control);
+    const int P = plan.npasses, d = P - *k;
+    uint32_t h[kRadix];
+    PL_CUDA(cudaMemcpyAsync(h, ctl->hist[d], sizeof h, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    uint64_t mx = 0;
+    for (int b = 0; b < kRadix; ++b) mx = h[b] > mx ? h[b] : mx;
+    const int rest = plan.key_bits - plan.digit_pos[d] - plan.digit_bits[d];      // prefix bits above this digit
+    if ((mx >> rest) <= (uint64_t)bucket_room(plan, *k, n) * 7 / 8) return POLYLAB_OK;
+    *k = 0;
+    if (o.stats) o.stats->bucket_fallback = 1;
+    PL_CUDA(cudaMemsetAsync(ctl->hist[d], 0, sizeof h, stream));
+    *launches += launch_key_hist(plan, 0, n, ws + L.keys[0], ctl, stream);
+    return POLYLAB_OK;
+}
+
 // ----------------------------------------------------------------------- shared tail of both paths
 
 // keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
-static int sort_reduce_emit(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
+struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish; };
+
+// Bucket path: k stable passes over the top k digits, then finish.cu.  The pairs are in (L.keys[0], coef0) and the
+// histogram of digit P-k is in ctl->hist[P-k].
+static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
+                            double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
+                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream)
+{
+    Control* ctl = (Control*)(ws + L.control);
+    void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
+    double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
+    const int P = plan.npasses;
+    for (int s = 0; s < k; ++s) {
+        const double* cin = (s == 0) ? coef0 : cbuf[s & 1];
+        *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
+                                      cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
+                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
+    }
+    tm.mark(POLYLAB_STAGE_SORT);
+    *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol, out_coef, out_exps, o.exp_bytes,
+                               out_capacity, (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), ctl, nullptr, stream);
+    tm.mark(POLYLAB_STAGE_REDUCE);
+    tm.mark(POLYLAB_STAGE_PRUNE);
+    PL_CUDA(cudaGetLastError());
+    if (o.stats) o.stats->kernel_launches += *launches;
+    Readback res;
+    PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    if (res.overflow) return kRetryNoBucket;
+    if (res.unsorted) return kRetrySafeRank;
+    tm.finish(o.stats);
+    if (o.stats) {
+        o.stats->distinct = res.distinct; o.stats->survivors = res.survivors;
+        o.stats->prefix_passes = k; o.stats->sort_passes = k; o.stats->refinish_tiles = (int32_t)res.refinish;
+    }
+    if (res.status != POLYLAB_OK) return res.status;
+    *out_nterms = (int64_t)res.survivors;
+    return (int64_t)res.survivors > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
+}
+
+static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream)
 {
+    if (k_bucket > 0)
+        return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
+                                tm, stream);
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
     const int P = plan.npasses;
     for (int p = 0; p < P; ++p) {
         const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
-        *launches += launch_sort_pass(plan, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1], cbuf[(p + 1) & 1],
-                                      (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
+        *launches += launch_sort_pass(plan, p, p + 1 < P ? p + 1 : -1, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1],
+                                      cbuf[(p + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
     }
     tm.mark(POLYLAB_STAGE_SORT);
@@ -282,7 +394,7 @@ size_t polylab_mul_simplify_workspace_bytes(int64_t na, int64_t nb, int32_t nvar
 
 static int simplify_once(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
                          const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
-                         int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream, bool safe_rank)
+                         int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream, const Attempt& at)
 {
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || nterms < 0 || nterms >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
@@ -325,11 +437,14 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     if (avail < L.total) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
 
-    // ---- S1 (+ histogram of the first digit), then the shared tail
-    launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0, stream);
+    // ---- S1 (+ histogram of the first pass's digit), then the shared tail
+    int k = choose_prefix_passes(plan, nterms, o, at);
+    launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
+    rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream);
+    if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
-    return sort_reduce_emit(plan, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
-                            safe_rank, stream);
+    return sort_reduce_emit(plan, k, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
+                            at.safe_rank, stream);
 }
 
 static bool wants_safe_rank(const polylab_opts* opts)
@@ -337,24 +452,42 @@ static bool wants_safe_rank(const polylab_opts* opts)
     return opts && (opts->flags & (POLYLAB_FLAG_SAFE_RANK | POLYLAB_FLAG_DEVICE_COUNT)) != 0;
 }
 
+// Runs `once(attempt)`; a failed self-check re-runs the call on a more conservative path (at most twice).
+extern "C++" {
+template <typename F>
+static int run_attempts(const polylab_opts* opts, F once)
+{
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; }
+    Attempt at = {wants_safe_rank(opts), true};
+    int rc = once(at);
+    if (rc == kRetryNoBucket) {
+        if (opts && opts->stats) opts->stats->bucket_fallback = 1;
+        at.allow_bucket = false;
+        rc = once(at);
+    }
+    if (rc == kRetrySafeRank) {
+        if (opts && opts->stats) opts->stats->rank_fallback = 1;
+        at.safe_rank = true;
+        at.allow_bucket = false;
+        rc = once(at);
+    }
+    return rc;
+}
+}  // extern "C++"
+
 int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
                      const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
                      int64_t* out_nterms, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; }
-    int rc = simplify_once(coef, exps, nterms, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
-                           workspace_bytes, cuda_stream, wants_safe_rank(opts));
-    if (rc == kRetrySafeRank) {
-        if (opts && opts->stats) opts->stats->rank_fallback = 1;
-        rc = simplify_once(coef, exps, nterms, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
-                           workspace_bytes, cuda_stream, true);
-    }
-    return rc;
+    return run_attempts(opts, [&](const Attempt& at) {
+        return simplify_once(coef, exps, nterms, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
+                             workspace_bytes, cuda_stream, at);
+    });
 }
 
 static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
                              double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
-                             void* workspace, size_t workspace_bytes, void* cuda_stream, bool safe_rank)
+                             void* workspace, size_t workspace_bytes, void* cuda_stream, const Attempt& at)
 {
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (!a || !b || a->nvars != b->nvars) return POLYLAB_ERR_INVALID_ARGUMENT;
@@ -411,28 +544,26 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
 
     // ---- S1 on the operands, X1 on packed keys (+ histogram of the first digit), then the shared tail
-    launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, false, stream);
-    launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, false, stream);
+    int k = choose_prefix_passes(plan_a, n, o, at);
+    launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, -1, stream);
+    launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, -1, stream);
     launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
-                                     (double*)(ws + L.coefs[0]), ctl, stream);
+                                     (double*)(ws + L.coefs[0]), ctl, k ? plan_a.npasses - k : 0, stream);
+    rc = bucket_precheck(plan_a, &k, n, ws, L, o, &launches, stream);
+    if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
-    return sort_reduce_emit(plan_a, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                            out_nterms, &launches, tm, safe_rank, stream);
+    return sort_reduce_emit(plan_a, k, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
+                            out_nterms, &launches, tm, at.safe_rank, stream);
 }
 
 int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
                          double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
                          void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; }
-    int rc = mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
-                               cuda_stream, wants_safe_rank(opts));
-    if (rc == kRetrySafeRank) {
-        if (opts && opts->stats) opts->stats->rank_fallback = 1;
-        rc = mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
-                               cuda_stream, true);
-    }
-    return rc;
+    return run_attempts(opts, [&](const Attempt& at) {
+        return mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
+                                 cuda_stream, at);
+    });
 }
 
 int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts, double* out_coef,

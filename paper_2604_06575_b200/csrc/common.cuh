@@ -58,6 +58,14 @@ __device__ __forceinline__ Key128 key_add(const Key128& a, const Key128& b)
     return r;
 }
 
+// do a and b agree on all bits at positions >= pos?  (the "prefix" of the bucket path, finish.cu)
+__host__ __device__ inline bool same_prefix(uint64_t a, uint64_t b, int pos) { return ((a ^ b) >> pos) == 0; }
+__host__ __device__ inline bool same_prefix(const Key128& a, const Key128& b, int pos)
+{
+    if (pos >= 64) return ((a.hi ^ b.hi) >> (pos - 64)) == 0;
+    return a.hi == b.hi && ((a.lo ^ b.lo) >> pos) == 0;
+}
+
 template <typename K> __device__ __forceinline__ K key_max();
 template <> __device__ __forceinline__ uint64_t key_max<uint64_t>() { return ~0ull; }
 template <> __device__ __forceinline__ Key128 key_max<Key128>() { Key128 k; k.lo = ~0ull; k.hi = ~0ull; return k; }
@@ -137,10 +145,13 @@ struct Control {
     uint32_t distinct;                       // U
     uint32_t survivors;                      // U'
     uint32_t unsorted;                       // S3 saw a key smaller than its predecessor (the sort was not stable)
+    uint32_t overflow;                       // bucket path: a bucket does not fit a finish tile (skewed prefix digits)
+    uint32_t refinish;                       // bucket path: finish tiles that needed the full local digit list
 };
 
 constexpr int kTicketReduce = kMaxPasses;
 constexpr int kTicketPrune = kMaxPasses + 1;
+constexpr int kTicketFinish = kMaxPasses + 2;
 
 // ------------------------------------------------------------------------- warp/block helpers
 
@@ -202,6 +213,19 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* w
     __syncthreads();
     *total = warp_scratch[NW];
     return warp_scratch[warp] + incl - x;
+}
+
+// Segmented-sum scan element: (any head seen, sum since the last head); used by S3 (reduce.cu, finish.cu).
+struct SegPair {
+    uint32_t f;
+    double v;
+};
+__device__ __forceinline__ SegPair seg_combine(const SegPair& l, const SegPair& r)
+{
+    SegPair o;
+    o.f = l.f | r.f;
+    o.v = r.f ? r.v : __dadd_rn(l.v, r.v);
+    return o;
 }
 
 // Decoupled look-back over single-word tile states: word = (value << 2) | flag.

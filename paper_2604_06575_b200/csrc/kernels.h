@@ -16,6 +16,11 @@ constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from sha
 constexpr int kPruneThreads = 256;
 constexpr int kPruneItems = 8;
 
+constexpr int kFinThreads = 512;    // bucket path (finish.cu): one block per SM
+constexpr int kFinCap = 6656;       // most records a finish tile can own (shared memory); tile t owns the buckets that start
+                                    // in positions [t*fin_tile, (t+1)*fin_tile), a bucket may be as long as kFinCap - fin_tile
+constexpr int kFinMinTile = 2560;   // smallest fin_tile the planner picks (workspace sizing)
+
 inline int sort_tile(int key_bytes) { return kSortThreads * (key_bytes == 8 ? kSortItems64 : kSortItems128); }
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
 constexpr int kPruneTile = kPruneThreads * kPruneItems;
@@ -24,31 +29,35 @@ constexpr int kPruneTile = kPruneThreads * kPruneItems;
 int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream);
 
 // S1: pack rows into keys (key_bytes from the plan), check e <= plan.bound (-> ctl->status), and, when
-// hist0 is true, accumulate the histogram of pass 0's digit into ctl->hist[0].
-int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, bool hist0,
+// hist_digit >= 0, accumulate the histogram of that plan digit into ctl->hist[hist_digit] (the first pass's digit).
+int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, int hist_digit,
                 cudaStream_t stream);
+
+// Histogram of plan digit `hist_digit` over packed keys into ctl->hist[hist_digit].
+int launch_key_hist(const Plan& plan, int hist_digit, int64_t n, const void* keys, Control* ctl, cudaStream_t stream);
 
 // S1 for the test entry point: always writes (hi, lo) pairs.
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
                      cudaStream_t stream);
 
 // X1: all products of packed operands: key = ka_i + kb_j, coef = fl(ca_i * cb_j); N = na*nb pairs written
-// to keys/coefs (emission order: i*nb + j); histogram of pass 0's digit into ctl->hist[0].
+// to keys/coefs (emission order: i*nb + j); histogram of plan digit `hist_digit` into ctl->hist[hist_digit].
 int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
-                         const Plan& plan, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
+                         const Plan& plan, void* keys, double* coefs, Control* ctl, int hist_digit, cudaStream_t stream);
 
 // Raw product without keys (polylab_expand): rows a_i + b_j, coefficients fl(ca_i*cb_j).
 int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const ExpView& eb, const double* cb, int64_t nb,
                       int nvars, double* out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream);
 
-// S2: one stable LSD radix pass (digit `pass` of the plan) of n (key, coef) pairs from (keys_in, coef_in)
-// to (keys_out, coef_out).  tile_state: ceil(n/tile) * 256 words, zero before the FIRST pass of a call and
-// reused by every later pass (flag parity alternates).  Also accumulates the next pass's histogram.
+// S2: one stable radix pass on plan digit `pass` of n (key, coef) pairs from (keys_in, coef_in) to (keys_out,
+// coef_out); needs ctl->hist[pass].  `next` >= 0: also accumulate the histogram of plan digit `next` (the digit of
+// the following pass) into ctl->hist[next].  `seq` = 0, 1, 2, ... counts the passes of the call: tile_state
+// (ceil(n/tile) * 256 words) is zero before pass seq 0 and reused by every later pass (flag parity alternates).
 // safe_rank: ballot-matching ranking (stable by construction); otherwise one shared atomic per record (see sort.cu).
 // debug_unstable: test hook, reverses the lane order of the atomic kernel.
-int launch_sort_pass(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in, void* keys_out,
-                     double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank, bool debug_unstable,
-                     cudaStream_t stream);
+int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
+                     void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
+                     bool debug_unstable, cudaStream_t stream);
 
 // S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U; sets ctl->unsorted
 // when a key is smaller than its predecessor.
@@ -68,5 +77,13 @@ int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coef
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
                         double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
                         Control* ctl, int64_t* out_count_device, cudaStream_t stream);
+
+// Bucket path (finish.cu): the pairs are sorted by their top `prefix_passes` plan digits; finish every bucket in
+// shared memory and emit the simplified polynomial (S2 rest + S3 + S4 + S5).  tile_start: ceil(n/fin_tile)+1 words;
+// tile_state: ceil(n/fin_tile) words, zeroed.  Sets ctl->overflow (nothing emitted) when a bucket is too long,
+// ctl->unsorted when the prefix order or the local order check fails, ctl->distinct, ctl->survivors.
+int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs, double tol,
+                  double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_start,
+                  uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaStream_t stream);
 
 }  // namespace polylab

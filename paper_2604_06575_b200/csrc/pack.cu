@@ -113,7 +113,7 @@ int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, in
 
 // ----------------------------------------------------------------------------------------------- S1
 
-// digit-0 histogram of a block: shared atomics, flushed with one global reduction per non-empty bin
+// first-pass digit histogram of a block: shared atomics, flushed with one global reduction per non-empty bin
 struct BlockHist {
     uint32_t* sh;
     __device__ void init(uint32_t* s) { sh = s; for (int b = threadIdx.x; b < kRadix; b += blockDim.x) sh[b] = 0u; }
@@ -137,14 +137,14 @@ __device__ __forceinline__ void pack_field(K& key, uint32_t e, int v, const Plan
 template <typename K, int ES, int WB>
 __global__ void __launch_bounds__(256) pack_rows_kernel(const uint8_t* __restrict__ base, int64_t nterms,
                                                         const __grid_constant__ Plan plan, K* __restrict__ keys,
-                                                        Control* ctl, int hist0)
+                                                        Control* ctl, int hd)
 {
     __shared__ uint32_t sh[kRadix];
     BlockHist bh;
-    if (hist0) { bh.init(sh); __syncthreads(); }
+    if (hd >= 0) { bh.init(sh); __syncthreads(); }
     const int rb = plan.nvars * ES;
-    const int dpos = plan.digit_pos[0];
-    const uint32_t dmask = (1u << plan.digit_bits[0]) - 1u;
+    const int dpos = plan.digit_pos[hd >= 0 ? hd : 0];
+    const uint32_t dmask = (1u << plan.digit_bits[hd >= 0 ? hd : 0]) - 1u;
     bool bad = false;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nterms; t += (int64_t)gridDim.x * blockDim.x) {
         const uint8_t* row = base + t * rb;
@@ -169,22 +169,22 @@ __global__ void __launch_bounds__(256) pack_rows_kernel(const uint8_t* __restric
             }
         }
         keys[t] = key;
-        if (hist0) bh.add(key_digit(key, dpos, dmask));
+        if (hd >= 0) bh.add(key_digit(key, dpos, dmask));
     }
     if (bad) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
-    if (hist0) { __syncthreads(); bh.flush(ctl->hist[0]); }
+    if (hd >= 0) { __syncthreads(); bh.flush(ctl->hist[hd]); }
 }
 
 // Any strides / alignment: one element load per variable.
 template <typename K>
 __global__ void __launch_bounds__(256) pack_strided_kernel(ExpView ev, int64_t nterms, const __grid_constant__ Plan plan,
-                                                           K* __restrict__ keys, Control* ctl, int hist0)
+                                                           K* __restrict__ keys, Control* ctl, int hd)
 {
     __shared__ uint32_t sh[kRadix];
     BlockHist bh;
-    if (hist0) { bh.init(sh); __syncthreads(); }
-    const int dpos = plan.digit_pos[0];
-    const uint32_t dmask = (1u << plan.digit_bits[0]) - 1u;
+    if (hd >= 0) { bh.init(sh); __syncthreads(); }
+    const int dpos = plan.digit_pos[hd >= 0 ? hd : 0];
+    const uint32_t dmask = (1u << plan.digit_bits[hd >= 0 ? hd : 0]) - 1u;
     bool bad = false;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nterms; t += (int64_t)gridDim.x * blockDim.x) {
         K key;
@@ -192,25 +192,25 @@ __global__ void __launch_bounds__(256) pack_strided_kernel(ExpView ev, int64_t n
         for (int v = 0; v < plan.nvars; ++v)
             pack_field(key, load_exp(ev.base, ev.exp_bytes, t * ev.term_stride + (int64_t)v * ev.var_stride), v, plan, bad);
         keys[t] = key;
-        if (hist0) bh.add(key_digit(key, dpos, dmask));
+        if (hd >= 0) bh.add(key_digit(key, dpos, dmask));
     }
     if (bad) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
-    if (hist0) { __syncthreads(); bh.flush(ctl->hist[0]); }
+    if (hd >= 0) { __syncthreads(); bh.flush(ctl->hist[hd]); }
 }
 
 template <typename K, int ES>
 static void launch_pack_rows_es(int wb, unsigned blocks, const ExpView& ev, int64_t nterms, const Plan& plan, K* keys,
-                                Control* ctl, int hist0, cudaStream_t stream)
+                                Control* ctl, int hd, cudaStream_t stream)
 {
     const uint8_t* base = (const uint8_t*)ev.base;
-    if (wb == 16) pack_rows_kernel<K, ES, 16><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
-    else if (wb == 4) pack_rows_kernel<K, ES, 4><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
-    else if (ES <= 2 && wb == 2) pack_rows_kernel<K, ES, (ES <= 2 ? 2 : 4)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
-    else pack_rows_kernel<K, ES, (ES == 1 ? 1 : ES)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hist0);
+    if (wb == 16) pack_rows_kernel<K, ES, 16><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hd);
+    else if (wb == 4) pack_rows_kernel<K, ES, 4><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hd);
+    else if (ES <= 2 && wb == 2) pack_rows_kernel<K, ES, (ES <= 2 ? 2 : 4)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hd);
+    else pack_rows_kernel<K, ES, (ES == 1 ? 1 : ES)><<<blocks, 256, 0, stream>>>(base, nterms, plan, keys, ctl, hd);
 }
 
 template <typename K>
-static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K* keys, Control* ctl, bool hist0,
+static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K* keys, Control* ctl, int hd,
                          cudaStream_t stream)
 {
     if (nterms <= 0) return 0;
@@ -220,26 +220,54 @@ static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K*
     if (ev.row_major_contiguous) {
         const int rb = plan.nvars * ev.exp_bytes;
         const int wb = (rb % 16 == 0) ? 16 : (rb % 4 == 0) ? 4 : (rb % 2 == 0) ? 2 : 1;
-        if (ev.exp_bytes == 1) launch_pack_rows_es<K, 1>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
-        else if (ev.exp_bytes == 2) launch_pack_rows_es<K, 2>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
-        else launch_pack_rows_es<K, 4>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hist0, stream);
+        if (ev.exp_bytes == 1) launch_pack_rows_es<K, 1>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hd, stream);
+        else if (ev.exp_bytes == 2) launch_pack_rows_es<K, 2>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hd, stream);
+        else launch_pack_rows_es<K, 4>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hd, stream);
     } else {
-        pack_strided_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(ev, nterms, plan, keys, ctl, hist0 ? 1 : 0);
+        pack_strided_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(ev, nterms, plan, keys, ctl, hd);
     }
     return 1;
 }
 
-int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, bool hist0,
+int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, int hd,
                 cudaStream_t stream)
 {
-    if (plan.key_bytes == 8) return launch_pack_t<uint64_t>(ev, nterms, plan, (uint64_t*)keys, ctl, hist0, stream);
-    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)keys, ctl, hist0, stream);
+    if (plan.key_bytes == 8) return launch_pack_t<uint64_t>(ev, nterms, plan, (uint64_t*)keys, ctl, hd, stream);
+    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)keys, ctl, hd, stream);
 }
 
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
                      cudaStream_t stream)
 {
-    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)out_hilo, ctl, false, stream);   // Key128 is (hi, lo)
+    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)out_hilo, ctl, -1, stream);   // Key128 is (hi, lo)
+}
+
+// Histogram of digit `hd` over already packed keys into ctl->hist[hd] (used when the bucket path is rejected after
+// S1 and the LSD passes need the histogram of digit 0 instead).
+template <typename K>
+__global__ void __launch_bounds__(256) key_hist_kernel(const K* __restrict__ keys, int64_t n, int dpos, uint32_t dmask,
+                                                       uint32_t* hist)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    bh.init(sh);
+    __syncthreads();
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x)
+        bh.add(key_digit(keys[t], dpos, dmask));
+    __syncthreads();
+    bh.flush(hist);
+}
+
+int launch_key_hist(const Plan& plan, int hd, int64_t n, const void* keys, Control* ctl, cudaStream_t stream)
+{
+    if (n <= 0 || hd < 0 || hd >= plan.npasses) return 0;
+    int64_t blocks = (n + 256 * 8 - 1) / (256 * 8);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    const int dpos = plan.digit_pos[hd];
+    const uint32_t dmask = (1u << plan.digit_bits[hd]) - 1u;
+    if (plan.key_bytes == 8) key_hist_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)keys, n, dpos, dmask, ctl->hist[hd]);
+    else key_hist_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)keys, n, dpos, dmask, ctl->hist[hd]);
+    return 1;
 }
 
 // ----------------------------------------------------------------------------------------------- X1
@@ -249,7 +277,7 @@ __global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict_
                                                             uint32_t na, const K* __restrict__ kb,
                                                             const double* __restrict__ cb, uint32_t nb,
                                                             K* __restrict__ keys, double* __restrict__ coefs, int dpos,
-                                                            uint32_t dmask, Control* ctl)
+                                                            uint32_t dmask, uint32_t* hist)
 {
     constexpr int ITEMS = 4;
     __shared__ uint32_t sh[kRadix];
@@ -270,23 +298,24 @@ __global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict_
         }
     }
     __syncthreads();
-    bh.flush(ctl->hist[0]);
+    bh.flush(hist);
 }
 
 int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
-                         const Plan& plan, void* keys, double* coefs, Control* ctl, cudaStream_t stream)
+                         const Plan& plan, void* keys, double* coefs, Control* ctl, int hd, cudaStream_t stream)
 {
     const int64_t n = na * nb;
     if (n <= 0) return 0;
     const unsigned blocks = (unsigned)((n + 1023) / 1024);
-    const int dpos = plan.npasses ? plan.digit_pos[0] : 0;
-    const uint32_t dmask = plan.npasses ? (1u << plan.digit_bits[0]) - 1u : 0u;
+    if (hd < 0 || hd >= plan.npasses) hd = 0;
+    const int dpos = plan.npasses ? plan.digit_pos[hd] : 0;
+    const uint32_t dmask = plan.npasses ? (1u << plan.digit_bits[hd]) - 1u : 0u;
     if (plan.key_bytes == 8)
         expand_packed_kernel<uint64_t><<<blocks, 256, 0, stream>>>((const uint64_t*)ka, ca, (uint32_t)na, (const uint64_t*)kb,
-                                                                   cb, (uint32_t)nb, (uint64_t*)keys, coefs, dpos, dmask, ctl);
+                                                                   cb, (uint32_t)nb, (uint64_t*)keys, coefs, dpos, dmask, ctl->hist[hd]);
     else
         expand_packed_kernel<Key128><<<blocks, 256, 0, stream>>>((const Key128*)ka, ca, (uint32_t)na, (const Key128*)kb, cb,
-                                                                 (uint32_t)nb, (Key128*)keys, coefs, dpos, dmask, ctl);
+                                                                 (uint32_t)nb, (Key128*)keys, coefs, dpos, dmask, ctl->hist[hd]);
     return 1;
 }
 

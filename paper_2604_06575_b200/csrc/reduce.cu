@@ -14,18 +14,6 @@ namespace polylab {
 
 // ----------------------------------------------------------------------------------------------- S3
 
-struct SegPair {          // (any head seen, sum since the last head)
-    uint32_t f;
-    double v;
-};
-__device__ __forceinline__ SegPair seg_combine(const SegPair& l, const SegPair& r)
-{
-    SegPair o;
-    o.f = l.f | r.f;
-    o.v = r.f ? r.v : __dadd_rn(l.v, r.v);
-    return o;
-}
-
 template <typename K, int THREADS, int ITEMS>
 __global__ void __launch_bounds__(THREADS)
 reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint32_t n, K* __restrict__ ukeys,

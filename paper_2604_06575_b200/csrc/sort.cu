@@ -253,24 +253,24 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 }
 
 template <typename K, int ITEMS, int MINB>
-static int launch_sort_pass_t(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in,
-                              void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                              bool debug_unstable, cudaStream_t stream)
+static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in,
+                              const double* coef_in, void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl,
+                              bool safe_rank, bool debug_unstable, cudaStream_t stream)
 {
     using S = SortSmem<K, kSortThreads, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
-    const bool has_next = pass + 1 < plan.npasses;
+    const bool has_next = next >= 0;
     PassArgs a;
     a.keys_in = keys_in; a.coef_in = coef_in; a.keys_out = keys_out; a.coef_out = coef_out;
     a.n = (uint32_t)n;
     a.dword = plan.digit_pos[pass] >> 5; a.dshift = plan.digit_pos[pass] & 31; a.dmask = (1u << plan.digit_bits[pass]) - 1u;
-    a.nword = has_next ? plan.digit_pos[pass + 1] >> 5 : 0;
-    a.nshift = has_next ? plan.digit_pos[pass + 1] & 31 : 0;
-    a.nmask = has_next ? (1u << plan.digit_bits[pass + 1]) - 1u : 0u;
+    a.nword = has_next ? plan.digit_pos[next] >> 5 : 0;
+    a.nshift = has_next ? plan.digit_pos[next] & 31 : 0;
+    a.nmask = has_next ? (1u << plan.digit_bits[next]) - 1u : 0u;
     a.tile_state = tile_state;
-    a.flag_partial = (pass & 1) ? 3u : 1u;                 // flag parity: no re-zeroing between passes
-    a.flag_inclusive = (pass & 1) ? 0u : 2u;
-    a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[pass + 1]; a.ticket = &ctl->ticket[pass];
+    a.flag_partial = (seq & 1) ? 3u : 1u;                  // flag parity: no re-zeroing between passes
+    a.flag_inclusive = (seq & 1) ? 0u : 2u;
+    a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[has_next ? next : kMaxPasses]; a.ticket = &ctl->ticket[seq];
     a.reverse_lanes = debug_unstable ? 1 : 0;
     if (safe_rank) {
         if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, false>(a, tiles, stream);
@@ -282,16 +282,16 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int64_t n, const void*
     return 1;
 }
 
-int launch_sort_pass(const Plan& plan, int pass, int64_t n, const void* keys_in, const double* coef_in, void* keys_out,
-                     double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank, bool debug_unstable,
-                     cudaStream_t stream)
+int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
+                     void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
+                     bool debug_unstable, cudaStream_t stream)
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
-        return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, n, keys_in, coef_in, keys_out, coef_out, tile_state,
-                                                             ctl, safe_rank, debug_unstable, stream);
-    return launch_sort_pass_t<Key128, kSortItems128, 3>(plan, pass, n, keys_in, coef_in, keys_out, coef_out, tile_state, ctl,
-                                                        safe_rank, debug_unstable, stream);
+        return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+                                                             tile_state, ctl, safe_rank, debug_unstable, stream);
+    return launch_sort_pass_t<Key128, kSortItems128, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+                                                        tile_state, ctl, safe_rank, debug_unstable, stream);
 }
 
 }  // namespace polylab

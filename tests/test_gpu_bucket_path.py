@@ -1,0 +1,152 @@
+"""-m gpu: the bucket path of the CUDA library (csrc/finish.cu: partition on the most significant digits, finish every
+bucket in shared memory, fused segmented sum / prune / unpack) against the CPU oracle under the same parity rule, its
+self-checks and its fallbacks.  POLYLAB_FLAG_DEBUG_FORCE_BUCKET lets small inputs reach the path."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2604_06575_b200 import binding as B
+from paper_2604_06575_b200 import workloads as W
+from gpu_util import assert_parity, dev
+
+pytestmark = pytest.mark.gpu
+
+FORCE = B.FLAG_DEBUG_FORCE_BUCKET
+
+
+def run(p, tol, flags=0, **kw):
+    c, e, st = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=flags, **kw)
+    torch.cuda.synchronize()
+    return c.cpu().numpy(), e.cpu().numpy(), st
+
+
+def pooled(n, nvars, dup, seed, hi=256, dtype=np.uint8):
+    """n terms drawn from a pool of n/dup uniform monomials (config 5's structure, any width), coef N(0,1)."""
+    r = np.random.default_rng(seed)
+    pool = r.integers(0, hi, size=(n // dup, nvars)).astype(dtype)
+    exps = pool[r.permutation(n) // dup]
+    return W.Poly(r.standard_normal(n), np.ascontiguousarray(exps))
+
+
+def test_config5_takes_the_bucket_path_by_default():
+    """2e6 terms of config 5: 16 digits, 2 prefix passes, then the finish; same answer as the LSD path."""
+    p, tol = W.config5(2_000_000)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    assert st.prefix_passes == 2 and st.sort_passes == 2 and st.bucket_fallback == 0 and st.rank_fallback == 0
+    assert st.distinct == 200_000 and st.survivors == 100_000 == len(c)
+    assert_parity(res, c, e)
+    c1, e1, st1 = run(p, tol, flags=B.FLAG_NO_BUCKET)
+    assert st1.prefix_passes == 0 and st1.sort_passes == 16
+    assert_parity(res, c1, e1)
+    assert (e == e1).all()
+    c2, e2, _ = run(p, tol)                                 # bit-reproducible run to run
+    assert (c.view(np.uint64) == c2.view(np.uint64)).all() and (e == e2).all()
+
+
+@pytest.mark.parametrize("n", [20, 10_000, 100_000, 300_000])
+def test_forced_bucket_path_small_config5(n):
+    p, tol = W.config5(n)
+    c, e, st = run(p, tol, flags=FORCE)
+    assert st.prefix_passes >= 1 and st.bucket_fallback == 0
+    assert len(c) == n // 20
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+
+
+def test_fast_digit_list_too_short_is_detected_and_resorted():
+    """With one fast digit (8 bits below the prefix) most tiles hold distinct keys that agree on it: the order check
+    must catch them and the tile must re-sort on every low digit."""
+    p, tol = W.config5(300_000)
+    c, e, st = run(p, tol, flags=FORCE | (1 << B.FLAG_DEBUG_NFAST_SHIFT))
+    assert st.prefix_passes == 1 and st.refinish_tiles > 0 and st.rank_fallback == 0
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+    c3, e3, st3 = run(p, tol, flags=FORCE)                  # default list: no tile needs it here
+    assert st3.refinish_tiles == 0
+    assert (e == e3).all() and (c.view(np.uint64) == c3.view(np.uint64)).all()
+
+
+def test_skewed_prefix_overflows_and_falls_back_to_lsd():
+    """Config 3's leading variables are mostly zero: one bucket holds a large share of the terms, does not fit a
+    tile, and the call must re-run on the LSD path with the same result."""
+    p, tol = W.config3(300_000)
+    c, e, st = run(p, tol, flags=FORCE)
+    assert st.bucket_fallback == 1 and st.prefix_passes == 0 and st.sort_passes == 4
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+
+
+def test_skewed_prefix_is_rejected_by_the_histogram_precheck():
+    """Default flags, 1.2e6 terms of config 3u (110-bit keys): the first prefix digit's histogram is far from flat, so
+    the bucket path is dropped before any pass runs."""
+    p, tol = W.config3u(1_200_000)
+    c, e, st = run(p, tol)
+    assert st.key_bits == 110 and st.bucket_fallback == 1 and st.prefix_passes == 0 and st.sort_passes == 14
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+
+
+def test_64_bit_keys_default_bucket_path():
+    p = pooled(1_200_000, 8, 4, seed=11)
+    c, e, st = run(p, 0.0)
+    assert st.key_bytes == 8 and st.prefix_passes == 2 and st.bucket_fallback == 0
+    assert len(c) == st.distinct
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_72_bit_keys_prefix_digit_in_its_own_word():
+    """9 variables of 8 bits: the top digit sits alone in the third 32-bit word of the key."""
+    p = pooled(200_000, 9, 5, seed=12)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.key_bits == 72 and st.key_bytes == 16 and st.prefix_passes == 1
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+@pytest.mark.parametrize("n", [1, 2, 33, 3000, 3584])
+def test_forced_one_bucket_of_equal_keys(n):
+    """All terms share one monomial: one bucket, one run, inside one finish tile."""
+    r = np.random.default_rng(n)
+    p = W.Poly(r.standard_normal(n), np.tile(np.array([[200, 3, 0, 77, 1, 2, 3, 4, 5]], np.uint8), (n, 1)))
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.prefix_passes >= 1 and st.bucket_fallback == 0 and len(c) == 1
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_forced_one_bucket_too_long_falls_back():
+    n = 20_000
+    r = np.random.default_rng(5)
+    exps = np.tile(np.array([[9, 9, 9, 9, 9]], np.uint8), (n, 1))
+    exps[:, 4] = r.integers(0, 256, n)                      # same prefix, 256 monomials
+    p = W.Poly(r.standard_normal(n), exps)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.bucket_fallback == 1 and len(c) == 256
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_forced_all_distinct_and_many_tiny_buckets():
+    """Every term its own monomial, three prefix passes' worth of tiny buckets inside each tile (ordinal passes > 1)."""
+    n = 100_003
+    r = np.random.default_rng(7)
+    exps = r.integers(0, 256, size=(n, 12)).astype(np.uint8)
+    p = W.Poly(r.standard_normal(n), exps)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.prefix_passes >= 1 and len(c) == len(np.unique(exps, axis=0))
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_bucket_path_prune_capacity_and_p_minus_p():
+    p, tol = W.config5(200_000)
+    with pytest.raises(B.PolylabError) as ei:
+        B.simplify(dev(p.coef), dev(p.exps), tol, out_capacity=100, flags=FORCE)
+    assert ei.value.status == B.ERR_OUTPUT_TOO_SMALL
+    q = W.Poly(np.concatenate([p.coef, -p.coef]), np.concatenate([p.exps, p.exps]))
+    c, e, st = run(q, 1e-12, flags=FORCE)
+    assert st.prefix_passes >= 1 and len(c) == 0
+
+
+def test_bucket_path_mul_simplify():
+    """Product of two 1100-term polynomials over 8 variables with exponents up to 127: 1.21e6 products, 64-bit keys."""
+    r = np.random.default_rng(21)
+    a = W.Poly(r.standard_normal(1100), r.integers(0, 128, size=(1100, 8)).astype(np.uint8))
+    b = W.Poly(r.standard_normal(1100), r.integers(0, 128, size=(1100, 8)).astype(np.uint8))
+    c, e, st = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), 0.0, return_stats=True)
+    assert st.prefix_passes >= 1 and st.bucket_fallback == 0
+    assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, 0.0), c.cpu().numpy(), e.cpu().numpy())
