@@ -217,7 +217,7 @@ static int choose_prefix_passes(const Plan& plan, int64_t n, const Opts& o, cons
     if (P < 1 || (!force && (P < 4 || n < (1 << 20)))) return 0;
     for (int k = 1; k <= P; ++k) {
         const int T = plan.key_bits - plan.digit_pos[P - k];
-        if (T >= 40 || (n >> T) < kFinCap - 3584) return (force || P - k >= 3) ? k : 0;
+        if (T >= 40 || (n >> T) < kFinMaxMeanBucket) return (force || P - k >= 3) ? k : 0;
     }
     return 0;
 }

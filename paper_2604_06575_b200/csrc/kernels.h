@@ -16,10 +16,12 @@ constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from sha
 constexpr int kPruneThreads = 256;
 constexpr int kPruneItems = 8;
 
-constexpr int kFinThreads = 512;    // bucket path (finish.cu): one block per SM
-constexpr int kFinCap = 6656;       // most records a finish tile can own (shared memory); tile t owns the buckets that start
-                                    // in positions [t*fin_tile, (t+1)*fin_tile), a bucket may be as long as kFinCap - fin_tile
-constexpr int kFinMinTile = 2560;   // smallest fin_tile the planner picks (workspace sizing)
+constexpr int kFinThreads = 512;    // bucket path (finish.cu): two blocks per SM
+constexpr int kFinCap = 8192;       // most records a finish tile can own (10 bytes of shared memory each); tile t owns the
+                                    // buckets that start in positions [t*fin_tile, (t+1)*fin_tile), so a bucket may be
+                                    // as long as kFinCap - fin_tile
+constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
+constexpr int kFinMinTile = 4096;   // smallest fin_tile the planner picks (workspace sizing)
 
 inline int sort_tile(int key_bytes) { return kSortThreads * (key_bytes == 8 ? kSortItems64 : kSortItems128); }
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
