@@ -136,7 +136,7 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.red_state = take(red_tiles * sizeof(uint32_t));
     L.prune_state = take(prune_tiles * sizeof(uint32_t));
     const size_t fin_tiles = (size_t)((n + kFinMinTile - 1) / kFinMinTile);
-    L.fin_state = take(fin_tiles * sizeof(uint32_t));
+    L.fin_state = take((fin_tiles + 1) * sizeof(uint32_t));
     L.zero_end = off;                                   // everything before this is zeroed per call
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.red_heads = take(red_tiles * sizeof(uint32_t));
@@ -284,7 +284,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
     }
     tm.mark(POLYLAB_STAGE_SORT);
-    *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol, out_coef, out_exps, o.exp_bytes,
+    *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol, kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes,
                                out_capacity, (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), ctl, nullptr, stream);
     tm.mark(POLYLAB_STAGE_REDUCE);
     tm.mark(POLYLAB_STAGE_PRUNE);

@@ -17,10 +17,15 @@
 //                        passes, one shared-memory atomic per record and sweep) and then by bucket ordinal, gathers
 //                        keys and coefficients through the permutation (they were just streamed, so the gather hits
 //                        L2), and -- records of equal monomials now being adjacent and no run crossing a tile -- does
-//                        the segmented sum (S3), the prune (S4, keep iff |s| > tol, reading A2), the order-preserving
-//                        compaction (look-back over the tiles' survivor counts) and the unpack (S5) straight into the
-//                        caller's output.  HBM traffic: N*(W+8) read, U'*(8+E) written; two blocks per SM overlap one
-//                        tile's loads with the other's shared-memory passes.
+//                        the segmented sum (S3) and the prune (S4, keep iff |s| > tol, reading A2) and leaves the
+//                        tile's survivors compacted in order at the tile's own position.  Tiles are independent (no
+//                        look-back: a tile only knows its count at the very end, and waiting in order for slow
+//                        predecessors left SMs idle); two blocks per SM overlap one tile's loads with the other's
+//                        shared-memory passes.
+//   tile_scan_kernel     exclusive scan of the tiles' survivor counts (one block).
+//   emit_kernel          S5: one thread per output term finds its tile in the scanned counts (binary search) and
+//                        unpacks the key into the caller's output -- order-preserving compaction across tiles.
+//                        HBM traffic of the three: N*(W+8) read, U'*(W+8) written and read, U'*(8+E) written.
 //
 // The local sort first uses only the `nfast` most significant digits below the prefix (enough to separate the
 // distinct keys of a bucket unless two of them share all those bits) and checks the order against the full keys while
@@ -152,19 +157,27 @@ struct FinishArgs {
     int nlow;                       // plan digits below the prefix: digits [0, nlow)
     int nfast;                      // how many of them (the most significant ones) the first attempt sorts on
     double tol;
+    void* ukeys;                    // survivors of tile t, compacted in order: (ukeys, usums)[tile_start[t] + q], q < tile_state[t]
+    double* usums;
+    Control* ctl;
+};
+
+struct EmitArgs {
+    const void* ukeys;
+    const double* usums;
+    uint32_t ntiles;
+    const uint32_t* tile_start;     // [ntiles + 1]
+    const uint32_t* tile_off;       // [ntiles + 1] exclusive scan of the tiles' survivor counts; [ntiles] = U'
     double* out_coef;
     void* out_exps;
     int exp_bytes;
     int words_u8;                   // out_exps may be written as 32-bit words of four u8 exponents
     int64_t out_capacity;
-    Control* ctl;
-    int64_t* out_count_device;
 };
 
 template <typename K>
-__device__ __forceinline__ void emit_term(const FinishArgs& a, const Plan& plan, uint64_t o, double s, const K& kk)
+__device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, uint64_t o, double s, const K& kk)
 {
-    if ((int64_t)o >= a.out_capacity) return;
     a.out_coef[o] = s;
     if (a.words_u8) {
         uint32_t* row = (uint32_t*)a.out_exps + o * (uint64_t)(plan.nvars >> 2);
@@ -366,16 +379,12 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
     uint32_t tile_keep;
     const uint32_t kexcl = block_exclusive_scan<THREADS>(nkeep + (last_keep ? 1u : 0u), scratch, &tile_keep);
-    if (warp == 0) {
-        const uint32_t r = warp_lookback_u32(a.tile_state, tile, tile_keep);
-        if (lane == 0) scratch[41] = r;
-    }
-    __syncthreads();
-    const uint32_t base = scratch[41];
 
-    // ---- S5: write the survivors in order
+    // ---- the tile's survivors, compacted in order at the tile's own place; S5 (emit_kernel) puts the tiles together
     {
-        uint64_t o = (uint64_t)base + kexcl;
+        K* __restrict__ uk = (K*)a.ukeys + lo;
+        double* __restrict__ us = a.usums + lo;
+        uint32_t o = kexcl;
         uint32_t k = 0;
         double a2 = 0.0;
         for (uint32_t j = 0; j < itn; ++j) {
@@ -384,8 +393,8 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                 if (hm & (1u << j)) {
                     if (first + j > 0) {
                         if (keep & (1u << k)) {
-                            const double total = (k == 0) ? __dadd_rn(carry.v, a2) : a2;
-                            emit_term<K>(a, plan, o, total, gkeys[py[first + j - 1]]);
+                            us[o] = (k == 0) ? __dadd_rn(carry.v, a2) : a2;
+                            uk[o] = gkeys[py[first + j - 1]];
                             ++o;
                         }
                         ++k;
@@ -394,16 +403,71 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                 } else a2 = __dadd_rn(a2, c);
             }
         }
-        if (last_keep) emit_term<K>(a, plan, o, incl.v, gkeys[py[n_loc - 1]]);
+        if (last_keep) { us[o] = incl.v; uk[o] = gkeys[py[n_loc - 1]]; }
     }
     {
         uint32_t tot_heads;                        // distinct monomials of the tile, for the statistics
         (void)block_exclusive_scan<THREADS>(nh, scratch, &tot_heads);
-        if (tid == 0 && tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);
+        if (tid == 0) {
+            if (tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);
+            a.tile_state[tile] = tile_keep;
+        }
     }
-    if (tile == a.ntiles - 1 && tid == 0) {
-        a.ctl->survivors = base + tile_keep;
-        if (a.out_count_device) *a.out_count_device = (int64_t)(base + tile_keep);
+}
+
+// ------------------------------------------------------------------------------- S4/S5 across tiles
+
+// Exclusive scan of the tiles' survivor counts, in place (one block); tile_off[ntiles] = U'.
+__global__ void __launch_bounds__(1024) tile_scan_kernel(uint32_t* __restrict__ tile_off, uint32_t ntiles, Control* ctl,
+                                                         int64_t* out_count_device)
+{
+    __shared__ uint32_t scratch[34];
+    __shared__ uint32_t running;
+    const unsigned tid = threadIdx.x;
+    if (tid == 0) running = 0u;
+    __syncthreads();
+    for (uint32_t base = 0; base < ntiles; base += 1024u * 4u) {
+        uint32_t v[4], sum = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t t = base + tid * 4u + j;
+            v[j] = t < ntiles ? tile_off[t] : 0u;
+            sum += v[j];
+        }
+        uint32_t total;
+        uint32_t excl = block_exclusive_scan<1024>(sum, scratch, &total) + running;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t t = base + tid * 4u + j;
+            if (t < ntiles) tile_off[t] = excl;
+            excl += v[j];
+        }
+        __syncthreads();
+        if (tid == 0) running += total;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        tile_off[ntiles] = running;
+        ctl->survivors = running;
+        if (out_count_device) *out_count_device = (int64_t)running;
+    }
+}
+
+// One thread per output term: find its tile in the scanned counts, fetch (key, sum), unpack (S5).
+template <typename K>
+__global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitArgs a, const __grid_constant__ Plan plan)
+{
+    const uint32_t total = a.tile_off[a.ntiles];
+    const uint64_t limit = min((uint64_t)total, (uint64_t)a.out_capacity);
+    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < limit; o += (uint64_t)gridDim.x * blockDim.x) {
+        uint32_t lo = 0, hi = a.ntiles;            // last tile t with tile_off[t] <= o
+        while (hi - lo > 1) {
+            const uint32_t mid = lo + (hi - lo) / 2;
+            if (a.tile_off[mid] <= (uint32_t)o) lo = mid;
+            else hi = mid;
+        }
+        const uint64_t src = (uint64_t)a.tile_start[lo] + ((uint32_t)o - a.tile_off[lo]);
+        emit_term<K>(a, plan, o, a.usums[src], ((const K*)a.ukeys)[src]);
     }
 }
 
@@ -411,8 +475,8 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
 
 template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
-                           const double* coefs, double tol, double* out_coef, void* out_exps, int exp_bytes,
-                           int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, Control* ctl,
+                           const double* coefs, double tol, void* ukeys, double* usums, double* out_coef, void* out_exps,
+                           int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, Control* ctl,
                            int64_t* out_count_device, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
@@ -430,24 +494,31 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     FinishArgs a;
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state;
-    a.pfx_pos = pfx_pos; a.nlow = nlow; a.nfast = nfast; a.tol = tol; a.out_coef = out_coef; a.out_exps = out_exps;
-    a.exp_bytes = exp_bytes;
-    a.words_u8 = (exp_bytes == 1 && (plan.nvars & 3) == 0 && ((uintptr_t)out_exps & 3) == 0) ? 1 : 0;
-    a.out_capacity = out_capacity; a.ctl = ctl; a.out_count_device = out_count_device;
+    a.pfx_pos = pfx_pos; a.nlow = nlow; a.nfast = nfast; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
     kern<<<ntiles, kFinThreads, smem, stream>>>(a, plan);
-    return 2;
+    tile_scan_kernel<<<1, 1024, 0, stream>>>(tile_state, ntiles, ctl, out_count_device);
+    EmitArgs e;
+    e.ukeys = ukeys; e.usums = usums; e.ntiles = ntiles; e.tile_start = tile_start; e.tile_off = tile_state;
+    e.out_coef = out_coef; e.out_exps = out_exps; e.exp_bytes = exp_bytes;
+    e.words_u8 = (exp_bytes == 1 && (plan.nvars & 3) == 0 && ((uintptr_t)out_exps & 3) == 0) ? 1 : 0;
+    e.out_capacity = out_capacity;
+    int64_t blocks = (n / 4 + 255) / 256;          // at most N outputs; grid-stride
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks < 1) blocks = 1;
+    emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
+    return 4;
 }
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
-                  double tol, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_start,
-                  uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaStream_t stream)
+                  double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
+                  uint32_t* tile_start, uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;
     if (plan.key_bytes == 8)
-        return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, out_coef, out_exps, exp_bytes,
-                                         out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
-    return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, out_coef, out_exps, exp_bytes,
-                                   out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
+        return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
+                                         exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
+    return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
+                                   exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
 }
 
 }  // namespace polylab
