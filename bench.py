@@ -10,8 +10,9 @@ north_star's roofline target is quoted on.  Prints ONE JSON line (rank 0).
 
   value     input terms/s, whole job, inputs resident in HBM, CUDA events around K calls of the C ABI
   e2e       the same metric through polylab_simplify_host: pinned host buffers, H2D and D2H inside the call
-  roofline  the radix-sort pass kernel (dominant): algorithmic bytes 2*N*(W+8) per launch / mean launch time,
-            timed live with the library's CUDA events on the call's stream (POLYLAB_FLAG_TIMING)
+  roofline  the longest kernel of the step, timed live with the library's CUDA events on the call's stream
+            (POLYLAB_FLAG_TIMING): on the bucket path the finish kernel (N*(W+8) read + U'*(W+8) written), on the LSD
+            path one radix pass (2*N*(W+8)); the radix pass and the sort+reduce pipeline are reported beside it
   cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same recipe (rank 0, N=1 only)
 
 --impl reference times the oracle alone (there is no reference implementation to install: the paper's
@@ -170,6 +171,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-bucket", action="store_true", help="POLYLAB_FLAG_NO_BUCKET: force the plain LSD path (A/B)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -196,18 +198,20 @@ def main():
     ws = B.Workspace(torch.device("cuda", local_rank))
     stats_log = []
 
+    xflags = B.FLAG_NO_BUCKET if args.no_bucket else 0
+
     def step_device():
         if kind == "simplify":
-            c, e, st = B.simplify(*dpolys[0], tol, workspace=ws, out=outbuf, return_stats=True, timing=True)
+            c, e, st = B.simplify(*dpolys[0], tol, workspace=ws, out=outbuf, return_stats=True, timing=True, flags=xflags)
             stats_log.append(st)
             return c.shape[0]
         if kind == "mul":
-            c, e, st = B.mul_simplify(*dpolys[0], *dpolys[1], tol, workspace=ws, return_stats=True, timing=True)
+            c, e, st = B.mul_simplify(*dpolys[0], *dpolys[1], tol, workspace=ws, return_stats=True, timing=True, flags=xflags)
             stats_log.append(st)
             return c.shape[0]
         pc, pe = dpolys[0]
         rc, re_ = B.expand(pc, pe, pc, pe)
-        c, e, st = B.mul_simplify(rc, re_, pc, pe, tol, workspace=ws, return_stats=True, timing=True)
+        c, e, st = B.mul_simplify(rc, re_, pc, pe, tol, workspace=ws, return_stats=True, timing=True, flags=xflags)
         stats_log.append(st)
         return c.shape[0]
 
@@ -250,24 +254,47 @@ def main():
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
     st = stats_log[-1]
     P, Wb = st.sort_passes, st.key_bytes
-    sort_ms = statistics.mean(s.stage_ms["sort"] for s in stats_log)
-    pass_ms = sort_ms / P if P else float("nan")
-    pass_bytes = 2.0 * st.sort_terms * (Wb + 8)
-    achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if P else 0.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"config{args.config}", {}).get("sort_pass_dram_bytes_per_launch")
+    S = Wb + 8
+    N, U, U1 = st.sort_terms, st.distinct, st.survivors
     stage_ms = {k: statistics.mean(s.stage_ms[k] for s in stats_log) for k in B.STAGES}
+    pass_ms = stage_ms["sort"] / P if P else float("nan")
+    pass_bytes = 2.0 * N * S
+    pass_gbs = pass_bytes / (pass_ms * 1e-3) / 1e9 if P else 0.0
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tinfo = json.load(open(tpath)).get(f"config{args.config}", {}) if os.path.exists(tpath) else {}
+    # what an LSD sort of the same keys plus the segmented sum must move: ceil(B/8) passes + one read + U records
+    lsd_digits = len(st.digit_bits)
+    lsd_bytes = lsd_digits * pass_bytes + N * S + U * S
     sr_ms = stage_ms["sort"] + stage_ms["reduce"]
-    sr_bytes = P * pass_bytes + st.sort_terms * (Wb + 8) + st.distinct * (Wb + 8)
-    roofline = {"bound": "hbm", "kernel": "sort_pass_kernel (one LSD radix pass, 8-bit digit)", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": pass_bytes, "launch_ms": pass_ms, "launches_per_step": P,
-                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                "sort_plus_reduce": {"ms": sr_ms, "algorithmic_bytes": sr_bytes, "GBps": sr_bytes / (sr_ms * 1e-3) / 1e9,
-                                     "frac": sr_bytes / (sr_ms * 1e-3) / 1e9 / peak},
-                "stage_ms": stage_ms}
+    pass_info = {"kernel": "sort_pass_kernel (one radix pass, 8-bit digit)", "launch_ms": pass_ms, "launches_per_step": P,
+                 "algorithmic_bytes_per_launch": pass_bytes, "achieved": pass_gbs, "frac": pass_gbs / peak,
+                 "traffic": tinfo.get("sort_pass_dram_bytes_per_launch")}
+    if st.prefix_passes > 0:
+        # bucket path: the finish kernel is the longest kernel of the step; it reads every pair once and writes the survivors
+        fin_ms = stage_ms["reduce"]
+        fin_bytes = float(N * S + U1 * S)
+        achieved = fin_bytes / (fin_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "finish_kernel (bucket path: shared-memory sort of each bucket + segmented sum + prune)",
+                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "traffic": tinfo.get("finish_dram_bytes_per_launch"), "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": fin_bytes, "launch_ms": fin_ms, "launches_per_step": 1,
+                    "limiter": "shared-memory / LSU pipe, not DRAM (ncu, profiles/): the kernel trades HBM passes for on-chip work",
+                    "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+    else:
+        roofline = {"bound": "hbm", "kernel": pass_info["kernel"], "achieved": pass_gbs, "peak": peak, "unit": "GB/s",
+                    "frac": pass_gbs / peak if peak else None, "traffic": pass_info["traffic"], "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": pass_bytes, "launch_ms": pass_ms, "launches_per_step": P,
+                    "frac_of_nominal_8TBs": pass_gbs / NOMINAL_HBM_GBS}
+    roofline["radix_pass"] = pass_info
+    # the north_star's pipeline figure: bytes an LSD sort + segmented sum of these keys must move / time of sort + reduce stages
+    roofline["sort_plus_reduce"] = {"ms": sr_ms, "lsd_algorithmic_bytes": lsd_bytes, "lsd_passes": lsd_digits,
+                                    "GBps_equivalent": lsd_bytes / (sr_ms * 1e-3) / 1e9,
+                                    "frac_of_peak": lsd_bytes / (sr_ms * 1e-3) / 1e9 / peak,
+                                    "frac_of_nominal_8TBs": lsd_bytes / (sr_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+                                    "note": "above 1.0 means the call beats the roofline of the LSD method by moving fewer bytes "
+                                            "(bucket path: %d passes over HBM instead of %d)" % (P, lsd_digits)}
+    roofline["stage_ms"] = stage_ms
+    roofline["path"] = "bucket" if st.prefix_passes > 0 else "lsd"
 
     # ---- end to end: host buffers, copies inside the C call
     e2e = None
@@ -318,7 +345,8 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": desc, "sort_terms_per_step": n_sort, "distinct": st.distinct, "survivors": int(n_out),
-                       "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "digit_bits": st.digit_bits,
+                       "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "prefix_passes": st.prefix_passes,
+                       "bucket_fallback": st.bucket_fallback, "refinish_tiles": st.refinish_tiles, "digit_bits": st.digit_bits,
                        "parallelism": f"replicas x{world} (no collective on the path)",
                        "l2": "inputs and workspace are far larger than the 126 MB L2" if n_sort * (Wb + 8) > 4e8 else
                              "working set fits L2 (no flush between steps; launch-latency bound)"},

@@ -110,7 +110,8 @@ typedef struct polylab_stats {
     int32_t rank_fallback;   /* 1 if the sorted-order check failed and the call re-ran with SAFE_RANK */
     float stage_ms[8];       /* with POLYLAB_FLAG_TIMING: device time of S0 (incl. read-back), S1 (+X1),
                                 S2 (all passes), S3, S4+S5; CUDA events on the call's stream.  On the bucket
-                                path S2 = the prefix passes and S3 = the fused finish (local sort + S3 + S4 + S5) */
+                                path S2 = the prefix passes, S3 = tile bounds + the finish kernel (local sort, S3, S4 per tile)
+                                and S4+S5 = the count scan + the emit/unpack kernel */
     int32_t prefix_passes;   /* > 0: the bucket path ran with this many prefix passes (then sort_passes == prefix_passes) */
     int32_t bucket_fallback; /* 1 if the bucket path was planned and abandoned (skewed digit histogram or a bucket
                                 too long for a tile); the result then comes from the LSD path */

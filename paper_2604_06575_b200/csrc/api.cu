@@ -284,9 +284,10 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
     }
     tm.mark(POLYLAB_STAGE_SORT);
-    *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol, kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes,
-                               out_capacity, (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), ctl, nullptr, stream);
-    tm.mark(POLYLAB_STAGE_REDUCE);
+    *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
+                               kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes, out_capacity,
+                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), ctl, nullptr,
+                               tm.on ? tm.ev[POLYLAB_STAGE_REDUCE + 1] : nullptr, stream);      // REDUCE = tiles, PRUNE = scan + emit
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
     if (o.stats) o.stats->kernel_launches += *launches;

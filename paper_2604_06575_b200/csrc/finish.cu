@@ -477,7 +477,7 @@ template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
                            const double* coefs, double tol, void* ukeys, double* usums, double* out_coef, void* out_exps,
                            int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, Control* ctl,
-                           int64_t* out_count_device, cudaStream_t stream)
+                           int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
     const int nlow = plan.npasses - prefix_passes;
@@ -496,6 +496,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     a.tile_start = tile_start; a.tile_state = tile_state;
     a.pfx_pos = pfx_pos; a.nlow = nlow; a.nfast = nfast; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
     kern<<<ntiles, kFinThreads, smem, stream>>>(a, plan);
+    if (after_tiles) cudaEventRecord(after_tiles, stream);
     tile_scan_kernel<<<1, 1024, 0, stream>>>(tile_state, ntiles, ctl, out_count_device);
     EmitArgs e;
     e.ukeys = ukeys; e.usums = usums; e.ntiles = ntiles; e.tile_start = tile_start; e.tile_off = tile_state;
@@ -511,14 +512,15 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaStream_t stream)
+                  uint32_t* tile_start, uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles,
+                  cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;
     if (plan.key_bytes == 8)
         return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                         exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
+                                         exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, after_tiles, stream);
     return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                   exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, stream);
+                                   exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, after_tiles, stream);
 }
 
 }  // namespace polylab
