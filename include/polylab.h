@@ -84,6 +84,9 @@ enum {
                                         (stats->prefix_passes > 0); otherwise (stats->bucket_fallback = 1) it runs the
                                         LSD passes.  Both paths give the same result up to summation order.  Not
                                         taken with POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
+    POLYLAB_FLAG_NO_FUSED_PACK = 16u, /* bucket path: always run S1 as its own kernel.  By default, when the exponent rows
+                                        are contiguous and 8 or 16 bytes long, the first radix pass packs the keys in
+                                        registers (no key array is written and re-read) */
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
                                         skew pre-check), so that small tests reach it and its overflow fallback */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose

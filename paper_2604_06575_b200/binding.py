@@ -27,6 +27,7 @@ FLAG_DEVICE_COUNT = 1
 FLAG_TIMING = 2
 FLAG_SAFE_RANK = 4
 FLAG_NO_BUCKET = 8
+FLAG_NO_FUSED_PACK = 16
 FLAG_DEBUG_FORCE_BUCKET = 0x20000000
 FLAG_DEBUG_UNSTABLE = 0x40000000
 FLAG_DEBUG_NFAST_SHIFT = 8

@@ -243,9 +243,10 @@ static int fast_digits(const Opts& o)
 // After S1/X1 accumulated the histogram of the first prefix digit: do its bins predict buckets that fit a tile?
 // (A necessary test only; tile_bounds_kernel has the last word.)  On rejection the LSD path needs digit 0's histogram.
 static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* ws, const Layout& L, const Opts& o,
-                           int* launches, cudaStream_t stream)
+                           int* launches, cudaStream_t stream, const ExpView* unpacked = nullptr)
 {
     if (*k == 0 || (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET)) return POLYLAB_OK;
+    // (the rejection branch below is the only one that needs `unpacked`)
     Control* ctl = (Control*)(ws + L.control);
     const int P = plan.npasses, d = P - *k;
     uint32_t h[kRadix];
@@ -258,7 +259,8 @@ static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* w
     *k = 0;
     if (o.stats) o.stats->bucket_fallback = 1;
     PL_CUDA(cudaMemsetAsync(ctl->hist[d], 0, sizeof h, stream));
-    *launches += launch_key_hist(plan, 0, n, ws + L.keys[0], ctl, stream);
+    if (unpacked) *launches += launch_pack(*unpacked, n, plan, ws + L.keys[0], ctl, 0, stream);   // S1 had been left to the first pass
+    else *launches += launch_key_hist(plan, 0, n, ws + L.keys[0], ctl, stream);
     return POLYLAB_OK;
 }
 
@@ -271,7 +273,7 @@ struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overfl
 // histogram of digit P-k is in ctl->hist[P-k].
 static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
-                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream)
+                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream, const ExpView* rows)
 {
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
@@ -281,7 +283,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
         const double* cin = (s == 0) ? coef0 : cbuf[s & 1];
         *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
                                       cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
-                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
+                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr);
     }
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
@@ -308,11 +310,12 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
 
 static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
-                            int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream)
+                            int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
+                            const ExpView* rows = nullptr)
 {
     if (k_bucket > 0)
         return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
-                                tm, stream);
+                                tm, stream, rows);
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
@@ -440,12 +443,14 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
 
     // ---- S1 (+ histogram of the first pass's digit), then the shared tail
     int k = choose_prefix_passes(plan, nterms, o, at);
-    launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
-    rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream);
+    const bool fuse = k > 0 && rows_fusable(ev, nvars) && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
+    if (fuse) launches += launch_row_hist(ev, nterms, plan, plan.npasses - k, ctl, stream);      // S1 itself runs inside the first pass
+    else launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
+    rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
     if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
     return sort_reduce_emit(plan, k, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
-                            at.safe_rank, stream);
+                            at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr);
 }
 
 static bool wants_safe_rank(const polylab_opts* opts)

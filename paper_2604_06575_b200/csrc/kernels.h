@@ -38,6 +38,12 @@ int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys,
 // Histogram of plan digit `hist_digit` over packed keys into ctl->hist[hist_digit].
 int launch_key_hist(const Plan& plan, int hist_digit, int64_t n, const void* keys, Control* ctl, cudaStream_t stream);
 
+// Can S1 be fused into the first radix pass for this exponent matrix?  (row-major, 16-byte aligned base, rows of 8 or 16 bytes)
+bool rows_fusable(const ExpView& ev, int nvars);
+
+// Histogram of plan digit `hist_digit` straight from such rows into ctl->hist[hist_digit] (no keys are written).
+int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hist_digit, Control* ctl, cudaStream_t stream);
+
 // S1 for the test entry point: always writes (hi, lo) pairs.
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
                      cudaStream_t stream);
@@ -55,11 +61,13 @@ int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const Exp
 // coef_out); needs ctl->hist[pass].  `next` >= 0: also accumulate the histogram of plan digit `next` (the digit of
 // the following pass) into ctl->hist[next].  `seq` = 0, 1, 2, ... counts the passes of the call: tile_state
 // (ceil(n/tile) * 256 words) is zero before pass seq 0 and reused by every later pass (flag parity alternates).
+// `rows` (rows_fusable() exponent matrix): S1 fused into the pass -- keys_in is ignored, the keys are packed in
+// registers from the rows, range-checked into ctl->status; atomic ranking only.
 // safe_rank: ballot-matching ranking (stable by construction); otherwise one shared atomic per record (see sort.cu).
 // debug_unstable: test hook, reverses the lane order of the atomic kernel.
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream);
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows = nullptr);
 
 // S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U; sets ctl->unsorted
 // when a key is smaller than its predecessor.

@@ -270,6 +270,98 @@ int launch_key_hist(const Plan& plan, int hd, int64_t n, const void* keys, Contr
     return 1;
 }
 
+// Histogram of plan digit `hd` straight from contiguous exponent rows of 8 or 16 bytes, without building the keys:
+// only the variables whose fields overlap the digit contribute (at most 8).  Used when S1 is fused into the first
+// radix pass of the bucket path (sort.cu), which needs this histogram before it can scatter.
+struct DigitParts {
+    int n;
+    uint8_t var[8];
+    int8_t lshift[8];       // contribution = e << lshift (lshift >= 0) or e >> -lshift, then & mask
+    uint32_t mask;
+};
+
+template <int RB, int ES>
+__global__ void __launch_bounds__(256) row_hist_kernel(const uint8_t* __restrict__ base, int64_t nterms, DigitParts dp,
+                                                       uint32_t* hist)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    bh.init(sh);
+    __syncthreads();
+    // four rows per thread and iteration: all four loads are issued before the first is used
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t0 < nterms; t0 += 4 * stride) {
+        uint32_t w[4][RB / 4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t t = t0 + u * stride;
+            if (t < nterms) {
+                if (RB == 16) {
+                    const uint4 q = __ldg((const uint4*)(base + t * RB));
+                    w[u][0] = q.x; w[u][RB / 4 > 1 ? 1 : 0] = q.y; w[u][RB / 4 > 2 ? 2 : 0] = q.z; w[u][RB / 4 > 3 ? 3 : 0] = q.w;
+                } else {
+                    const uint2 q = __ldg((const uint2*)(base + t * RB));
+                    w[u][0] = q.x; w[u][RB / 4 > 1 ? 1 : 0] = q.y;
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (t0 + u * stride >= nterms) break;
+            uint32_t d = 0;
+            for (int i = 0; i < dp.n; ++i) {
+                const int v = dp.var[i];
+                uint32_t e;
+                const int wi = ES == 4 ? v : ES == 2 ? (v >> 1) : (v >> 2);      // selects, not a dynamically indexed array
+                uint32_t x = w[u][0];
+                if (RB / 4 > 1 && wi == 1) x = w[u][RB / 4 > 1 ? 1 : 0];
+                if (RB / 4 > 2 && wi == 2) x = w[u][RB / 4 > 2 ? 2 : 0];
+                if (RB / 4 > 3 && wi == 3) x = w[u][RB / 4 > 3 ? 3 : 0];
+                if (ES == 4) e = x;
+                else if (ES == 2) e = (x >> (16 * (v & 1))) & 0xffffu;
+                else e = (x >> (8 * (v & 3))) & 0xffu;
+                const int ls = dp.lshift[i];
+                d |= ls >= 0 ? (e << ls) : (e >> -ls);
+            }
+            bh.add(d & dp.mask);
+        }
+    }
+    __syncthreads();
+    bh.flush(hist);
+}
+
+bool rows_fusable(const ExpView& ev, int nvars)
+{
+    const int rb = nvars * ev.exp_bytes;
+    return ev.row_major_contiguous && (rb == 8 || rb == 16);
+}
+
+int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hd, Control* ctl, cudaStream_t stream)
+{
+    if (nterms <= 0 || !rows_fusable(ev, plan.nvars) || hd < 0 || hd >= plan.npasses) return 0;
+    DigitParts dp;
+    dp.n = 0;
+    const int dpos = plan.digit_pos[hd], dbits = plan.digit_bits[hd];
+    dp.mask = (1u << dbits) - 1u;
+    for (int v = 0; v < plan.nvars; ++v) {
+        const int lo = plan.shift[v], hi = lo + plan.width[v];
+        if (plan.width[v] == 0 || hi <= dpos || lo >= dpos + dbits) continue;
+        dp.var[dp.n] = (uint8_t)v;
+        dp.lshift[dp.n] = (int8_t)(lo - dpos);
+        ++dp.n;
+    }
+    const int rb = plan.nvars * ev.exp_bytes;
+    int64_t blocks = (nterms + 256 * 8 - 1) / (256 * 8);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    const uint8_t* base = (const uint8_t*)ev.base;
+    uint32_t* hist = ctl->hist[hd];
+#define POLYLAB_RH(RB, ES) row_hist_kernel<RB, ES><<<(unsigned)blocks, 256, 0, stream>>>(base, nterms, dp, hist)
+    if (rb == 16) { if (ev.exp_bytes == 1) POLYLAB_RH(16, 1); else if (ev.exp_bytes == 2) POLYLAB_RH(16, 2); else POLYLAB_RH(16, 4); }
+    else { if (ev.exp_bytes == 1) POLYLAB_RH(8, 1); else if (ev.exp_bytes == 2) POLYLAB_RH(8, 2); else POLYLAB_RH(8, 4); }
+#undef POLYLAB_RH
+    return 1;
+}
+
 // ----------------------------------------------------------------------------------------------- X1
 
 template <typename K>

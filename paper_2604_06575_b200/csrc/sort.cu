@@ -40,7 +40,50 @@ struct PassArgs {
     uint32_t* hist_next;
     uint32_t* ticket;
     int reverse_lanes;          // POLYLAB_FLAG_DEBUG_UNSTABLE: the atomic kernel maps lane l to record 31 - l
+    // S1 fused into the pass (ROWS > 0): keys are packed in registers from contiguous exponent rows of ROWS bytes
+    const uint8_t* rows;
+    int exp_bytes;
+    int32_t* status;
 };
+
+// Step S1 inside the radix pass: exponent row t (ROWS = 8 or 16 contiguous bytes) -> key, with the range check of
+// pack.cu (an exponent above plan.bound sets `bad`).  BYTES: u8 exponents, every field 8 bits wide and unbounded, rows
+// as long as the key: the key is the byte-reversed row.
+template <typename K, int ROWS, bool BYTES>
+__device__ __forceinline__ K pack_row_inline(const PassArgs& a, const Plan& plan, uint32_t t, bool& bad)
+{
+    uint32_t w[ROWS / 4];
+    if (ROWS == 16) {
+        const uint4 q = __ldg((const uint4*)(a.rows + (size_t)t * ROWS));
+        w[0] = q.x; w[ROWS / 4 > 1 ? 1 : 0] = q.y; w[ROWS / 4 > 2 ? 2 : 0] = q.z; w[ROWS / 4 > 3 ? 3 : 0] = q.w;
+    } else {
+        const uint2 q = __ldg((const uint2*)(a.rows + (size_t)t * ROWS));
+        w[0] = q.x; w[ROWS / 4 > 1 ? 1 : 0] = q.y;
+    }
+    K key;
+    key_zero(key);
+    if (BYTES) {
+        uint64_t h[ROWS / 8];
+#pragma unroll
+        for (int i = 0; i < ROWS / 8; ++i)
+            h[i] = ((uint64_t)__byte_perm(w[2 * i], 0u, 0x0123) << 32) | (uint64_t)__byte_perm(w[2 * i + 1], 0u, 0x0123);
+        key_from_halves(key, h[0], h[ROWS / 8 - 1]);
+        return key;
+    }
+    const int es = a.exp_bytes;
+#pragma unroll
+    for (int k = 0; k < ROWS; ++k) {
+        if (k * es < ROWS) {
+            uint32_t e;
+            if (es == 4) e = w[(k < ROWS / 4) ? k : 0];
+            else if (es == 2) e = (w[(k < ROWS / 2) ? (k >> 1) : 0] >> (16 * (k & 1))) & 0xffffu;
+            else e = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
+            bad |= e > plan.bound[k];
+            key_or_field(key, e, plan.shift[k]);
+        }
+    }
+    return key;
+}
 
 // lanes of the warp holding the same digit d (< 256) as the calling lane; all 32 lanes participate
 __device__ __forceinline__ unsigned match_digit_all(uint32_t d)
@@ -60,9 +103,9 @@ __device__ __forceinline__ unsigned match_digit_all(uint32_t d)
 // values in ascending lane order on sm_100a (measured, profiles/r1b_shared_atomics.md; not documented), which
 // is what makes the pass stable; the reduce step verifies the sorted order and the call falls back to the
 // ballot-matching kernel (RANK_ATOMIC = false) if it ever does not hold.
-template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC>
-__device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char* smem_raw, uint32_t tile, uint32_t tile_base,
-                                               uint32_t tile_n)
+template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC, int ROWS, bool BYTES = false>
+__device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* plan, unsigned char* smem_raw, uint32_t tile,
+                                               uint32_t tile_base, uint32_t tile_n)
 {
     using S = SortSmem<K, THREADS, ITEMS>;
     constexpr int NW = S::NW;
@@ -83,12 +126,16 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, unsigned char*
     // ---- load keys: warp w owns records [w*32*ITEMS, (w+1)*32*ITEMS) of the tile, item j of lane l is j*32+l
     const uint32_t chunk = warp * 32u * ITEMS + ((RANK_ATOMIC && a.reverse_lanes) ? 31u - lane : lane);
     K key[ITEMS];
+    bool bad = false;
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
-        if (FULL || li < tile_n) key[j] = keys_in[tile_base + li];
-        else key[j] = key_max<K>();
+        if (FULL || li < tile_n) {
+            if (ROWS > 0) key[j] = pack_row_inline<K, (ROWS > 0 ? ROWS : 8), BYTES>(a, *plan, tile_base + li, bad);
+            else key[j] = keys_in[tile_base + li];
+        } else key[j] = key_max<K>();
     }
+    if (ROWS > 0 && bad) atomicMax(a.status, (int)POLYLAB_ERR_EXPONENT_RANGE);
 #define POLYLAB_DIGIT(j) ((key_word(key[j], a.dword) >> a.dshift) & a.dmask)
 
     // ---- rank within the warp, in record order (stable)
@@ -235,8 +282,29 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_c
     const uint32_t tile = scratch[NW + 2];
     const uint32_t tile_base = tile * (uint32_t)TILE;
     const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
-    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, RANK_ATOMIC>(a, smem_raw, tile, tile_base, tile_n);
-    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, RANK_ATOMIC>(a, smem_raw, tile, tile_base, tile_n);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, RANK_ATOMIC, 0>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, RANK_ATOMIC, 0>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+}
+
+// The same pass with S1 fused in: reads exponent rows instead of keys (first pass of the bucket path).
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, int ROWS, bool BYTES>
+__global__ void __launch_bounds__(THREADS, MINB) sort_pass_rows_kernel(const __grid_constant__ PassArgs a, const __grid_constant__ Plan plan)
+{
+    using S = SortSmem<K, THREADS, ITEMS>;
+    constexpr int TILE = S::TILE, NW = S::NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* whist = (uint32_t*)(smem_raw + S::stage_bytes);
+    uint32_t* scratch = whist + NW * kRadix + 3 * kRadix;
+
+    const unsigned tid = threadIdx.x;
+    if (tid == 0) scratch[NW + 2] = atomicAdd(a.ticket, 1u);
+    for (int i = tid; i < (NW + 1) * kRadix; i += THREADS) whist[i] = 0u;
+    __syncthreads();
+    const uint32_t tile = scratch[NW + 2];
+    const uint32_t tile_base = tile * (uint32_t)TILE;
+    const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, ROWS, BYTES>(a, &plan, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES>(a, &plan, smem_raw, tile, tile_base, tile_n);
 }
 
 template <typename K, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
@@ -255,7 +323,7 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 template <typename K, int ITEMS, int MINB>
 static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in,
                               const double* coef_in, void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl,
-                              bool safe_rank, bool debug_unstable, cudaStream_t stream)
+                              bool safe_rank, bool debug_unstable, const ExpView* rows, cudaStream_t stream)
 {
     using S = SortSmem<K, kSortThreads, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
@@ -272,6 +340,22 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     a.flag_inclusive = (seq & 1) ? 0u : 2u;
     a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[has_next ? next : kMaxPasses]; a.ticket = &ctl->ticket[seq];
     a.reverse_lanes = debug_unstable ? 1 : 0;
+    a.rows = nullptr; a.exp_bytes = 0; a.status = &ctl->status;
+    if (rows) {
+        a.rows = (const uint8_t*)rows->base; a.exp_bytes = rows->exp_bytes;
+        bool fast = rows->exp_bytes == 1 && plan.nvars * rows->exp_bytes == (int)sizeof(K);
+        for (int v = 0; v < plan.nvars && fast; ++v) fast = plan.width[v] == 8 && plan.bound[v] >= 255u;
+        const int rb = plan.nvars * rows->exp_bytes;
+        auto go = [&](auto kern) {
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
+            kern<<<tiles, kSortThreads, S::bytes(), stream>>>(a, plan);
+        };
+        constexpr int KB = (int)sizeof(K);          // the byte-reversal path needs rows as long as the key
+        if (fast) { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, KB, true>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, KB, true>); }
+        else if (rb == 16) { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, 16, false>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, 16, false>); }
+        else { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, 8, false>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, 8, false>); }
+        return 1;
+    }
     if (safe_rank) {
         if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, false>(a, tiles, stream);
         else launch_sort_pass_k<K, ITEMS, MINB, false, false>(a, tiles, stream);
@@ -284,14 +368,14 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
 
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream)
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows)
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                             tile_state, ctl, safe_rank, debug_unstable, stream);
+                                                             tile_state, ctl, safe_rank, debug_unstable, rows, stream);
     return launch_sort_pass_t<Key128, kSortItems128, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                        tile_state, ctl, safe_rank, debug_unstable, stream);
+                                                        tile_state, ctl, safe_rank, debug_unstable, rows, stream);
 }
 
 }  // namespace polylab

@@ -150,3 +150,32 @@ def test_bucket_path_mul_simplify():
     c, e, st = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), 0.0, return_stats=True)
     assert st.prefix_passes >= 1 and st.bucket_fallback == 0
     assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, 0.0), c.cpu().numpy(), e.cpu().numpy())
+
+
+# ------------------------------------------------------------------ S1 fused into the first radix pass
+
+@pytest.mark.parametrize("case", ["u8x16_bytes", "u8x16_narrow", "u8x8", "u16x8", "u32x4", "u32x2", "u16x4"])
+def test_fused_pack_matches_separate_pack(case):
+    """Rows of 8 or 16 contiguous bytes are packed inside the first prefix pass; the result must be bit-identical to
+    the run with S1 as its own kernel (POLYLAB_FLAG_NO_FUSED_PACK), and in parity with the oracle."""
+    n = 120_000
+    nvars, dtype, hi = {"u8x16_bytes": (16, np.uint8, 256), "u8x16_narrow": (16, np.uint8, 100), "u8x8": (8, np.uint8, 256),
+                        "u16x8": (8, np.uint16, 5000), "u32x4": (4, np.uint32, 70000), "u32x2": (2, np.uint32, 1 << 20),
+                        "u16x4": (4, np.uint16, 40000)}[case]
+    p = pooled(n, nvars, 4, seed=31 + nvars, hi=hi, dtype=dtype)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    c0, e0, st0 = run(p, 0.0, flags=FORCE | B.FLAG_NO_FUSED_PACK)
+    assert st.prefix_passes >= 1 and st0.prefix_passes == st.prefix_passes
+    assert st.kernel_launches == st0.kernel_launches          # row histogram instead of the pack kernel
+    assert (e == e0).all() and (c.view(np.uint64) == c0.view(np.uint64)).all()
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_fused_pack_checks_caller_bounds():
+    p = pooled(50_000, 16, 4, seed=41, hi=200)
+    with pytest.raises(B.PolylabError) as ei:
+        B.simplify(dev(p.coef), dev(p.exps), 0.0, max_exp=[150] * 16, flags=FORCE)
+    assert ei.value.status == B.ERR_EXPONENT_RANGE
+    c, e, st = B.simplify(dev(p.coef), dev(p.exps), 0.0, max_exp=[255] * 16, flags=FORCE, return_stats=True)
+    assert st.prefix_passes >= 1
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c.cpu().numpy(), e.cpu().numpy())
