@@ -237,7 +237,7 @@ static int bucket_room(const Plan& plan, int k, int64_t n)
 static int fast_digits(const Opts& o)
 {
     const int dbg = (int)((o.flags >> POLYLAB_FLAG_DEBUG_NFAST_SHIFT) & 0xfu);
-    return dbg ? dbg : 3;          // 24 bits below the prefix separate the distinct keys of a bucket with high probability
+    return dbg;                    // 0 = no limit: as many bits below the prefix as fit the 27-bit composite sort word
 }
 
 // After S1/X1 accumulated the histogram of the first prefix digit: do its bins predict buckets that fit a tile?

@@ -71,79 +71,85 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ 
 
 struct FinishSmem {
     static constexpr int NW = kFinThreads / 32;
-    // [sort word u32][perm X u16][ordinal u16] = 8 bytes per record, reused for the gathered coefficients once the
-    // sort is done; then [perm Y u16], per-warp histograms, bin starts, scratch
-    static constexpr size_t off_sw = 0;
-    static constexpr size_t off_px = (size_t)kFinCap * 4;
-    static constexpr size_t off_ord = off_px + (size_t)kFinCap * 2;
-    static constexpr size_t off_py = off_ord + (size_t)kFinCap * 2;
-    static constexpr size_t off_whist = off_py + (size_t)kFinCap * 2;
-    static constexpr size_t off_scratch = off_whist + (size_t)NW * kRadix * 4;
+    // [X u32][Y u32]: ping-pong buffers of sort elements, reused for the gathered coefficients (8 bytes per record) once
+    // the sort is done; [P u16]: head flags, then bucket ordinals, then the final permutation; per-warp histograms; scratch
+    static constexpr size_t off_x = 0;
+    static constexpr size_t off_y = (size_t)kFinCap * 4;
+    static constexpr size_t off_p = off_y + (size_t)kFinCap * 4;
+    static constexpr size_t off_whist = off_p + (size_t)kFinCap * 2;
+    static constexpr size_t off_scratch = off_whist + (size_t)NW * kFinBins * 2;
     static constexpr size_t bytes = off_scratch + 64 * 4;
 };
 
-// Exclusive scan of one value per thread over the first 256 threads of the block (warps 0..7 only call this; they
-// meet on named barrier 1, the other warps are not involved).  wtot: 9 words of shared memory.
-__device__ __forceinline__ uint32_t scan256_exclusive(uint32_t x, uint32_t* wtot)
-{
-    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
-    uint32_t incl = x;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t y = __shfl_up_sync(kFullMask, incl, o);
-        if (lane >= (unsigned)o) incl += y;
-    }
-    if (lane == 31) wtot[warp] = incl;
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    uint32_t before = 0;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) before += (w < (int)warp) ? wtot[w] : 0u;
-    return before + incl - x;
-}
-
-// One stable counting-sort pass over the permutation: pout = pin reordered by the digit (src[r] >> shift) & mask of
-// record r.  Warp w owns the contiguous chunk [w*per, (w+1)*per) of positions and row w of the histogram.
+// One stable counting-sort pass on a digit of `dbits` <= 9 bits.  A sort element is one 32-bit word: the record's index
+// in the tile in its low 13 bits, the not yet consumed sort bits above (least significant digit first), so a pass
+// reads its input sequentially and never dereferences an index.  FIRST: the input is the composite sort word itself
+// (up to 27 bits), position = record index.  Warp w owns the contiguous chunk [w*per, (w+1)*per) of positions and row w of
+// the histogram: 512 16-bit counters, two per word, bumped with one shared-memory atomic per record and sweep.
 // Sweep 1 counts; the bins are then turned into the first output slot of every (warp, digit) pair; sweep 2 takes slots
 // with the same atomic in the same order.  Stability rests on the order in which one warp's shared-memory atomics to
-// one address return (lane order within an instruction, program order across instructions: measured on sm_100a,
+// one word return (lane order within an instruction, program order across instructions: measured on sm_100a,
 // profiles/r1b_shared_atomics.md) and is re-verified by the caller's order check.
-template <typename SRC>
-__device__ __forceinline__ void local_pass(const SRC* __restrict__ src, int shift, uint32_t mask, const uint16_t* pin,
-                                           uint16_t* pout, uint32_t n_loc, uint32_t* whist, uint32_t* scratch)
+template <bool FIRST>
+__device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int dbits, uint32_t n_loc,
+                                           uint32_t* whist, uint32_t* scratch)
 {
-    constexpr int NW = FinishSmem::NW;
+    constexpr int NW = FinishSmem::NW, ROW = kFinBins / 2;    // words per histogram row
+    static_assert(kFinBins == kFinThreads, "one thread per bin in the scan step");
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    uint32_t* my_hist = whist + warp * kRadix;
+    const uint32_t mask = (1u << dbits) - 1u;
+    uint32_t* my_hist = whist + warp * ROW;
 #pragma unroll
-    for (int b = 0; b < kRadix / 32; ++b) my_hist[b * 32 + lane] = 0u;
+    for (int b = 0; b < ROW / 32; ++b) my_hist[b * 32 + lane] = 0u;
     __syncwarp();
     const uint32_t per = (((n_loc + NW - 1) / NW) + 31u) & ~31u;
     const uint32_t wbeg = min(warp * per, n_loc), wend = min(wbeg + per, n_loc);
-    for (uint32_t i = wbeg + lane; i < wend; i += 32u)
-        atomicAdd(&my_hist[((uint32_t)src[pin[i]] >> shift) & mask], 1u);
+    for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
+        const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
+        atomicAdd(&my_hist[d >> 1], 1u << ((d & 1u) * 16u));
+    }
     __syncthreads();
-    if (tid < kRadix) {
+    {
+        uint16_t* h16 = (uint16_t*)whist;                      // [NW][kFinBins], bin b of warp w at w*kFinBins + b
         uint32_t c[NW];
         uint32_t count = 0;
 #pragma unroll
-        for (int w = 0; w < NW; ++w) c[w] = whist[w * kRadix + tid];
+        for (int w = 0; w < NW; ++w) c[w] = h16[w * kFinBins + tid];
 #pragma unroll
         for (int w = 0; w < NW; ++w) { const uint32_t x = c[w]; c[w] = count; count += x; }
-        const uint32_t bin_start = scan256_exclusive(count, scratch);
+        uint32_t total;
+        const uint32_t bin_start = block_exclusive_scan<kFinThreads>(count, scratch, &total);
 #pragma unroll
-        for (int w = 0; w < NW; ++w) whist[w * kRadix + tid] = bin_start + c[w];
+        for (int w = 0; w < NW; ++w) h16[w * kFinBins + tid] = (uint16_t)(bin_start + c[w]);
     }
     __syncthreads();
     for (uint32_t base = wbeg; base < wend; base += 32u) {
         const uint32_t i = base + lane;
         if (i < wend) {
-            const uint32_t r = pin[i];
-            const uint32_t slot = atomicAdd(&my_hist[((uint32_t)src[r] >> shift) & mask], 1u);
-            pout[slot] = (uint16_t)r;
+            const uint32_t e = in[i];
+            const uint32_t d = (FIRST ? e : (e >> 13)) & mask;
+            const uint32_t sh = (d & 1u) * 16u;
+            const uint32_t slot = (atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh) & 0xffffu;
+            out[slot] = FIRST ? (i | ((e >> dbits) << 13)) : ((e & 0x1fffu) | ((e >> (13 + dbits)) << 13));
         }
         __syncwarp();
     }
     __syncthreads();
+}
+
+// all passes over `nbits` sort bits (9 per pass); returns with the result in *cur (swaps *cur / *oth as it goes)
+template <bool FIRST0>
+__device__ __forceinline__ void local_sort_bits(uint32_t** cur, uint32_t** oth, int nbits, uint32_t n_loc, uint32_t* whist,
+                                                uint32_t* scratch)
+{
+    bool first = FIRST0;
+    for (int done = 0; done < nbits; done += kFinDigit) {
+        const int dbits = min(kFinDigit, nbits - done);
+        if (first) local_pass<true>(*cur, *oth, dbits, n_loc, whist, scratch);
+        else local_pass<false>(*cur, *oth, dbits, n_loc, whist, scratch);
+        first = false;
+        uint32_t* t = *cur; *cur = *oth; *oth = t;
+    }
 }
 
 struct FinishArgs {
@@ -154,8 +160,7 @@ struct FinishArgs {
     const uint32_t* tile_start;     // [ntiles + 1]
     uint32_t* tile_state;           // [ntiles] look-back words, zero before the kernel
     int pfx_pos;                    // the prefix is the key bits at positions >= pfx_pos
-    int nlow;                       // plan digits below the prefix: digits [0, nlow)
-    int nfast;                      // how many of them (the most significant ones) the first attempt sorts on
+    int fast_bits;                  // most key bits below the prefix the first attempt sorts on (test hook; 32 = no limit)
     double tol;
     void* ukeys;                    // survivors of tile t, compacted in order: (ukeys, usums)[tile_start[t] + q], q < tile_state[t]
     double* usums;
@@ -194,31 +199,20 @@ __device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, u
         store_exp(a.out_exps, a.exp_bytes, (int64_t)o * plan.nvars + v, key_get_field(kk, plan.shift[v], plan.width[v]));
 }
 
-// digits [d, e) starting at digit d that fit one 32-bit sort word; returns e, the word's position and width
-__device__ __forceinline__ int digit_group(const Plan& plan, int d, int nlow, int* gpos, int* gw)
-{
-    *gpos = plan.digit_pos[d];
-    int e = d;
-    while (e < nlow && plan.digit_pos[e] + plan.digit_bits[e] - *gpos <= 32) ++e;
-    *gw = plan.digit_pos[e - 1] + plan.digit_bits[e - 1] - *gpos;
-    return e;
-}
-
 // ------------------------------------------------------------------------------------ finish kernel
 
 template <typename K>
 __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_constant__ FinishArgs a, const __grid_constant__ Plan plan)
 {
     constexpr int THREADS = kFinThreads, CAP = kFinCap, NW = THREADS / 32;
-    static_assert(CAP <= 65536 && CAP / THREADS <= 32, "16-bit permutation entries, 32-bit head masks");
+    static_assert(CAP <= 8192 && CAP / THREADS <= 32, "13-bit record indices in the sort elements, 32-bit head masks");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint32_t* sw = (uint32_t*)(smem_raw + FinishSmem::off_sw);
-    uint16_t* px = (uint16_t*)(smem_raw + FinishSmem::off_px);
-    uint16_t* ord = (uint16_t*)(smem_raw + FinishSmem::off_ord);
-    uint16_t* py = (uint16_t*)(smem_raw + FinishSmem::off_py);
+    uint32_t* bx = (uint32_t*)(smem_raw + FinishSmem::off_x);
+    uint32_t* by = (uint32_t*)(smem_raw + FinishSmem::off_y);
+    uint16_t* py = (uint16_t*)(smem_raw + FinishSmem::off_p);              // head flags -> ordinals -> final permutation
     uint32_t* whist = (uint32_t*)(smem_raw + FinishSmem::off_whist);
     uint32_t* scratch = (uint32_t*)(smem_raw + FinishSmem::off_scratch);   // [0..NW+1] scans, [40] tile, [41] base
-    double* scs = (double*)smem_raw;               // coefficients in sorted order, over sw / px / ord once the sort is done
+    double* scs = (double*)smem_raw;               // coefficients in sorted order, over X / Y once the sort is done
     __shared__ uint32_t wagg_f[NW];
     __shared__ double wagg_v[NW];
 
@@ -235,14 +229,13 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     const uint32_t itn = (n_loc + THREADS - 1) / THREADS;      // sorted positions per thread in the blocked phases
     const uint32_t first = tid * itn;
 
-    int d_start = (a.nfast < a.nlow) ? a.nlow - a.nfast : 0;
+    // raw sort bits of the fast attempt: the (up to 32) key bits just below the prefix
+    const int rbits = min(32, a.pfx_pos);
+    bool full = (rbits == 0);                      // nothing below the prefix: only the ordinal is sorted on
     uint32_t hm = 0, nh = 0;
     double acc = 0.0;
     while (true) {
-        // ---- stream the keys once: bucket heads, the first group's sort word, identity permutations
-        int gpos = 0, gw = 0;
-        int e = d_start;
-        if (d_start < a.nlow) e = digit_group(plan, d_start, a.nlow, &gpos, &gw);
+        // ---- stream the keys once: bucket heads and the raw sort bits
         bool descending = false;
         for (uint32_t i = tid; i < n_loc; i += THREADS) {
             const K k = gkeys[i];
@@ -252,46 +245,65 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                 head = !same_prefix(k, kp, a.pfx_pos);
                 descending |= head && key_lt(k, kp);
             }
-            sw[i] = gw ? key_get_field(k, gpos, gw) : 0u;
-            ord[i] = head ? 1 : 0;
-            px[i] = (uint16_t)i;
-            py[i] = (uint16_t)i;
+            bx[i] = full ? i : key_get_field(k, a.pfx_pos - rbits, rbits);
+            py[i] = head ? 1 : 0;
         }
         if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
         __syncthreads();
 
-        // ---- bucket ordinal of every record (buckets are contiguous: the input is sorted by prefix)
+        // ---- bucket ordinal of every record (buckets are contiguous: the input is sorted by prefix); fast attempt:
+        // composite sort word = ordinal above the top fb raw bits, ob + fb <= 27 so that 13 index bits fit beside what
+        // is left after the first 9-bit pass
         uint32_t nbuckets;
+        int ob = 0, fb = 0;
         {
             uint32_t cnt = 0;
             for (uint32_t j = 0; j < itn; ++j)
-                if (first + j < n_loc) cnt += ord[first + j];
+                if (first + j < n_loc) cnt += py[first + j];
             uint32_t o = block_exclusive_scan<THREADS>(cnt, scratch, &nbuckets);
-            for (uint32_t j = 0; j < itn; ++j)
-                if (first + j < n_loc) { o += ord[first + j]; ord[first + j] = (uint16_t)(o - 1u); }
+            while (nbuckets > 1 && ((nbuckets - 1u) >> ob) != 0u) ++ob;
+            fb = min(min(27 - ob, rbits), a.fast_bits);
+            for (uint32_t j = 0; j < itn; ++j) {
+                if (first + j < n_loc) {
+                    o += py[first + j];
+                    py[first + j] = (uint16_t)(o - 1u);
+                    if (!full) bx[first + j] = ((o - 1u) << fb) | (fb ? (bx[first + j] >> (rbits - fb)) : 0u);
+                }
+            }
         }
         __syncthreads();
 
-        // ---- local sort: the digits of [d_start, nlow) low to high, then the ordinal; the result lands in py
-        int nord = 0;
-        for (int ob = 0; nbuckets > 1 && ((nbuckets - 1u) >> ob) != 0u; ob += kRadixBits) ++nord;
-        uint16_t* pin = (((a.nlow - d_start) + nord) & 1) ? px : py;
-        uint16_t* pout = (pin == px) ? py : px;
-        for (int d = d_start; d < a.nlow;) {
-            if (d != d_start) {                    // next group of digits: cut a new sort word out of the keys
-                e = digit_group(plan, d, a.nlow, &gpos, &gw);
-                for (uint32_t i = tid; i < n_loc; i += THREADS) sw[i] = key_get_field(gkeys[i], gpos, gw);
+        // ---- local sort; the final permutation lands in py
+        uint32_t* cur = bx;
+        uint32_t* oth = by;
+        if (!full) {
+            local_sort_bits<true>(&cur, &oth, ob + fb, n_loc, whist, scratch);
+            if (ob + fb == 0)                      // one bucket, no bits: identity
+                for (uint32_t i = tid; i < n_loc; i += THREADS) cur[i] = i;
+        } else {
+            // every bit below the prefix, 18 at a time from the least significant up, cut out of the keys through the
+            // current permutation; then the ordinal
+            for (int gpos = 0; gpos < a.pfx_pos; gpos += 18) {
+                const int gw = min(18, a.pfx_pos - gpos);
+                for (uint32_t i = tid; i < n_loc; i += THREADS) {
+                    const uint32_t r = cur[i] & 0x1fffu;
+                    cur[i] = r | (key_get_field(gkeys[r], gpos, gw) << 13);
+                }
                 __syncthreads();
+                local_sort_bits<false>(&cur, &oth, gw, n_loc, whist, scratch);
             }
-            for (; d < e; ++d) {
-                local_pass<uint32_t>(sw, plan.digit_pos[d] - gpos, (1u << plan.digit_bits[d]) - 1u, pin, pout, n_loc, whist, scratch);
-                uint16_t* t = pin; pin = pout; pout = t;
+            if (ob > 0) {
+                for (uint32_t i = tid; i < n_loc; i += THREADS) {
+                    const uint32_t r = cur[i] & 0x1fffu;
+                    cur[i] = r | ((uint32_t)py[r] << 13);
+                }
+                __syncthreads();
+                local_sort_bits<false>(&cur, &oth, ob, n_loc, whist, scratch);
             }
         }
-        for (int q = 0; q < nord; ++q) {
-            local_pass<uint16_t>(ord, q * kRadixBits, (uint32_t)kRadix - 1u, pin, pout, n_loc, whist, scratch);
-            uint16_t* t = pin; pin = pout; pout = t;
-        }
+        __syncthreads();
+        for (uint32_t i = tid; i < n_loc; i += THREADS) py[i] = (uint16_t)(cur[i] & 0x1fffu);
+        __syncthreads();
 
         // ---- gather through the permutation: heads of runs of equal keys, sums since the last head, order check
         hm = 0; nh = 0; acc = 0.0;
@@ -306,7 +318,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                     const uint32_t r = py[first + j];
                     const K kk = gkeys[r];
                     const double c = gcoef[r];
-                    scs[first + j] = c;            // own positions only; sw / px / ord are dead after the last pass
+                    scs[first + j] = c;            // own positions only; X / Y are dead after the last pass
                     const bool head = !hp || !key_eq(kk, kp);
                     viol |= hp && key_lt(kk, kp);
                     if (head) { hm |= 1u << j; ++nh; acc = c; }
@@ -317,11 +329,11 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
             }
         }
         if (!__syncthreads_or(viol ? 1 : 0)) break;
-        if (d_start == 0) {                        // every digit was sorted on and the order is still wrong
+        if (full) {                                // every bit was sorted on and the order is still wrong
             if (tid == 0) a.ctl->unsorted = 1u;
             break;
         }
-        d_start = 0;
+        full = true;
         if (tid == 0) atomicAdd(&a.ctl->refinish, 1u);
     }
 
@@ -494,7 +506,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     FinishArgs a;
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state;
-    a.pfx_pos = pfx_pos; a.nlow = nlow; a.nfast = nfast; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
+    a.pfx_pos = pfx_pos; a.fast_bits = nfast > 0 ? nfast * 8 : 32; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
     kern<<<ntiles, kFinThreads, smem, stream>>>(a, plan);
     if (after_tiles) cudaEventRecord(after_tiles, stream);
     tile_scan_kernel<<<1, 1024, 0, stream>>>(tile_state, ntiles, ctl, out_count_device);

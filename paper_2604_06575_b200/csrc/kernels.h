@@ -20,6 +20,8 @@ constexpr int kFinThreads = 512;    // bucket path (finish.cu): two blocks per S
 constexpr int kFinCap = 8192;       // most records a finish tile can own (10 bytes of shared memory each); tile t owns the
                                     // buckets that start in positions [t*fin_tile, (t+1)*fin_tile), so a bucket may be
                                     // as long as kFinCap - fin_tile
+constexpr int kFinDigit = 9;         // local sort: 9-bit digits, 512 bins
+constexpr int kFinBins = 1 << kFinDigit;
 constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
 constexpr int kFinMinTile = 4096;   // smallest fin_tile the planner picks (workspace sizing)
 
