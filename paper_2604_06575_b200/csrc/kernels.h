@@ -10,7 +10,7 @@ namespace polylab {
 // Tile sizes of the streaming kernels (records per thread block); also used by the workspace query.
 constexpr int kSortThreads = 256;
 constexpr int kSortItems64 = 16;    // 4096-record tiles of (u64 key, f64 coef)
-constexpr int kSortItems128 = 12;   // 3072-record tiles of (u128 key, f64 coef)
+constexpr int kSortItems128 = 20;   // 5120-record tiles of (u128 key, f64 coef), two blocks per SM (swept on B200: 12x3 4.26, 16x2 4.08, 20x2 4.04, 24x2 4.74 ms for two passes of config 5)
 constexpr int kReduceThreads = 256;
 constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from shared memory
 constexpr int kPruneThreads = 256;

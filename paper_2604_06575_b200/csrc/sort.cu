@@ -374,7 +374,7 @@ int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, c
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
                                                              tile_state, ctl, safe_rank, debug_unstable, rows, stream);
-    return launch_sort_pass_t<Key128, kSortItems128, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+    return launch_sort_pass_t<Key128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
                                                         tile_state, ctl, safe_rank, debug_unstable, rows, stream);
 }
 
