@@ -90,27 +90,40 @@ struct FinishSmem {
 // with the same atomic in the same order.  Stability rests on the order in which one warp's shared-memory atomics to
 // one word return (lane order within an instruction, program order across instructions: measured on sm_100a,
 // profiles/r1b_shared_atomics.md) and is re-verified by the caller's order check.
-template <bool FIRST>
+template <bool FIRST, bool RANKS>
 __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int dbits, uint32_t n_loc,
-                                           uint32_t* whist, uint32_t* scratch)
+                                           uint32_t* whist, uint32_t* scratch, uint16_t* ranks)
 {
     constexpr int NW = FinishSmem::NW, ROW = kFinBins / 2;    // words per histogram row
     static_assert(kFinBins == kFinThreads, "one thread per bin in the scan step");
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t mask = (1u << dbits) - 1u;
     uint32_t* my_hist = whist + warp * ROW;
+    uint16_t* h16 = (uint16_t*)whist;                          // [NW][kFinBins], bin b of warp w at w*kFinBins + b
 #pragma unroll
     for (int b = 0; b < ROW / 32; ++b) my_hist[b * 32 + lane] = 0u;
     __syncwarp();
     const uint32_t per = (((n_loc + NW - 1) / NW) + 31u) & ~31u;
     const uint32_t wbeg = min(warp * per, n_loc), wend = min(wbeg + per, n_loc);
-    for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
-        const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
-        atomicAdd(&my_hist[d >> 1], 1u << ((d & 1u) * 16u));
+    if (RANKS) {
+        // sweep 1 counts AND ranks: the atomic's old value is the record's rank among its warp's records of the digit
+        for (uint32_t base = wbeg; base < wend; base += 32u) {
+            const uint32_t i = base + lane;
+            if (i < wend) {
+                const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
+                const uint32_t sh = (d & 1u) * 16u;
+                ranks[i] = (uint16_t)(atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh);
+            }
+            __syncwarp();
+        }
+    } else {
+        for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
+            const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
+            atomicAdd(&my_hist[d >> 1], 1u << ((d & 1u) * 16u));
+        }
     }
     __syncthreads();
     {
-        uint16_t* h16 = (uint16_t*)whist;                      // [NW][kFinBins], bin b of warp w at w*kFinBins + b
         uint32_t c[NW];
         uint32_t count = 0;
 #pragma unroll
@@ -123,30 +136,44 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
         for (int w = 0; w < NW; ++w) h16[w * kFinBins + tid] = (uint16_t)(bin_start + c[w]);
     }
     __syncthreads();
-    for (uint32_t base = wbeg; base < wend; base += 32u) {
-        const uint32_t i = base + lane;
-        if (i < wend) {
+    if (RANKS) {
+        // sweep 2 needs no atomics and no order: slot = first slot of (warp, digit) + rank
+        const uint16_t* my16 = h16 + warp * kFinBins;
+#pragma unroll 4
+        for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
             const uint32_t e = in[i];
             const uint32_t d = (FIRST ? e : (e >> 13)) & mask;
-            const uint32_t sh = (d & 1u) * 16u;
-            const uint32_t slot = (atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh) & 0xffffu;
+            const uint32_t slot = (uint32_t)my16[d] + ranks[i];
             out[slot] = FIRST ? (i | ((e >> dbits) << 13)) : ((e & 0x1fffu) | ((e >> (13 + dbits)) << 13));
         }
-        __syncwarp();
+    } else {
+        for (uint32_t base = wbeg; base < wend; base += 32u) {
+            const uint32_t i = base + lane;
+            if (i < wend) {
+                const uint32_t e = in[i];
+                const uint32_t d = (FIRST ? e : (e >> 13)) & mask;
+                const uint32_t sh = (d & 1u) * 16u;
+                const uint32_t slot = (atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh) & 0xffffu;
+                out[slot] = FIRST ? (i | ((e >> dbits) << 13)) : ((e & 0x1fffu) | ((e >> (13 + dbits)) << 13));
+            }
+            __syncwarp();
+        }
     }
     __syncthreads();
 }
 
 // all passes over `nbits` sort bits (9 per pass); returns with the result in *cur (swaps *cur / *oth as it goes)
-template <bool FIRST0>
+// RANKS: a free 16-bit-per-record array is available for the ranks (fast attempt: the ordinal array is dead once the
+// composite sort word exists), which halves the atomics
+template <bool FIRST0, bool RANKS>
 __device__ __forceinline__ void local_sort_bits(uint32_t** cur, uint32_t** oth, int nbits, uint32_t n_loc, uint32_t* whist,
-                                                uint32_t* scratch)
+                                                uint32_t* scratch, uint16_t* ranks)
 {
     bool first = FIRST0;
     for (int done = 0; done < nbits; done += kFinDigit) {
         const int dbits = min(kFinDigit, nbits - done);
-        if (first) local_pass<true>(*cur, *oth, dbits, n_loc, whist, scratch);
-        else local_pass<false>(*cur, *oth, dbits, n_loc, whist, scratch);
+        if (first) local_pass<true, RANKS>(*cur, *oth, dbits, n_loc, whist, scratch, ranks);
+        else local_pass<false, RANKS>(*cur, *oth, dbits, n_loc, whist, scratch, ranks);
         first = false;
         uint32_t* t = *cur; *cur = *oth; *oth = t;
     }
@@ -277,7 +304,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
         uint32_t* cur = bx;
         uint32_t* oth = by;
         if (!full) {
-            local_sort_bits<true>(&cur, &oth, ob + fb, n_loc, whist, scratch);
+            local_sort_bits<true, true>(&cur, &oth, ob + fb, n_loc, whist, scratch, py);
             if (ob + fb == 0)                      // one bucket, no bits: identity
                 for (uint32_t i = tid; i < n_loc; i += THREADS) cur[i] = i;
         } else {
@@ -290,7 +317,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                     cur[i] = r | (key_get_field(gkeys[r], gpos, gw) << 13);
                 }
                 __syncthreads();
-                local_sort_bits<false>(&cur, &oth, gw, n_loc, whist, scratch);
+                local_sort_bits<false, false>(&cur, &oth, gw, n_loc, whist, scratch, nullptr);
             }
             if (ob > 0) {
                 for (uint32_t i = tid; i < n_loc; i += THREADS) {
@@ -298,7 +325,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                     cur[i] = r | ((uint32_t)py[r] << 13);
                 }
                 __syncthreads();
-                local_sort_bits<false>(&cur, &oth, ob, n_loc, whist, scratch);
+                local_sort_bits<false, false>(&cur, &oth, ob, n_loc, whist, scratch, nullptr);
             }
         }
         __syncthreads();
