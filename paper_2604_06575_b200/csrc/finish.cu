@@ -264,6 +264,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
         bool descending = false;
+#pragma unroll 4
         for (uint32_t i = tid; i < n_loc; i += THREADS) {
             const K k = gkeys[i];
             bool head = true;
