@@ -64,6 +64,26 @@ def workload(config: int, nterms, seed_offset: int = 0):
     raise SystemExit(f"unknown config {config}")
 
 
+def max_over_ranks(dist, value: float, device) -> float:
+    """The slowest rank's time: what a multi-GPU number is quoted on (all_reduce MAX; identity without a process group)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed_offset(rank: int) -> int:
+    """Replicas only: rank r simplifies its own polynomial of the same shape, seeded by r."""
+    return int(rank)
+
+
+def aggregate_value(n_sort_terms: int, world: int, ms_per_step: float) -> float:
+    """Whole-job throughput: the terms all ranks processed / the slowest rank's time per step."""
+    return n_sort_terms * world / (ms_per_step * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -192,7 +212,7 @@ def main():
     B.lib()                                             # fail loudly if libpolylab.so is missing
     steps, warmup = max(args.steps, 1), max(args.warmup, 3)
 
-    kind, polys, tol, desc, n_sort = workload(args.config, args.nterms, seed_offset=rank)
+    kind, polys, tol, desc, n_sort = workload(args.config, args.nterms, seed_offset=replica_seed_offset(rank))
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     dpolys = [(dev(p.coef), dev(p.exps)) for p in polys]
     ws = B.Workspace(torch.device("cuda", local_rank))
@@ -239,12 +259,9 @@ def main():
     barrier()
     clocks = sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(dist, ms_total, "cuda")
     ms_per_step = ms_total / steps
-    value = n_sort * world / (ms_per_step * 1e-3)
+    value = aggregate_value(n_sort, world, ms_per_step)
 
     # ---- roofline of the dominant kernel: one radix pass moves 2*N*(W+8) algorithmic bytes
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -319,13 +336,10 @@ def main():
         e1.record()
         barrier()
         ms2 = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms2], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t.item())
+        ms2 = max_over_ranks(dist, ms2, "cuda")
         esize = e.element_size() if isinstance(e, torch.Tensor) else e.dtype.itemsize
         d2h = int(c.shape[0]) * (8 + int(e.shape[1]) * esize)
-        e2e = {"value": n_sort * world / (ms2 / k2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        e2e = {"value": aggregate_value(n_sort, world, ms2 / k2), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h) + 8, "steps": k2, "ms_per_step": ms2 / k2}
         del hp
 
