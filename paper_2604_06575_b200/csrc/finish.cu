@@ -65,6 +65,12 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ 
         else hi = mid;
     }
     tile_start[t] = lo;
+    // a tile starts a new bucket: its first prefix must be above the record before it (finish_kernel checks the order
+    // inside a tile; together they prove that every bucket is contiguous, i.e. that the prefix passes were stable)
+    if (lo < n) {
+        const K kb = keys[lo - 1], kf = keys[lo];
+        if (!key_lt(kb, kf) || same_prefix(kb, kf, pfx_pos)) ctl->unsorted = 1u;
+    }
 }
 
 // --------------------------------------------------------------------------------- local radix pass

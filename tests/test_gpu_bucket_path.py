@@ -179,3 +179,13 @@ def test_fused_pack_checks_caller_bounds():
     c, e, st = B.simplify(dev(p.coef), dev(p.exps), 0.0, max_exp=[255] * 16, flags=FORCE, return_stats=True)
     assert st.prefix_passes >= 1
     assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c.cpu().numpy(), e.cpu().numpy())
+
+
+def test_unstable_prefix_passes_are_detected_on_the_bucket_path():
+    """POLYLAB_FLAG_DEBUG_UNSTABLE breaks the stability of the radix passes; with two prefix passes the array is then not
+    sorted by prefix, the finish kernel's prefix-order checks (inside a tile and at every tile start) must see it and the
+    call must re-run on the LSD path with ballot ranking."""
+    p, tol = W.config5(2_000_000)
+    c, e, st = run(p, tol, flags=B.FLAG_DEBUG_UNSTABLE)
+    assert st.rank_fallback == 1 and st.prefix_passes == 0 and st.sort_passes == 16
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
