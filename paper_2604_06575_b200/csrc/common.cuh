@@ -96,6 +96,8 @@ __device__ __forceinline__ uint32_t key_get_field(const Key128& k, int shift, in
 // key from its most / least significant 64-bit halves (for a 64-bit key both arguments are the key)
 __device__ __forceinline__ void key_from_halves(uint64_t& k, uint64_t hi, uint64_t lo) { (void)hi; k = lo; }
 __device__ __forceinline__ void key_from_halves(Key128& k, uint64_t hi, uint64_t lo) { k.hi = hi; k.lo = lo; }
+__device__ __forceinline__ uint64_t key_top64(uint64_t k) { return k; }          // most significant 64 bits of a key
+__device__ __forceinline__ uint64_t key_top64(const Key128& k) { return k.hi; }
 __device__ __forceinline__ void key_zero(uint64_t& k) { k = 0; }
 __device__ __forceinline__ void key_zero(Key128& k) { k.lo = 0; k.hi = 0; }
 

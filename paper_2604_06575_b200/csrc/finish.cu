@@ -270,17 +270,47 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
         bool descending = false;
-#pragma unroll 4
-        for (uint32_t i = tid; i < n_loc; i += THREADS) {
-            const K k = gkeys[i];
-            bool head = true;
-            if (i > 0) {
-                const K kp = gkeys[i - 1];
-                head = !same_prefix(k, kp, a.pfx_pos);
-                descending |= head && key_lt(k, kp);
+        if (a.pfx_pos >= 8 * (int)sizeof(K) - 64) {
+            // the prefix lies in the key's most significant 64 bits: only those are fetched from the left neighbour, and
+            // four records per thread are in flight (all loads issued before the first use)
+            for (uint32_t i0 = tid; i0 < n_loc; i0 += 4 * THREADS) {
+                K k[4];
+                uint64_t ph[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * THREADS;
+                    key_zero(k[u]);
+                    ph[u] = 0;
+                    if (i < n_loc) {
+                        k[u] = gkeys[i];
+                        if (i > 0) ph[u] = *(const uint64_t*)(gkeys + (i - 1));     // Key128 is stored (hi, lo)
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * THREADS;
+                    if (i < n_loc) {
+                        const int hs = a.pfx_pos - (8 * (int)sizeof(K) - 64);              // prefix position inside the top half
+                        const uint64_t pk = key_top64(k[u]) >> hs, pp = ph[u] >> hs;
+                        const bool head = (i == 0) || pk != pp;
+                        descending |= (i > 0) && pk < pp;
+                        bx[i] = full ? i : key_get_field(k[u], a.pfx_pos - rbits, rbits);
+                        py[i] = head ? 1 : 0;
+                    }
+                }
             }
-            bx[i] = full ? i : key_get_field(k, a.pfx_pos - rbits, rbits);
-            py[i] = head ? 1 : 0;
+        } else {
+            for (uint32_t i = tid; i < n_loc; i += THREADS) {
+                const K k = gkeys[i];
+                bool head = true;
+                if (i > 0) {
+                    const K kp = gkeys[i - 1];
+                    head = !same_prefix(k, kp, a.pfx_pos);
+                    descending |= head && key_lt(k, kp);
+                }
+                bx[i] = full ? i : key_get_field(k, a.pfx_pos - rbits, rbits);
+                py[i] = head ? 1 : 0;
+            }
         }
         if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
         __syncthreads();
