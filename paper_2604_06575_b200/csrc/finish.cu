@@ -246,6 +246,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     uint32_t* whist = (uint32_t*)(smem_raw + FinishSmem::off_whist);
     uint32_t* scratch = (uint32_t*)(smem_raw + FinishSmem::off_scratch);   // [0..NW+1] scans, [40] tile, [41] base
     double* scs = (double*)smem_raw;               // coefficients in sorted order, over X / Y once the sort is done
+    static_assert((size_t)FinishSmem::NW * kFinBins * 2 >= (size_t)kFinCap * 2, "the inverse permutation borrows the histogram rows");
     __shared__ uint32_t wagg_f[NW];
     __shared__ double wagg_v[NW];
 
@@ -368,6 +369,16 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
         __syncthreads();
         for (uint32_t i = tid; i < n_loc; i += THREADS) py[i] = (uint16_t)(cur[i] & 0x1fffu);
         __syncthreads();
+        // coefficients into sorted order through the INVERSE permutation: the global read is coalesced (a gather would
+        // touch one 32-byte sector per 8-byte coefficient), the permuted write goes to shared memory
+        {
+            uint16_t* inv = (uint16_t*)whist;      // the histograms are dead until the next pass
+            for (uint32_t i = tid; i < n_loc; i += THREADS) inv[py[i]] = (uint16_t)i;
+            __syncthreads();
+#pragma unroll 4
+            for (uint32_t i = tid; i < n_loc; i += THREADS) scs[inv[i]] = gcoef[i];
+            __syncthreads();
+        }
 
         // ---- gather through the permutation: heads of runs of equal keys, sums since the last head, order check
         hm = 0; nh = 0; acc = 0.0;
@@ -381,8 +392,7 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
                 if (first + j < n_loc) {
                     const uint32_t r = py[first + j];
                     const K kk = gkeys[r];
-                    const double c = gcoef[r];
-                    scs[first + j] = c;            // own positions only; X / Y are dead after the last pass
+                    const double c = scs[first + j];
                     const bool head = !hp || !key_eq(kk, kp);
                     viol |= hp && key_lt(kk, kp);
                     if (head) { hm |= 1u << j; ++nh; acc = c; }
