@@ -113,12 +113,19 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
     const uint32_t wbeg = min(warp * per, n_loc), wend = min(wbeg + per, n_loc);
     if (RANKS) {
         // sweep 1 counts AND ranks: the atomic's old value is the record's rank among its warp's records of the digit
-        for (uint32_t base = wbeg; base < wend; base += 32u) {
-            const uint32_t i = base + lane;
-            if (i < wend) {
-                const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
+        for (uint32_t base = wbeg; base < wend; base += 64u) {      // two rounds per iteration: both loads first
+            const uint32_t i0 = base + lane, i1 = i0 + 32u;
+            const uint32_t e0 = (i0 < wend) ? in[i0] : 0u, e1 = (i1 < wend) ? in[i1] : 0u;
+            if (i0 < wend) {
+                const uint32_t d = (FIRST ? e0 : (e0 >> 13)) & mask;
                 const uint32_t sh = (d & 1u) * 16u;
-                ranks[i] = (uint16_t)(atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh);
+                ranks[i0] = (uint16_t)(atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh);
+            }
+            __syncwarp();
+            if (i1 < wend) {
+                const uint32_t d = (FIRST ? e1 : (e1 >> 13)) & mask;
+                const uint32_t sh = (d & 1u) * 16u;
+                ranks[i1] = (uint16_t)(atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh);
             }
             __syncwarp();
         }
