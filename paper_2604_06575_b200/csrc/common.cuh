@@ -152,6 +152,7 @@ struct Control {
     uint32_t unsorted;                       // S3 saw a key smaller than its predecessor (the sort was not stable)
     uint32_t overflow;                       // bucket path: a bucket does not fit a finish tile (skewed prefix digits)
     uint32_t refinish;                       // bucket path: finish tiles that needed the full local digit list
+    uint32_t fin_count;                      // bucket path: tiles that own records (length of the work list)
 };
 
 constexpr int kTicketReduce = kMaxPasses;

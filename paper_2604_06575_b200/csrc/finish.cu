@@ -22,7 +22,7 @@
 //                        look-back: a tile only knows its count at the very end, and waiting in order for slow
 //                        predecessors left SMs idle); two blocks per SM overlap one tile's loads with the other's
 //                        shared-memory passes.
-//   tile_scan_kernel     exclusive scan of the tiles' survivor counts (one block).
+//   tile_sum_kernel, tile_scan_kernel   exclusive scan of the tiles' survivor counts (chunk sums, then the scan).
 //   emit_kernel          S5: one thread per output term finds its tile in the scanned counts (binary search) and
 //                        unpacks the key into the caller's output -- order-preserving compaction across tiles.
 //                        HBM traffic of the three: N*(W+8) read, U'*(W+8) written and read, U'*(8+E) written.
@@ -41,35 +41,60 @@ namespace polylab {
 
 // ------------------------------------------------------------------------------------- tile bounds
 
+// start of tile t: the first position >= t*fin_tile where the prefix changes (0 for t = 0, n past the end)
 template <typename K>
-__global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ keys, uint32_t n, int pfx_pos,
-                                                          uint32_t fin_tile, uint32_t ntiles,
-                                                          uint32_t* __restrict__ tile_start, Control* ctl)
+__device__ __forceinline__ uint32_t tile_first_change(const K* __restrict__ keys, uint32_t n, int pfx_pos, uint32_t fin_tile,
+                                                      uint32_t t, bool* overflow)
 {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t > ntiles) return;
-    if (t == 0) { tile_start[0] = 0u; return; }
+    if (t == 0) return 0u;
     const uint64_t s64 = (uint64_t)t * fin_tile;
-    if (s64 >= n) { tile_start[t] = n; return; }
+    if (s64 >= n) return n;
     const uint32_t s = (uint32_t)s64;
     const K ref = keys[s - 1];
     uint32_t lo = s, hi = (uint32_t)min((uint64_t)n, s64 + (uint64_t)(kFinCap - fin_tile));
     if (hi < n && same_prefix(keys[hi], ref, pfx_pos)) {      // the bucket of record s-1 runs past what a tile can own
-        ctl->overflow = 1u;
-        tile_start[t] = s;
-        return;
+        *overflow = true;
+        return s;
     }
     while (lo < hi) {                                         // smallest p in [lo, hi] whose prefix differs (p == n counts)
         const uint32_t mid = lo + (hi - lo) / 2;
         if (same_prefix(keys[mid], ref, pfx_pos)) lo = mid + 1;
         else hi = mid;
     }
-    tile_start[t] = lo;
-    // a tile starts a new bucket: its first prefix must be above the record before it (finish_kernel checks the order
-    // inside a tile; together they prove that every bucket is contiguous, i.e. that the prefix passes were stable)
-    if (lo < n) {
-        const K kb = keys[lo - 1], kf = keys[lo];
-        if (!key_lt(kb, kf) || same_prefix(kb, kf, pfx_pos)) ctl->unsorted = 1u;
+    return lo;
+}
+
+template <typename K>
+__global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ keys, uint32_t n, int pfx_pos,
+                                                          uint32_t fin_tile, uint32_t ntiles,
+                                                          uint32_t* __restrict__ tile_start, uint32_t* __restrict__ worklist,
+                                                          Control* ctl)
+{
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    bool overflow = false, owns = false;
+    if (t <= ntiles) {
+        const uint32_t lo = tile_first_change(keys, n, pfx_pos, fin_tile, t, &overflow);
+        tile_start[t] = lo;
+        if (t < ntiles) {
+            const uint32_t hi = tile_first_change(keys, n, pfx_pos, fin_tile, t + 1, &overflow);
+            owns = (uint64_t)lo < ((uint64_t)t + 1) * fin_tile && hi > lo;        // a bucket starts inside the tile
+        }
+        // a tile starts a new bucket: its first prefix must be above the record before it (finish_kernel checks the
+        // order inside a tile; together they prove that every bucket is contiguous, i.e. that the prefix passes were stable)
+        if (t > 0 && lo < n && !overflow) {
+            const K kb = keys[lo - 1], kf = keys[lo];
+            if (!key_lt(kb, kf) || same_prefix(kb, kf, pfx_pos)) ctl->unsorted = 1u;
+        }
+        if (overflow) ctl->overflow = 1u;
+    }
+    // work list of the tiles that own records (any order: tiles are independent), one atomic per warp
+    const unsigned m = __ballot_sync(kFullMask, owns);
+    if (m) {
+        const unsigned lane = lane_id();
+        uint32_t base = 0;
+        if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(&ctl->fin_count, (uint32_t)__popc(m));
+        base = __shfl_sync(kFullMask, base, __ffs(m) - 1);
+        if (owns) worklist[base + __popc(m & lanemask_lt())] = t;
     }
 }
 
@@ -83,7 +108,9 @@ struct FinishSmem {
     static constexpr size_t off_y = (size_t)kFinCap * 4;
     static constexpr size_t off_p = off_y + (size_t)kFinCap * 4;
     static constexpr size_t off_whist = off_p + (size_t)kFinCap * 2;
-    static constexpr size_t off_scratch = off_whist + (size_t)NW * kFinBins * 2;
+    // the histogram rows double as the inverse permutation (16 bits per record) between the sort and the sums
+    static constexpr size_t whist_bytes = (size_t)NW * kFinBins * 2 > (size_t)kFinCap * 2 ? (size_t)NW * kFinBins * 2 : (size_t)kFinCap * 2;
+    static constexpr size_t off_scratch = off_whist + whist_bytes;
     static constexpr size_t bytes = off_scratch + 64 * 4;
 };
 
@@ -101,7 +128,8 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
                                            uint32_t* whist, uint32_t* scratch, uint16_t* ranks)
 {
     constexpr int NW = FinishSmem::NW, ROW = kFinBins / 2;    // words per histogram row
-    static_assert(kFinBins == kFinThreads, "one thread per bin in the scan step");
+    constexpr int BPT = kFinBins / kFinThreads;               // bins per thread in the scan step
+    static_assert(BPT >= 1 && BPT * kFinThreads == kFinBins, "whole bins per thread in the scan step");
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t mask = (1u << dbits) - 1u;
     uint32_t* my_hist = whist + warp * ROW;
@@ -137,16 +165,22 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
     }
     __syncthreads();
     {
-        uint32_t c[NW];
+        uint32_t c[BPT][NW];
         uint32_t count = 0;
 #pragma unroll
-        for (int w = 0; w < NW; ++w) c[w] = h16[w * kFinBins + tid];
+        for (int q = 0; q < BPT; ++q)
 #pragma unroll
-        for (int w = 0; w < NW; ++w) { const uint32_t x = c[w]; c[w] = count; count += x; }
+            for (int w = 0; w < NW; ++w) c[q][w] = h16[w * kFinBins + tid * BPT + q];
+#pragma unroll
+        for (int q = 0; q < BPT; ++q)
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { const uint32_t x = c[q][w]; c[q][w] = count; count += x; }
         uint32_t total;
         const uint32_t bin_start = block_exclusive_scan<kFinThreads>(count, scratch, &total);
 #pragma unroll
-        for (int w = 0; w < NW; ++w) h16[w * kFinBins + tid] = (uint16_t)(bin_start + c[w]);
+        for (int q = 0; q < BPT; ++q)
+#pragma unroll
+            for (int w = 0; w < NW; ++w) h16[w * kFinBins + tid * BPT + q] = (uint16_t)(bin_start + c[q][w]);
     }
     __syncthreads();
     if (RANKS) {
@@ -198,7 +232,8 @@ struct FinishArgs {
     uint32_t n, ntiles;
     uint32_t fin_tile;              // positions per tile; a tile owns at most kFinCap records
     const uint32_t* tile_start;     // [ntiles + 1]
-    uint32_t* tile_state;           // [ntiles] look-back words, zero before the kernel
+    const uint32_t* worklist;       // the ctl->fin_count tiles that own records
+    uint32_t* tile_state;           // [ntiles + 1] survivors per tile, zero before the kernel
     int pfx_pos;                    // the prefix is the key bits at positions >= pfx_pos
     int fast_bits;                  // most key bits below the prefix the first attempt sorts on (test hook; 32 = no limit)
     double tol;
@@ -242,7 +277,7 @@ __device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, u
 // ------------------------------------------------------------------------------------ finish kernel
 
 template <typename K>
-__global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_constant__ FinishArgs a, const __grid_constant__ Plan plan)
+__global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(const __grid_constant__ FinishArgs a, const __grid_constant__ Plan plan)
 {
     constexpr int THREADS = kFinThreads, CAP = kFinCap, NW = THREADS / 32;
     static_assert(CAP <= 8192 && CAP / THREADS <= 32, "13-bit record indices in the sort elements, 32-bit head masks");
@@ -253,15 +288,14 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
     uint32_t* whist = (uint32_t*)(smem_raw + FinishSmem::off_whist);
     uint32_t* scratch = (uint32_t*)(smem_raw + FinishSmem::off_scratch);   // [0..NW+1] scans, [40] tile, [41] base
     double* scs = (double*)smem_raw;               // coefficients in sorted order, over X / Y once the sort is done
-    static_assert((size_t)FinishSmem::NW * kFinBins * 2 >= (size_t)kFinCap * 2, "the inverse permutation borrows the histogram rows");
+    static_assert(FinishSmem::whist_bytes >= (size_t)kFinCap * 2, "the inverse permutation borrows the histogram rows");
     __shared__ uint32_t wagg_f[NW];
     __shared__ double wagg_v[NW];
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (a.ctl->overflow) return;                   // set by tile_bounds_kernel: the call will re-run on the LSD path
-    if (tid == 0) scratch[40] = atomicAdd(&a.ctl->ticket[kTicketFinish], 1u);
-    __syncthreads();
-    const uint32_t tile = scratch[40];
+    if (blockIdx.x >= a.ctl->fin_count) return;    // the grid is sized for the most tiles that can own records
+    const uint32_t tile = a.worklist[blockIdx.x];
     const uint32_t lo = a.tile_start[tile], hi = a.tile_start[tile + 1];
     uint32_t n_loc = 0;
     if ((uint64_t)lo < ((uint64_t)tile + 1) * a.fin_tile && hi > lo) n_loc = min(hi - lo, (uint32_t)CAP);
@@ -510,39 +544,59 @@ __global__ void __launch_bounds__(kFinThreads, 2) finish_kernel(const __grid_con
 
 // ------------------------------------------------------------------------------- S4/S5 across tiles
 
-// Exclusive scan of the tiles' survivor counts, in place (one block); tile_off[ntiles] = U'.
-__global__ void __launch_bounds__(1024) tile_scan_kernel(uint32_t* __restrict__ tile_off, uint32_t ntiles, Control* ctl,
+// Exclusive scan of the tiles' survivor counts, in place, in two small kernels: per-chunk sums, then every block adds the
+// sums of the chunks before it to the scan of its own chunk; tile_off[ntiles] = U'.
+constexpr uint32_t kScanChunk = 1024u * 4u;
+
+__global__ void __launch_bounds__(1024) tile_sum_kernel(const uint32_t* __restrict__ tile_cnt, uint32_t ntiles,
+                                                        uint32_t* __restrict__ chunk_sum)
+{
+    __shared__ uint32_t scratch[34];
+    const uint32_t base = blockIdx.x * kScanChunk;
+    uint32_t sum = 0;
+#pragma unroll
+    for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t t = base + j * 1024u + threadIdx.x;
+        if (t < ntiles) sum += tile_cnt[t];
+    }
+    uint32_t total;
+    (void)block_exclusive_scan<1024>(sum, scratch, &total);
+    if (threadIdx.x == 0) chunk_sum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) tile_scan_kernel(uint32_t* __restrict__ tile_off, uint32_t ntiles,
+                                                         const uint32_t* __restrict__ chunk_sum, Control* ctl,
                                                          int64_t* out_count_device)
 {
     __shared__ uint32_t scratch[34];
-    __shared__ uint32_t running;
     const unsigned tid = threadIdx.x;
-    if (tid == 0) running = 0u;
-    __syncthreads();
-    for (uint32_t base = 0; base < ntiles; base += 1024u * 4u) {
-        uint32_t v[4], sum = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t t = base + tid * 4u + j;
-            v[j] = t < ntiles ? tile_off[t] : 0u;
-            sum += v[j];
-        }
-        uint32_t total;
-        uint32_t excl = block_exclusive_scan<1024>(sum, scratch, &total) + running;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t t = base + tid * 4u + j;
-            if (t < ntiles) tile_off[t] = excl;
-            excl += v[j];
-        }
-        __syncthreads();
-        if (tid == 0) running += total;
+    uint32_t before = 0;                           // survivors of the chunks before this block's (at most 1024 chunks)
+    {
+        uint32_t x = 0;
+        for (uint32_t c = tid; c < blockIdx.x; c += 1024u) x += chunk_sum[c];
+        (void)block_exclusive_scan<1024>(x, scratch, &before);
         __syncthreads();
     }
-    if (tid == 0) {
-        tile_off[ntiles] = running;
-        ctl->survivors = running;
-        if (out_count_device) *out_count_device = (int64_t)running;
+    const uint32_t base = blockIdx.x * kScanChunk;
+    uint32_t v[4], sum = 0;
+#pragma unroll
+    for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t t = base + tid * 4u + j;
+        v[j] = t < ntiles ? tile_off[t] : 0u;
+        sum += v[j];
+    }
+    uint32_t total;
+    uint32_t excl = block_exclusive_scan<1024>(sum, scratch, &total) + before;
+#pragma unroll
+    for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t t = base + tid * 4u + j;
+        if (t < ntiles) tile_off[t] = excl;
+        excl += v[j];
+    }
+    if (blockIdx.x == gridDim.x - 1 && tid == 0) {
+        tile_off[ntiles] = before + total;
+        ctl->survivors = before + total;
+        if (out_count_device) *out_count_device = (int64_t)(before + total);
     }
 }
 
@@ -569,14 +623,14 @@ __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitA
 template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
                            const double* coefs, double tol, void* ukeys, double* usums, double* out_coef, void* out_exps,
-                           int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, Control* ctl,
-                           int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
+                           int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist,
+                           uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
     const int nlow = plan.npasses - prefix_passes;
     const int pfx_pos = plan.digit_pos[nlow];
     tile_bounds_kernel<K><<<(ntiles + 1 + 255) / 256, 256, 0, stream>>>((const K*)keys, (uint32_t)n, pfx_pos, (uint32_t)fin_tile,
-                                                                       ntiles, tile_start, ctl);
+                                                                       ntiles, tile_start, worklist, ctl);
     auto kern = finish_kernel<K>;
     constexpr size_t smem = FinishSmem::bytes;
     static bool attr_set = false;
@@ -586,11 +640,16 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     }
     FinishArgs a;
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
-    a.tile_start = tile_start; a.tile_state = tile_state;
+    a.tile_start = tile_start; a.tile_state = tile_state; a.worklist = worklist;
     a.pfx_pos = pfx_pos; a.fast_bits = nfast > 0 ? nfast * 8 : 32; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
-    kern<<<ntiles, kFinThreads, smem, stream>>>(a, plan);
+    // a tile owns records only if a bucket starts in it: at most one tile per bucket, at most 2^T buckets
+    const int T = plan.key_bits - pfx_pos;
+    const uint32_t fin_blocks = (T < 31 && (1u << T) < ntiles) ? (1u << T) : ntiles;
+    kern<<<fin_blocks, kFinThreads, smem, stream>>>(a, plan);
     if (after_tiles) cudaEventRecord(after_tiles, stream);
-    tile_scan_kernel<<<1, 1024, 0, stream>>>(tile_state, ntiles, ctl, out_count_device);
+    const uint32_t nchunks = (ntiles + kScanChunk - 1) / kScanChunk;
+    tile_sum_kernel<<<nchunks, 1024, 0, stream>>>(tile_state, ntiles, chunk_sum);
+    tile_scan_kernel<<<nchunks, 1024, 0, stream>>>(tile_state, ntiles, chunk_sum, ctl, out_count_device);
     EmitArgs e;
     e.ukeys = ukeys; e.usums = usums; e.ntiles = ntiles; e.tile_start = tile_start; e.tile_off = tile_state;
     e.out_coef = out_coef; e.out_exps = out_exps; e.exp_bytes = exp_bytes;
@@ -600,20 +659,20 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (blocks < 1) blocks = 1;
     emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
-    return 4;
+    return 5;
 }
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles,
-                  cudaStream_t stream)
+                  uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist, uint32_t* chunk_sum, Control* ctl,
+                  int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;
     if (plan.key_bytes == 8)
         return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                         exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, after_tiles, stream);
+                                         exp_bytes, out_capacity, tile_start, tile_state, worklist, chunk_sum, ctl, out_count_device, after_tiles, stream);
     return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                   exp_bytes, out_capacity, tile_start, tile_state, ctl, out_count_device, after_tiles, stream);
+                                   exp_bytes, out_capacity, tile_start, tile_state, worklist, chunk_sum, ctl, out_count_device, after_tiles, stream);
 }
 
 }  // namespace polylab

@@ -16,14 +16,15 @@ constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from sha
 constexpr int kPruneThreads = 256;
 constexpr int kPruneItems = 8;
 
-constexpr int kFinThreads = 512;    // bucket path (finish.cu): two blocks per SM
-constexpr int kFinCap = 8192;       // most records a finish tile can own (10 bytes of shared memory each); tile t owns the
+constexpr int kFinBlocksPerSM = 4;
+constexpr int kFinThreads = 256;    // bucket path (finish.cu): four blocks per SM (swept on B200: 512 x 8192 x 2 4.83 ms, 256 x 4608 x 4 4.29 ms)
+constexpr int kFinCap = 4608;       // most records a finish tile can own (10 bytes of shared memory each); tile t owns the
                                     // buckets that start in positions [t*fin_tile, (t+1)*fin_tile), so a bucket may be
                                     // as long as kFinCap - fin_tile
 constexpr int kFinDigit = 9;         // local sort: 9-bit digits, 512 bins
 constexpr int kFinBins = 1 << kFinDigit;
 constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
-constexpr int kFinMinTile = 4096;   // smallest fin_tile the planner picks (workspace sizing)
+constexpr int kFinMinTile = 512;    // smallest fin_tile the planner picks (workspace sizing)
 
 inline int sort_tile(int key_bytes) { return kSortThreads * (key_bytes == 8 ? kSortItems64 : kSortItems128); }
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
@@ -92,12 +93,12 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
 
 // Bucket path (finish.cu): the pairs are sorted by their top `prefix_passes` plan digits; finish every bucket in
 // shared memory and emit the simplified polynomial (S2 rest + S3 + S4 + S5).  (ukeys, usums): scratch for n pairs.
-// tile_start, tile_state: ceil(n/fin_tile)+1 words each, tile_state zeroed.  after_tiles (optional): recorded
+// tile_start, tile_state, worklist: ceil(n/fin_tile)+1 words each, tile_state zeroed; chunk_sum: ceil(tiles/4096) words.  after_tiles (optional): recorded
 // between the finish kernel and the scan/emit kernels, for the stage timing.  Sets ctl->overflow (nothing emitted) when a bucket is too long,
 // ctl->unsorted when the prefix order or the local order check fails, ctl->distinct, ctl->survivors.
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles,
-                  cudaStream_t stream);
+                  uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist, uint32_t* chunk_sum, Control* ctl,
+                  int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream);
 
 }  // namespace polylab
