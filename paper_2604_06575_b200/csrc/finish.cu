@@ -294,7 +294,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (a.ctl->overflow) return;                   // set by tile_bounds_kernel: the call will re-run on the LSD path
-    if (blockIdx.x >= a.ctl->fin_count) return;    // the grid is sized for the most tiles that can own records
+    const uint32_t fin_count = a.ctl->fin_count;
+    if (blockIdx.x == 0 && tid == 0 && fin_count > gridDim.x) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
+    if (blockIdx.x >= fin_count) return;           // the grid is sized for the most tiles that can own records
     const uint32_t tile = a.worklist[blockIdx.x];
     const uint32_t lo = a.tile_start[tile], hi = a.tile_start[tile + 1];
     uint32_t n_loc = 0;

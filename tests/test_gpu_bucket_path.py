@@ -189,3 +189,33 @@ def test_unstable_prefix_passes_are_detected_on_the_bucket_path():
     c, e, st = run(p, tol, flags=B.FLAG_DEBUG_UNSTABLE)
     assert st.rank_fallback == 1 and st.prefix_passes == 0 and st.sort_passes == 16
     assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_randomised_shapes_both_paths(seed):
+    """Random variable counts, dtypes, exponent ranges, duplication and sizes: the forced bucket path and the LSD path
+    must both be in parity with the oracle and agree on the monomial set (a poor man's fuzzer; compute-sanitizer is
+    not available on the GPU pool)."""
+    r = np.random.default_rng(1000 + seed)
+    dtype = [np.uint8, np.uint16, np.uint32][int(r.integers(0, 3))]
+    nvars = int(r.integers(1, 17))
+    his = r.choice([1, 2, 4, 16, 200, 256, 1000, 60000][: {np.uint8: 6, np.uint16: 8, np.uint32: 8}[dtype]], size=nvars)
+    while sum(int(h - 1).bit_length() for h in his) > 128:          # keep the key within 128 bits
+        his[int(r.integers(0, nvars))] = 2
+    n = int(r.choice([1, 7, 300, 4607, 4609, 20_000, 60_001]))
+    dup = int(r.choice([1, 2, 5, 50]))
+    pool = np.stack([r.integers(0, h, size=max(1, n // dup)) for h in his], axis=1).astype(dtype)
+    exps = np.ascontiguousarray(pool[r.integers(0, len(pool), size=n)])
+    coef = r.standard_normal(n)
+    if seed % 4 == 0:
+        coef[: n // 2] = -coef[n - n // 2:][::-1]                    # some cancellation
+    tol = [0.0, 1e-14, 0.5][seed % 3]
+    p = W.Poly(coef, exps)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol, flags=FORCE)
+    assert_parity(res, c, e)
+    c0, e0, st0 = run(p, tol, flags=B.FLAG_NO_BUCKET)
+    assert st0.prefix_passes == 0
+    assert_parity(res, c0, e0)
+    if tol == 0.0:
+        assert (e == e0).all()
