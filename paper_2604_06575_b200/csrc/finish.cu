@@ -7,34 +7,37 @@
 // finished on chip.  This file is that finish:
 //
 //   tile_bounds_kernel   cuts the prefix-sorted array into tiles of whole buckets: tile t owns the buckets that
-//                        START in positions [t*TILE, (t+1)*TILE); tile_start[t] is found by a binary search for the
+//                        START in positions [t*TILE, (t+1)*TILE); a tile's start is found by a binary search for the
 //                        first change of prefix at or after t*TILE.  A bucket longer than CAP - TILE sets
 //                        ctl->overflow and the call falls back to the plain LSD path.  TILE is chosen per call
-//                        (api.cu): CAP minus room for the longest bucket expected from N / 2^T.
-//   finish_kernel        one block per tile (<= CAP records).  Shared memory holds 10 bytes per record, not the record:
-//                        a 32-bit "sort word" cut out of the key, its bucket ordinal and two 16-bit permutation
-//                        buffers.  The block sorts the permutation by the sort word's digits (stable counting-sort
-//                        passes, one shared-memory atomic per record and sweep) and then by bucket ordinal, gathers
-//                        keys and coefficients through the permutation (they were just streamed, so the gather hits
-//                        L2), and -- records of equal monomials now being adjacent and no run crossing a tile -- does
-//                        the segmented sum (S3) and the prune (S4, keep iff |s| > tol, reading A2) and leaves the
-//                        tile's survivors compacted in order at the tile's own position.  Tiles are independent (no
+//                        (api.cu): CAP minus room for the longest bucket expected from N / 2^T.  Tiles that own
+//                        records go on a work list; every tile start is checked to be a strict prefix increase.
+//   finish_kernel        one block per work-list tile (<= CAP = 4608 records, 256 threads, four blocks per SM).
+//                        Shared memory holds 10 bytes per record, not the record: two 32-bit ping-pong buffers of sort
+//                        elements (record index in the low 13 bits, the not yet consumed sort bits above) and one
+//                        16-bit array (head flags -> bucket ordinals -> ranks -> final permutation).  The block
+//                        streams its keys once (bucket heads, the key bits below the prefix), builds the composite
+//                        sort word "bucket ordinal above the top key bits" (<= 27 bits), sorts it with stable
+//                        counting-sort passes on 9-bit digits, brings the coefficients into sorted order through the
+//                        inverse permutation (coalesced read), gathers the keys through the permutation (L2 hits),
+//                        and -- records of equal monomials now being adjacent and no run crossing a tile -- does the
+//                        segmented sum (S3) and the prune (S4, keep iff |s| > tol, reading A2) and leaves the tile's
+//                        survivors compacted in order at the tile's own position.  Tiles are independent (no
 //                        look-back: a tile only knows its count at the very end, and waiting in order for slow
-//                        predecessors left SMs idle); two blocks per SM overlap one tile's loads with the other's
-//                        shared-memory passes.
+//                        predecessors left SMs idle).
 //   tile_sum_kernel, tile_scan_kernel   exclusive scan of the tiles' survivor counts (chunk sums, then the scan).
 //   emit_kernel          S5: one thread per output term finds its tile in the scanned counts (binary search) and
 //                        unpacks the key into the caller's output -- order-preserving compaction across tiles.
-//                        HBM traffic of the three: N*(W+8) read, U'*(W+8) written and read, U'*(8+E) written.
+//                        HBM traffic of all of them: N*(W+8) read, U'*(W+8) written and read, U'*(8+E) written.
 //
-// The local sort first uses only the `nfast` most significant digits below the prefix (enough to separate the
-// distinct keys of a bucket unless two of them share all those bits) and checks the order against the full keys while
-// it computes the head flags; a tile that fails the check re-sorts on every low digit, re-cutting the sort word from
-// the keys for each group of digits (ctl->refinish counts such tiles).
+// The local sort first uses only as many key bits below the prefix as fit the composite sort word (enough to separate
+// the distinct keys of a bucket unless two of them share all those bits) and checks the order against the full keys
+// while it computes the head flags; a tile that fails the check re-sorts on every bit below the prefix, 18 at a time,
+// cutting them out of the keys through the current permutation (ctl->refinish counts such tiles).
 //
 // Summation order (reading A6): equal keys keep their input order through every stable step; a tile sums left to
 // right inside a thread and by a fixed shuffle tree across threads -- a function of the data layout only, so
-// results are bit-reproducible run to run.
+// results are bit-reproducible run to run (the work list's order varies, the tiles' results do not).
 #include "kernels.h"
 
 namespace polylab {
