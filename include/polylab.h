@@ -87,6 +87,10 @@ enum {
     POLYLAB_FLAG_NO_FUSED_PACK = 16u, /* bucket path: always run S1 as its own kernel.  By default, when the exponent rows
                                         are contiguous and 8 or 16 bytes long, the first radix pass packs the keys in
                                         registers (no key array is written and re-read) */
+    POLYLAB_FLAG_EXACT_BOUNDS = 32u,  /* S0 always reads every exponent.  By default a simplify call with >= 2^22 terms and
+                                        no max_exp_host takes the maxima of a sample of the rows, sizes the key fields by
+                                        their bit lengths, and lets S1's range check verify every row; a violation
+                                        re-runs the call with full bounds (stats->bounds_retry = 1).  Same result. */
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
                                         skew pre-check), so that small tests reach it and its overflow fallback */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
@@ -120,6 +124,8 @@ typedef struct polylab_stats {
                                 too long for a tile); the result then comes from the LSD path */
     int32_t refinish_tiles;  /* bucket path: tiles whose fast local sort failed the order check and re-sorted fully */
     int32_t plan_digits;     /* ceil(B/8): digits of the key layout = entries of digit_bits = LSD passes the plan needs */
+    int32_t bounds_sampled;  /* 1 if S0 ran on a sample of the rows (see POLYLAB_FLAG_EXACT_BOUNDS) */
+    int32_t bounds_retry;    /* 1 if the sampled bounds were violated and the call re-ran with full bounds */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

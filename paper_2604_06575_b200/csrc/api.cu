@@ -15,10 +15,12 @@ static thread_local char g_cuda_error[256] = "";
 // ballot ranking on the LSD path; a bucket of the bucket path was too long -> re-run on the LSD path
 constexpr int kRetrySafeRank = -1000;
 constexpr int kRetryNoBucket = -1001;
+constexpr int kRetryExactBounds = -1002;       // an exponent exceeded the field sized from the sampled maxima
 
 struct Attempt {
     bool safe_rank;        // ballot-matching radix passes, LSD path only
     bool allow_bucket;     // may take the bucket path (finish.cu)
+    bool exact_bounds;     // S0 reads every row (otherwise large inputs are sampled and S1's range check verifies)
 };
 
 static bool cuda_failed(cudaError_t e, const char* what)
@@ -31,6 +33,8 @@ static bool cuda_failed(cudaError_t e, const char* what)
     do {                                                         \
         if (cuda_failed((call), #call)) return POLYLAB_ERR_CUDA; \
     } while (0)
+
+constexpr int64_t kSampleBoundsMinTerms = (int64_t)1 << 22;   // below this S0 reads every row
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 static inline int bitlen(uint64_t x) { int b = 0; while (x) { ++b; x >>= 1; } return b; }
@@ -162,11 +166,12 @@ static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb)
 static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
 {
     if (!st) return;
-    const int32_t launches = st->kernel_launches, fallback = st->rank_fallback, bfall = st->bucket_fallback;
+    const int32_t launches = st->kernel_launches, fallback = st->rank_fallback, bfall = st->bucket_fallback, bretry = st->bounds_retry;
     memset(st, 0, sizeof *st);
     st->kernel_launches = launches;
     st->rank_fallback = fallback;
     st->bucket_fallback = bfall;
+    st->bounds_retry = bretry;
     st->key_bits = plan.key_bits;
     st->key_bytes = plan.key_bytes;
     st->sort_passes = plan.npasses;
@@ -423,21 +428,30 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     // ---- S0: per-variable maxima (from the caller, or from the data with one read-back)
     uint64_t m[kMaxVars];
     uint32_t bound[kMaxVars];
+    bool sampled = false;
     if (o.max_exp_host) {
         for (int v = 0; v < nvars; ++v) { m[v] = o.max_exp_host[v]; bound[v] = o.max_exp_host[v]; }
     } else {
+        // Large inputs: maxima of a 0.3 % sample of the rows.  A field only needs the maximum's BIT LENGTH, so the bound is
+        // widened to the field's capacity and S1's range check proves that no unsampled exponent exceeds it; if one does,
+        // the call re-runs with S0 over every row.
+        sampled = !at.exact_bounds && nterms >= kSampleBoundsMinTerms && !(o.flags & POLYLAB_FLAG_EXACT_BOUNDS);
         PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
-        launches += launch_bounds(ev, nterms, nvars, ctl, 0, stream);
+        launches += sampled ? launch_bounds_sample(ev, nterms, nvars, ctl, 0, stream) : launch_bounds(ev, nterms, nvars, ctl, 0, stream);
         uint32_t mh[kMaxVars];
         PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp[0], sizeof(uint32_t) * nvars, cudaMemcpyDeviceToHost, stream));
         PL_CUDA(cudaStreamSynchronize(stream));
-        for (int v = 0; v < nvars; ++v) { m[v] = mh[v]; bound[v] = mh[v]; }
+        for (int v = 0; v < nvars; ++v) {
+            const uint32_t mv = sampled ? (bitlen(mh[v]) >= 32 ? 0xffffffffu : (1u << bitlen(mh[v])) - 1u) : mh[v];
+            m[v] = mv; bound[v] = mv;
+        }
     }
     tm.mark(POLYLAB_STAGE_BOUNDS);
     Plan plan;
     rc = make_plan(nvars, m, bound, &plan);
     if (rc != POLYLAB_OK) return rc;
     fill_stats(o.stats, plan, nterms);
+    if (o.stats) o.stats->bounds_sampled = sampled ? 1 : 0;
 
     const Layout L = make_layout(nterms, plan.key_bytes, 0, 0);
     if (avail < L.total) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
@@ -451,8 +465,9 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
     if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
-    return sort_reduce_emit(plan, k, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
-                            at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr);
+    rc = sort_reduce_emit(plan, k, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
+                          at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr);
+    return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
 }
 
 static bool wants_safe_rank(const polylab_opts* opts)
@@ -465,20 +480,25 @@ extern "C++" {
 template <typename F>
 static int run_attempts(const polylab_opts* opts, F once)
 {
-    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; }
-    Attempt at = {wants_safe_rank(opts), true};
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; opts->stats->bounds_retry = 0; }
+    Attempt at = {wants_safe_rank(opts), true, false};
     int rc = once(at);
-    if (rc == kRetryNoBucket) {
-        if (opts && opts->stats) opts->stats->bucket_fallback = 1;
-        at.allow_bucket = false;
+    for (int tries = 0; tries < 3 && (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank); ++tries) {
+        polylab_stats* st = opts ? opts->stats : nullptr;
+        if (rc == kRetryExactBounds) {             // each retry only ever tightens the attempt, so three suffice
+            if (st) st->bounds_retry = 1;
+            at.exact_bounds = true;
+        } else if (rc == kRetryNoBucket) {
+            if (st) st->bucket_fallback = 1;
+            at.allow_bucket = false;
+        } else {
+            if (st) st->rank_fallback = 1;
+            at.safe_rank = true;
+            at.allow_bucket = false;
+        }
         rc = once(at);
     }
-    if (rc == kRetrySafeRank) {
-        if (opts && opts->stats) opts->stats->rank_fallback = 1;
-        at.safe_rank = true;
-        at.allow_bucket = false;
-        rc = once(at);
-    }
+    if (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank) rc = POLYLAB_ERR_INTERNAL;
     return rc;
 }
 }  // extern "C++"

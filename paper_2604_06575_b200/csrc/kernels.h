@@ -33,6 +33,10 @@ constexpr int kPruneTile = kPruneThreads * kPruneItems;
 // S0: per-variable maxima of an exponent matrix into ctl->max_exp[which][v] (atomicMax).
 int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream);
 
+// S0 on a sample: 1184 evenly spaced segments of 512 rows.  The caller sizes the fields from the sampled maxima's bit
+// lengths and relies on S1's range check to catch an exponent the sample missed (then S0 runs in full).
+int launch_bounds_sample(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream);
+
 // S1: pack rows into keys (key_bytes from the plan), check e <= plan.bound (-> ctl->status), and, when
 // hist_digit >= 0, accumulate the histogram of that plan digit into ctl->hist[hist_digit] (the first pass's digit).
 int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, int hist_digit,

@@ -85,6 +85,39 @@ __global__ void __launch_bounds__(THREADS) bounds_stream_kernel(const uint4* __r
     if (tid < nvars && smax[tid]) atomicMax(&gmax[tid], smax[tid]);
 }
 
+// Maxima over a SAMPLE of the rows: block b sweeps rows [b*seg_stride, b*seg_stride + seg_rows).  Any strides.
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS) bounds_sample_kernel(ExpView ev, int64_t nterms, int nvars, int64_t seg_stride,
+                                                                int seg_rows, uint32_t* gmax)
+{
+    __shared__ uint32_t smax[kMaxVars];
+    const int tid = threadIdx.x;
+    if (tid < nvars) smax[tid] = 0u;
+    __syncthreads();
+    const int rows_per_iter = THREADS / nvars;
+    if (tid < rows_per_iter * nvars) {
+        const int v = tid % nvars, r = tid / nvars;
+        const int64_t t0 = (int64_t)blockIdx.x * seg_stride;
+        const int64_t t1 = min(nterms, t0 + seg_rows);
+        uint32_t m = 0u;
+        const int64_t voff = (int64_t)v * ev.var_stride;
+#pragma unroll 4
+        for (int64_t t = t0 + r; t < t1; t += rows_per_iter)
+            m = max(m, load_exp(ev.base, ev.exp_bytes, t * ev.term_stride + voff));
+        if (m) atomicMax(&smax[v], m);
+    }
+    __syncthreads();
+    if (tid < nvars && smax[tid]) atomicMax(&gmax[tid], smax[tid]);
+}
+
+int launch_bounds_sample(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream)
+{
+    if (nterms <= 0) return 0;
+    constexpr int kSegs = 148 * 8, kSegRows = 512;
+    bounds_sample_kernel<256><<<kSegs, 256, 0, stream>>>(ev, nterms, nvars, nterms / kSegs, kSegRows, ctl->max_exp[which]);
+    return 1;
+}
+
 int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream)
 {
     if (nterms <= 0) return 0;

@@ -219,3 +219,25 @@ def test_randomised_shapes_both_paths(seed):
     assert_parity(res, c0, e0)
     if tol == 0.0:
         assert (e == e0).all()
+
+
+# ------------------------------------------------------------------ S0 on a sample of the rows
+
+def test_sampled_bounds_are_verified_and_retried():
+    """>= 2^22 terms: S0 reads a sample of the rows and S1's range check verifies the rest.  An exponent the sample misses
+    (one row of 200 among values below 16) must be caught and the call re-run with full bounds -- same result as
+    POLYLAB_FLAG_EXACT_BOUNDS."""
+    n = (1 << 22) + 12_344
+    p = pooled(n, 8, 8, seed=51, hi=16)
+    c, e, st = run(p, 0.0)
+    assert st.bounds_sampled == 1 and st.bounds_retry == 0 and st.key_bits == 32
+    res = oracle.simplify(p.coef, p.exps, 0.0)
+    assert_parity(res, c, e)
+    p.exps[1000, 3] = 200                                   # rows 512..3500 of every stride are not sampled
+    res = oracle.simplify(p.coef, p.exps, 0.0)
+    c, e, st = run(p, 0.0)
+    assert st.bounds_retry == 1 and st.bounds_sampled == 0 and st.key_bits == 36
+    assert_parity(res, c, e)
+    c1, e1, st1 = run(p, 0.0, flags=B.FLAG_EXACT_BOUNDS)
+    assert st1.bounds_retry == 0 and st1.bounds_sampled == 0
+    assert (e == e1).all() and (c.view(np.uint64) == c1.view(np.uint64)).all()
