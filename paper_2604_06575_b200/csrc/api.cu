@@ -303,6 +303,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     Readback res;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));
+    if (res.status == POLYLAB_ERR_EXPONENT_RANGE) return res.status;   // keys built from out-of-range exponents prove nothing below
     if (res.overflow) return kRetryNoBucket;
     if (res.unsorted) return kRetrySafeRank;
     tm.finish(o.stats);
@@ -360,6 +361,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     struct { int32_t status; uint32_t distinct, survivors, unsorted; } res;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));
+    if (res.status == POLYLAB_ERR_EXPONENT_RANGE) return res.status;   // keys built from out-of-range exponents prove nothing below
     if (res.unsorted) return safe_rank ? (int)POLYLAB_ERR_INTERNAL : kRetrySafeRank;
     tm.finish(o.stats);
     if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; }

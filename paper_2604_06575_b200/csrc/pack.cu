@@ -309,7 +309,8 @@ int launch_key_hist(const Plan& plan, int hd, int64_t n, const void* keys, Contr
 struct DigitParts {
     int n;
     uint8_t var[8];
-    int8_t lshift[8];       // contribution = e << lshift (lshift >= 0) or e >> -lshift, then & mask
+    int8_t lshift[8];       // contribution = min(e, emax) << lshift (lshift >= 0) or >> -lshift, then & mask
+    uint32_t emax[8];       // the variable's bound: the fused pass clamps an out-of-range exponent the same way
     uint32_t mask;
 };
 
@@ -353,6 +354,7 @@ __global__ void __launch_bounds__(256) row_hist_kernel(const uint8_t* __restrict
                 if (ES == 4) e = x;
                 else if (ES == 2) e = (x >> (16 * (v & 1))) & 0xffffu;
                 else e = (x >> (8 * (v & 3))) & 0xffu;
+                e = min(e, dp.emax[i]);
                 const int ls = dp.lshift[i];
                 d |= ls >= 0 ? (e << ls) : (e >> -ls);
             }
@@ -381,6 +383,7 @@ int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hd,
         if (plan.width[v] == 0 || hi <= dpos || lo >= dpos + dbits) continue;
         dp.var[dp.n] = (uint8_t)v;
         dp.lshift[dp.n] = (int8_t)(lo - dpos);
+        dp.emax[dp.n] = plan.bound[v];
         ++dp.n;
     }
     const int rb = plan.nvars * ev.exp_bytes;

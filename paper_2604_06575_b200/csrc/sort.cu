@@ -78,7 +78,9 @@ __device__ __forceinline__ K pack_row_inline(const PassArgs& a, const Plan& plan
             if (es == 4) e = w[(k < ROWS / 4) ? k : 0];
             else if (es == 2) e = (w[(k < ROWS / 2) ? (k >> 1) : 0] >> (16 * (k & 1))) & 0xffffu;
             else e = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
-            bad |= e > plan.bound[k];
+            // an out-of-range exponent is reported AND clamped: the digit histogram was built from the rows with the same
+            // clamp (pack.cu, row_hist_kernel), and the scatter must agree with it bin for bin
+            if (e > plan.bound[k]) { bad = true; e = plan.bound[k]; }
             key_or_field(key, e, plan.shift[k]);
         }
     }

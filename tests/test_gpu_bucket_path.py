@@ -241,3 +241,24 @@ def test_sampled_bounds_are_verified_and_retried():
     c1, e1, st1 = run(p, 0.0, flags=B.FLAG_EXACT_BOUNDS)
     assert st1.bounds_retry == 0 and st1.bounds_sampled == 0
     assert (e == e1).all() and (c.view(np.uint64) == c1.view(np.uint64)).all()
+
+
+def test_out_of_range_exponents_on_the_fused_path_are_reported_not_scattered():
+    """Caller bounds far too small (4-bit fields, exponents up to 199): the fused pass clamps what it reports, so its
+    scatter still agrees with the digit histogram built from the rows, and the call returns the range error."""
+    p = pooled(300_000, 16, 4, seed=61, hi=200)
+    for _ in range(3):
+        with pytest.raises(B.PolylabError) as ei:
+            B.simplify(dev(p.coef), dev(p.exps), 0.0, max_exp=[15] * 16, flags=FORCE)
+        assert ei.value.status == B.ERR_EXPONENT_RANGE
+    c, e, st = run(p, 0.0, flags=FORCE)                     # the library is still healthy afterwards
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+def test_sampled_bounds_retry_on_the_bucket_path_with_fused_pack():
+    n = (1 << 22) + 8_000
+    p = pooled(n, 16, 8, seed=52, hi=16)
+    p.exps[2000, 5] = 200                                   # not in the sample
+    c, e, st = run(p, 0.0)
+    assert st.bounds_retry == 1 and st.key_bits == 68 and st.prefix_passes == 2
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
