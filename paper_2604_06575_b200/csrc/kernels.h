@@ -8,7 +8,8 @@
 namespace polylab {
 
 // Tile sizes of the streaming kernels (records per thread block); also used by the workspace query.
-constexpr int kSortThreads = 256;
+constexpr int kSortThreads64 = 256;
+constexpr int kSortThreads128 = 256;
 constexpr int kSortItems64 = 16;    // 4096-record tiles of (u64 key, f64 coef)
 constexpr int kSortItems128 = 20;   // 5120-record tiles of (u128 key, f64 coef), two blocks per SM (swept on B200: 12x3 4.26, 16x2 4.08, 20x2 4.04, 24x2 4.74 ms for two passes of config 5)
 constexpr int kReduceThreads = 256;
@@ -26,7 +27,7 @@ constexpr int kFinBins = 1 << kFinDigit;
 constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
 constexpr int kFinMinTile = 512;    // smallest fin_tile the planner picks (workspace sizing)
 
-inline int sort_tile(int key_bytes) { return kSortThreads * (key_bytes == 8 ? kSortItems64 : kSortItems128); }
+inline int sort_tile(int key_bytes) { return key_bytes == 8 ? kSortThreads64 * kSortItems64 : kSortThreads128 * kSortItems128; }
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
 constexpr int kPruneTile = kPruneThreads * kPruneItems;
 

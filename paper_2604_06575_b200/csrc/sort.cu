@@ -179,23 +179,26 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 
     // ---- per-bin: exclusive offsets over warps, tile count, next-digit histogram, look-back publication
     const unsigned b = tid;
+    const bool bt = tid < (unsigned)kRadix;              // the first 256 threads own one bin each
     uint32_t count = 0;
+    uint32_t* my_state = a.tile_state + (size_t)tile * kRadix + (bt ? b : 0u);
+    if (bt) {
 #pragma unroll
-    for (int w = 0; w < NW; ++w) {
-        const uint32_t c = whist[w * kRadix + b];
-        whist[w * kRadix + b] = count;
-        count += c;
-    }
-    uint32_t* my_state = a.tile_state + (size_t)tile * kRadix + b;
-    st_volatile_u32(my_state, (count << 2) | (tile == 0 ? a.flag_inclusive : a.flag_partial));
-    if (NEXT) {
-        const uint32_t c2 = bhist2[b];
-        if (c2) atomicAdd(&a.hist_next[b], c2);
+        for (int w = 0; w < NW; ++w) {
+            const uint32_t c = whist[w * kRadix + b];
+            whist[w * kRadix + b] = count;
+            count += c;
+        }
+        st_volatile_u32(my_state, (count << 2) | (tile == 0 ? a.flag_inclusive : a.flag_partial));
+        if (NEXT) {
+            const uint32_t c2 = bhist2[b];
+            if (c2) atomicAdd(&a.hist_next[b], c2);
+        }
     }
     uint32_t total;
     const uint32_t bin_start = block_exclusive_scan<THREADS>(count, scratch, &total);
-    sm_bin_start[b] = bin_start;
-    const uint32_t gbase = block_exclusive_scan<THREADS>(a.hist_this[b], scratch, &total);   // syncs: sm_bin_start visible
+    if (bt) sm_bin_start[b] = bin_start;
+    const uint32_t gbase = block_exclusive_scan<THREADS>(bt ? a.hist_this[b] : 0u, scratch, &total);   // syncs: sm_bin_start visible
 
     // ---- scatter keys into shared memory at their position in the sorted tile
 #pragma unroll
@@ -219,7 +222,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
     // is the longest stall of the kernel when done one dependent load at a time (profiles/r1b), so LB states are
     // fetched per round trip and consumed in order up to the first inclusive one (or the first not yet published).
     uint32_t excl = 0;
-    if (tile > 0) {
+    if (tile > 0 && bt) {
         constexpr int LB = 8;
         int64_t t = (int64_t)tile - 1;                       // nearest predecessor not consumed yet
         bool done = false;
@@ -241,7 +244,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         }
         st_volatile_u32(my_state, ((excl + count) << 2) | a.flag_inclusive);
     }
-    sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
+    if (bt) sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
     __syncthreads();
 
     // ---- write keys: slot s of the sorted tile, contiguous per bin
@@ -270,7 +273,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
 __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_constant__ PassArgs a)
 {
-    static_assert(THREADS == kRadix, "one thread per bin");
+    static_assert(THREADS >= kRadix && THREADS % 32 == 0, "the first 256 threads own one bin each");
     using S = SortSmem<K, THREADS, ITEMS>;
     constexpr int TILE = S::TILE, NW = S::NW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -309,25 +312,25 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_rows_kernel(const __g
     else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES>(a, &plan, smem_raw, tile, tile_base, tile_n);
 }
 
-template <typename K, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
 static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t stream)
 {
-    using S = SortSmem<K, kSortThreads, ITEMS>;
-    auto kern = sort_pass_kernel<K, kSortThreads, ITEMS, MINB, NEXT, RANK_ATOMIC>;
+    using S = SortSmem<K, THREADS, ITEMS>;
+    auto kern = sort_pass_kernel<K, THREADS, ITEMS, MINB, NEXT, RANK_ATOMIC>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
         attr_set = true;
     }
-    kern<<<tiles, kSortThreads, S::bytes(), stream>>>(a);
+    kern<<<tiles, THREADS, S::bytes(), stream>>>(a);
 }
 
-template <typename K, int ITEMS, int MINB>
+template <typename K, int THREADS, int ITEMS, int MINB>
 static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in,
                               const double* coef_in, void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl,
                               bool safe_rank, bool debug_unstable, const ExpView* rows, cudaStream_t stream)
 {
-    using S = SortSmem<K, kSortThreads, ITEMS>;
+    using S = SortSmem<K, THREADS, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
     const bool has_next = next >= 0;
     PassArgs a;
@@ -350,20 +353,20 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
         const int rb = plan.nvars * rows->exp_bytes;
         auto go = [&](auto kern) {
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
-            kern<<<tiles, kSortThreads, S::bytes(), stream>>>(a, plan);
+            kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);
         };
         constexpr int KB = (int)sizeof(K);          // the byte-reversal path needs rows as long as the key
-        if (fast) { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, KB, true>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, KB, true>); }
-        else if (rb == 16) { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, 16, false>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, 16, false>); }
-        else { if (has_next) go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, true, 8, false>); else go(sort_pass_rows_kernel<K, kSortThreads, ITEMS, MINB, false, 8, false>); }
+        if (fast) { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, KB, true>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, KB, true>); }
+        else if (rb == 16) { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 16, false>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, 16, false>); }
+        else { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 8, false>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, 8, false>); }
         return 1;
     }
     if (safe_rank) {
-        if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, false>(a, tiles, stream);
-        else launch_sort_pass_k<K, ITEMS, MINB, false, false>(a, tiles, stream);
+        if (has_next) launch_sort_pass_k<K, THREADS, ITEMS, MINB, true, false>(a, tiles, stream);
+        else launch_sort_pass_k<K, THREADS, ITEMS, MINB, false, false>(a, tiles, stream);
     } else {
-        if (has_next) launch_sort_pass_k<K, ITEMS, MINB, true, true>(a, tiles, stream);
-        else launch_sort_pass_k<K, ITEMS, MINB, false, true>(a, tiles, stream);
+        if (has_next) launch_sort_pass_k<K, THREADS, ITEMS, MINB, true, true>(a, tiles, stream);
+        else launch_sort_pass_k<K, THREADS, ITEMS, MINB, false, true>(a, tiles, stream);
     }
     return 1;
 }
@@ -374,9 +377,9 @@ int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, c
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
-        return launch_sort_pass_t<uint64_t, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+        return launch_sort_pass_t<uint64_t, kSortThreads64, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
                                                              tile_state, ctl, safe_rank, debug_unstable, rows, stream);
-    return launch_sort_pass_t<Key128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+    return launch_sort_pass_t<Key128, kSortThreads128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
                                                         tile_state, ctl, safe_rank, debug_unstable, rows, stream);
 }
 
