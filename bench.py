@@ -61,6 +61,13 @@ def workload(config: int, nterms, seed_offset: int = 0):
         p, tol = W.config5(nterms or 200_000_000, seed_offset)
         return "simplify", (p,), tol, (f"config5: simplify {p.nterms} terms, nvars=16, exps U{{0..255}} (128-bit keys), pool of "
                                        f"{p.nterms // 10} monomials x10, half cancelling, tol=1e-14"), p.nterms
+    if config == 6:                                     # not a BASELINE.json config: the paper's own Fig. 2 workload, d = 4
+        p = W.p_d(4)
+        return "cubic", (p,), 0.0, ("paper Fig. 2: simplify(p_4^3), 5 variables, 126 monomials (PAPER.md:543, 584, 586): raw p*p "
+                                    "(15,876 terms) times p = 2,000,376 products in one sort"), 126 * 126 + 126 ** 3
+    if config == 7:                                     # not a BASELINE.json config: config 3's intent, reading A15
+        p, tol = W.config3u(nterms or 10_000_000, seed_offset)
+        return "simplify", (p,), tol, f"config3u: simplify {p.nterms} terms, nvars=10, 3 nonzero vars with exps U{{1..1024}} u16 (110-bit keys, mostly unique)", p.nterms
     raise SystemExit(f"unknown config {config}")
 
 
@@ -138,20 +145,20 @@ def time_oracle(kind, polys, tol):
     elif kind == "mul":
         oracle.mul_simplify(polys[0].coef, polys[0].exps, polys[1].coef, polys[1].exps, tol)
     else:
-        p = polys[0]
-        c, e = oracle.mul_simplify(p.coef, p.exps, p.coef, p.exps, tol).pruned
-        oracle.mul_simplify(c, e, p.coef, p.exps.astype(np.uint32), tol)
+        p = polys[0]                                    # the same work as the timed GPU step: raw p*p, then (p*p)*p merged once
+        c, e = oracle.expand(p.coef, p.exps, p.coef, p.exps)
+        oracle.mul_simplify(c, e, p.coef, p.exps.astype(e.dtype), tol)
     return time.perf_counter() - t0
 
 
 def oracle_sample(config: int, budget_s: float):
     """A bounded sample of the workload for the CPU oracle: same recipe, fewer terms (about budget_s of CPU work)."""
-    if config in (1, 2, 4):
+    if config in (1, 2, 4, 6):
         return workload(config, None)                   # the oracle finishes these in seconds
     probe_n = 1_000_000
     kind, polys, tol, _, n = workload(config, probe_n)
     rate = n / time_oracle(kind, polys, tol)
-    full = 10_000_000 if config == 3 else 200_000_000
+    full = 10_000_000 if config in (3, 7) else 200_000_000
     n_s = int(min(full, max(probe_n, rate * budget_s)) // 20 * 20)
     return workload(config, n_s)
 
@@ -186,7 +193,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--config", type=int, default=5, help="1-5: BASELINE.json configs; 6: the paper's p_4^3; 7: config 3u")
     ap.add_argument("--nterms", type=int, default=None, help="override the config's term count (debugging)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
