@@ -81,6 +81,16 @@ def max_over_ranks(dist, value: float, device) -> float:
     return float(t.item())
 
 
+def lsu_pipe(wavefronts_per_launch, launch_ms: float, sms: int = 148, sm_mhz: float = 1965.0):
+    """The finish kernel's real limiter: LSU data-pipe wavefronts (ncu count of the committed capture, profiles/traffic.json)
+    per live launch time, against one wavefront per clock and SM (B300_MICROARCH.md; 148 SMs at the 1965 MHz maximum)."""
+    if not wavefronts_per_launch:
+        return None
+    peak = sms * sm_mhz * 1e6
+    ach = wavefronts_per_launch / (launch_ms * 1e-3)
+    return {"wavefronts_per_launch_ncu": wavefronts_per_launch, "achieved_per_s": ach, "peak_per_s": peak, "frac": ach / peak}
+
+
 def replica_seed_offset(rank: int) -> int:
     """Replicas only: rank r simplifies its own polynomial of the same shape, seeded by r."""
     return int(rank)
@@ -303,6 +313,7 @@ def main():
                     "traffic": tinfo.get("finish_dram_bytes_per_launch"), "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": fin_bytes, "launch_ms": fin_ms, "launches_per_step": 1,
                     "limiter": "shared-memory / LSU pipe, not DRAM (ncu, profiles/): the kernel trades HBM passes for on-chip work",
+                    "lsu_pipe": lsu_pipe(tinfo.get("finish_lsu_wavefronts_per_launch"), fin_ms),
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
     else:
         roofline = {"bound": "hbm", "kernel": pass_info["kernel"], "achieved": pass_gbs, "peak": peak, "unit": "GB/s",
