@@ -306,7 +306,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     if ((uint64_t)lo < ((uint64_t)tile + 1) * a.fin_tile && hi > lo) n_loc = min(hi - lo, (uint32_t)CAP);
     const K* __restrict__ gkeys = (const K*)a.keys + lo;
     const double* __restrict__ gcoef = a.coefs + lo;
-    const uint32_t itn = (n_loc + THREADS - 1) / THREADS;      // sorted positions per thread in the blocked phases
+    // sorted positions per thread in the blocked phases; odd, so that the threads' strided shared-memory accesses
+    // (stride itn elements) spread over all banks
+    const uint32_t itn = ((n_loc + THREADS - 1) / THREADS) | 1u;
     const uint32_t first = tid * itn;
 
     // raw sort bits of the fast attempt: the (up to 32) key bits just below the prefix
