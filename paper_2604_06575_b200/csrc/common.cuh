@@ -139,6 +139,26 @@ __device__ __forceinline__ void store_exp(void* base, int exp_bytes, int64_t idx
     else ((uint32_t*)base)[idx] = e;
 }
 
+// 32-bit word `w` of the unpacked exponent row of key kk (S5) when rows are written as words: exp_bytes 1 -> variables
+// 4w..4w+3, 2 -> 2w, 2w+1, 4 -> w.  Usable when nvars * exp_bytes is a multiple of 4 and the output base is 4-byte aligned.
+template <typename K>
+__device__ __forceinline__ uint32_t unpack_row_word(const Plan& plan, const K& kk, int w, int exp_bytes)
+{
+    if (exp_bytes == 4) return key_get_field(kk, plan.shift[w], plan.width[w]);
+    if (exp_bytes == 2)
+        return key_get_field(kk, plan.shift[2 * w], plan.width[2 * w]) |
+               (key_get_field(kk, plan.shift[2 * w + 1], plan.width[2 * w + 1]) << 16);
+    return key_get_field(kk, plan.shift[4 * w], plan.width[4 * w]) |
+           (key_get_field(kk, plan.shift[4 * w + 1], plan.width[4 * w + 1]) << 8) |
+           (key_get_field(kk, plan.shift[4 * w + 2], plan.width[4 * w + 2]) << 16) |
+           (key_get_field(kk, plan.shift[4 * w + 3], plan.width[4 * w + 3]) << 24);
+}
+__host__ inline int row_words(int nvars, int exp_bytes, const void* out_exps)
+{
+    const int rb = nvars * exp_bytes;
+    return (rb % 4 == 0 && ((uintptr_t)out_exps & 3) == 0) ? rb / 4 : 0;      // 0: rows cannot be written as words
+}
+
 // --------------------------------------------------------------------------- control block
 
 // Small device-side state at the head of the workspace, zeroed at the start of every call.

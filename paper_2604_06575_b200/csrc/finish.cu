@@ -254,7 +254,7 @@ struct EmitArgs {
     double* out_coef;
     void* out_exps;
     int exp_bytes;
-    int words_u8;                   // out_exps may be written as 32-bit words of four u8 exponents
+    int wpr;                        // > 0: rows are written as this many 32-bit words (common.cuh, row_words)
     int64_t out_capacity;
 };
 
@@ -262,15 +262,9 @@ template <typename K>
 __device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, uint64_t o, double s, const K& kk)
 {
     a.out_coef[o] = s;
-    if (a.words_u8) {
-        uint32_t* row = (uint32_t*)a.out_exps + o * (uint64_t)(plan.nvars >> 2);
-        for (int v = 0; v < plan.nvars; v += 4) {
-            const uint32_t w = key_get_field(kk, plan.shift[v], plan.width[v]) |
-                               (key_get_field(kk, plan.shift[v + 1], plan.width[v + 1]) << 8) |
-                               (key_get_field(kk, plan.shift[v + 2], plan.width[v + 2]) << 16) |
-                               (key_get_field(kk, plan.shift[v + 3], plan.width[v + 3]) << 24);
-            row[v >> 2] = w;
-        }
+    if (a.wpr > 0) {
+        uint32_t* row = (uint32_t*)a.out_exps + o * (uint64_t)a.wpr;
+        for (int w = 0; w < a.wpr; ++w) row[w] = unpack_row_word(plan, kk, w, a.exp_bytes);
         return;
     }
     for (int v = 0; v < plan.nvars; ++v)
@@ -660,7 +654,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     EmitArgs e;
     e.ukeys = ukeys; e.usums = usums; e.ntiles = ntiles; e.tile_start = tile_start; e.tile_off = tile_state;
     e.out_coef = out_coef; e.out_exps = out_exps; e.exp_bytes = exp_bytes;
-    e.words_u8 = (exp_bytes == 1 && (plan.nvars & 3) == 0 && ((uintptr_t)out_exps & 3) == 0) ? 1 : 0;
+    e.wpr = row_words(plan.nvars, exp_bytes, out_exps);
     e.out_capacity = out_capacity;
     int64_t blocks = (n / 4 + 255) / 256;          // at most N outputs; grid-stride
     if (blocks > 148 * 16) blocks = 148 * 16;

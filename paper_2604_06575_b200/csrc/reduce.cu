@@ -215,10 +215,11 @@ template <typename K, int THREADS, int ITEMS>
 __global__ void __launch_bounds__(THREADS)
 prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usums, double tol,
                     const __grid_constant__ Plan plan, double* __restrict__ out_coef, void* out_exps, int exp_bytes,
-                    int64_t out_capacity, uint32_t* tile_state, Control* ctl, int64_t* out_count_device)
+                    int wpr, int64_t out_capacity, uint32_t* tile_state, Control* ctl, int64_t* out_count_device)
 {
     constexpr int TILE = THREADS * ITEMS, NW = THREADS / 32;
     __shared__ uint32_t scratch[NW + 2];
+    __shared__ uint16_t sel[TILE];                     // the tile's survivors, compacted: positions inside the tile
     __shared__ uint32_t sm_tile, sm_base;
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t U = ctl->distinct;
@@ -254,18 +255,32 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
             if (lane == 0) sm_base = r;
         }
         __syncthreads();
-        uint64_t o = (uint64_t)sm_base + excl;
+        // survivors' positions, compacted in order; then the block writes them together so that consecutive threads
+        // store consecutive words of the output (a thread writing its own 8 rows touched 32 sectors per store)
+        {
+            uint32_t q = excl;
 #pragma unroll
-        for (int j = 0; j < ITEMS; ++j) {
-            if (keep & (1u << j)) {
-                if ((int64_t)o < out_capacity) {
-                    out_coef[o] = s[j];
-                    const K kk = ukeys[tile_base + first + j];
+            for (int j = 0; j < ITEMS; ++j)
+                if (keep & (1u << j)) sel[q++] = (uint16_t)(first + j);
+        }
+        __syncthreads();
+        const uint64_t obase = sm_base;
+        for (uint32_t i = tid; i < total; i += THREADS)
+            if ((int64_t)(obase + i) < out_capacity) out_coef[obase + i] = usums[tile_base + sel[i]];
+        if (wpr > 0) {
+            uint32_t* __restrict__ ow = (uint32_t*)out_exps;
+            for (uint32_t f = tid; f < total * (uint32_t)wpr; f += THREADS) {
+                const uint32_t i = f / (uint32_t)wpr, w = f - i * (uint32_t)wpr;
+                if ((int64_t)(obase + i) < out_capacity)
+                    ow[(obase + i) * (uint64_t)wpr + w] = unpack_row_word(plan, ukeys[tile_base + sel[i]], (int)w, exp_bytes);
+            }
+        } else {
+            for (uint32_t i = tid; i < total; i += THREADS) {
+                if ((int64_t)(obase + i) < out_capacity) {
+                    const K kk = ukeys[tile_base + sel[i]];
                     for (int v = 0; v < plan.nvars; ++v)
-                        store_exp(out_exps, exp_bytes, (int64_t)o * plan.nvars + v,
-                                  key_get_field(kk, plan.shift[v], plan.width[v]));
+                        store_exp(out_exps, exp_bytes, (int64_t)(obase + i) * plan.nvars + v, key_get_field(kk, plan.shift[v], plan.width[v]));
                 }
-                ++o;
             }
         }
         if (tile_base + tile_n == U && tid == 0) {
@@ -284,12 +299,12 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (plan.key_bytes == 8)
         prune_unpack_kernel<uint64_t, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
-            (const uint64_t*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, out_capacity, tile_state, ctl,
-            out_count_device);
+            (const uint64_t*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
+            out_capacity, tile_state, ctl, out_count_device);
     else
         prune_unpack_kernel<Key128, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
-            (const Key128*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, out_capacity, tile_state, ctl,
-            out_count_device);
+            (const Key128*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
+            out_capacity, tile_state, ctl, out_count_device);
     return 1;
 }
 
