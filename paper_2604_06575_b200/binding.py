@@ -109,10 +109,13 @@ def lib():
         mul = [pp, pp, dbl, po, vp, vp, i64, vp, vp, sz, vp]
         L.polylab_mul_simplify.argtypes = mul
         L.polylab_mul_simplify_host.argtypes = mul
+        L.polylab_pow_simplify_workspace_bytes.argtypes = [i64, i32, i32, i64, po]
+        L.polylab_pow_simplify_workspace_bytes.restype = sz
+        L.polylab_pow_simplify.argtypes = [pp, i32, dbl, po, vp, vp, i64, vp, vp, sz, vp]
         L.polylab_expand.argtypes = [pp, pp, po, vp, vp, vp, sz, vp]
         L.polylab_pack_keys.argtypes = [vp, i64, i32, po, vp, ctypes.POINTER(i32), vp, sz, vp]
         for name in ("polylab_simplify", "polylab_simplify_host", "polylab_mul_simplify", "polylab_mul_simplify_host",
-                     "polylab_expand", "polylab_pack_keys", "polylab_version"):
+                     "polylab_expand", "polylab_pack_keys", "polylab_version", "polylab_pow_simplify"):
             getattr(L, name).restype = ctypes.c_int
         L.polylab_status_string.argtypes = [ctypes.c_int]
         L.polylab_status_string.restype = ctypes.c_char_p
@@ -289,6 +292,33 @@ def mul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tenso
     rc = lib().polylab_mul_simplify(ctypes.byref(pa), ctypes.byref(pb), float(tol), ctypes.byref(o), out_coef.data_ptr(),
                                     out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(),
                                     _stream_ptr(stream))
+    _check(rc)
+    k = count.value
+    res = (out_coef[:k], out_exps[:k])
+    return (*res, _stats(st)) if return_stats else res
+
+
+def pow_simplify(coef: torch.Tensor, exps: torch.Tensor, power: int, tol: float = 0.0, *, out_capacity: Optional[int] = None,
+                 workspace: Optional[Workspace] = None, stream=None, return_stats: bool = False, flags: int = 0):
+    """polylab_pow_simplify on device tensors: simplify(p^power); the intermediate powers stay inside the workspace.
+    out_capacity bounds every power's term count (default: min(nterms^power, 2^22))."""
+    coef, exps, strides = _dev_poly(coef, exps)
+    if strides is not None:
+        exps = exps.contiguous()
+    n, nvars = int(exps.shape[0]), int(exps.shape[1])
+    cap = int(out_capacity) if out_capacity is not None else max(1, min(max(n, 1) ** max(int(power), 1), 1 << 22))
+    keep = []
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep)
+    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
+    out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
+    wsb = int(lib().polylab_pow_simplify_workspace_bytes(n, nvars, int(power), cap, ctypes.byref(o)))
+    if wsb == 0 and n > 0 and power > 1:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "out_capacity * nterms must be < 2^30")
+    ws = _ws(coef.device, workspace).get(max(wsb, 256))
+    pp = _Poly(coef.data_ptr(), exps.data_ptr(), n, nvars)
+    count = ctypes.c_int64(0)
+    rc = lib().polylab_pow_simplify(ctypes.byref(pp), int(power), float(tol), ctypes.byref(o), out_coef.data_ptr(),
+                                    out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])

@@ -390,6 +390,8 @@ using namespace polylab;
 
 extern "C" {
 
+static int opts_exp_bytes_fwd(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
+
 size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
 {
     (void)nvars; (void)opts;
@@ -594,6 +596,86 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
         return mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
                                  cuda_stream, at);
     });
+}
+
+// ------------------------------------------------------------------------------- powers (N2)
+
+struct PowLayout { size_t coef[2], exps[2], inner, inner_bytes, total; };
+
+static PowLayout pow_layout(int64_t np, int nvars, int es, int64_t cap, const polylab_opts* opts)
+{
+    PowLayout P;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
+    for (int i = 0; i < 2; ++i) { P.coef[i] = take((size_t)cap * sizeof(double)); P.exps[i] = take((size_t)cap * nvars * es); }
+    P.inner_bytes = polylab_mul_simplify_workspace_bytes(cap, np, nvars, opts);
+    P.inner = take(P.inner_bytes);
+    P.total = off + 256;
+    return P;
+}
+
+size_t polylab_pow_simplify_workspace_bytes(int64_t nterms, int32_t nvars, int32_t power, int64_t out_capacity,
+                                            const polylab_opts* opts)
+{
+    if (nterms < 0 || nvars < 1 || power < 0 || out_capacity < 0) return 0;
+    if (power <= 1) return polylab_simplify_workspace_bytes(nterms, nvars, opts);
+    const int64_t cap = out_capacity > nterms ? out_capacity : nterms;
+    if (nterms > 0 && cap >= POLYLAB_MAX_TERMS / nterms) return 0;              // a product could exceed the term limit
+    const PowLayout P = pow_layout(nterms, nvars, opts_exp_bytes_fwd(opts), cap, opts);
+    return P.inner_bytes ? P.total : 0;
+}
+
+int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const polylab_opts* opts,
+                         double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (!p || power < 0 || !out_nterms || out_capacity < 0 || !(tol >= 0.0) || isinf(tol)) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int nvars = p->nvars;
+    const int64_t np = p->nterms;
+    if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || np < 0 || np >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (opts && (opts->max_exp_host || (opts->flags & POLYLAB_FLAG_DEVICE_COUNT) || opts->term_stride != 0 || opts->var_stride != 0))
+        return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int es = opts_exp_bytes_fwd(opts);
+    if (es != POLYLAB_EXP_U8 && es != POLYLAB_EXP_U16 && es != POLYLAB_EXP_U32) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (power == 0) {                                    // p^0 = 1, also for the zero polynomial (the empty product)
+        *out_nterms = 1;
+        if (out_capacity < 1) return POLYLAB_ERR_OUTPUT_TOO_SMALL;
+        if (!out_coef || !out_exps) return POLYLAB_ERR_INVALID_ARGUMENT;
+        const double one = 1.0;
+        PL_CUDA(cudaMemcpyAsync(out_coef, &one, sizeof one, cudaMemcpyHostToDevice, stream));
+        PL_CUDA(cudaMemsetAsync(out_exps, 0, (size_t)nvars * es, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        return POLYLAB_OK;
+    }
+    if (power == 1 || np == 0)
+        return polylab_simplify(p->coef, p->exps, np, nvars, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace,
+                                workspace_bytes, cuda_stream);
+    if (!p->coef || !p->exps || !workspace || (out_capacity > 0 && (!out_coef || !out_exps))) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int64_t cap = out_capacity > np ? out_capacity : np;
+    if (cap >= POLYLAB_MAX_TERMS / np) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const PowLayout P = pow_layout(np, nvars, es, cap, opts);
+    unsigned char* ws = align_ptr(workspace);
+    if (!P.inner_bytes || workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + P.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+
+    polylab_poly cur = *p;
+    int64_t count = 0;
+    for (int step = 2; step <= power; ++step) {
+        const bool last = step == power;
+        double* dc = last ? out_coef : (double*)(ws + P.coef[step & 1]);
+        void* de = last ? out_exps : (void*)(ws + P.exps[step & 1]);
+        const int rc = polylab_mul_simplify(&cur, p, last ? tol : 0.0, opts, dc, de, last ? out_capacity : cap, &count, ws + P.inner,
+                                            P.inner_bytes, cuda_stream);
+        if (rc != POLYLAB_OK) {
+            if (rc == POLYLAB_ERR_OUTPUT_TOO_SMALL) *out_nterms = count;
+            return rc;
+        }
+        if (!last && count > out_capacity) { *out_nterms = count; return POLYLAB_ERR_OUTPUT_TOO_SMALL; }
+        cur.coef = dc; cur.exps = de; cur.nterms = count;
+        if (count == 0) break;                           // the zero polynomial stays zero
+    }
+    *out_nterms = count;
+    return POLYLAB_OK;
 }
 
 int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_opts* opts, double* out_coef,

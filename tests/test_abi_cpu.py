@@ -29,7 +29,7 @@ def test_header_symbols_exported(L):
     names = _declared_functions()
     assert {"polylab_simplify", "polylab_mul_simplify", "polylab_expand", "polylab_pack_keys", "polylab_simplify_host",
             "polylab_mul_simplify_host", "polylab_simplify_workspace_bytes", "polylab_mul_simplify_workspace_bytes",
-            "polylab_status_string", "polylab_version"} <= set(names)
+            "polylab_status_string", "polylab_version", "polylab_pow_simplify", "polylab_pow_simplify_workspace_bytes"} <= set(names)
     for n in names:
         assert hasattr(L, n), f"{n} declared in include/polylab.h but not exported"
 
@@ -116,6 +116,38 @@ def test_host_side_argument_errors(L):
     cnt.value = -7
     assert g(ctypes.byref(pa), ctypes.byref(pb), 0.0, None, one, one, 25, ctypes.addressof(cnt), one, 1 << 20, None) == B.OK
     assert cnt.value == 0
+
+
+def test_pow_simplify_host_side_checks(L):
+    """polylab_pow_simplify: argument errors and the workspace query, no GPU involved."""
+    from paper_2604_06575_b200 import binding as B
+    cnt = ctypes.c_int64(-7)
+    one = ctypes.c_void_p(16)
+    f = L.polylab_pow_simplify
+    p = B._Poly(16, 16, 10, 3)
+
+    def call(poly=p, power=3, tol=0.0, opts=None, cap=100, cntp=ctypes.addressof(cnt), ws=one, wsb=1 << 30):
+        return f(ctypes.byref(poly) if poly is not None else None, power, tol, opts, one, one, cap, cntp, ws, wsb, None)
+
+    assert call(power=-1) == B.ERR_INVALID_ARGUMENT
+    assert call(poly=None) == B.ERR_INVALID_ARGUMENT
+    assert call(tol=float("nan")) == B.ERR_INVALID_ARGUMENT
+    assert call(cntp=None) == B.ERR_INVALID_ARGUMENT
+    assert call(poly=B._Poly(16, 16, 10, 0)) == B.ERR_INVALID_ARGUMENT
+    assert call(ws=None) == B.ERR_INVALID_ARGUMENT
+    assert call(wsb=1024) == B.ERR_WORKSPACE_TOO_SMALL
+    o = B._Opts()
+    o.term_stride, o.var_stride = 1, 10                      # strided operands are not supported by the power routine
+    assert call(opts=ctypes.byref(o)) == B.ERR_INVALID_ARGUMENT
+    o = B._Opts()
+    bounds = (ctypes.c_uint32 * 3)(1, 1, 1)
+    o.max_exp_host = ctypes.cast(bounds, ctypes.POINTER(ctypes.c_uint32))
+    assert call(opts=ctypes.byref(o)) == B.ERR_INVALID_ARGUMENT
+    assert call(poly=B._Poly(16, 16, 1 << 20, 3), cap=1 << 20) == B.ERR_INVALID_ARGUMENT     # a product could reach 2^30 terms
+    q = L.polylab_pow_simplify_workspace_bytes
+    assert q(200, 20, 1, 1000, None) == L.polylab_simplify_workspace_bytes(200, 20, None)
+    assert q(200, 20, 3, 300_000, None) >= L.polylab_mul_simplify_workspace_bytes(300_000, 200, 20, None)
+    assert q(200, 20, -1, 1000, None) == 0 and q(1 << 20, 3, 2, 1 << 20, None) == 0
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):
