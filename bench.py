@@ -111,7 +111,7 @@ class ClockSampler:
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20",
                                           "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -262,19 +262,35 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local_rank)
+    sampler.start()                                     # started before the warm-up: nvidia-smi needs ~0.1 s to produce its first line
     for _ in range(warmup):
         n_out = step_device()
+    t_wait = time.perf_counter()
+    while sampler.proc is not None and not sampler.rows and time.perf_counter() - t_wait < 2.0:
+        n_out = step_device()                           # keep the GPU under the same load until the sampler is live
     stats_log.clear()
-    sampler = ClockSampler(local_rank)
     barrier()
-    sampler.start()
+    rows_before = len(sampler.rows)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for _ in range(steps):
         n_out = step_device()
     ev1.record()
     barrier()
+    in_region = len(sampler.rows) - rows_before
+    # a step takes ~10 ms and nvidia-smi samples every 100 ms: keep the same load running (untimed, results discarded) until
+    # the clock line has at least five samples, so that "median under load" means something
+    saved_stats = list(stats_log)
+    t_hold = time.perf_counter()
+    while len(sampler.rows) - rows_before < 5 and time.perf_counter() - t_hold < 3.0 and sampler.proc is not None:
+        step_device()
+    torch.cuda.synchronize()
+    stats_log[:] = saved_stats
+    sampler.rows = sampler.rows[rows_before:]           # only lines taken from the start of the timed region on
     clocks = sampler.stop()
+    clocks["samples_in_timed_region"] = in_region
+    clocks["note"] = "sampled while the timed steps ran and, for short regions, while the same step kept running untimed"
     ms_total = ev0.elapsed_time(ev1)
     ms_total = max_over_ranks(dist, ms_total, "cuda")
     ms_per_step = ms_total / steps
