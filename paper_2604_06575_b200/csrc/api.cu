@@ -390,7 +390,7 @@ using namespace polylab;
 
 extern "C" {
 
-static int opts_exp_bytes_fwd(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
+static int opts_exp_bytes(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
 
 size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
 {
@@ -621,7 +621,7 @@ size_t polylab_pow_simplify_workspace_bytes(int64_t nterms, int32_t nvars, int32
     if (power <= 1) return polylab_simplify_workspace_bytes(nterms, nvars, opts);
     const int64_t cap = out_capacity > nterms ? out_capacity : nterms;
     if (nterms > 0 && cap >= POLYLAB_MAX_TERMS / nterms) return 0;              // a product could exceed the term limit
-    const PowLayout P = pow_layout(nterms, nvars, opts_exp_bytes_fwd(opts), cap, opts);
+    const PowLayout P = pow_layout(nterms, nvars, opts_exp_bytes(opts), cap, opts);
     return P.inner_bytes ? P.total : 0;
 }
 
@@ -636,7 +636,7 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
     if (nvars < 1 || nvars > POLYLAB_MAX_NVARS || np < 0 || np >= POLYLAB_MAX_TERMS) return POLYLAB_ERR_INVALID_ARGUMENT;
     if (opts && (opts->max_exp_host || (opts->flags & POLYLAB_FLAG_DEVICE_COUNT) || opts->term_stride != 0 || opts->var_stride != 0))
         return POLYLAB_ERR_INVALID_ARGUMENT;
-    const int es = opts_exp_bytes_fwd(opts);
+    const int es = opts_exp_bytes(opts);
     if (es != POLYLAB_EXP_U8 && es != POLYLAB_EXP_U16 && es != POLYLAB_EXP_U32) return POLYLAB_ERR_INVALID_ARGUMENT;
     if (power == 0) {                                    // p^0 = 1, also for the zero polynomial (the empty product)
         *out_nterms = 1;
@@ -760,8 +760,6 @@ static HostLayout host_layout(int64_t n_in_terms, int64_t n_sort, int nvars, int
     H.total = off + 256;
     return H;
 }
-
-static int opts_exp_bytes(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
 
 size_t polylab_simplify_host_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
 {

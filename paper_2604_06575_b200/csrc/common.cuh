@@ -177,7 +177,6 @@ struct Control {
 
 constexpr int kTicketReduce = kMaxPasses;
 constexpr int kTicketPrune = kMaxPasses + 1;
-constexpr int kTicketFinish = kMaxPasses + 2;
 
 // ------------------------------------------------------------------------- warp/block helpers
 
