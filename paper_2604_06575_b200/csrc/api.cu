@@ -250,7 +250,7 @@ static int fast_digits(const Opts& o)
 // After S1/X1 accumulated the histogram of the first prefix digit: do its bins predict buckets that fit a tile?
 // (A necessary test only; tile_bounds_kernel has the last word.)  On rejection the LSD path needs digit 0's histogram.
 static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* ws, const Layout& L, const Opts& o,
-                           int* launches, cudaStream_t stream, const ExpView* unpacked = nullptr)
+                           int* launches, cudaStream_t stream, const ExpView* unpacked = nullptr, const ExpandSrc* xs = nullptr)
 {
     if (*k == 0 || (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET)) return POLYLAB_OK;
     // (the rejection branch below is the only one that needs `unpacked`)
@@ -266,7 +266,8 @@ static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* w
     *k = 0;
     if (o.stats) o.stats->bucket_fallback = 1;
     PL_CUDA(cudaMemsetAsync(ctl->hist[d], 0, sizeof h, stream));
-    if (unpacked) *launches += launch_pack(*unpacked, n, plan, ws + L.keys[0], ctl, 0, stream);   // S1 had been left to the first pass
+    if (xs) *launches += launch_expand_hist(*xs, plan, 0, ctl, stream);                             // X1 stays in the first pass
+    else if (unpacked) *launches += launch_pack(*unpacked, n, plan, ws + L.keys[0], ctl, 0, stream);   // S1 had been left to the first pass
     else *launches += launch_key_hist(plan, 0, n, ws + L.keys[0], ctl, stream);
     return POLYLAB_OK;
 }
@@ -280,7 +281,8 @@ struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overfl
 // histogram of digit P-k is in ctl->hist[P-k].
 static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
-                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream, const ExpView* rows)
+                            int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream, const ExpView* rows,
+                            const ExpandSrc* xs)
 {
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
@@ -290,7 +292,8 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
         const double* cin = (s == 0) ? coef0 : cbuf[s & 1];
         *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
                                       cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
-                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr);
+                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr,
+                                      s == 0 ? xs : nullptr);
     }
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
@@ -319,11 +322,11 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
 static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
-                            const ExpView* rows = nullptr)
+                            const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr)
 {
     if (k_bucket > 0)
         return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
-                                tm, stream, rows);
+                                tm, stream, rows, xs);
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
@@ -332,7 +335,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
         const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
         *launches += launch_sort_pass(plan, p, p + 1 < P ? p + 1 : -1, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1],
                                       cbuf[(p + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
-                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream);
+                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, nullptr, p == 0 ? xs : nullptr);
     }
     tm.mark(POLYLAB_STAGE_SORT);
     const void* skeys = kbuf[P & 1];
@@ -579,13 +582,18 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     int k = choose_prefix_passes(plan_a, n, o, at);
     launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, -1, stream);
     launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, -1, stream);
-    launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
-                                     (double*)(ws + L.coefs[0]), ctl, k ? plan_a.npasses - k : 0, stream);
-    rc = bucket_precheck(plan_a, &k, n, ws, L, o, &launches, stream);
+    // X1 runs inside the first radix pass (the products are formed in registers and never stored) unless the ballot
+    // ranking kernel is asked for or there is no pass at all; only the first digit's histogram is built up front
+    const ExpandSrc xs = {ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb};
+    const bool fuse = plan_a.npasses > 0 && !at.safe_rank && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
+    if (fuse) launches += launch_expand_hist(xs, plan_a, k ? plan_a.npasses - k : 0, ctl, stream);
+    else launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
+                                          (double*)(ws + L.coefs[0]), ctl, k ? plan_a.npasses - k : 0, stream);
+    rc = bucket_precheck(plan_a, &k, n, ws, L, o, &launches, stream, nullptr, fuse ? &xs : nullptr);
     if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
     return sort_reduce_emit(plan_a, k, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                            out_nterms, &launches, tm, at.safe_rank, stream);
+                            out_nterms, &launches, tm, at.safe_rank, stream, nullptr, fuse ? &xs : nullptr);
 }
 
 int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,

@@ -73,9 +73,22 @@ int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const Exp
 // registers from the rows, range-checked into ctl->status; atomic ranking only.
 // safe_rank: ballot-matching ranking (stable by construction); otherwise one shared atomic per record (see sort.cu).
 // debug_unstable: test hook, reverses the lane order of the atomic kernel.
+// `xs` (packed operands of a product): X1 fused into the pass -- keys_in / coef_in are ignored, record q = i*nb + j is
+// formed in registers as (ka_i + kb_j, fl(ca_i * cb_j)); atomic ranking only.
+struct ExpandSrc {
+    const void* ka;
+    const double* ca;
+    int64_t na;
+    const void* kb;
+    const double* cb;
+    int64_t nb;
+};
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream, const ExpView* rows = nullptr);
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr);
+
+// Histogram of plan digit `hist_digit` over the na*nb products of packed operands, without storing them.
+int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hist_digit, Control* ctl, cudaStream_t stream);
 
 // S3: segmented sum over sorted pairs -> (ukeys[U], usums[U]) ascending, ctl->distinct = U; sets ctl->unsorted
 // when a key is smaller than its predecessor.

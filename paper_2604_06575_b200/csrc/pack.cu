@@ -447,6 +447,41 @@ int launch_expand_packed(const void* ka, const double* ca, int64_t na, const voi
     return 1;
 }
 
+// Histogram of one digit over all products, nothing stored (X1 fused into the first radix pass needs it up front).
+template <typename K>
+__global__ void __launch_bounds__(256) expand_hist_kernel(const K* __restrict__ ka, uint32_t na, const K* __restrict__ kb,
+                                                          uint32_t nb, int dpos, uint32_t dmask, uint32_t* hist)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    bh.init(sh);
+    __syncthreads();
+    const uint32_t n = na * nb;
+    for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += gridDim.x * blockDim.x) {
+        const uint32_t i = q / nb, j = q - i * nb;
+        bh.add(key_digit(key_add(ka[i], kb[j]), dpos, dmask));
+    }
+    __syncthreads();
+    bh.flush(hist);
+}
+
+int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hd, Control* ctl, cudaStream_t stream)
+{
+    const int64_t n = xs.na * xs.nb;
+    if (n <= 0 || hd < 0 || hd >= plan.npasses) return 0;
+    int64_t blocks = (n + 256 * 8 - 1) / (256 * 8);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    const int dpos = plan.digit_pos[hd];
+    const uint32_t dmask = (1u << plan.digit_bits[hd]) - 1u;
+    if (plan.key_bytes == 8)
+        expand_hist_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)xs.ka, (uint32_t)xs.na, (const uint64_t*)xs.kb,
+                                                                          (uint32_t)xs.nb, dpos, dmask, ctl->hist[hd]);
+    else
+        expand_hist_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)xs.ka, (uint32_t)xs.na, (const Key128*)xs.kb,
+                                                                        (uint32_t)xs.nb, dpos, dmask, ctl->hist[hd]);
+    return 1;
+}
+
 // Raw product in (coef, exps) form, no keys: polylab_expand (reading A10).
 __global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, const double* __restrict__ ca, uint32_t na,
                                                          ExpView eb, const double* __restrict__ cb, uint32_t nb,

@@ -44,7 +44,14 @@ struct PassArgs {
     const uint8_t* rows;
     int exp_bytes;
     int32_t* status;
+    // X1 fused into the pass (ROWS == kLoadProducts): record q = i*xnb + j is the product of term i of a and term j of b
+    const void* xa_keys;
+    const void* xb_keys;
+    const double* xa_coef;
+    const double* xb_coef;
+    uint32_t xnb;
 };
+constexpr int kLoadProducts = -1;
 
 // Step S1 inside the radix pass: exponent row t (ROWS = 8 or 16 contiguous bytes) -> key, with the range check of
 // pack.cu (an exponent above plan.bound sets `bad`).  BYTES: u8 exponents, every field 8 bits wide and unbounded, rows
@@ -134,7 +141,11 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         const uint32_t li = chunk + j * 32u;
         if (FULL || li < tile_n) {
             if (ROWS > 0) key[j] = pack_row_inline<K, (ROWS > 0 ? ROWS : 8), BYTES>(a, *plan, tile_base + li, bad);
-            else key[j] = keys_in[tile_base + li];
+            else if (ROWS == kLoadProducts) {
+                // step X1 in registers: key = ka_i + kb_j (fields never carry into each other), the product is never stored
+                const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
+                key[j] = key_add(((const K*)a.xa_keys)[i], ((const K*)a.xb_keys)[jj]);
+            } else key[j] = keys_in[tile_base + li];
         } else key[j] = key_max<K>();
     }
     if (ROWS > 0 && bad) atomicMax(a.status, (int)POLYLAB_ERR_EXPONENT_RANGE);
@@ -215,7 +226,10 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
-        c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
+        if (ROWS == kLoadProducts) {
+            const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
+            c[j] = (FULL || li < tile_n) ? __dmul_rn(a.xa_coef[i], a.xb_coef[jj]) : 0.0;     // one IEEE multiplication, never contracted
+        } else c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
     }
 
     // ---- decoupled look-back: number of records with digit b in all earlier tiles.  The walk over the predecessors
@@ -328,7 +342,7 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 template <typename K, int THREADS, int ITEMS, int MINB>
 static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in,
                               const double* coef_in, void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl,
-                              bool safe_rank, bool debug_unstable, const ExpView* rows, cudaStream_t stream)
+                              bool safe_rank, bool debug_unstable, const ExpView* rows, const ExpandSrc* xs, cudaStream_t stream)
 {
     using S = SortSmem<K, THREADS, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
@@ -346,6 +360,17 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[has_next ? next : kMaxPasses]; a.ticket = &ctl->ticket[seq];
     a.reverse_lanes = debug_unstable ? 1 : 0;
     a.rows = nullptr; a.exp_bytes = 0; a.status = &ctl->status;
+    a.xa_keys = nullptr; a.xb_keys = nullptr; a.xa_coef = nullptr; a.xb_coef = nullptr; a.xnb = 1;
+    if (xs) {
+        a.xa_keys = xs->ka; a.xb_keys = xs->kb; a.xa_coef = xs->ca; a.xb_coef = xs->cb; a.xnb = (uint32_t)xs->nb;
+        auto go = [&](auto kern) {
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
+            kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);
+        };
+        if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, kLoadProducts, false>);
+        else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, kLoadProducts, false>);
+        return 1;
+    }
     if (rows) {
         a.rows = (const uint8_t*)rows->base; a.exp_bytes = rows->exp_bytes;
         bool fast = rows->exp_bytes == 1 && plan.nvars * rows->exp_bytes == (int)sizeof(K);
@@ -373,14 +398,14 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
 
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream, const ExpView* rows)
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows, const ExpandSrc* xs)
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortThreads64, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                             tile_state, ctl, safe_rank, debug_unstable, rows, stream);
+                                                             tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
     return launch_sort_pass_t<Key128, kSortThreads128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                        tile_state, ctl, safe_rank, debug_unstable, rows, stream);
+                                                        tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
 }
 
 }  // namespace polylab

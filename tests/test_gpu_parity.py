@@ -446,3 +446,29 @@ def test_unstable_rank_is_detected_and_falls_back():
                               flags=B.FLAG_DEBUG_UNSTABLE)
     assert st.rank_fallback == 1
     assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol), c.cpu().numpy(), e.cpu().numpy())
+
+
+@pytest.mark.parametrize("shape", ["c2", "c4sq", "wide128", "tiny"])
+def test_fused_expand_matches_materialised_products(shape):
+    """X1 runs inside the first radix pass by default (products formed in registers, never stored); with
+    POLYLAB_FLAG_NO_FUSED_PACK the products are materialised first.  Same order of records -> bit-identical results."""
+    r = np.random.default_rng(77)
+    if shape == "c2":
+        a, b, tol = W.config2(700)
+    elif shape == "c4sq":
+        p, tol = W.config4()
+        a, b = p, p
+    elif shape == "wide128":
+        a = W.Poly(r.standard_normal(900), r.integers(0, 100, size=(900, 12)).astype(np.uint8))
+        b = W.Poly(r.standard_normal(40), r.integers(0, 100, size=(40, 12)).astype(np.uint8))
+        tol = 0.0
+    else:
+        a = W.Poly(np.array([1.0, 2.0]), np.array([[1, 0], [0, 1]], np.uint8))
+        b = W.Poly(np.array([1.0, -2.0]), np.array([[1, 0], [0, 1]], np.uint8))
+        tol = 0.0
+    r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True)
+    r1 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_NO_FUSED_PACK)
+    c0, e0, c1, e1 = r0[0].cpu().numpy(), r0[1].cpu().numpy(), r1[0].cpu().numpy(), r1[1].cpu().numpy()
+    assert (e0 == e1).all() and (c0.view(np.uint64) == c1.view(np.uint64)).all()
+    assert r0[2].kernel_launches == r1[2].kernel_launches
+    assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol), c0, e0)
