@@ -26,8 +26,8 @@
 //                        look-back: a tile only knows its count at the very end, and waiting in order for slow
 //                        predecessors left SMs idle).
 //   tile_sum_kernel, tile_scan_kernel   exclusive scan of the tiles' survivor counts (chunk sums, then the scan).
-//   emit_kernel          S5: one thread per output term finds its tile in the scanned counts (binary search) and
-//                        unpacks the key into the caller's output -- order-preserving compaction across tiles.
+//   emit_kernel          S5: one warp per work-list tile copies the tile's survivors to the tile's scanned offset and
+//                        unpacks the keys into the caller's output -- order-preserving compaction across tiles.
 //                        HBM traffic of all of them: N*(W+8) read, U'*(W+8) written and read, U'*(8+E) written.
 //
 // The local sort first uses only as many key bits below the prefix as fit the composite sort word (enough to separate
@@ -256,6 +256,9 @@ struct EmitArgs {
     int exp_bytes;
     int wpr;                        // > 0: rows are written as this many 32-bit words (common.cuh, row_words)
     int64_t out_capacity;
+    const uint32_t* worklist;       // the tiles that own records (ctl->fin_count of them, at most max_list processed by finish_kernel)
+    uint32_t max_list;
+    const Control* ctl;
 };
 
 template <typename K>
@@ -601,21 +604,22 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(uint32_t* __restrict__ 
     }
 }
 
-// One thread per output term: find its tile in the scanned counts, fetch (key, sum), unpack (S5).
+// S5: one warp per work-list tile copies the tile's survivors to their final place (the tile's scanned offset) and unpacks
+// the keys -- no search, consecutive lanes read and write consecutive terms.  Tiles without records are not on the list.
 template <typename K>
 __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitArgs a, const __grid_constant__ Plan plan)
 {
-    const uint32_t total = a.tile_off[a.ntiles];
-    const uint64_t limit = min((uint64_t)total, (uint64_t)a.out_capacity);
-    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < limit; o += (uint64_t)gridDim.x * blockDim.x) {
-        uint32_t lo = 0, hi = a.ntiles;            // last tile t with tile_off[t] <= o
-        while (hi - lo > 1) {
-            const uint32_t mid = lo + (hi - lo) / 2;
-            if (a.tile_off[mid] <= (uint32_t)o) lo = mid;
-            else hi = mid;
+    const uint32_t nlist = min(a.ctl->fin_count, a.max_list);
+    const unsigned lane = lane_id();
+    const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
+    for (uint32_t q = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); q < nlist; q += nwarps) {
+        const uint32_t t = a.worklist[q];
+        const uint32_t off = a.tile_off[t], cnt = a.tile_off[t + 1] - off;
+        const uint64_t src = a.tile_start[t];
+        for (uint32_t i = lane; i < cnt; i += 32u) {
+            const uint64_t o = (uint64_t)off + i;
+            if ((int64_t)o < a.out_capacity) emit_term<K>(a, plan, o, a.usums[src + i], ((const K*)a.ukeys)[src + i]);
         }
-        const uint64_t src = (uint64_t)a.tile_start[lo] + ((uint32_t)o - a.tile_off[lo]);
-        emit_term<K>(a, plan, o, a.usums[src], ((const K*)a.ukeys)[src]);
     }
 }
 
@@ -656,8 +660,9 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     e.out_coef = out_coef; e.out_exps = out_exps; e.exp_bytes = exp_bytes;
     e.wpr = row_words(plan.nvars, exp_bytes, out_exps);
     e.out_capacity = out_capacity;
-    int64_t blocks = (n / 4 + 255) / 256;          // at most N outputs; grid-stride
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    e.worklist = worklist; e.max_list = fin_blocks; e.ctl = ctl;
+    int64_t blocks = ((int64_t)fin_blocks + 7) / 8;          // one warp per work-list tile, grid-stride
+    if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks < 1) blocks = 1;
     emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
     return 5;
