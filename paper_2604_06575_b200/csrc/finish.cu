@@ -307,6 +307,12 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     // (stride itn elements) spread over all banks
     const uint32_t itn = ((n_loc + THREADS - 1) / THREADS) | 1u;
     const uint32_t first = tid * itn;
+    // pull the tile's keys and coefficients towards L2 now: the key stream below is read in batches and the coefficients
+    // only after the sort, and both would otherwise wait out a full DRAM round trip when their turn comes
+    for (uint32_t i = tid * 8u; i < n_loc; i += THREADS * 8u)                 // one 128-byte line of keys (64-bit keys: half a line)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(gkeys + i));
+    for (uint32_t i = tid * 16u; i < n_loc; i += THREADS * 16u)               // one 128-byte line of coefficients
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(gcoef + i));
 
     // raw sort bits of the fast attempt: the (up to 32) key bits just below the prefix
     const int rbits = min(32, a.pfx_pos);
