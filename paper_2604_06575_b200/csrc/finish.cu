@@ -128,8 +128,10 @@ struct FinishSmem {
 // profiles/r1b_shared_atomics.md) and is re-verified by the caller's order check.
 template <bool FIRST, bool RANKS>
 __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int dbits, uint32_t n_loc,
-                                           uint32_t* whist, uint32_t* scratch, uint16_t* ranks)
+                                           uint32_t* whist, uint32_t* scratch, uint16_t* ranks, int pre = 0)
 {
+    // pre (FIRST only): the input words are shifted right by this before use (a one-bucket tile sorts on the raw key bits
+    // as they were cut, without a pass that rewrites them)
     constexpr int NW = FinishSmem::NW, ROW = kFinBins / 2;    // words per histogram row
     constexpr int BPT = kFinBins / kFinThreads;               // bins per thread in the scan step
     static_assert(BPT >= 1 && BPT * kFinThreads == kFinBins, "whole bins per thread in the scan step");
@@ -146,7 +148,7 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
         // sweep 1 counts AND ranks: the atomic's old value is the record's rank among its warp's records of the digit
         for (uint32_t base = wbeg; base < wend; base += 64u) {      // two rounds per iteration: both loads first
             const uint32_t i0 = base + lane, i1 = i0 + 32u;
-            const uint32_t e0 = (i0 < wend) ? in[i0] : 0u, e1 = (i1 < wend) ? in[i1] : 0u;
+            const uint32_t e0 = (i0 < wend) ? (FIRST ? in[i0] >> pre : in[i0]) : 0u, e1 = (i1 < wend) ? (FIRST ? in[i1] >> pre : in[i1]) : 0u;
             if (i0 < wend) {
                 const uint32_t d = (FIRST ? e0 : (e0 >> 13)) & mask;
                 const uint32_t sh = (d & 1u) * 16u;
@@ -162,7 +164,7 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
         }
     } else {
         for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
-            const uint32_t d = (FIRST ? in[i] : (in[i] >> 13)) & mask;
+            const uint32_t d = (FIRST ? (in[i] >> pre) : (in[i] >> 13)) & mask;
             atomicAdd(&my_hist[d >> 1], 1u << ((d & 1u) * 16u));
         }
     }
@@ -191,7 +193,7 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
         const uint16_t* my16 = h16 + warp * kFinBins;
 #pragma unroll 4
         for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
-            const uint32_t e = in[i];
+            const uint32_t e = FIRST ? (in[i] >> pre) : in[i];
             const uint32_t d = (FIRST ? e : (e >> 13)) & mask;
             const uint32_t slot = (uint32_t)my16[d] + ranks[i];
             out[slot] = FIRST ? (i | ((e >> dbits) << 13)) : ((e & 0x1fffu) | ((e >> (13 + dbits)) << 13));
@@ -200,7 +202,7 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
         for (uint32_t base = wbeg; base < wend; base += 32u) {
             const uint32_t i = base + lane;
             if (i < wend) {
-                const uint32_t e = in[i];
+                const uint32_t e = FIRST ? (in[i] >> pre) : in[i];
                 const uint32_t d = (FIRST ? e : (e >> 13)) & mask;
                 const uint32_t sh = (d & 1u) * 16u;
                 const uint32_t slot = (atomicAdd(&my_hist[d >> 1], 1u << sh) >> sh) & 0xffffu;
@@ -217,12 +219,12 @@ __device__ __forceinline__ void local_pass(const uint32_t* __restrict__ in, uint
 // composite sort word exists), which halves the atomics
 template <bool FIRST0, bool RANKS>
 __device__ __forceinline__ void local_sort_bits(uint32_t** cur, uint32_t** oth, int nbits, uint32_t n_loc, uint32_t* whist,
-                                                uint32_t* scratch, uint16_t* ranks)
+                                                uint32_t* scratch, uint16_t* ranks, int pre = 0)
 {
     bool first = FIRST0;
     for (int done = 0; done < nbits; done += kFinDigit) {
         const int dbits = min(kFinDigit, nbits - done);
-        if (first) local_pass<true, RANKS>(*cur, *oth, dbits, n_loc, whist, scratch, ranks);
+        if (first) local_pass<true, RANKS>(*cur, *oth, dbits, n_loc, whist, scratch, ranks, pre);
         else local_pass<false, RANKS>(*cur, *oth, dbits, n_loc, whist, scratch, ranks);
         first = false;
         uint32_t* t = *cur; *cur = *oth; *oth = t;
@@ -321,7 +323,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     double acc = 0.0;
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
-        bool descending = false;
+        bool descending = false, later_head = false;
         if (a.pfx_pos >= 8 * (int)sizeof(K) - 64) {
             // the prefix lies in the key's most significant 64 bits: only those are fetched from the left neighbour, and
             // four records per thread are in flight (all loads issued before the first use)
@@ -346,6 +348,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                         const uint64_t pk = key_top64(k[u]) >> hs, pp = ph[u] >> hs;
                         const bool head = (i == 0) || pk != pp;
                         descending |= (i > 0) && pk < pp;
+                        later_head |= head && i > 0;
                         bx[i] = full ? i : key_get_field(k[u], a.pfx_pos - rbits, rbits);
                         py[i] = head ? 1 : 0;
                     }
@@ -359,20 +362,25 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                     const K kp = gkeys[i - 1];
                     head = !same_prefix(k, kp, a.pfx_pos);
                     descending |= head && key_lt(k, kp);
+                    later_head |= head;
                 }
                 bx[i] = full ? i : key_get_field(k, a.pfx_pos - rbits, rbits);
                 py[i] = head ? 1 : 0;
             }
         }
         if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
-        __syncthreads();
+        const bool one_bucket = !__syncthreads_or(later_head ? 1 : 0) && !full;
 
         // ---- bucket ordinal of every record (buckets are contiguous: the input is sorted by prefix); fast attempt:
         // composite sort word = ordinal above the top fb raw bits, ob + fb <= 27 so that 13 index bits fit beside what
-        // is left after the first 9-bit pass
-        uint32_t nbuckets;
-        int ob = 0, fb = 0;
-        {
+        // is left after the first 9-bit pass.  A tile with a single bucket (the usual case when buckets are longer than the
+        // tile step) needs neither: it sorts on the raw bits as cut, shifted on the fly by the first pass.
+        uint32_t nbuckets = 1;
+        int ob = 0, fb = 0, pre = 0;
+        if (one_bucket) {
+            fb = min(min(27, rbits), a.fast_bits);
+            pre = rbits - fb;
+        } else {
             uint32_t cnt = 0;
             for (uint32_t j = 0; j < itn; ++j)
                 if (first + j < n_loc) cnt += py[first + j];
@@ -393,7 +401,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         uint32_t* cur = bx;
         uint32_t* oth = by;
         if (!full) {
-            local_sort_bits<true, true>(&cur, &oth, ob + fb, n_loc, whist, scratch, py);
+            local_sort_bits<true, true>(&cur, &oth, ob + fb, n_loc, whist, scratch, py, pre);
             if (ob + fb == 0)                      // one bucket, no bits: identity
                 for (uint32_t i = tid; i < n_loc; i += THREADS) cur[i] = i;
         } else {
