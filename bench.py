@@ -10,9 +10,10 @@ north_star's roofline target is quoted on.  Prints ONE JSON line (rank 0).
 
   value     input terms/s, whole job, inputs resident in HBM, CUDA events around K calls of the C ABI
   e2e       the same metric through polylab_simplify_host: pinned host buffers, H2D and D2H inside the call
-  roofline  the longest kernel of the step, timed live with the library's CUDA events on the call's stream
-            (POLYLAB_FLAG_TIMING): on the bucket path the finish kernel (N*(W+8) read + U'*(W+8) written), on the LSD
-            path one radix pass (2*N*(W+8)); the radix pass and the sort+reduce pipeline are reported beside it
+  roofline  the kernel with the largest share of the step, timed live with the library's CUDA events on the call's
+            stream (POLYLAB_FLAG_TIMING): the radix pass (2*N*(W+8) per launch, all launches counted) or, on the bucket path
+            when it takes longer, the finish kernel (N*(W+8) read + U'*(W+8) written); the other one, the radix pass and the
+            sort+reduce pipeline figure are reported beside it
   cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same recipe (rank 0, N=1 only)
 
 --impl reference times the oracle alone (there is no reference implementation to install: the paper's
@@ -319,23 +320,30 @@ def main():
     pass_info = {"kernel": "sort_pass_kernel (one radix pass, 8-bit digit)", "launch_ms": pass_ms, "launches_per_step": P,
                  "algorithmic_bytes_per_launch": pass_bytes, "achieved": pass_gbs, "frac": pass_gbs / peak,
                  "traffic": tinfo.get("sort_pass_dram_bytes_per_launch")}
+    pass_roof = {"bound": "hbm", "kernel": pass_info["kernel"], "achieved": pass_gbs, "peak": peak, "unit": "GB/s",
+                 "frac": pass_gbs / peak if peak else None, "traffic": pass_info["traffic"], "peak_source": peak_src,
+                 "algorithmic_bytes_per_launch": pass_bytes, "launch_ms": pass_ms, "launches_per_step": P,
+                 "share_of_step": stage_ms["sort"] / ms_per_step, "frac_of_nominal_8TBs": pass_gbs / NOMINAL_HBM_GBS}
+    roofline = pass_roof
     if st.prefix_passes > 0:
-        # bucket path: the finish kernel is the longest kernel of the step; it reads every pair once and writes the survivors
+        # bucket path: the finish kernel reads every pair once and writes the survivors
         fin_ms = stage_ms["reduce"]
         fin_bytes = float(N * S + U1 * S)
         achieved = fin_bytes / (fin_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "finish_kernel (bucket path: shared-memory sort of each bucket + segmented sum + prune)",
+        fin_roof = {"bound": "hbm", "kernel": "finish_kernel (bucket path: shared-memory sort of each bucket + segmented sum + prune)",
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                     "traffic": tinfo.get("finish_dram_bytes_per_launch"), "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": fin_bytes, "launch_ms": fin_ms, "launches_per_step": 1,
+                    "share_of_step": fin_ms / ms_per_step,
                     "limiter": "shared-memory / LSU pipe, not DRAM (ncu, profiles/): the kernel trades HBM passes for on-chip work",
                     "lsu_pipe": lsu_pipe(tinfo.get("finish_lsu_wavefronts_per_launch"), fin_ms),
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
-    else:
-        roofline = {"bound": "hbm", "kernel": pass_info["kernel"], "achieved": pass_gbs, "peak": peak, "unit": "GB/s",
-                    "frac": pass_gbs / peak if peak else None, "traffic": pass_info["traffic"], "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": pass_bytes, "launch_ms": pass_ms, "launches_per_step": P,
-                    "frac_of_nominal_8TBs": pass_gbs / NOMINAL_HBM_GBS}
+        # the dominant kernel is the one with the larger share of the step: the radix pass (all its launches) or the finish
+        if fin_ms > stage_ms["sort"]:
+            roofline = fin_roof
+        else:
+            roofline = dict(pass_roof)
+            roofline["finish_kernel"] = fin_roof
     roofline["radix_pass"] = pass_info
     # the north_star's pipeline figure: bytes an LSD sort + segmented sum of these keys must move / time of sort + reduce stages
     roofline["sort_plus_reduce"] = {"ms": sr_ms, "lsd_algorithmic_bytes": lsd_bytes, "lsd_passes": lsd_digits,

@@ -426,13 +426,16 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
             }
         }
         __syncthreads();
-        for (uint32_t i = tid; i < n_loc; i += THREADS) py[i] = (uint16_t)(cur[i] & 0x1fffu);
-        __syncthreads();
-        // coefficients into sorted order through the INVERSE permutation: the global read is coalesced (a gather would
-        // touch one 32-byte sector per 8-byte coefficient), the permuted write goes to shared memory
+        // the final permutation (sorted position -> record) and its inverse; coefficients then reach sorted order through
+        // the INVERSE permutation: the global read is coalesced (a gather would touch one 32-byte sector per 8-byte
+        // coefficient), the permuted write goes to shared memory
         {
             uint16_t* inv = (uint16_t*)whist;      // the histograms are dead until the next pass
-            for (uint32_t i = tid; i < n_loc; i += THREADS) inv[py[i]] = (uint16_t)i;
+            for (uint32_t i = tid; i < n_loc; i += THREADS) {
+                const uint32_t r = cur[i] & 0x1fffu;
+                py[i] = (uint16_t)r;
+                inv[r] = (uint16_t)i;
+            }
             __syncthreads();
 #pragma unroll 4
             for (uint32_t i = tid; i < n_loc; i += THREADS) scs[inv[i]] = gcoef[i];
