@@ -525,8 +525,12 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         }
     }
     const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
-    uint32_t tile_keep;
-    const uint32_t kexcl = block_exclusive_scan<THREADS>(nkeep + (last_keep ? 1u : 0u), scratch, &tile_keep);
+    // one scan for two counts (each at most CAP < 2^16): survivors in the low half, heads (distinct monomials) in the high half
+    uint32_t tile_keep, tot_heads;
+    uint32_t kexcl = block_exclusive_scan<THREADS>((nkeep + (last_keep ? 1u : 0u)) | (nh << 16), scratch, &tile_keep);
+    kexcl &= 0xffffu;
+    tot_heads = tile_keep >> 16;
+    tile_keep &= 0xffffu;
 
     // ---- the tile's survivors, compacted in order at the tile's own place; S5 (emit_kernel) puts the tiles together
     {
@@ -553,13 +557,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         }
         if (last_keep) { us[o] = incl.v; uk[o] = gkeys[py[n_loc - 1]]; }
     }
-    {
-        uint32_t tot_heads;                        // distinct monomials of the tile, for the statistics
-        (void)block_exclusive_scan<THREADS>(nh, scratch, &tot_heads);
-        if (tid == 0) {
-            if (tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);
-            a.tile_state[tile] = tile_keep;
-        }
+    if (tid == 0) {
+        if (tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);      // distinct monomials, for the statistics
+        a.tile_state[tile] = tile_keep;
     }
 }
 
