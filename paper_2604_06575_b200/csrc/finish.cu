@@ -319,8 +319,8 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     // raw sort bits of the fast attempt: the (up to 32) key bits just below the prefix
     const int rbits = min(32, a.pfx_pos);
     bool full = (rbits == 0);                      // nothing below the prefix: only the ordinal is sorted on
-    uint32_t hm = 0, nh = 0;
-    double acc = 0.0;
+    uint32_t hm = 0, nh = 0, keep = 0, nkeep = 0, nclosed = 0;
+    double acc = 0.0, part0 = 0.0;
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
         bool descending = false, later_head = false;
@@ -444,6 +444,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
 
         // ---- gather through the permutation: heads of runs of equal keys, sums since the last head, order check
         hm = 0; nh = 0; acc = 0.0;
+        keep = 0; nkeep = 0; nclosed = 0; part0 = 0.0;
         bool viol = false;
         {
             K kp;
@@ -457,8 +458,16 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                     const double c = scs[first + j];
                     const bool head = !hp || !key_eq(kk, kp);
                     viol |= hp && key_lt(kk, kp);
-                    if (head) { hm |= 1u << j; ++nh; acc = c; }
-                    else acc = __dadd_rn(acc, c);
+                    if (head) {
+                        // S4 for the runs that END here (a run ends where the next head is met): a run that also began
+                        // in this thread has its whole sum in acc; the first one needs the other threads' part (below)
+                        if (first + j > 0) {
+                            if (nclosed == 0) part0 = acc;
+                            else if (fabs(acc) > a.tol) { keep |= 1u << nclosed; ++nkeep; }    // NaN compares false: dropped (A12)
+                            ++nclosed;
+                        }
+                        hm |= 1u << j; ++nh; acc = c;
+                    } else acc = __dadd_rn(acc, c);
                     kp = kk;
                     hp = true;
                 }
@@ -504,26 +513,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         incl = seg_combine(wp, incl);
     }
 
-    // ---- S4: which of the runs that END in this thread survive (a run ends where the next head is met; the run still
-    // open at the end of the tile is closed by the last thread, whose inclusive scan value is its sum)
-    uint32_t keep = 0, nkeep = 0;
-    {
-        uint32_t k = 0;
-        double a2 = 0.0;
-        for (uint32_t j = 0; j < itn; ++j) {
-            if (first + j < n_loc) {
-                const double c = scs[first + j];
-                if (hm & (1u << j)) {
-                    if (first + j > 0) {
-                        const double total = (k == 0) ? __dadd_rn(carry.v, a2) : a2;
-                        if (fabs(total) > a.tol) { keep |= 1u << k; ++nkeep; }     // NaN compares false: dropped (A12)
-                        ++k;
-                    }
-                    a2 = c;
-                } else a2 = __dadd_rn(a2, c);
-            }
-        }
-    }
+    // ---- S4 for the first run that ends in this thread (its head lies in an earlier thread); the run still open at the
+    // end of the tile is closed by the last thread, whose inclusive scan value is its sum
+    if (nclosed > 0 && fabs(__dadd_rn(carry.v, part0)) > a.tol) { keep |= 1u; ++nkeep; }
     const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
     // one scan for two counts (each at most CAP < 2^16): survivors in the low half, heads (distinct monomials) in the high half
     uint32_t tile_keep, tot_heads;
