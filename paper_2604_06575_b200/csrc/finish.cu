@@ -463,7 +463,11 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                         // in this thread has its whole sum in acc; the first one needs the other threads' part (below)
                         if (first + j > 0) {
                             if (nclosed == 0) part0 = acc;
-                            else if (fabs(acc) > a.tol) { keep |= 1u << nclosed; ++nkeep; }    // NaN compares false: dropped (A12)
+                            else if (fabs(acc) > a.tol) {                  // NaN compares false: dropped (A12)
+                                keep |= 1u << nclosed;
+                                ++nkeep;
+                                scs[first + j - 1] = acc;                  // the run's sum, parked on its last record (own position)
+                            }
                             ++nclosed;
                         }
                         hm |= 1u << j; ++nh; acc = c;
@@ -515,7 +519,15 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
 
     // ---- S4 for the first run that ends in this thread (its head lies in an earlier thread); the run still open at the
     // end of the tile is closed by the last thread, whose inclusive scan value is its sum
-    if (nclosed > 0 && fabs(__dadd_rn(carry.v, part0)) > a.tol) { keep |= 1u; ++nkeep; }
+    const uint32_t chm = (first == 0) ? (hm & ~1u) : hm;        // the heads that close a run (every head but the tile's first record)
+    if (nclosed > 0) {
+        const double total0 = __dadd_rn(carry.v, part0);
+        if (fabs(total0) > a.tol) {
+            keep |= 1u;
+            ++nkeep;
+            scs[first + (__ffs(chm) - 1) - 1] = total0;             // its last record is the one before that head (maybe the previous thread's: nobody else touches it)
+        }
+    }
     const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
     // one scan for two counts (each at most CAP < 2^16): survivors in the low half, heads (distinct monomials) in the high half
     uint32_t tile_keep, tot_heads;
@@ -530,21 +542,12 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         double* __restrict__ us = a.usums + lo;
         uint32_t o = kexcl;
         uint32_t k = 0;
-        double a2 = 0.0;
-        for (uint32_t j = 0; j < itn; ++j) {
-            if (first + j < n_loc) {
-                const double c = scs[first + j];
-                if (hm & (1u << j)) {
-                    if (first + j > 0) {
-                        if (keep & (1u << k)) {
-                            us[o] = (k == 0) ? __dadd_rn(carry.v, a2) : a2;
-                            uk[o] = gkeys[py[first + j - 1]];
-                            ++o;
-                        }
-                        ++k;
-                    }
-                    a2 = c;
-                } else a2 = __dadd_rn(a2, c);
+        for (uint32_t m = chm; m != 0u; m &= m - 1u, ++k) {         // the runs that end in this thread, in order
+            if (keep & (1u << k)) {
+                const uint32_t pos = first + (__ffs(m) - 1) - 1;    // the run's last record, where its sum was parked
+                us[o] = scs[pos];
+                uk[o] = gkeys[py[pos]];
+                ++o;
             }
         }
         if (last_keep) { us[o] = incl.v; uk[o] = gkeys[py[n_loc - 1]]; }
