@@ -84,9 +84,10 @@ enum {
                                         (stats->prefix_passes > 0); otherwise (stats->bucket_fallback = 1) it runs the
                                         LSD passes.  Both paths give the same result up to summation order.  Not
                                         taken with POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
-    POLYLAB_FLAG_NO_FUSED_PACK = 16u, /* bucket path: always run S1 as its own kernel.  By default, when the exponent rows
-                                        are contiguous and 8 or 16 bytes long, the first radix pass packs the keys in
-                                        registers (no key array is written and re-read) */
+    POLYLAB_FLAG_NO_FUSED_PACK = 16u, /* always run S1 (pack) and X1 (expand) as kernels of their own.  By default the first
+                                        radix pass forms its keys in registers: from the exponent rows on the bucket path
+                                        (contiguous rows of 8 or 16 bytes), from the packed operands for a product
+                                        (the na*nb products are then never stored).  Same result, bit for bit. */
     POLYLAB_FLAG_EXACT_BOUNDS = 32u,  /* S0 always reads every exponent.  By default a simplify call with >= 2^22 terms and
                                         no max_exp_host takes the maxima of a sample of the rows, sizes the key fields by
                                         their bit lengths, and lets S1's range check verify every row; a violation
