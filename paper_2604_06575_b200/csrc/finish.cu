@@ -394,8 +394,8 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                     if (!full) bx[first + j] = ((o - 1u) << fb) | (fb ? (bx[first + j] >> (rbits - fb)) : 0u);
                 }
             }
+            __syncthreads();
         }
-        __syncthreads();
 
         // ---- local sort; the final permutation lands in py
         uint32_t* cur = bx;
