@@ -674,7 +674,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     e.out_capacity = out_capacity;
     e.worklist = worklist; e.max_list = fin_blocks; e.ctl = ctl;
     int64_t blocks = ((int64_t)fin_blocks + 7) / 8;          // one warp per work-list tile, grid-stride
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > 148 * 64) blocks = 148 * 64;
     if (blocks < 1) blocks = 1;
     emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
     return 5;
