@@ -143,7 +143,7 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.fin_state = take((fin_tiles + 1) * sizeof(uint32_t));
     L.zero_end = off;                                   // everything before this is zeroed per call
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
-    L.fin_wl = take((fin_tiles + 1) * sizeof(uint32_t));
+    L.fin_wl = take((fin_tiles + 1) * sizeof(uint4));
     L.fin_chunks = take((fin_tiles / 4096 + 2) * sizeof(uint32_t));
     L.red_heads = take(red_tiles * sizeof(uint32_t));
     L.red_hb = take(red_tiles * sizeof(uint32_t));
@@ -298,7 +298,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
                                kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes, out_capacity,
-                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint32_t*)(ws + L.fin_wl), (uint32_t*)(ws + L.fin_chunks), ctl, nullptr,
+                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint32_t*)(ws + L.fin_chunks), ctl, nullptr,
                                tm.on ? tm.ev[POLYLAB_STAGE_REDUCE + 1] : nullptr, stream);      // REDUCE = tiles, PRUNE = scan + emit
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());

@@ -70,16 +70,17 @@ __device__ __forceinline__ uint32_t tile_first_change(const K* __restrict__ keys
 template <typename K>
 __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ keys, uint32_t n, int pfx_pos,
                                                           uint32_t fin_tile, uint32_t ntiles,
-                                                          uint32_t* __restrict__ tile_start, uint32_t* __restrict__ worklist,
+                                                          uint32_t* __restrict__ tile_start, uint4* __restrict__ worklist,
                                                           Control* ctl)
 {
     const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     bool overflow = false, owns = false;
+    uint32_t lo = 0, hi = 0;
     if (t <= ntiles) {
-        const uint32_t lo = tile_first_change(keys, n, pfx_pos, fin_tile, t, &overflow);
+        lo = tile_first_change(keys, n, pfx_pos, fin_tile, t, &overflow);
         tile_start[t] = lo;
         if (t < ntiles) {
-            const uint32_t hi = tile_first_change(keys, n, pfx_pos, fin_tile, t + 1, &overflow);
+            hi = tile_first_change(keys, n, pfx_pos, fin_tile, t + 1, &overflow);
             owns = (uint64_t)lo < ((uint64_t)t + 1) * fin_tile && hi > lo;        // a bucket starts inside the tile
         }
         // a tile starts a new bucket: its first prefix must be above the record before it (finish_kernel checks the
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ 
         uint32_t base = 0;
         if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(&ctl->fin_count, (uint32_t)__popc(m));
         base = __shfl_sync(kFullMask, base, __ffs(m) - 1);
-        if (owns) worklist[base + __popc(m & lanemask_lt())] = t;
+        if (owns) worklist[base + __popc(m & lanemask_lt())] = make_uint4(t, lo, hi, 0u);     // tile, first record, end
     }
 }
 
@@ -237,7 +238,7 @@ struct FinishArgs {
     uint32_t n, ntiles;
     uint32_t fin_tile;              // positions per tile; a tile owns at most kFinCap records
     const uint32_t* tile_start;     // [ntiles + 1]
-    const uint32_t* worklist;       // the ctl->fin_count tiles that own records
+    const uint4* worklist;          // the ctl->fin_count tiles that own records: (tile, first record, end, -)
     uint32_t* tile_state;           // [ntiles + 1] survivors per tile, zero before the kernel
     int pfx_pos;                    // the prefix is the key bits at positions >= pfx_pos
     int fast_bits;                  // most key bits below the prefix the first attempt sorts on (test hook; 32 = no limit)
@@ -258,7 +259,7 @@ struct EmitArgs {
     int exp_bytes;
     int wpr;                        // > 0: rows are written as this many 32-bit words (common.cuh, row_words)
     int64_t out_capacity;
-    const uint32_t* worklist;       // the tiles that own records (ctl->fin_count of them, at most max_list processed by finish_kernel)
+    const uint4* worklist;          // the tiles that own records (ctl->fin_count of them, at most max_list processed by finish_kernel)
     uint32_t max_list;
     const Control* ctl;
 };
@@ -299,10 +300,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     const uint32_t fin_count = a.ctl->fin_count;
     if (blockIdx.x == 0 && tid == 0 && fin_count > gridDim.x) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
     if (blockIdx.x >= fin_count) return;           // the grid is sized for the most tiles that can own records
-    const uint32_t tile = a.worklist[blockIdx.x];
-    const uint32_t lo = a.tile_start[tile], hi = a.tile_start[tile + 1];
-    uint32_t n_loc = 0;
-    if ((uint64_t)lo < ((uint64_t)tile + 1) * a.fin_tile && hi > lo) n_loc = min(hi - lo, (uint32_t)CAP);
+    const uint4 wl = a.worklist[blockIdx.x];       // one load instead of three dependent ones
+    const uint32_t tile = wl.x, lo = wl.y, hi = wl.z;
+    const uint32_t n_loc = hi > lo ? min(hi - lo, (uint32_t)CAP) : 0u;
     const K* __restrict__ gkeys = (const K*)a.keys + lo;
     const double* __restrict__ gcoef = a.coefs + lo;
     // sorted positions per thread in the blocked phases; odd, so that the threads' strided shared-memory accesses
@@ -625,9 +625,10 @@ __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitA
     const unsigned lane = lane_id();
     const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
     for (uint32_t q = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); q < nlist; q += nwarps) {
-        const uint32_t t = a.worklist[q];
+        const uint4 wl = a.worklist[q];
+        const uint32_t t = wl.x;
         const uint32_t off = a.tile_off[t], cnt = a.tile_off[t + 1] - off;
-        const uint64_t src = a.tile_start[t];
+        const uint64_t src = wl.y;
         for (uint32_t i = lane; i < cnt; i += 32u) {
             const uint64_t o = (uint64_t)off + i;
             if ((int64_t)o < a.out_capacity) emit_term<K>(a, plan, o, a.usums[src + i], ((const K*)a.ukeys)[src + i]);
@@ -640,7 +641,7 @@ __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitA
 template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
                            const double* coefs, double tol, void* ukeys, double* usums, double* out_coef, void* out_exps,
-                           int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist,
+                           int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint4* worklist,
                            uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
@@ -682,7 +683,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist, uint32_t* chunk_sum, Control* ctl,
+                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
                   int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;

@@ -111,12 +111,12 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
 
 // Bucket path (finish.cu): the pairs are sorted by their top `prefix_passes` plan digits; finish every bucket in
 // shared memory and emit the simplified polynomial (S2 rest + S3 + S4 + S5).  (ukeys, usums): scratch for n pairs.
-// tile_start, tile_state, worklist: ceil(n/fin_tile)+1 words each, tile_state zeroed; chunk_sum: ceil(tiles/4096) words.  after_tiles (optional): recorded
+// tile_start, tile_state: ceil(n/fin_tile)+1 words each, tile_state zeroed; worklist: as many uint4; chunk_sum: ceil(tiles/4096) words.  after_tiles (optional): recorded
 // between the finish kernel and the scan/emit kernels, for the stage timing.  Sets ctl->overflow (nothing emitted) when a bucket is too long,
 // ctl->unsorted when the prefix order or the local order check fails, ctl->distinct, ctl->survivors.
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, uint32_t* worklist, uint32_t* chunk_sum, Control* ctl,
+                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
                   int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream);
 
 }  // namespace polylab
