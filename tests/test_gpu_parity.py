@@ -472,3 +472,21 @@ def test_fused_expand_matches_materialised_products(shape):
     assert (e0 == e1).all() and (c0.view(np.uint64) == c1.view(np.uint64)).all()
     assert r0[2].kernel_launches == r1[2].kernel_launches
     assert_parity(oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol), c0, e0)
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_randomised_products_all_paths(seed):
+    """Random operand sizes, variable counts, dtypes and exponent ranges: the default product path (X1 fused into the
+    first pass), the materialising path, the forced bucket path and the ballot-ranking path all in parity with the oracle."""
+    r = np.random.default_rng(70_000 + seed)
+    dtype = [np.uint8, np.uint16, np.uint32][int(r.integers(0, 3))]
+    nvars = int(r.integers(1, 13))
+    hi = int(r.choice([2, 4, 16, 100]))
+    na, nb = int(r.choice([1, 7, 200, 1100])), int(r.choice([1, 5, 64, 1100]))
+    a = W.Poly(r.standard_normal(na), r.integers(0, hi, size=(na, nvars)).astype(dtype))
+    b = W.Poly(r.standard_normal(nb), r.integers(0, hi, size=(nb, nvars)).astype(dtype))
+    tol = [0.0, 1e-13][seed % 2]
+    res = oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol)
+    for flags in (0, B.FLAG_DEBUG_FORCE_BUCKET, B.FLAG_NO_FUSED_PACK, B.FLAG_SAFE_RANK):
+        c, e = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, flags=flags)
+        assert_parity(res, c.cpu().numpy(), e.cpu().numpy())
