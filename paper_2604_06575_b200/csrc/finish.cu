@@ -451,6 +451,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
             key_zero(kp);
             bool hp = false;
             if (first > 0 && first < n_loc) { kp = gkeys[py[first - 1]]; hp = true; }
+#pragma unroll 2
             for (uint32_t j = 0; j < itn; ++j) {
                 if (first + j < n_loc) {
                     const uint32_t r = py[first + j];
