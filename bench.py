@@ -403,6 +403,8 @@ def main():
             "config": {"workload": desc, "sort_terms_per_step": n_sort, "distinct": st.distinct, "survivors": int(n_out),
                        "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "prefix_passes": st.prefix_passes,
                        "bucket_fallback": st.bucket_fallback, "refinish_tiles": st.refinish_tiles, "digit_bits": st.digit_bits,
+                       "bounds": ("S0 on a 0.3 % sample of the rows, every row verified by S1's range check (DESIGN.md reading B4; "
+                                  "reading every row adds 0.47 ms on config 5)") if st.bounds_sampled else "S0 reads every row",
                        "parallelism": f"replicas x{world} (no collective on the path)",
                        "l2": "inputs and workspace are far larger than the 126 MB L2" if n_sort * (Wb + 8) > 4e8 else
                              "working set fits L2 (no flush between steps; launch-latency bound)"},
