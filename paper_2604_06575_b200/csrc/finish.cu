@@ -98,7 +98,9 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ 
         uint32_t base = 0;
         if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(&ctl->fin_count, (uint32_t)__popc(m));
         base = __shfl_sync(kFullMask, base, __ffs(m) - 1);
-        if (owns) worklist[base + __popc(m & lanemask_lt())] = make_uint4(t, lo, hi, 0u);     // tile, first record, end
+        // tile, first record, end, and whether its first and last record share their prefix (then, if the array is sorted
+        // by prefix, the tile holds a single bucket)
+        if (owns) worklist[base + __popc(m & lanemask_lt())] = make_uint4(t, lo, hi, same_prefix(keys[lo], keys[hi - 1], pfx_pos) ? 1u : 0u);
     }
 }
 
@@ -321,10 +323,36 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     bool full = (rbits == 0);                      // nothing below the prefix: only the ordinal is sorted on
     uint32_t hm = 0, nh = 0, keep = 0, nkeep = 0, nclosed = 0;
     double acc = 0.0, part0 = 0.0;
+    bool try_single = wl.w != 0u && !full;        // first and last record share the prefix: probably one bucket
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
         bool descending = false, later_head = false;
-        if (a.pfx_pos >= 8 * (int)sizeof(K) - 64) {
+        if (try_single) {
+            // one-bucket candidate: no neighbour is needed, every prefix must equal the first record's (four records per
+            // thread in flight); a record that differs sends the tile through the general stream below
+            const K k0 = gkeys[0];
+            for (uint32_t i0 = tid; i0 < n_loc; i0 += 4 * THREADS) {
+                K k[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * THREADS;
+                    k[u] = k0;
+                    if (i < n_loc) k[u] = gkeys[i];
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * THREADS;
+                    if (i < n_loc) {
+                        later_head |= !same_prefix(k[u], k0, a.pfx_pos);
+                        bx[i] = key_get_field(k[u], a.pfx_pos - rbits, rbits);
+                    }
+                }
+            }
+            if (__syncthreads_or(later_head ? 1 : 0)) {   // not a single bucket after all (or not sorted): general path
+                try_single = false;
+                continue;
+            }
+        } else if (a.pfx_pos >= 8 * (int)sizeof(K) - 64) {
             // the prefix lies in the key's most significant 64 bits: only those are fetched from the left neighbour, and
             // four records per thread are in flight (all loads issued before the first use)
             for (uint32_t i0 = tid; i0 < n_loc; i0 += 4 * THREADS) {
@@ -369,7 +397,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
             }
         }
         if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
-        const bool one_bucket = !__syncthreads_or(later_head ? 1 : 0) && !full;
+        const bool one_bucket = try_single || (!__syncthreads_or(later_head ? 1 : 0) && !full);
 
         // ---- bucket ordinal of every record (buckets are contiguous: the input is sorted by prefix); fast attempt:
         // composite sort word = ordinal above the top fb raw bits, ob + fb <= 27 so that 13 index bits fit beside what
@@ -484,6 +512,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
             break;
         }
         full = true;
+        try_single = false;
         if (tid == 0) atomicAdd(&a.ctl->refinish, 1u);
     }
 
