@@ -57,8 +57,12 @@ static inline void acc_init(acc_t* q, int64_t first)
 static inline void acc_add(acc_t* q, double x)
 {
     const double t = q->s + x;
-    if (fabs(q->s) >= fabs(x)) q->c += (q->s - t) + x;
-    else                       q->c += (x - t) + q->s;
+    /* reading A12: non-finite values propagate as in a plain sum -- once the running sum is +-inf or NaN
+     * the compensation (which would compute inf - inf) is left alone, so the value stays +-inf / NaN */
+    if (isfinite(t)) {
+        if (fabs(q->s) >= fabs(x)) q->c += (q->s - t) + x;
+        else                       q->c += (x - t) + q->s;
+    }
     q->s = t;
     q->a += fabs(x);
     q->n += 1;

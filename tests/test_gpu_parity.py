@@ -281,6 +281,17 @@ def test_tolerance_semantics_gpu():
     assert e[:, 0].tolist() == [1] and c.tolist() == [5e-324]
 
 
+def test_nonfinite_coefficients_gpu():
+    """Reading A12 on both sides: +-inf sums are kept, inf - inf and NaN sums are dropped."""
+    inf = float("inf")
+    coef = np.array([inf, 1.0, 2.0, -inf, 3.0, inf, -inf, 4.0, 1.5, float("nan"), 7.0])
+    exps = np.array([[0], [0], [1], [1], [1], [2], [2], [2], [3], [4], [4]], np.uint8)
+    c, e = gpu_simplify(coef, exps, 0.5)
+    assert e[:, 0].tolist() == [0, 1, 3] and c.tolist() == [inf, -inf, 1.5]
+    res = oracle.simplify(coef, exps, 0.5)
+    assert res.pruned[0].tolist() == c.tolist() and res.pruned[1][:, 0].tolist() == e[:, 0].tolist()
+
+
 def test_strides_column_major_and_dtypes():
     p, tol = W.config3(50_000)
     res = oracle.simplify(p.coef, p.exps, tol)

@@ -196,6 +196,20 @@ def test_tolerance_semantics(method):
 
 
 @pytest.mark.parametrize("method", METHODS)
+def test_nonfinite_coefficients_propagate(method):
+    """Reading A12: +-inf propagates through a monomial's sum like in a plain sum (kept: |inf| > tol);
+    inf + (-inf) = NaN and NaN fail the predicate and are dropped.  The values are those of IEEE addition."""
+    inf = float("inf")
+    coef = np.array([inf, 1.0, 2.0, -inf, 3.0, inf, -inf, 4.0, 1.5, float("nan"), 7.0])
+    exps = np.array([[0], [0], [1], [1], [1], [2], [2], [2], [3], [4], [4]], np.uint8)
+    res = oracle.simplify(coef, exps, 0.5, method=method)
+    assert res.rows[:, 0].tolist() == [0, 1, 2, 3, 4]
+    assert res.sum[0] == inf and res.sum[1] == -inf and math.isnan(res.sum[2]) and res.sum[3] == 1.5 and math.isnan(res.sum[4])
+    assert res.keep.tolist() == [True, True, False, True, False]
+    assert res.abs[0] == inf and res.count.tolist() == [2, 3, 3, 1, 2]
+
+
+@pytest.mark.parametrize("method", METHODS)
 def test_exponent_dtypes_and_empty(method):
     r = np.random.default_rng(2)
     rows = r.integers(0, 200, (300, 5))
