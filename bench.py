@@ -82,10 +82,11 @@ def max_over_ranks(dist, value: float, device) -> float:
     return float(t.item())
 
 
-def lsu_pipe(wavefronts_per_launch, launch_ms: float, sms: int = 148, sm_mhz: float = 1965.0):
+def lsu_pipe(wavefronts_per_launch, launch_ms: float, sms: int, sm_mhz: float):
     """The finish kernel's real limiter: LSU data-pipe wavefronts (ncu count of the committed capture, profiles/traffic.json)
-    per live launch time, against one wavefront per clock and SM (B300_MICROARCH.md; 148 SMs at the 1965 MHz maximum)."""
-    if not wavefronts_per_launch:
+    per live launch time, against one wavefront per clock and SM (B300_MICROARCH.md); `sms` from the device properties,
+    `sm_mhz` the SM clock sampled during the timed region."""
+    if not wavefronts_per_launch or not sms or not sm_mhz:
         return None
     peak = sms * sm_mhz * 1e6
     ach = wavefronts_per_launch / (launch_ms * 1e-3)
@@ -162,16 +163,146 @@ def time_oracle(kind, polys, tol):
     return time.perf_counter() - t0
 
 
-def oracle_sample(config: int, budget_s: float):
-    """A bounded sample of the workload for the CPU oracle: same recipe, fewer terms (about budget_s of CPU work)."""
-    if config in (1, 2, 4, 6):
-        return workload(config, None)                   # the oracle finishes these in seconds
-    probe_n = 1_000_000
-    kind, polys, tol, _, n = workload(config, probe_n)
-    rate = n / time_oracle(kind, polys, tol)
-    full = 10_000_000 if config in (3, 7) else 200_000_000
-    n_s = int(min(full, max(probe_n, rate * budget_s)) // 20 * 20)
-    return workload(config, n_s)
+ORACLE_SAMPLE_TERMS = {5: 10_000_000}     # config 5: a fixed 1e7-term sample of the same recipe (~5 s on one core)
+
+
+def oracle_sample(config: int):
+    """The workload the CPU oracle is timed on: the bench workload itself (same seeded arrays) for every config of at most
+    1e7 terms; for config 5 a fixed 1e7-term sample of the same recipe -- the same sample in both arms."""
+    return workload(config, ORACLE_SAMPLE_TERMS.get(config))
+
+
+def sample_note(config: int, desc: str) -> str:
+    return (f"{desc} (bounded sample of the bench workload, same recipe)" if config in ORACLE_SAMPLE_TERMS
+            else f"{desc} (the bench workload itself, same seeded arrays)")
+
+
+def rows_strictly_ascending(rows: np.ndarray) -> bool:
+    """Canonical order of the output (reading A1): every row lexicographically above its predecessor."""
+    rows = np.ascontiguousarray(rows)
+    if rows.shape[0] < 2:
+        return True
+    be = rows if rows.dtype == np.uint8 else np.ascontiguousarray(rows.astype(">u4"))
+    k = be.view(f"S{be.shape[1] * be.dtype.itemsize}").reshape(-1)      # byte strings compare like the rows
+    return bool((k[1:] > k[:-1]).all())
+
+
+def parity_of_timed_output(kind, polys, tol, out_c, out_e, slice_value=None):
+    """The output of the TIMED configuration against the CPU oracle (outside the timed region; SURVEY 8(c) parity rule).
+    slice_value None: every monomial.  Otherwise a KEY SLICE: the monomials whose first exponent equals slice_value -- the
+    oracle simplifies exactly the input terms of the slice (a numpy mask on the inputs: every contribution to these
+    monomials is in it), the output is filtered by the same mask, rules (1)-(4) apply in full; rule (4) (strictly
+    ascending) is checked over ALL output rows in either case."""
+    from oracle import oracle, parity
+    oc, oe = out_c.cpu().numpy(), out_e.cpu().numpy()
+    t0 = time.perf_counter()
+    if kind == "simplify":
+        p = polys[0]
+        if slice_value is None:
+            res = oracle.simplify(p.coef, p.exps, tol)
+        else:
+            m = p.exps[:, 0] == slice_value
+            res = oracle.simplify(p.coef[m], np.ascontiguousarray(p.exps[m]), tol)
+    elif kind == "mul":
+        res = oracle.mul_simplify(polys[0].coef, polys[0].exps, polys[1].coef, polys[1].exps, tol)
+    else:
+        p = polys[0]
+        c, e = oracle.expand(p.coef, p.exps, p.coef, p.exps)
+        res = oracle.mul_simplify(c, e, p.coef, p.exps.astype(e.dtype), tol)
+    oracle_s = time.perf_counter() - t0
+    if slice_value is not None:
+        mo = oe[:, 0] == slice_value
+        rep = parity.check(res, oc[mo], oe[mo])
+    else:
+        rep = parity.check(res, oc, oe)
+    asc = rows_strictly_ascending(oe)
+    return {"ok": bool(rep.ok and asc), "matched": rep.matched, "exempt": rep.exempt, "max_rel_dev": rep.max_rel_dev,
+            "oracle_distinct": rep.n_oracle_distinct, "oracle_survivors": rep.n_expected, "candidate_terms": rep.n_candidate,
+            "all_rows_strictly_ascending": asc, "output_terms": int(oc.shape[0]),
+            "slice": (f"monomials with exponent[0] == {slice_value}: {rep.n_oracle_distinct} of the input's monomials, every "
+                      "contribution included" if slice_value is not None else "every monomial"),
+            "errors": rep.errors[:3]}, oracle_s
+
+
+def algorithmic_bytes(kind, n_in_rows, E, N, W, P, U, U1):
+    """what the pack -> LSD sort -> segmented sum -> prune -> unpack method must move for this input."""
+    S = W + 8
+    b = 0.0
+    if kind == "simplify":
+        b += n_in_rows * E + N * (E + W)          # S0 + S1
+    b += N * W                                    # one histogram read of the keys (0 when fused)
+    b += P * 2.0 * N * S + N * S + U * S + U * S + U1 * (8 + E)
+    return b
+
+
+def measure_other_config(B, torch, cfg, variant, steps, warmup, peak, ws):
+    """One of the non-headline configs: device-resident timing through the C ABI, parity of that output, the oracle on the
+    same arrays."""
+    kind, polys, tol, desc, n_sort = workload(cfg, None)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    d = [(dev(p.coef), dev(p.exps)) for p in polys]
+    last = {}
+
+    def step():
+        if kind == "simplify":
+            c, e, st = B.simplify(*d[0], tol, workspace=ws, return_stats=True, timing=True)
+        elif kind == "mul":
+            c, e, st = B.mul_simplify(*d[0], *d[1], tol, workspace=ws, return_stats=True, timing=True)
+        elif variant == "A":                      # config 4, two chained mul+simplify passes (reading A16)
+            qc, qe, st0 = B.mul_simplify(*d[0], *d[0], tol, workspace=ws, return_stats=True, timing=True)
+            c, e, st = B.mul_simplify(qc, qe, *d[0], tol, workspace=ws, return_stats=True, timing=True)
+            last["n_sort"] = st0.sort_terms + st.sort_terms
+            last["launches"] = st0.kernel_launches + st.kernel_launches
+        else:                                     # raw p*p, then (p*p)*p merged in one sort
+            rc, re_ = B.expand(*d[0], *d[0])
+            c, e, st = B.mul_simplify(rc, re_, *d[0], tol, workspace=ws, return_stats=True, timing=True)
+            last["n_sort"] = rc.shape[0] + st.sort_terms
+            last["launches"] = 1 + st.kernel_launches
+        last["out"], last["st"] = (c, e), st
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    st = last["st"]
+    n_sort = last.get("n_sort", st.sort_terms)
+    c, e = last["out"]
+    if variant == "A":
+        from oracle import oracle, parity
+        p = polys[0]
+        t0 = time.perf_counter()
+        q = oracle.mul_simplify(p.coef, p.exps, p.coef, p.exps, tol)
+        qc, qe = q.pruned
+        res = oracle.mul_simplify(qc, qe, p.coef, p.exps.astype(qe.dtype), tol)
+        osec = time.perf_counter() - t0
+        rep = parity.check(res, c.cpu().numpy(), e.cpu().numpy())
+        par = {"ok": bool(rep.ok), "matched": rep.matched, "exempt": rep.exempt, "max_rel_dev": rep.max_rel_dev,
+               "slice": "every monomial", "errors": rep.errors[:3]}
+    else:
+        par, osec = parity_of_timed_output(kind, polys, tol, c, e)
+    E = polys[0].exps.shape[1] * polys[0].exps.dtype.itemsize
+    W, P, U, U1 = st.key_bytes, len(st.digit_bits), max(st.distinct, 0), int(c.shape[0])
+    ab = algorithmic_bytes(kind, polys[0].nterms, E, st.sort_terms, W, P, U, U1)
+    gbs = ab / (ms * 1e-3) / 1e9
+    return {"config": ({1: "1", 2: "2", 3: "3", 4: "4" + (variant or "B"), 6: "paper p_4^3", 7: "3u"}[cfg]), "workload": desc,
+            "ms_per_step": ms, "terms_per_s": n_sort / (ms * 1e-3), "sort_terms_per_step": int(n_sort),
+            "distinct": int(U), "survivors": U1, "key_bits": st.key_bits, "lsd_passes_of_the_plan": P,
+            "algorithmic_GB_lsd_method": ab / 1e9, "GBps_equivalent": gbs, "frac_of_measured_peak": gbs / peak,
+            "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS, "stage_ms_last_call": st.stage_ms, "path": path_name(st),
+            "rank_fallback": st.rank_fallback, "bucket_fallback": st.bucket_fallback, "bounds_retry": st.bounds_retry,
+            "kernel_launches_per_step": last.get("launches", st.kernel_launches),
+            "oracle_seconds_same_arrays_1core": osec, "oracle_terms_per_s": n_sort / osec if osec else None, "parity": par}
+
+
+def path_name(st) -> str:
+    if getattr(st, "table_path", 0):
+        return "table"
+    return "bucket" if st.prefix_passes > 0 else "lsd"
 
 
 def run_reference(args):
@@ -181,14 +312,13 @@ def run_reference(args):
         return
     from oracle import oracle
     oracle.build()
-    total = max(args.steps + args.warmup, 1)
-    kind, polys, tol, desc, n = oracle_sample(args.config, budget_s=min(8.0, 60.0 / total))
+    kind, polys, tol, desc, n = oracle_sample(args.config)
     for _ in range(args.warmup):
         time_oracle(kind, polys, tol)
     t = [time_oracle(kind, polys, tol) for _ in range(args.steps)]
     sec = sum(t) / len(t)
     v = n / sec
-    sample = f"{desc} (bounded sample of the bench workload, same recipe)"
+    sample = sample_note(args.config, desc)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -210,6 +340,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bucket", action="store_true", help="POLYLAB_FLAG_NO_BUCKET: force the plain LSD path (A/B)")
+    ap.add_argument("--no-parity", action="store_true", help="skip the oracle check of the timed output")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the other_configs table (configs 1-4, 3u, p_4^3)")
+    ap.add_argument("--flags", type=int, default=0, help="extra POLYLAB_FLAG_* bits for the timed calls (A/B runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -236,21 +369,25 @@ def main():
     ws = B.Workspace(torch.device("cuda", local_rank))
     stats_log = []
 
-    xflags = B.FLAG_NO_BUCKET if args.no_bucket else 0
+    xflags = (B.FLAG_NO_BUCKET if args.no_bucket else 0) | args.flags
+    last_out = {}
 
     def step_device():
         if kind == "simplify":
             c, e, st = B.simplify(*dpolys[0], tol, workspace=ws, out=outbuf, return_stats=True, timing=True, flags=xflags)
             stats_log.append(st)
+            last_out["ce"] = (c, e)
             return c.shape[0]
         if kind == "mul":
             c, e, st = B.mul_simplify(*dpolys[0], *dpolys[1], tol, workspace=ws, return_stats=True, timing=True, flags=xflags)
             stats_log.append(st)
+            last_out["ce"] = (c, e)
             return c.shape[0]
         pc, pe = dpolys[0]
         rc, re_ = B.expand(pc, pe, pc, pe)
         c, e, st = B.mul_simplify(rc, re_, pc, pe, tol, workspace=ws, return_stats=True, timing=True, flags=xflags)
         stats_log.append(st)
+        last_out["ce"] = (c, e)
         return c.shape[0]
 
     outbuf = None
@@ -279,6 +416,7 @@ def main():
         n_out = step_device()
     ev1.record()
     barrier()
+    timed_out = tuple(t.clone() for t in last_out["ce"])    # the output of the last TIMED step, for the parity check below
     in_region = len(sampler.rows) - rows_before
     # a step takes ~10 ms and nvidia-smi samples every 100 ms: keep the same load running (untimed, results discarded) until
     # the clock line has at least five samples, so that "median under load" means something
@@ -336,7 +474,8 @@ def main():
                     "algorithmic_bytes_per_launch": fin_bytes, "launch_ms": fin_ms, "launches_per_step": 1,
                     "share_of_step": fin_ms / ms_per_step,
                     "limiter": "shared-memory / LSU pipe, not DRAM (ncu, profiles/): the kernel trades HBM passes for on-chip work",
-                    "lsu_pipe": lsu_pipe(tinfo.get("finish_lsu_wavefronts_per_launch"), fin_ms),
+                    "lsu_pipe": lsu_pipe(tinfo.get("finish_lsu_wavefronts_per_launch"), fin_ms,
+                                         torch.cuda.get_device_properties(local_rank).multi_processor_count, clocks.get("sm_mhz")),
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
         # the dominant kernel is the one with the larger share of the step: the radix pass (all its launches) or the finish
         if fin_ms > stage_ms["sort"]:
@@ -353,7 +492,7 @@ def main():
                                     "note": "above 1.0 means the call beats the roofline of the LSD method by moving fewer bytes "
                                             "(bucket path: %d passes over HBM instead of %d)" % (P, lsd_digits)}
     roofline["stage_ms"] = stage_ms
-    roofline["path"] = "bucket" if st.prefix_passes > 0 else "lsd"
+    roofline["path"] = path_name(st)
 
     # ---- end to end: host buffers, copies inside the C call
     e2e = None
@@ -385,14 +524,36 @@ def main():
                "d2h_bytes_per_step": int(d2h) + 8, "steps": k2, "ms_per_step": ms2 / k2}
         del hp
 
+    # ---- parity of the timed output against the oracle (outside the timed region): every monomial for the configs of at most
+    # 1e7 terms, an oracle key slice (1/256 of the monomials, all their contributions) for config 5
+    par = None
+    if rank == 0 and not args.no_parity:
+        sl = 37 if (kind == "simplify" and n_sort > 20_000_000) else None
+        par, _ = parity_of_timed_output(kind, polys, tol, timed_out[0], timed_out[1], sl)
+        par["distinct_reported"] = int(st.distinct)
+        if args.config == 5 and args.nterms is None:     # the generator fixes these by construction (reading A18)
+            par["recipe_counts_ok"] = bool(st.distinct == n_sort // 10 and int(timed_out[0].shape[0]) == n_sort // 20)
+            par["ok"] = bool(par["ok"] and par["recipe_counts_ok"])
+    del timed_out
+
+    # ---- the other configs (rank 0, N=1): a few milliseconds each on the GPU, seconds each for the oracle
+    others = None
+    if rank == 0 and world == 1 and not args.no_other_configs and args.config == 5 and args.nterms is None:
+        dpolys.clear()                               # release the 2e8-term inputs and output buffers first
+        outbuf = polys = None
+        torch.cuda.empty_cache()
+        others = []
+        for cfg, variant in ((1, None), (2, None), (3, None), (4, "A"), (4, "B"), (7, None), (6, None)):
+            others.append(measure_other_config(B, torch, cfg, variant, 10, 3, peak, ws))
+
     # ---- CPU oracle on a bounded sample (rank 0, N=1)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        k_s, p_s, tol_s, desc_s, n_s = oracle_sample(args.config, budget_s=8.0)   # the probe overestimates the rate
+        k_s, p_s, tol_s, desc_s, n_s = oracle_sample(args.config)
         sec = time_oracle(k_s, p_s, tol_s)
         cpu = {"value": n_s / sec, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": sec,
-               "sample": f"{desc_s} (bounded sample, same recipe as the bench workload)",
-               "host_cpus": os.cpu_count()}
+               "sample": sample_note(args.config, desc_s), "host_cpus": os.cpu_count()}
+        del p_s
 
     if rank == 0:
         launches = sum(s.kernel_launches for s in stats_log) + (steps if kind == "cubic" else 0)
@@ -402,13 +563,15 @@ def main():
             "data": "synthetic",
             "config": {"workload": desc, "sort_terms_per_step": n_sort, "distinct": st.distinct, "survivors": int(n_out),
                        "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "prefix_passes": st.prefix_passes,
-                       "bucket_fallback": st.bucket_fallback, "refinish_tiles": st.refinish_tiles, "digit_bits": st.digit_bits,
+                       "bucket_fallback": st.bucket_fallback, "rank_fallback": st.rank_fallback, "bounds_retry": st.bounds_retry,
+                       "refinish_tiles": st.refinish_tiles, "digit_bits": st.digit_bits, "path": path_name(st),
                        "bounds": ("S0 on a 0.3 % sample of the rows, every row verified by S1's range check (DESIGN.md reading B4; "
                                   "reading every row adds 0.47 ms on config 5)") if st.bounds_sampled else "S0 reads every row",
                        "parallelism": f"replicas x{world} (no collective on the path)",
                        "l2": "inputs and workspace are far larger than the 126 MB L2" if n_sort * (Wb + 8) > 4e8 else
                              "working set fits L2 (no flush between steps; launch-latency bound)"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "parity": par, "other_configs": others,
         }))
     if dist is not None:
         dist.destroy_process_group()

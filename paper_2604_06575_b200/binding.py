@@ -238,9 +238,10 @@ def simplify(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_ex
     wsb = simplify_workspace_bytes(n, nvars)
     ws = _ws(coef.device, workspace).get(max(wsb, 256))
     count = ctypes.c_int64(0)
-    rc = lib().polylab_simplify(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
-                                out_coef.data_ptr(), out_exps.data_ptr(), cap, ctypes.addressof(count),
-                                ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_simplify(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
+                                    out_coef.data_ptr(), out_exps.data_ptr(), cap, ctypes.addressof(count),
+                                    ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])
@@ -257,9 +258,10 @@ def simplify_async(coef: torch.Tensor, exps: torch.Tensor, tol: float, max_exp: 
     o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=FLAG_DEVICE_COUNT, strides=strides, status_device=status, keep=keep)
     wsb = simplify_workspace_bytes(n, nvars)
     ws = _ws(coef.device, workspace).get(max(wsb, 256))
-    rc = lib().polylab_simplify(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
-                                out_coef.data_ptr(), out_exps.data_ptr(), int(out_coef.shape[0]), out_count.data_ptr(),
-                                ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_simplify(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
+                                    out_coef.data_ptr(), out_exps.data_ptr(), int(out_coef.shape[0]), out_count.data_ptr(),
+                                    ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     return _stats(st)
 
@@ -289,9 +291,10 @@ def mul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tenso
     pa = _Poly(a_coef.data_ptr(), a_exps.data_ptr(), na, nvars)
     pb = _Poly(b_coef.data_ptr(), b_exps.data_ptr(), nb, nvars)
     count = ctypes.c_int64(0)
-    rc = lib().polylab_mul_simplify(ctypes.byref(pa), ctypes.byref(pb), float(tol), ctypes.byref(o), out_coef.data_ptr(),
-                                    out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(),
-                                    _stream_ptr(stream))
+    with torch.cuda.device(a_coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_mul_simplify(ctypes.byref(pa), ctypes.byref(pb), float(tol), ctypes.byref(o), out_coef.data_ptr(),
+                                        out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(),
+                                        _stream_ptr(stream))
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])
@@ -317,8 +320,9 @@ def pow_simplify(coef: torch.Tensor, exps: torch.Tensor, power: int, tol: float 
     ws = _ws(coef.device, workspace).get(max(wsb, 256))
     pp = _Poly(coef.data_ptr(), exps.data_ptr(), n, nvars)
     count = ctypes.c_int64(0)
-    rc = lib().polylab_pow_simplify(ctypes.byref(pp), int(power), float(tol), ctypes.byref(o), out_coef.data_ptr(),
-                                    out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_pow_simplify(ctypes.byref(pp), int(power), float(tol), ctypes.byref(o), out_coef.data_ptr(),
+                                        out_exps.data_ptr(), cap, ctypes.addressof(count), ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])
@@ -338,8 +342,9 @@ def expand(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tensor, b_e
     ws = torch.empty(SMALL_WORKSPACE_BYTES, dtype=torch.uint8, device=a_coef.device)
     pa = _Poly(a_coef.data_ptr(), a_exps.data_ptr(), na, nvars)
     pb = _Poly(b_coef.data_ptr(), b_exps.data_ptr(), nb, nvars)
-    rc = lib().polylab_expand(ctypes.byref(pa), ctypes.byref(pb), ctypes.byref(o), out_coef.data_ptr(), out_exps.data_ptr(),
-                              ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    with torch.cuda.device(a_coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_expand(ctypes.byref(pa), ctypes.byref(pb), ctypes.byref(o), out_coef.data_ptr(), out_exps.data_ptr(),
+                                  ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     return out_coef[:n], out_exps[:n]
 
@@ -355,8 +360,9 @@ def pack_keys(exps: torch.Tensor, max_exp: Optional[Sequence[int]] = None, strea
     out = torch.zeros((max(n, 1), 2), dtype=torch.int64, device=exps.device)
     ws = torch.empty(SMALL_WORKSPACE_BYTES, dtype=torch.uint8, device=exps.device)
     bits = ctypes.c_int32(0)
-    rc = lib().polylab_pack_keys(exps.data_ptr(), n, nvars, ctypes.byref(o), out.data_ptr(), ctypes.byref(bits),
-                                 ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    with torch.cuda.device(exps.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_pack_keys(exps.data_ptr(), n, nvars, ctypes.byref(o), out.data_ptr(), ctypes.byref(bits),
+                                     ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc)
     return out[:n], bits.value
 

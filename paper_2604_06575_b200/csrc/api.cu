@@ -552,8 +552,12 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     uint64_t m[kMaxVars];
     uint32_t ba[kMaxVars], bb[kMaxVars];
     const uint32_t emax = exp_max_of(o.exp_bytes);
+    bool check_sums = false;                  // caller bounds that allow a sum above exp_type's range: checked on the device
     if (o.max_exp_host) {
-        for (int v = 0; v < nvars; ++v) { ba[v] = bb[v] = o.max_exp_host[v]; m[v] = 2ull * o.max_exp_host[v]; }
+        for (int v = 0; v < nvars; ++v) {
+            ba[v] = bb[v] = o.max_exp_host[v]; m[v] = 2ull * o.max_exp_host[v];
+            check_sums |= m[v] > emax;
+        }
     } else {
         PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
         launches += launch_bounds(eva, na, nvars, ctl, 0, stream);
@@ -577,6 +581,7 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     const Layout L = make_layout(n, plan_a.key_bytes, na, nb);
     if (avail < L.total) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
+    if (check_sums) launches += launch_sum_range_check(eva, na, evb, nb, nvars, emax, ctl, stream);
 
     // ---- S1 on the operands, X1 on packed keys (+ histogram of the first digit), then the shared tail
     int k = choose_prefix_passes(plan_a, n, o, at);

@@ -82,6 +82,9 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const K* __restrict__ 
         if (t < ntiles) {
             hi = tile_first_change(keys, n, pfx_pos, fin_tile, t + 1, &overflow);
             owns = (uint64_t)lo < ((uint64_t)t + 1) * fin_tile && hi > lo;        // a bucket starts inside the tile
+            // in a prefix-sorted array a tile without a bucket start has lo == hi (both searches find the same change);
+            // anything else would leave the records of [lo, hi) to nobody
+            if (hi != lo && !owns && !overflow) ctl->unsorted = 1u;
         }
         // a tile starts a new bucket: its first prefix must be above the record before it (finish_kernel checks the
         // order inside a tile; together they prove that every bucket is contiguous, i.e. that the prefix passes were stable)
@@ -681,11 +684,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
                                                                        ntiles, tile_start, worklist, ctl);
     auto kern = finish_kernel<K>;
     constexpr size_t smem = FinishSmem::bytes;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
-    }
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device: set on every launch
     FinishArgs a;
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state; a.worklist = worklist;
@@ -705,7 +704,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     e.out_capacity = out_capacity;
     e.worklist = worklist; e.max_list = fin_blocks; e.ctl = ctl;
     int64_t blocks = ((int64_t)fin_blocks + 7) / 8;          // one warp per work-list tile, grid-stride
-    if (blocks > 148 * 64) blocks = 148 * 64;
+    if (blocks > sm_count() * 64) blocks = sm_count() * 64;
     if (blocks < 1) blocks = 1;
     emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
     return 5;

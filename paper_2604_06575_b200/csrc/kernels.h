@@ -27,6 +27,20 @@ constexpr int kFinBins = 1 << kFinDigit;
 constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
 constexpr int kFinMinTile = 512;    // smallest fin_tile the planner picks (workspace sizing)
 
+// Number of SMs of the current device (grid sizing); queried once per device, 148 on a B200.
+inline int sm_count()
+{
+    static int cached[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
+    if (cached[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached[dev] = n;
+    }
+    return cached[dev];
+}
+
 inline int sort_tile(int key_bytes) { return key_bytes == 8 ? kSortThreads64 * kSortItems64 : kSortThreads128 * kSortItems128; }
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
 constexpr int kPruneTile = kPruneThreads * kPruneItems;
@@ -37,6 +51,11 @@ int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, in
 // S0 on a sample: 1184 evenly spaced segments of 512 rows.  The caller sizes the fields from the sampled maxima's bit
 // lengths and relies on S1's range check to catch an exponent the sample missed (then S0 runs in full).
 int launch_bounds_sample(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream);
+
+// Product with caller bounds: true maxima of both operands into ctl->max_exp (which must be zero), then
+// max_a[v] + max_b[v] > emax -> ctl->status = POLYLAB_ERR_EXPONENT_RANGE (the exponent sums must fit exp_type, reading A8).
+int launch_sum_range_check(const ExpView& ea, int64_t na, const ExpView& eb, int64_t nb, int nvars, uint32_t emax, Control* ctl,
+                           cudaStream_t stream);
 
 // S1: pack rows into keys (key_bytes from the plan), check e <= plan.bound (-> ctl->status), and, when
 // hist_digit >= 0, accumulate the histogram of that plan digit into ctl->hist[hist_digit] (the first pass's digit).

@@ -113,7 +113,8 @@ __global__ void __launch_bounds__(THREADS) bounds_sample_kernel(ExpView ev, int6
 int launch_bounds_sample(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, int which, cudaStream_t stream)
 {
     if (nterms <= 0) return 0;
-    constexpr int kSegs = 148 * 8, kSegRows = 512;
+    const int kSegs = sm_count() * 8;
+    constexpr int kSegRows = 512;
     bounds_sample_kernel<256><<<kSegs, 256, 0, stream>>>(ev, nterms, nvars, nterms / kSegs, kSegRows, ctl->max_exp[which]);
     return 1;
 }
@@ -127,7 +128,7 @@ int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, in
         const int rb = nvars * ev.exp_bytes;
         const int64_t nbytes = nterms * rb;
         int64_t k = (nbytes / 16 + (int64_t)T * 8 - 1) / ((int64_t)T * 8) / rb;      // ~8 words per thread
-        const int64_t kmax = (148 * 16 + rb - 1) / rb;
+        const int64_t kmax = (sm_count() * 16 + rb - 1) / rb;
         if (k > kmax) k = kmax;
         if (k < 1) k = 1;
         const unsigned blocks = (unsigned)(k * rb);
@@ -139,9 +140,25 @@ int launch_bounds(const ExpView& ev, int64_t nterms, int nvars, Control* ctl, in
     }
     const int rows_per_iter = T / nvars;
     int64_t blocks = (nterms + (int64_t)rows_per_iter * 16 - 1) / ((int64_t)rows_per_iter * 16);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     bounds_kernel<T><<<(unsigned)blocks, T, 0, stream>>>(ev, nterms, nvars, ctl->max_exp[which]);
     return 1;
+}
+
+// A product's exponent sums must fit exp_type (reading A8).  With bounds from the data the host checks max_a + max_b; with
+// caller bounds (no read-back) the operands' true maxima are taken on the device and compared here.
+__global__ void sum_range_check_kernel(Control* ctl, int nvars, uint32_t emax)
+{
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v < nvars && (uint64_t)ctl->max_exp[0][v] + ctl->max_exp[1][v] > emax) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+}
+
+int launch_sum_range_check(const ExpView& ea, int64_t na, const ExpView& eb, int64_t nb, int nvars, uint32_t emax, Control* ctl,
+                           cudaStream_t stream)
+{
+    int launches = launch_bounds(ea, na, nvars, ctl, 0, stream) + launch_bounds(eb, nb, nvars, ctl, 1, stream);
+    sum_range_check_kernel<<<1, kMaxVars, 0, stream>>>(ctl, nvars, emax);
+    return launches + 1;
 }
 
 // ----------------------------------------------------------------------------------------------- S1
@@ -248,7 +265,7 @@ static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K*
 {
     if (nterms <= 0) return 0;
     int64_t blocks = (nterms + 256 * 4 - 1) / (256 * 4);       // >= 4 rows per thread once the grid saturates
-    if (blocks > 148 * 32) blocks = 148 * 32;
+    if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     if (blocks < 1) blocks = 1;
     if (ev.row_major_contiguous) {
         const int rb = plan.nvars * ev.exp_bytes;
@@ -295,7 +312,7 @@ int launch_key_hist(const Plan& plan, int hd, int64_t n, const void* keys, Contr
 {
     if (n <= 0 || hd < 0 || hd >= plan.npasses) return 0;
     int64_t blocks = (n + 256 * 8 - 1) / (256 * 8);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     const int dpos = plan.digit_pos[hd];
     const uint32_t dmask = (1u << plan.digit_bits[hd]) - 1u;
     if (plan.key_bytes == 8) key_hist_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)keys, n, dpos, dmask, ctl->hist[hd]);
@@ -388,7 +405,7 @@ int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hd,
     }
     const int rb = plan.nvars * ev.exp_bytes;
     int64_t blocks = (nterms + 256 * 8 - 1) / (256 * 8);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     const uint8_t* base = (const uint8_t*)ev.base;
     uint32_t* hist = ctl->hist[hd];
 #define POLYLAB_RH(RB, ES) row_hist_kernel<RB, ES><<<(unsigned)blocks, 256, 0, stream>>>(base, nterms, dp, hist)
@@ -470,7 +487,7 @@ int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hd, Control* c
     const int64_t n = xs.na * xs.nb;
     if (n <= 0 || hd < 0 || hd >= plan.npasses) return 0;
     int64_t blocks = (n + 256 * 8 - 1) / (256 * 8);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     const int dpos = plan.digit_pos[hd];
     const uint32_t dmask = (1u << plan.digit_bits[hd]) - 1u;
     if (plan.key_bytes == 8)
@@ -511,7 +528,7 @@ int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const Exp
     const int64_t n = na * nb;
     if (n <= 0) return 0;
     int64_t blocks = (n + 255) / 256;
-    if (blocks > 148 * 32) blocks = 148 * 32;
+    if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     expand_raw_kernel<<<(unsigned)blocks, 256, 0, stream>>>(ea, ca, (uint32_t)na, eb, cb, (uint32_t)nb, nvars, out_coef,
                                                             out_exps, &ctl_status->status);
     return 1;

@@ -162,22 +162,40 @@ reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint
     }
 }
 
-// Adds the leading fragments of later tiles to segments that cross tile boundaries, left to right.
+// Adds the leading fragments of later tiles to segments that cross tile boundaries.  One warp per tile that is the FIRST
+// continuation of a segment: the fragments of the following tiles are taken 32 at a time, summed by a fixed butterfly
+// (every lane ends with the same value) and added chunk by chunk -- a fixed function of the layout, and the error of a run
+// of n equal keys grows as (n / (32 * tile) + 5 + ...) * 2^-53 * A_m instead of n / tile (a run of 2^30 records stays far
+// inside the 1e-12 * A_m bound).
 __global__ void __launch_bounds__(256) reduce_fixup_kernel(uint32_t ntiles, double* __restrict__ usums, ReduceScratch sc)
 {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned lane = lane_id();
     if (t == 0 || t >= ntiles) return;
-    if (!sc.tile_cont[t] || sc.tile_heads[t - 1] == 0) return;      // not the first continuation of a segment
+    if (!sc.tile_cont[t] || sc.tile_heads[t - 1] == 0) return;      // not the first continuation of a segment (warp-uniform)
     const uint32_t slot = sc.tile_hb[t] - 1;
     double s = usums[slot];
-    uint32_t u = t;
+    uint32_t u0 = t;
     while (true) {
-        s = __dadd_rn(s, sc.tile_frag[u]);
-        if (sc.tile_heads[u] > 0) break;
-        ++u;
-        if (u >= ntiles || !sc.tile_cont[u]) break;
+        // lane l looks at tile u0 + l: it belongs to the chain iff every tile in (u0, u0 + l] continues the segment and no
+        // tile in [u0, u0 + l) holds a head (a tile with a head ends the chain, its own fragment included)
+        const uint32_t u = u0 + lane;
+        const bool in = u < ntiles;
+        const bool cont = in && (u == t || sc.tile_cont[u]);
+        const bool head = in && sc.tile_heads[u] > 0;
+        const unsigned stop_before = __ballot_sync(kFullMask, !cont);       // first lane that is not part of the chain
+        const unsigned stop_after = __ballot_sync(kFullMask, head);         // first lane that ends it
+        int last = 31;                                                       // last lane whose fragment is added
+        if (stop_before) last = min(last, __ffs(stop_before) - 2);
+        if (stop_after) last = min(last, __ffs(stop_after) - 1);
+        double f = ((int)lane <= last) ? sc.tile_frag[u] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) f = __dadd_rn(f, __shfl_xor_sync(kFullMask, f, o));
+        if (last >= 0) s = __dadd_rn(s, f);
+        if (last < 31) break;
+        u0 += 32u;
     }
-    usums[slot] = s;
+    if (lane == 0) usums[slot] = s;
 }
 
 template <typename K>
@@ -187,15 +205,11 @@ static int launch_reduce_t(int64_t n, const void* keys, const double* coefs, voi
     constexpr int TILE = kReduceTile;
     const size_t smem = (size_t)TILE * (sizeof(K) + sizeof(double));
     auto kern = reduce_kernel<K, kReduceThreads, kReduceItems>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
-    }
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device: set on every launch
     const unsigned tiles = (unsigned)((n + TILE - 1) / TILE);
     kern<<<tiles, kReduceThreads, smem, stream>>>((const K*)keys, coefs, (uint32_t)n, (K*)ukeys, usums, sc, ctl);
     if (tiles > 1) {
-        reduce_fixup_kernel<<<(tiles + 255) / 256, 256, 0, stream>>>(tiles, usums, sc);
+        reduce_fixup_kernel<<<(unsigned)(((uint64_t)tiles * 32 + 255) / 256), 256, 0, stream>>>(tiles, usums, sc);
         return 2;
     }
     return 1;
@@ -296,7 +310,7 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
 {
     if (max_units <= 0) return 0;
     int64_t blocks = (max_units + kPruneTile - 1) / kPruneTile;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     if (plan.key_bytes == 8)
         prune_unpack_kernel<uint64_t, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const uint64_t*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),

@@ -331,11 +331,7 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 {
     using S = SortSmem<K, THREADS, ITEMS>;
     auto kern = sort_pass_kernel<K, THREADS, ITEMS, MINB, NEXT, RANK_ATOMIC>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
-        attr_set = true;
-    }
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());   // per device: set on every launch
     kern<<<tiles, THREADS, S::bytes(), stream>>>(a);
 }
 

@@ -1,0 +1,137 @@
+"""-m gpu: the CUDA path against the CPU oracle at the sizes BASELINE.json STATES (north_star: parity "on all five
+configs"), in the launch configuration bench.py times: config 3 at its full 1e7 terms; the config 5 recipe at sizes
+that take the sampled S0, the fused byte-reversal pack and two prefix passes exactly as the 2e8-term bench run does; a
+narrow-first-variable variant whose finish tiles hold ONE bucket of ~3000 records (the geometry of the 2e8-term run,
+reached here at 2.4e7 terms).  The full 2e8-term config 5 output is checked by bench.py itself on an oracle key slice
+(its input alone takes a minute to draw), see `parity` in bench.py's JSON line.  Also the robustness cases the
+advisor asked for: products with caller bounds whose sums overflow exp_type, one run of 1e7 equal keys."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2604_06575_b200 import binding as B
+from paper_2604_06575_b200 import workloads as W
+from gpu_util import assert_parity, dev
+
+pytestmark = pytest.mark.gpu
+
+
+def run(p, tol, flags=0, **kw):
+    c, e, st = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=flags, **kw)
+    torch.cuda.synchronize()
+    return c.cpu().numpy(), e.cpu().numpy(), st
+
+
+def test_config3_at_its_stated_size():
+    """BASELINE.json config 3, all 1e7 terms: 7,680 monomials (reading A15), every one checked."""
+    p, tol = W.config3(10_000_000)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    rep = assert_parity(res, c, e)
+    assert len(res.sum) == 7680 and rep.matched == len(c) == int(res.keep.sum())
+    assert st.sort_terms == 10_000_000 and st.rank_fallback == 0
+
+
+def test_config3u_at_its_stated_size():
+    """Config 3's intent (A15): 1e7 mostly unique terms, 110-bit keys."""
+    p, tol = W.config3u(10_000_000)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    assert_parity(res, c, e)
+    assert st.key_bytes == 16 and st.rank_fallback == 0
+
+
+@pytest.mark.parametrize("n", [(1 << 22) + 16, 20_000_020])
+def test_config5_recipe_in_the_bench_configuration(n):
+    """Default flags, >= 2^22 terms plus a ragged tail: sampled S0 + byte-reversal fused pack + 2 prefix passes + finish,
+    the combination bench.py times at 2e8 terms -- full parity, every monomial."""
+    p, tol = W.config5(n)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    assert st.bounds_sampled == 1 and st.bounds_retry == 0
+    assert st.prefix_passes == 2 and st.sort_passes == 2 and st.key_bytes == 16 and st.key_bits == 128
+    assert st.bucket_fallback == 0 and st.rank_fallback == 0
+    assert st.distinct == n // 10 and st.survivors == n // 20 == len(c)
+    rep = assert_parity(res, c, e)
+    assert rep.matched == n // 20
+
+
+def test_one_bucket_per_finish_tile_geometry():
+    """The 2e8-term run finishes ONE bucket of ~3052 records per tile (tiles of 512 positions).  The same geometry at
+    2.4e7 terms: variable 0 is 3 bits wide, so two prefix passes give T = 13 prefix bits and buckets of ~2930."""
+    n = 24_000_000
+    r = np.random.default_rng(77)
+    pool = r.integers(0, 256, size=(n // 10, 16), dtype=np.uint8)
+    pool[:, 0] &= 7
+    base = r.standard_normal((n // 10, 10))
+    base[: n // 20, 5:] = -base[: n // 20, :5]              # config 5's cancelling half (A18)
+    perm = r.permutation(n)
+    p = W.Poly(base.reshape(-1)[perm], np.ascontiguousarray(pool[perm // 10]))
+    tol = 1e-14
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    assert st.key_bits == 123 and st.prefix_passes == 2 and st.bucket_fallback == 0 and st.rank_fallback == 0
+    assert st.bounds_sampled == 1
+    rep = assert_parity(res, c, e)
+    assert rep.matched == len(c) == int(res.keep.sum())
+
+
+def test_mul_with_caller_bounds_fits_and_overflows():
+    """polylab_mul_simplify with opts->max_exp_host (advisor, round 1): fields are sized for 2*bound; sums that do not fit
+    exp_type must be reported (POLYLAB_ERR_EXPONENT_RANGE), not truncated."""
+    r = np.random.default_rng(5)
+    na, nb = 300, 200
+    a = W.Poly(r.standard_normal(na), r.integers(0, 101, size=(na, 3)).astype(np.uint8))
+    b = W.Poly(r.standard_normal(nb), r.integers(0, 101, size=(nb, 3)).astype(np.uint8))
+    res = oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, 0.0)
+    # bound 100: 2*100 fits u8 -- no device check needed
+    c, e, st = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), 0.0, max_exp=[100, 100, 100], return_stats=True)
+    assert_parity(res, c.cpu().numpy(), e.cpu().numpy())
+    # bound 200: 2*200 does not fit u8, the data's sums (<= 200) do -- checked on the device, passes
+    c, e, st = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), 0.0, max_exp=[200, 200, 200], return_stats=True)
+    assert_parity(res, c.cpu().numpy(), e.cpu().numpy())
+    assert st.key_bits == 27
+    # one sum of 300 in variable 1
+    a2 = W.Poly(a.coef.copy(), a.exps.copy())
+    b2 = W.Poly(b.coef.copy(), b.exps.copy())
+    a2.exps[17, 1] = 200
+    b2.exps[3, 1] = 100
+    with pytest.raises(B.PolylabError) as ei:
+        B.mul_simplify(dev(a2.coef), dev(a2.exps), dev(b2.coef), dev(b2.exps), 0.0, max_exp=[200, 200, 200])
+    assert ei.value.status == B.ERR_EXPONENT_RANGE
+    # the same through bounds from the data
+    with pytest.raises(B.PolylabError) as ei:
+        B.mul_simplify(dev(a2.coef), dev(a2.exps), dev(b2.coef), dev(b2.exps), 0.0)
+    assert ei.value.status == B.ERR_EXPONENT_RANGE
+    # u16: 40000 + 30000 overflows, caller bound 40000
+    a3 = W.Poly(np.ones(2), np.array([[40000, 1], [2, 3]], np.uint16))
+    b3 = W.Poly(np.ones(2), np.array([[30000, 1], [2, 3]], np.uint16))
+    with pytest.raises(B.PolylabError) as ei:
+        B.mul_simplify(dev(a3.coef), dev(a3.exps), dev(b3.coef), dev(b3.exps), 0.0, max_exp=[40000, 3])
+    assert ei.value.status == B.ERR_EXPONENT_RANGE
+
+
+@pytest.mark.parametrize("n", [10_000_000])
+def test_one_run_of_1e7_equal_keys(n):
+    """A single monomial 1e7 times: the run crosses 4,341 reduce tiles; the cross-tile fix-up sums the tile fragments by
+    a fixed tree (reduce.cu), so the error stays far inside 1e-12 * A_m."""
+    r = np.random.default_rng(n)
+    coef = r.standard_normal(n)
+    exps = np.tile(np.array([[3, 1, 4, 1, 5]], np.uint8), (n, 1))
+    c, e, st = run(W.Poly(coef, exps), 0.0)
+    exact = math.fsum(coef.tolist())
+    A = float(np.abs(coef).sum())
+    assert len(c) == 1 and e.tolist() == [[3, 1, 4, 1, 5]]
+    assert abs(c[0] - exact) <= 1e-12 * A
+    assert abs(c[0] - exact) <= 64 * 2.0 ** -53 * A          # tree, not a chain of 4,341 sequential additions
+    # two runs that both cross many tiles, with a third short one between them
+    exps2 = exps.copy()
+    exps2[: n // 2, 0] = 2
+    exps2[n // 2: n // 2 + 7, 0] = 9
+    res = oracle.simplify(coef, exps2, 0.0)
+    c2, e2, _ = run(W.Poly(coef, exps2), 0.0)
+    assert_parity(res, c2, e2)
+    assert len(c2) == 3
