@@ -92,6 +92,20 @@ enum {
                                         no max_exp_host takes the maxima of a sample of the rows, sizes the key fields by
                                         their bit lengths, and lets S1's range check verify every row; a violation
                                         re-runs the call with full bounds (stats->bounds_retry = 1).  Same result. */
+    POLYLAB_FLAG_NO_TABLE = 64u,      /* never take the table path.  By default a call with 2^15 <= N <= 2^26 terms whose key fits 63 bits
+                                        first merges like terms in a table (the packed key itself as the index when 2^B slots
+                                        are affordable, else a hash table) with order-independent fixed-point accumulators,
+                                        and sorts only the U distinct monomials (stats->table_path = 1 dense, 2 hash).  If
+                                        more than min(N/4, 2^20) distinct monomials turn up the call continues on the sort
+                                        path (stats->table_fallback = 1).  Results obey the same parity rule; on this path
+                                        they are also invariant under permutations of the input terms.  Not taken with
+                                        POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
+    POLYLAB_FLAG_NO_SMALL = 128u,     /* never take the one-block path.  By default at most 8192 terms (or products, or distinct
+                                        monomials left by the table path; 4096 with 128-bit keys) are sorted and summed by a
+                                        single thread block in shared memory (stats->small_path = 1): two launches instead of
+                                        a dozen.  Not taken with POLYLAB_FLAG_SAFE_RANK / POLYLAB_FLAG_DEVICE_COUNT. */
+    POLYLAB_FLAG_DEBUG_FORCE_TABLE = 0x10000000u,  /* test hook: take the table path at any size up to 2^20 terms (abandoned only beyond 16384 distinct monomials) */
+    POLYLAB_FLAG_DEBUG_FORCE_HASH = 0x08000000u,   /* test hook: use the hash table even where the dense table applies */
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
                                         skew pre-check), so that small tests reach it and its overflow fallback */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
@@ -127,6 +141,10 @@ typedef struct polylab_stats {
     int32_t plan_digits;     /* ceil(B/8): digits of the key layout = entries of digit_bits = LSD passes the plan needs */
     int32_t bounds_sampled;  /* 1 if S0 ran on a sample of the rows (see POLYLAB_FLAG_EXACT_BOUNDS) */
     int32_t bounds_retry;    /* 1 if the sampled bounds were violated and the call re-ran with full bounds */
+    int32_t table_path;      /* 1: like terms were merged in a dense table (no sort at all); 2: in a hash table, and only the
+                                distinct monomials were sorted (see POLYLAB_FLAG_NO_TABLE); 0: sort path */
+    int32_t table_fallback;  /* 1 if the table path was tried and abandoned (too many distinct monomials) */
+    int32_t small_path;      /* 1 if one thread block did the sort and the segmented sum (see POLYLAB_FLAG_NO_SMALL) */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

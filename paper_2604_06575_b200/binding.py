@@ -29,6 +29,10 @@ FLAG_SAFE_RANK = 4
 FLAG_NO_BUCKET = 8
 FLAG_NO_FUSED_PACK = 16
 FLAG_EXACT_BOUNDS = 32
+FLAG_NO_TABLE = 64
+FLAG_NO_SMALL = 128
+FLAG_DEBUG_FORCE_TABLE = 0x10000000
+FLAG_DEBUG_FORCE_HASH = 0x08000000
 FLAG_DEBUG_FORCE_BUCKET = 0x20000000
 FLAG_DEBUG_UNSTABLE = 0x40000000
 FLAG_DEBUG_NFAST_SHIFT = 8
@@ -50,7 +54,8 @@ class _Stats(ctypes.Structure):
                 ("survivors", ctypes.c_int64), ("kernel_launches", ctypes.c_int32), ("rank_fallback", ctypes.c_int32),
                 ("stage_ms", ctypes.c_float * 8), ("prefix_passes", ctypes.c_int32), ("bucket_fallback", ctypes.c_int32),
                 ("refinish_tiles", ctypes.c_int32), ("plan_digits", ctypes.c_int32), ("bounds_sampled", ctypes.c_int32),
-                ("bounds_retry", ctypes.c_int32)]
+                ("bounds_retry", ctypes.c_int32), ("table_path", ctypes.c_int32), ("table_fallback", ctypes.c_int32),
+                ("small_path", ctypes.c_int32)]
 
 
 class _Opts(ctypes.Structure):
@@ -80,6 +85,9 @@ class Stats:
     refinish_tiles: int = 0
     bounds_sampled: int = 0
     bounds_retry: int = 0
+    table_path: int = 0
+    table_fallback: int = 0
+    small_path: int = 0
 
 
 _lib = None
@@ -191,7 +199,8 @@ def _stats(st: _Stats) -> Stats:
     return Stats(st.key_bits, st.key_bytes, st.sort_passes, list(st.digit_bits)[:st.plan_digits], st.sort_terms,
                  st.distinct, st.survivors, st.kernel_launches, {k: float(st.stage_ms[i]) for i, k in enumerate(STAGES)},
                  rank_fallback=st.rank_fallback, prefix_passes=st.prefix_passes, bucket_fallback=st.bucket_fallback,
-                 refinish_tiles=st.refinish_tiles, bounds_sampled=st.bounds_sampled, bounds_retry=st.bounds_retry)
+                 refinish_tiles=st.refinish_tiles, bounds_sampled=st.bounds_sampled, bounds_retry=st.bounds_retry,
+                 table_path=st.table_path, table_fallback=st.table_fallback, small_path=st.small_path)
 
 
 def _dev_poly(coef: torch.Tensor, exps: torch.Tensor, strides=None):

@@ -21,6 +21,7 @@ struct Attempt {
     bool safe_rank;        // ballot-matching radix passes, LSD path only
     bool allow_bucket;     // may take the bucket path (finish.cu)
     bool exact_bounds;     // S0 reads every row (otherwise large inputs are sampled and S1's range check verifies)
+    bool allow_table;      // may take the table path (table.cu); only the first attempt does
 };
 
 static bool cuda_failed(cudaError_t e, const char* what)
@@ -124,8 +125,41 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 
 struct Layout {
     size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
+    size_t tab_state, tab, tab_bytes;
     size_t keys[2], coefs[2], ka, kb, total;
 };
+
+// Table path (table.cu): the dense table indexes 2^B slots with the key itself (B <= 22 and no more slots than
+// max(N, 65536)); the hash table has room for `limit` distinct keys at load <= 1/2.
+static int64_t table_max_dense_slots(int64_t n)
+{
+    if (n > kTableMaxTerms) return 0;
+    int64_t s = n > 65536 ? n : 65536;
+    if (s > ((int64_t)1 << kTableDenseMaxBits)) s = (int64_t)1 << kTableDenseMaxBits;
+    return s;
+}
+static uint32_t table_limit(int64_t n, bool forced)
+{
+    if (forced) return (uint32_t)(n < 1024 ? 1024 : n > 16384 ? 16384 : n);   // test hook: small inputs are never abandoned
+    int64_t l = n / 4;
+    if (l > (int64_t)kTableMaxDistinct) l = kTableMaxDistinct;
+    return (uint32_t)(l < 1 ? 1 : l);
+}
+static uint32_t table_capacity(uint32_t limit)
+{
+    uint32_t c = 1024;
+    while (c < 2u * limit) c <<= 1;
+    return c;
+}
+static size_t table_hash_bytes(uint32_t limit) { return (size_t)table_capacity(limit) * sizeof(TableSlot) + (size_t)limit * 16 + 512; }
+static size_t table_region_bytes(int64_t n)
+{
+    if (n < 1 || n > kTableMaxTerms) return 0;
+    const size_t dense = (size_t)table_max_dense_slots(n) * 20 + 768;
+    size_t hash = table_hash_bytes(table_limit(n, false));
+    { const size_t f = table_hash_bytes(table_limit(n, true)); if (f > hash) hash = f; }
+    return dense > hash ? dense : hash;
+}
 
 static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
 {
@@ -141,7 +175,10 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.prune_state = take(prune_tiles * sizeof(uint32_t));
     const size_t fin_tiles = (size_t)((n + kFinMinTile - 1) / kFinMinTile);
     L.fin_state = take((fin_tiles + 1) * sizeof(uint32_t));
+    L.tab_state = take(((size_t)table_max_dense_slots(n) / table_dense_tile() + 2) * sizeof(uint32_t));
     L.zero_end = off;                                   // everything before this is zeroed per call
+    L.tab_bytes = table_region_bytes(n);
+    L.tab = take(L.tab_bytes);
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.fin_wl = take((fin_tiles + 1) * sizeof(uint4));
     L.fin_chunks = take((fin_tiles / 4096 + 2) * sizeof(uint32_t));
@@ -167,7 +204,9 @@ static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
 {
     if (!st) return;
     const int32_t launches = st->kernel_launches, fallback = st->rank_fallback, bfall = st->bucket_fallback, bretry = st->bounds_retry;
+    const int32_t tfall = st->table_fallback;
     memset(st, 0, sizeof *st);
+    st->table_fallback = tfall;
     st->kernel_launches = launches;
     st->rank_fallback = fallback;
     st->bucket_fallback = bfall;
@@ -319,6 +358,13 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     return (int64_t)res.survivors > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
 }
 
+// At most kSmallCap pairs: one thread block does S2-S5 (small.cu).  The sort path's test hooks mean the multi-kernel path.
+static bool small_eligible(int64_t n, const Plan& plan, const Opts& o)
+{
+    if (n > small_cap(plan.key_bytes) || (o.flags & (POLYLAB_FLAG_NO_SMALL | POLYLAB_FLAG_SAFE_RANK))) return false;
+    return !(o.flags & (POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE | (0xfu << POLYLAB_FLAG_DEBUG_NFAST_SHIFT)));
+}
+
 static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
@@ -331,28 +377,38 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
     const int P = plan.npasses;
-    for (int p = 0; p < P; ++p) {
-        const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
-        *launches += launch_sort_pass(plan, p, p + 1 < P ? p + 1 : -1, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1],
-                                      cbuf[(p + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
-                                      (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, nullptr, p == 0 ? xs : nullptr);
-    }
-    tm.mark(POLYLAB_STAGE_SORT);
-    const void* skeys = kbuf[P & 1];
-    const double* scoef = (P == 0) ? coef0 : cbuf[P & 1];
-    void* ukeys = kbuf[(P + 1) & 1];
-    double* usums = cbuf[(P + 1) & 1];
-    ReduceScratch sc;
-    sc.tile_state = (uint32_t*)(ws + L.red_state);
-    sc.tile_heads = (uint32_t*)(ws + L.red_heads);
-    sc.tile_hb = (uint32_t*)(ws + L.red_hb);
-    sc.tile_frag = (double*)(ws + L.red_frag);
-    sc.tile_cont = (uint8_t*)(ws + L.red_cont);
-    *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
-    tm.mark(POLYLAB_STAGE_REDUCE);
     const bool dev_count = (o.flags & POLYLAB_FLAG_DEVICE_COUNT) != 0;
-    *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
-                                     (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+    const bool small = xs == nullptr && !safe_rank && small_eligible(n, plan, o);   // (its ranking is the atomic one)
+    if (small) {
+        tm.mark(POLYLAB_STAGE_SORT);
+        *launches += launch_block_sort_reduce(plan, kbuf[0], coef0, nullptr, (uint32_t)n, kbuf[1], cbuf[1], ctl, stream);
+        tm.mark(POLYLAB_STAGE_REDUCE);
+        *launches += launch_prune_unpack(plan, n, kbuf[1], cbuf[1], tol, out_coef, out_exps, o.exp_bytes, out_capacity,
+                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+        if (o.stats) { o.stats->small_path = 1; o.stats->sort_passes = 0; }
+    } else {
+        for (int p = 0; p < P; ++p) {
+            const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
+            *launches += launch_sort_pass(plan, p, p + 1 < P ? p + 1 : -1, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1],
+                                          cbuf[(p + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
+                                          (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, nullptr, p == 0 ? xs : nullptr);
+        }
+        tm.mark(POLYLAB_STAGE_SORT);
+        const void* skeys = kbuf[P & 1];
+        const double* scoef = (P == 0) ? coef0 : cbuf[P & 1];
+        void* ukeys = kbuf[(P + 1) & 1];
+        double* usums = cbuf[(P + 1) & 1];
+        ReduceScratch sc;
+        sc.tile_state = (uint32_t*)(ws + L.red_state);
+        sc.tile_heads = (uint32_t*)(ws + L.red_heads);
+        sc.tile_hb = (uint32_t*)(ws + L.red_hb);
+        sc.tile_frag = (double*)(ws + L.red_frag);
+        sc.tile_cont = (uint8_t*)(ws + L.red_cont);
+        *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
+        tm.mark(POLYLAB_STAGE_REDUCE);
+        *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
+                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+    }
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
     if (o.stats) o.stats->kernel_launches += *launches;
@@ -369,6 +425,96 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     tm.finish(o.stats);
     if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; }
     if (res.status != POLYLAB_OK) return res.status;
+    *out_nterms = (int64_t)res.survivors;
+    return (int64_t)res.survivors > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
+}
+
+// ---------------------------------------------------------------------------------------- table path
+
+static bool table_eligible(const Plan& plan, int64_t n, const Opts& o, const Attempt& at)
+{
+    if (!at.allow_table || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_TABLE | POLYLAB_FLAG_DEVICE_COUNT | POLYLAB_FLAG_SAFE_RANK))) return false;
+    // the sort path's test hooks mean the sort path
+    if (o.flags & (POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE | (0xfu << POLYLAB_FLAG_DEBUG_NFAST_SHIFT))) return false;
+    if (plan.key_bytes != 8 || plan.key_bits > 63 || plan.npasses < 1 || n > kTableMaxTerms) return false;
+    if (o.flags & POLYLAB_FLAG_DEBUG_FORCE_TABLE) return n <= ((int64_t)1 << 20);
+    return n >= kTableMinTerms;
+}
+
+// Merges the N records of `src` in a table and emits the simplified polynomial.  *done = false: the table was abandoned
+// (too many distinct monomials) and nothing was emitted -- the caller continues on the sort path.
+static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, TableSrc src, double tol, const Opts& o,
+                      double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
+                      cudaStream_t stream, bool* done)
+{
+    *done = false;
+    Control* ctl = (Control*)(ws + L.control);
+    const bool forced = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_TABLE) != 0;
+    const bool dense = !(o.flags & POLYLAB_FLAG_DEBUG_FORCE_HASH) && plan.key_bits <= kTableDenseMaxBits &&
+                       ((int64_t)1 << plan.key_bits) <= table_max_dense_slots(n);
+    src.n = (uint32_t)n;
+    TableArgs t;
+    memset(&t, 0, sizeof t);
+    t.ctl = ctl;
+    int lg = 0;
+    while (((int64_t)1 << lg) < n) ++lg;
+    t.p = 62 - lg > 40 ? 40 : 62 - lg;                 // limb width: N terms of p bits never overflow 62 bits
+    unsigned char* base = ws + L.tab;
+    if (dense) {
+        const size_t slots = (size_t)1 << plan.key_bits;
+        t.nord = (uint32_t)slots;
+        t.acc_hi = (unsigned long long*)base;
+        t.acc_lo = t.acc_hi + slots;
+        t.meta = (uint32_t*)(t.acc_lo + slots);
+        PL_CUDA(cudaMemsetAsync(base, 0, slots * 20, stream));
+    } else {
+        t.limit = table_limit(n, forced);
+        const uint32_t cap = table_capacity(t.limit);
+        t.cmask = cap - 1u;
+        t.slots = (TableSlot*)base;
+        t.acc_hi = (unsigned long long*)(base + (size_t)cap * sizeof(TableSlot));
+        t.acc_lo = t.acc_hi + t.limit;
+        PL_CUDA(cudaMemsetAsync(base, 0, (size_t)cap * sizeof(TableSlot) + (size_t)t.limit * 16, stream));
+    }
+    *launches += launch_table_insert(src, t, dense, stream);
+    struct Tail { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish, fin_count, tab_count, tab_overflow; } res;
+    if (!dense) {
+        PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        if (res.status == POLYLAB_ERR_EXPONENT_RANGE) { *done = true; return res.status; }
+        if (res.tab_overflow || res.tab_count > t.limit) {
+            if (o.stats) o.stats->table_fallback = 1;
+            return POLYLAB_OK;
+        }
+        t.nord = res.tab_count;
+    }
+    *launches += launch_table_accum(src, t, dense, stream);
+    *done = true;
+    if (!dense) {
+        // (key, sum)[U] -> the ordinary sort / prune / unpack over U records
+        const int64_t U = t.nord;
+        *launches += launch_table_finalize(t, (uint64_t*)(ws + L.keys[0]), (double*)(ws + L.coefs[0]), stream);
+        if (!small_eligible(U, plan, o)) {
+            PL_CUDA(cudaMemsetAsync(ctl->hist, 0, sizeof ctl->hist, stream));      // S1 counted the N records into one of them
+            *launches += launch_key_hist(plan, 0, U, ws + L.keys[0], ctl, stream);
+        }
+        if (o.stats) { o.stats->table_path = 2; o.stats->sort_terms = n; }
+        const int rc = sort_reduce_emit(plan, 0, U, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
+                                        out_nterms, launches, tm, false, stream);
+        return rc == kRetrySafeRank ? kRetrySafeRank : rc;
+    }
+    tm.mark(POLYLAB_STAGE_SORT);
+    tm.mark(POLYLAB_STAGE_REDUCE);
+    *launches += launch_table_dense_emit(t, plan, tol, out_coef, out_exps, o.exp_bytes, out_capacity, (uint32_t*)(ws + L.tab_state), stream);
+    tm.mark(POLYLAB_STAGE_PRUNE);
+    PL_CUDA(cudaGetLastError());
+    if (o.stats) o.stats->kernel_launches += *launches;
+    PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    if (res.status != POLYLAB_OK) return res.status;
+    if (res.unsorted) return POLYLAB_ERR_INTERNAL;
+    tm.finish(o.stats);
+    if (o.stats) { o.stats->distinct = res.distinct; o.stats->survivors = res.survivors; o.stats->table_path = 1; o.stats->sort_passes = 0; }
     *out_nterms = (int64_t)res.survivors;
     return (int64_t)res.survivors > out_capacity ? POLYLAB_ERR_OUTPUT_TOO_SMALL : POLYLAB_OK;
 }
@@ -466,9 +612,19 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
 
     // ---- S1 (+ histogram of the first pass's digit), then the shared tail
     int k = choose_prefix_passes(plan, nterms, o, at);
-    const bool fuse = k > 0 && rows_fusable(ev, nvars) && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
+    const bool try_table = table_eligible(plan, nterms, o, at);
+    const bool fuse = !try_table && k > 0 && rows_fusable(ev, nvars) && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
     if (fuse) launches += launch_row_hist(ev, nterms, plan, plan.npasses - k, ctl, stream);      // S1 itself runs inside the first pass
     else launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
+    if (try_table) {
+        tm.mark(POLYLAB_STAGE_PACK);
+        TableSrc src;
+        memset(&src, 0, sizeof src);
+        src.keys = (const uint64_t*)(ws + L.keys[0]); src.coef = coef;
+        bool done = false;
+        rc = table_path(plan, nterms, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
+        if (done || rc != POLYLAB_OK) return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
+    }
     rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
     if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
@@ -487,11 +643,12 @@ extern "C++" {
 template <typename F>
 static int run_attempts(const polylab_opts* opts, F once)
 {
-    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; opts->stats->bounds_retry = 0; }
-    Attempt at = {wants_safe_rank(opts), true, false};
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; opts->stats->bounds_retry = 0; opts->stats->table_fallback = 0; }
+    Attempt at = {wants_safe_rank(opts), true, false, true};
     int rc = once(at);
     for (int tries = 0; tries < 3 && (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank); ++tries) {
         polylab_stats* st = opts ? opts->stats : nullptr;
+        if (rc != kRetryExactBounds) at.allow_table = false;
         if (rc == kRetryExactBounds) {             // each retry only ever tightens the attempt, so three suffice
             if (st) st->bounds_retry = 1;
             at.exact_bounds = true;
@@ -590,7 +747,16 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     // X1 runs inside the first radix pass (the products are formed in registers and never stored) unless the ballot
     // ranking kernel is asked for or there is no pass at all; only the first digit's histogram is built up front
     const ExpandSrc xs = {ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb};
-    const bool fuse = plan_a.npasses > 0 && !at.safe_rank && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
+    if (table_eligible(plan_a, n, o, at)) {
+        tm.mark(POLYLAB_STAGE_PACK);
+        TableSrc src;
+        memset(&src, 0, sizeof src);
+        src.ka = ws + L.ka; src.ca = a->coef; src.kb = ws + L.kb; src.cb = b->coef; src.nb = (uint32_t)nb;
+        bool done = false;
+        rc = table_path(plan_a, n, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
+        if (done || rc != POLYLAB_OK) return rc;
+    }
+    const bool fuse = plan_a.npasses > 0 && !at.safe_rank && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK) && !small_eligible(n, plan_a, o);      // (at.safe_rank already excludes fusing)
     if (fuse) launches += launch_expand_hist(xs, plan_a, k ? plan_a.npasses - k : 0, ctl, stream);
     else launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
                                           (double*)(ws + L.coefs[0]), ctl, k ? plan_a.npasses - k : 0, stream);

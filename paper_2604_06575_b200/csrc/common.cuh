@@ -173,6 +173,8 @@ struct Control {
     uint32_t overflow;                       // bucket path: a bucket does not fit a finish tile (skewed prefix digits)
     uint32_t refinish;                       // bucket path: finish tiles that needed the full local digit list
     uint32_t fin_count;                      // bucket path: tiles that own records (length of the work list)
+    uint32_t tab_count;                      // table path: distinct keys inserted so far (= U after the insert pass)
+    uint32_t tab_overflow;                   // table path: more distinct keys than the table was sized for -> sort path
 };
 
 constexpr int kTicketReduce = kMaxPasses;
@@ -192,6 +194,19 @@ __device__ __forceinline__ unsigned match_digit(uint32_t d, bool valid)
         const bool bit = (d >> b) & 1u;
         const unsigned m = __ballot_sync(kFullMask, bit);
         mask &= bit ? m : ~m;
+    }
+    return mask;
+}
+
+// lanes of the warp holding the same digit d (< 256) as the calling lane; all 32 lanes participate
+__device__ __forceinline__ unsigned match_digit_all(uint32_t d)
+{
+    unsigned mask = kFullMask;
+#pragma unroll
+    for (int b = 0; b < kRadixBits; ++b) {
+        const unsigned x = 0u - ((d >> b) & 1u);            // all ones iff bit b of d is set
+        const unsigned m = __ballot_sync(kFullMask, x != 0u);
+        mask &= ~(m ^ x);                                   // keep the lanes whose bit b equals ours
     }
     return mask;
 }

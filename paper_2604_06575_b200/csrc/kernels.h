@@ -138,4 +138,52 @@ int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, 
                   uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
                   int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream);
 
+// Small inputs (small.cu): S2 + S3 of at most small_cap() (key, coef) pairs in ONE thread block -- radix sort of a permutation
+// in shared memory, segmented sum; (ukeys, usums)[U] ascending and ctl->distinct = U as launch_reduce leaves them (then
+// launch_prune_unpack).  Sets ctl->unsorted if its atomic ranking turned out unstable.
+// n_device (optional, DEVICE): the pair count is read on the device (clamped) instead of `n`.
+constexpr int kSmallCap = 8192;          // 64-bit keys; half of it for 128-bit keys
+inline int small_cap(int key_bytes) { return key_bytes == 8 ? kSmallCap : kSmallCap / 2; }
+int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
+                             void* ukeys, double* usums, Control* ctl, cudaStream_t stream);
+
+// Table path (table.cu): merge like terms in a dense or hash table before any sort.
+struct __align__(16) TableSlot {
+    uint64_t key1;          // packed key + 1; 0 = empty
+    uint32_t ord;           // dense ordinal of the key, 0..U-1 (index into the accumulators)
+    uint32_t meta;          // largest biased coefficient exponent seen + 1; 2048 = a non-finite coefficient; 0 = untouched
+};
+struct TableSrc {           // the N records: packed keys + coefficients, or (keys == nullptr) the products of packed operands
+    const uint64_t* keys;
+    const double* coef;
+    const void* ka;
+    const double* ca;
+    const void* kb;
+    const double* cb;
+    uint32_t nb;
+    uint32_t n;
+};
+struct TableArgs {
+    TableSlot* slots;       // hash: [cmask + 1]
+    uint32_t cmask;
+    uint32_t limit;         // hash: most distinct keys before the path is abandoned
+    uint32_t* meta;         // dense: [2^B]
+    unsigned long long* acc_hi;   // [nord] fixed-point accumulators (two limbs of p bits)
+    unsigned long long* acc_lo;
+    uint32_t nord;          // dense: 2^B; hash: U (known after the insert pass)
+    uint32_t nsm;           // set by launch_table_accum: ordinals below this are accumulated in shared memory
+    int p;                  // limb width in bits
+    Control* ctl;
+};
+constexpr int64_t kTableMaxTerms = (int64_t)1 << 26;      // the fixed-point error bound is derived for N <= 2^26 (table.cu)
+constexpr int64_t kTableMinTerms = (int64_t)1 << 15;
+constexpr int kTableDenseMaxBits = 22;
+constexpr uint32_t kTableMaxDistinct = 1u << 20;
+inline uint32_t table_dense_tile() { return 256u * 8u; }
+int launch_table_insert(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
+int launch_table_accum(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
+int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cudaStream_t stream);
+int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, double* out_coef, void* out_exps, int exp_bytes,
+                            int64_t out_capacity, uint32_t* tile_state, cudaStream_t stream);
+
 }  // namespace polylab

@@ -225,6 +225,71 @@ __global__ void __launch_bounds__(256) pack_rows_kernel(const uint8_t* __restric
     if (hd >= 0) { __syncthreads(); bh.flush(ctl->hist[hd]); }
 }
 
+// Contiguous rows whose size is not a multiple of 16 bytes (10 one-byte variables, 6 two-byte ones, ...): a thread reading
+// its own row would issue narrow, misaligned loads (five 2-byte loads for a 10-byte row).  Instead the block brings a tile
+// of `tile_rows` consecutive rows into shared memory with aligned 16-byte asynchronous copies (cp.async), double-buffered:
+// the next tile is in flight while every thread picks its rows of the current one out of shared memory.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+
+template <typename K, int ES>
+__global__ void __launch_bounds__(256) pack_rows_staged_kernel(const uint8_t* __restrict__ base, int64_t nterms, int tile_rows,
+                                                               const __grid_constant__ Plan plan, K* __restrict__ keys,
+                                                               Control* ctl, int hd)
+{
+    extern __shared__ __align__(16) unsigned char stage[];          // two buffers of tile_rows * row bytes + 16, each 16-byte aligned
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    if (hd >= 0) { bh.init(sh); }
+    const int rb = plan.nvars * ES;
+    const int dpos = plan.digit_pos[hd >= 0 ? hd : 0];
+    const uint32_t dmask = (1u << plan.digit_bits[hd >= 0 ? hd : 0]) - 1u;
+    const int64_t nbytes = nterms * rb;
+    const int bufsz = (tile_rows * rb + 16 + 15) & ~15;
+    const int64_t step = (int64_t)gridDim.x * tile_rows;
+    auto issue = [&](int buf, int64_t t0) {                          // rows [t0, t0 + tile_rows) -> stage + buf * bufsz
+        if (t0 < nterms) {
+            const int nr = (int)min((int64_t)tile_rows, nterms - t0);
+            const int64_t b0 = t0 * rb, b1 = b0 + (int64_t)nr * rb, a0 = b0 & ~(int64_t)15;
+            unsigned char* dst = stage + (size_t)buf * bufsz;
+            for (int64_t off = a0 + 16 * (int64_t)threadIdx.x; off < b1; off += 16 * 256) {
+                if (off + 16 <= nbytes) cp_async16(dst + (off - a0), base + off);
+                else for (int64_t b = off; b < nbytes; ++b) dst[b - a0] = base[b];         // the array's last, partial word
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    bool bad = false;
+    int64_t t0 = (int64_t)blockIdx.x * tile_rows;
+    issue(0, t0);
+    for (int it = 0; t0 < nterms; ++it, t0 += step) {
+        const int cur = it & 1;
+        issue(cur ^ 1, t0 + step);                                  // (the buffer was released by the barrier that ended the last round)
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncthreads();                                            // tile `cur` has landed for every thread
+        const int nr = (int)min((int64_t)tile_rows, nterms - t0);
+        const int64_t b0 = t0 * rb, a0 = b0 & ~(int64_t)15;
+        const unsigned char* src = stage + (size_t)cur * bufsz + (b0 - a0);
+        for (int r = threadIdx.x; r < nr; r += 256) {
+            const unsigned char* row = src + (int64_t)r * rb;
+            K key;
+            key_zero(key);
+            for (int v = 0; v < plan.nvars; ++v) {
+                const uint32_t e = ES == 1 ? row[v] : ES == 2 ? ((const uint16_t*)row)[v] : ((const uint32_t*)row)[v];
+                pack_field(key, e, v, plan, bad);
+            }
+            keys[t0 + r] = key;
+            if (hd >= 0) bh.add(key_digit(key, dpos, dmask));
+        }
+        __syncthreads();                                            // tile `cur` has been read: its buffer may be refilled
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (bad) atomicMax(&ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+    if (hd >= 0) { __syncthreads(); bh.flush(ctl->hist[hd]); }
+}
+
 // Any strides / alignment: one element load per variable.
 template <typename K>
 __global__ void __launch_bounds__(256) pack_strided_kernel(ExpView ev, int64_t nterms, const __grid_constant__ Plan plan,
@@ -267,7 +332,18 @@ static int launch_pack_t(const ExpView& ev, int64_t nterms, const Plan& plan, K*
     int64_t blocks = (nterms + 256 * 4 - 1) / (256 * 4);       // >= 4 rows per thread once the grid saturates
     if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     if (blocks < 1) blocks = 1;
-    if (ev.row_major_contiguous) {
+    if (ev.row_major_contiguous && (plan.nvars * ev.exp_bytes) % 16 != 0) {
+        const int rb = plan.nvars * ev.exp_bytes;
+        int tile_rows = 16384 / rb;                              // at most 16 KB of rows per tile, two tiles in shared memory
+        tile_rows = tile_rows > 1024 ? 1024 : tile_rows < 32 ? 32 : tile_rows / 32 * 32;
+        int64_t sblocks = (nterms + tile_rows - 1) / tile_rows;
+        if (sblocks > sm_count() * 6) sblocks = sm_count() * 6;
+        const size_t smem = 2 * (((size_t)tile_rows * rb + 16 + 15) & ~(size_t)15);
+        const uint8_t* base = (const uint8_t*)ev.base;
+        if (ev.exp_bytes == 1) pack_rows_staged_kernel<K, 1><<<(unsigned)sblocks, 256, smem, stream>>>(base, nterms, tile_rows, plan, keys, ctl, hd);
+        else if (ev.exp_bytes == 2) pack_rows_staged_kernel<K, 2><<<(unsigned)sblocks, 256, smem, stream>>>(base, nterms, tile_rows, plan, keys, ctl, hd);
+        else pack_rows_staged_kernel<K, 4><<<(unsigned)sblocks, 256, smem, stream>>>(base, nterms, tile_rows, plan, keys, ctl, hd);
+    } else if (ev.row_major_contiguous) {
         const int rb = plan.nvars * ev.exp_bytes;
         const int wb = (rb % 16 == 0) ? 16 : (rb % 4 == 0) ? 4 : (rb % 2 == 0) ? 2 : 1;
         if (ev.exp_bytes == 1) launch_pack_rows_es<K, 1>(wb, (unsigned)blocks, ev, nterms, plan, keys, ctl, hd, stream);

@@ -94,19 +94,6 @@ __device__ __forceinline__ K pack_row_inline(const PassArgs& a, const Plan& plan
     return key;
 }
 
-// lanes of the warp holding the same digit d (< 256) as the calling lane; all 32 lanes participate
-__device__ __forceinline__ unsigned match_digit_all(uint32_t d)
-{
-    unsigned mask = kFullMask;
-#pragma unroll
-    for (int b = 0; b < kRadixBits; ++b) {
-        const unsigned x = 0u - ((d >> b) & 1u);            // all ones iff bit b of d is set
-        const unsigned m = __ballot_sync(kFullMask, x != 0u);
-        mask &= ~(m ^ x);                                   // keep the lanes whose bit b equals ours
-    }
-    return mask;
-}
-
 // RANK_ATOMIC: rank a record among the warp's records of the same digit with ONE shared-memory atomic (the old
 // value of the warp's counter).  Lanes of one warp instruction that hit the same counter receive their old
 // values in ascending lane order on sm_100a (measured, profiles/r1b_shared_atomics.md; not documented), which

@@ -67,8 +67,9 @@ def test_workspace_queries(L):
     small = L.polylab_simplify_workspace_bytes(1000, 4, None)
     big = L.polylab_simplify_workspace_bytes(100_000, 4, None)
     assert 0 < small < big
-    # two 16-byte key buffers + two coefficient buffers dominate: 48 B per term
-    assert 48 * 100_000 <= big <= 48 * 100_000 + (1 << 21)
+    # two 16-byte key buffers + two coefficient buffers dominate: 48 B per term (+ 20 B per slot of the table path's
+    # dense table, at most max(N, 65536) slots)
+    assert 48 * 100_000 <= big <= 68 * 100_000 + (1 << 21)
     assert L.polylab_mul_simplify_workspace_bytes(2000, 2000, 6, None) >= 48 * 4_000_000
     assert L.polylab_mul_simplify_workspace_bytes(1 << 20, 1 << 20, 6, None) == 0      # na*nb >= 2^30
     assert L.polylab_simplify_workspace_bytes(-1, 4, None) == 0

@@ -214,11 +214,16 @@ def test_randomised_shapes_both_paths(seed):
     res = oracle.simplify(p.coef, p.exps, tol)
     c, e, st = run(p, tol, flags=FORCE)
     assert_parity(res, c, e)
-    c0, e0, st0 = run(p, tol, flags=B.FLAG_NO_BUCKET)
-    assert st0.prefix_passes == 0
+    c0, e0, st0 = run(p, tol, flags=B.FLAG_NO_BUCKET | B.FLAG_NO_TABLE)
+    assert st0.prefix_passes == 0 and st0.table_path == 0
     assert_parity(res, c0, e0)
     if tol == 0.0:
         assert (e == e0).all()
+    if sum(int(h - 1).bit_length() for h in his) <= 63:             # the table path (table.cu), dense or hash, and hash alone
+        for fl in (B.FLAG_DEBUG_FORCE_TABLE, B.FLAG_DEBUG_FORCE_TABLE | B.FLAG_DEBUG_FORCE_HASH):
+            c1, e1, st1 = run(p, tol, flags=fl)
+            assert_parity(res, c1, e1)
+            assert st1.table_path in (1, 2) or st1.table_fallback == 1 or st1.key_bits == 0
 
 
 # ------------------------------------------------------------------ S0 on a sample of the rows

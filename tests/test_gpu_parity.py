@@ -346,7 +346,7 @@ def test_128_one_bit_variables_and_wide_fields():
     full[:, :] |= (np.arange(128) % 2 == 0).astype(np.uint8) & full           # keep all 128 fields live
     coef = r.standard_normal(3000)
     c, e, st = B.simplify(dev(coef), dev(full), return_stats=True)
-    assert st.key_bits == 128 and st.key_bytes == 16 and st.sort_passes == 16
+    assert st.key_bits == 128 and st.key_bytes == 16 and len(st.digit_bits) == 16
     assert_parity(oracle.simplify(coef, full), c.cpu().numpy(), e.cpu().numpy())
     big = r.integers(0, 2 ** 32, size=(4000, 3), dtype=np.uint64).astype(np.uint32)
     big[0:3999:3] = big[1:4000:3]
@@ -431,12 +431,12 @@ def test_safe_rank_kernel_matches_default(cfg):
     same monomials, bit-identical sums (the summation tree is the same when the sorted order is the same)."""
     if cfg == "c2":
         a, b, tol = W.config2(300)
-        r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True)
+        r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_NO_TABLE)
         r1 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_SAFE_RANK)
         res = oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol)
     else:
         p, tol = (W.config3(300_000) if cfg == "c3" else W.config5(300_000))
-        r0 = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True)
+        r0 = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=B.FLAG_NO_TABLE)    # the sort path
         r1 = B.simplify(dev(p.coef), dev(p.exps), tol, return_stats=True, flags=B.FLAG_SAFE_RANK)
         res = oracle.simplify(p.coef, p.exps, tol)
     assert r0[2].rank_fallback == 0 and r1[2].rank_fallback == 0
@@ -477,8 +477,9 @@ def test_fused_expand_matches_materialised_products(shape):
         a = W.Poly(np.array([1.0, 2.0]), np.array([[1, 0], [0, 1]], np.uint8))
         b = W.Poly(np.array([1.0, -2.0]), np.array([[1, 0], [0, 1]], np.uint8))
         tol = 0.0
-    r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True)
-    r1 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_NO_FUSED_PACK)
+    r0 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True, flags=B.FLAG_NO_TABLE)
+    r1 = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, return_stats=True,
+                        flags=B.FLAG_NO_FUSED_PACK | B.FLAG_NO_TABLE)
     c0, e0, c1, e1 = r0[0].cpu().numpy(), r0[1].cpu().numpy(), r1[0].cpu().numpy(), r1[1].cpu().numpy()
     assert (e0 == e1).all() and (c0.view(np.uint64) == c1.view(np.uint64)).all()
     assert r0[2].kernel_launches == r1[2].kernel_launches
@@ -498,6 +499,7 @@ def test_randomised_products_all_paths(seed):
     b = W.Poly(r.standard_normal(nb), r.integers(0, hi, size=(nb, nvars)).astype(dtype))
     tol = [0.0, 1e-13][seed % 2]
     res = oracle.mul_simplify(a.coef, a.exps, b.coef, b.exps, tol)
-    for flags in (0, B.FLAG_DEBUG_FORCE_BUCKET, B.FLAG_NO_FUSED_PACK, B.FLAG_SAFE_RANK):
+    for flags in (0, B.FLAG_NO_TABLE, B.FLAG_DEBUG_FORCE_TABLE, B.FLAG_DEBUG_FORCE_TABLE | B.FLAG_DEBUG_FORCE_HASH,
+                  B.FLAG_DEBUG_FORCE_BUCKET, B.FLAG_NO_FUSED_PACK | B.FLAG_NO_TABLE, B.FLAG_SAFE_RANK):
         c, e = B.mul_simplify(dev(a.coef), dev(a.exps), dev(b.coef), dev(b.exps), tol, flags=flags)
         assert_parity(res, c.cpu().numpy(), e.cpu().numpy())
