@@ -299,9 +299,78 @@ def measure_other_config(B, torch, cfg, variant, steps, warmup, peak, ws):
             "oracle_seconds_same_arrays_1core": osec, "oracle_terms_per_s": n_sort / osec if osec else None, "parity": par}
 
 
+def measure_matrix_product(B, torch, steps, warmup, ws):
+    """Table 7's matrix-mtimes shape (5-variable polynomials, a 3x3 matrix product): ONE batched call
+    (polylab_matmul_simplify) against the same product through separate calls (27 polylab_expand + 9 polylab_simplify), both
+    device-resident through the C ABI; parity of the batched output against one oracle call per entry."""
+    from oracle import oracle, parity
+    r = np.random.Generator(np.random.PCG64(20260321 + 77))
+    m = k = n = 3
+    nvars, nt = 5, 40
+
+    def matrix(rows, cols):
+        c = r.standard_normal(rows * cols * nt)
+        e = r.integers(0, 4, size=(rows * cols * nt, nvars)).astype(np.uint8)
+        return c, e, np.arange(rows * cols + 1, dtype=np.int64) * nt
+    A, Bm = matrix(m, k), matrix(k, n)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dA, dB = (dev(A[0]), dev(A[1])), (dev(Bm[0]), dev(Bm[1]))
+    sl = lambda d, off, i: (d[0][off[i]:off[i + 1]], d[1][off[i]:off[i + 1]])
+
+    def batched():
+        return B.matmul_simplify(dA[0], dA[1], A[2], dB[0], dB[1], Bm[2], m, k, n, 0.0, workspace=ws, return_stats=True)
+
+    def separate():
+        outs = []
+        for i in range(m):
+            for j in range(n):
+                parts = [B.expand(*sl(dA, A[2], i * k + l), *sl(dB, Bm[2], l * n + j)) for l in range(k)]
+                outs.append(B.simplify(torch.cat([p[0] for p in parts]), torch.cat([p[1] for p in parts]), 0.0, workspace=ws))
+        return outs
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps, out
+    ms_b, (c, e, off, st) = timed(batched)
+    ms_s, _ = timed(separate)
+    c, e = c.cpu().numpy(), e.cpu().numpy()
+    ok, matched, worst = True, 0, 0.0
+    t0 = time.perf_counter()
+    for i in range(m):
+        for j in range(n):
+            cs, es = zip(*[oracle.expand(A[0][A[2][i * k + l]:A[2][i * k + l + 1]], A[1][A[2][i * k + l]:A[2][i * k + l + 1]],
+                                         Bm[0][Bm[2][l * n + j]:Bm[2][l * n + j + 1]], Bm[1][Bm[2][l * n + j]:Bm[2][l * n + j + 1]])
+                           for l in range(k)])
+            res = oracle.simplify(np.concatenate(cs), np.concatenate(es), 0.0)
+            q = i * n + j
+            rep = parity.check(res, c[off[q]:off[q + 1]], e[off[q]:off[q + 1]])
+            ok, matched, worst = ok and rep.ok, matched + rep.matched, max(worst, rep.max_rel_dev)
+    osec = time.perf_counter() - t0
+    nprod = m * n * k * nt * nt
+    return {"config": "matrix mtimes 3x3 (batched, SURVEY 8(f) N3)",
+            "workload": f"simplify(A*B), A and B 3x3 polynomial matrices, {nt} terms per entry over {nvars} variables: {nprod} term products "
+                        "(the shape of Table 7's matrix rows, PAPER.md:560)",
+            "ms_per_step": ms_b, "terms_per_s": nprod / (ms_b * 1e-3), "sort_terms_per_step": nprod,
+            "ms_per_step_separate_calls": ms_s, "speedup_over_separate_calls": ms_s / ms_b,
+            "separate_calls": "27 polylab_expand + 9 polylab_simplify through the same binding",
+            "survivors": int(off[-1]), "key_bits": st.key_bits, "path": path_name(st), "kernel_launches_per_step": st.kernel_launches,
+            "oracle_seconds_same_arrays_1core": osec,
+            "parity": {"ok": bool(ok), "matched": matched, "max_rel_dev": worst, "slice": "every entry, every monomial"}}
+
+
 def path_name(st) -> str:
     if getattr(st, "table_path", 0):
-        return "table"
+        return "table (dense)" if st.table_path == 1 else ("table (hash) + one-block sort" if st.small_path else "table (hash) + lsd")
+    if getattr(st, "small_path", 0):
+        return "one block"
     return "bucket" if st.prefix_passes > 0 else "lsd"
 
 
@@ -545,6 +614,7 @@ def main():
         others = []
         for cfg, variant in ((1, None), (2, None), (3, None), (4, "A"), (4, "B"), (7, None), (6, None)):
             others.append(measure_other_config(B, torch, cfg, variant, 10, 3, peak, ws))
+        others.append(measure_matrix_product(B, torch, 10, 3, ws))
 
     # ---- CPU oracle on a bounded sample (rank 0, N=1)
     cpu = None

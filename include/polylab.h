@@ -216,6 +216,46 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
                          void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * Batched operations on polynomial MATRICES (Table 4: matrix mtimes, sum, prod; section 3.4;
+ * the rows of Table 7, where per-entry launches make the paper's GPU backends lose to its CPU class).
+ * A batch is many scalar polynomials over the same nvars variables stored back to back: entry e owns the terms
+ * [offsets_host[e], offsets_host[e+1]) of (coef, exps); offsets_host is a HOST array of nentries + 1 non-decreasing values
+ * starting at 0 (an entry may be empty: the zero polynomial).  A matrix is a batch in row-major entry order.
+ * One call simplifies every entry: the entry index is the most significant field of the packed key, so a single sort /
+ * segmented sum / prune / unpack serves them all.  Outputs: the simplified entries concatenated in entry order, each in
+ * canonical monomial order, in out_coef[out_capacity] / out_exps[out_capacity x nvars] (DEVICE); out_offsets_host (HOST,
+ * nentries + 1 values) receives where each entry starts (out_offsets_host[nentries] = total number of terms).  Survivors
+ * beyond out_capacity -> POLYLAB_ERR_OUTPUT_TOO_SMALL with out_offsets_host filled in.  Exponents: row-major, opts->exp_type;
+ * opts->max_exp_host, strides and POLYLAB_FLAG_DEVICE_COUNT are not supported (POLYLAB_ERR_INVALID_ARGUMENT); nvars <= 127.
+ * The calls synchronise the stream.
+ */
+typedef struct polylab_batch {
+    const double* coef;           /* DEVICE [offsets_host[nentries]]                     */
+    const void* exps;             /* DEVICE [offsets_host[nentries] x nvars], row-major  */
+    const int64_t* offsets_host;  /* HOST [nentries + 1]                                 */
+    int64_t nentries;
+    int32_t nvars;
+} polylab_batch;
+
+/* simplify every entry of a batch (for a matrix `sum` along a dimension: lay the summands of one result entry back to back) */
+size_t polylab_simplify_batched_workspace_bytes(int64_t nterms, int64_t nentries, int32_t nvars, const polylab_opts* opts);
+int polylab_simplify_batched(const polylab_batch* p, double tol, const polylab_opts* opts,
+                             double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_offsets_host,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * simplify(A*B) for polynomial matrices A (m x k) and B (k x n): entry (i, j) = sum over l of A(i,l)*B(l,j), every product
+ * of scalar polynomials formed term by term (coefficient products rounded once, exponent sums) and all of them merged in
+ * one pass.  The result has m*n entries, row-major.  nproducts = the sum over (i, j, l) of nterms(A(i,l)) * nterms(B(l,j)),
+ * which must be < POLYLAB_MAX_TERMS; out_capacity = nproducts always suffices.
+ */
+size_t polylab_matmul_simplify_workspace_bytes(int64_t nproducts, int64_t a_nterms, int64_t b_nterms, int64_t m, int64_t k, int64_t n,
+                                               int32_t nvars, const polylab_opts* opts);
+int polylab_matmul_simplify(const polylab_batch* a, int32_t m, int32_t k, const polylab_batch* b, int32_t n, double tol,
+                            const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                            int64_t* out_offsets_host, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
  * The raw product a*b without merging (reading A10): out_coef[na*nb], out_exps[na*nb x nvars] row-major,
  * term (i,j) at index i*nb + j.  workspace: POLYLAB_SMALL_WORKSPACE_BYTES.  Exponent sums that do not fit
  * exp_type -> POLYLAB_ERR_EXPONENT_RANGE (the call synchronises to report it).

@@ -64,6 +64,11 @@ class _Opts(ctypes.Structure):
                 ("status_device", ctypes.c_void_p), ("stats", ctypes.POINTER(_Stats))]
 
 
+class _Batch(ctypes.Structure):
+    _fields_ = [("coef", ctypes.c_void_p), ("exps", ctypes.c_void_p), ("offsets_host", ctypes.POINTER(ctypes.c_int64)),
+                ("nentries", ctypes.c_int64), ("nvars", ctypes.c_int32)]
+
+
 class _Poly(ctypes.Structure):
     _fields_ = [("coef", ctypes.c_void_p), ("exps", ctypes.c_void_p), ("nterms", ctypes.c_int64), ("nvars", ctypes.c_int32)]
 
@@ -120,6 +125,15 @@ def lib():
         L.polylab_pow_simplify_workspace_bytes.argtypes = [i64, i32, i32, i64, po]
         L.polylab_pow_simplify_workspace_bytes.restype = sz
         L.polylab_pow_simplify.argtypes = [pp, i32, dbl, po, vp, vp, i64, vp, vp, sz, vp]
+        pb = ctypes.POINTER(_Batch)
+        L.polylab_simplify_batched_workspace_bytes.argtypes = [i64, i64, i32, po]
+        L.polylab_simplify_batched_workspace_bytes.restype = sz
+        L.polylab_simplify_batched.argtypes = [pb, dbl, po, vp, vp, i64, vp, vp, sz, vp]
+        L.polylab_simplify_batched.restype = ctypes.c_int
+        L.polylab_matmul_simplify_workspace_bytes.argtypes = [i64, i64, i64, i64, i64, i64, i32, po]
+        L.polylab_matmul_simplify_workspace_bytes.restype = sz
+        L.polylab_matmul_simplify.argtypes = [pb, i32, i32, pb, i32, dbl, po, vp, vp, i64, vp, vp, sz, vp]
+        L.polylab_matmul_simplify.restype = ctypes.c_int
         L.polylab_expand.argtypes = [pp, pp, po, vp, vp, vp, sz, vp]
         L.polylab_pack_keys.argtypes = [vp, i64, i32, po, vp, ctypes.POINTER(i32), vp, sz, vp]
         for name in ("polylab_simplify", "polylab_simplify_host", "polylab_mul_simplify", "polylab_mul_simplify_host",
@@ -335,6 +349,74 @@ def pow_simplify(coef: torch.Tensor, exps: torch.Tensor, power: int, tol: float 
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])
+    return (*res, _stats(st)) if return_stats else res
+
+
+def _batch(coef: torch.Tensor, exps: torch.Tensor, offsets, keep: list):
+    coef, exps, strides = _dev_poly(coef, exps)
+    if strides is not None:
+        exps = exps.contiguous()
+    off = np.ascontiguousarray(np.asarray(offsets, dtype=np.int64))
+    if off.ndim != 1 or off.shape[0] < 1 or int(off[-1]) != int(coef.shape[0]):
+        raise PolylabError(ERR_INVALID_ARGUMENT, "offsets must be a 1-D array of nentries + 1 values ending at the term count")
+    keep.extend([coef, exps, off])
+    return _Batch(coef.data_ptr(), exps.data_ptr(), off.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), off.shape[0] - 1,
+                  int(exps.shape[1])), coef, exps, off
+
+
+def simplify_batched(coef: torch.Tensor, exps: torch.Tensor, offsets, tol: float = 0.0, *, out_capacity: Optional[int] = None,
+                     workspace: Optional[Workspace] = None, stream=None, return_stats: bool = False, flags: int = 0):
+    """polylab_simplify_batched: entry e = terms [offsets[e], offsets[e+1]); returns (coef, exps, out_offsets) with the
+    simplified entries concatenated in entry order (polynomial matrices, sum)."""
+    keep = []
+    bt, coef, exps, off = _batch(coef, exps, offsets, keep)
+    n, ne, nvars = int(coef.shape[0]), int(off.shape[0] - 1), int(exps.shape[1])
+    cap = n if out_capacity is None else int(out_capacity)
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep)
+    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
+    out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
+    out_off = np.zeros(ne + 1, dtype=np.int64)
+    wsb = int(lib().polylab_simplify_batched_workspace_bytes(n, ne, nvars, ctypes.byref(o)))
+    ws = _ws(coef.device, workspace).get(max(wsb, 256))
+    with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_simplify_batched(ctypes.byref(bt), float(tol), ctypes.byref(o), out_coef.data_ptr(), out_exps.data_ptr(), cap,
+                                            out_off.ctypes.data, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    k = int(out_off[-1])
+    res = (out_coef[:k], out_exps[:k], out_off)
+    return (*res, _stats(st)) if return_stats else res
+
+
+def matmul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, a_offsets, b_coef: torch.Tensor, b_exps: torch.Tensor, b_offsets,
+                    m: int, k: int, n: int, tol: float = 0.0, *, out_capacity: Optional[int] = None,
+                    workspace: Optional[Workspace] = None, stream=None, return_stats: bool = False, flags: int = 0):
+    """polylab_matmul_simplify: simplify(A*B) for polynomial matrices A (m x k) and B (k x n) given as row-major batches;
+    returns (coef, exps, out_offsets) of the m*n entries (Table 4)."""
+    keep = []
+    ba, a_coef, a_exps, aoff = _batch(a_coef, a_exps, a_offsets, keep)
+    bb, b_coef, b_exps, boff = _batch(b_coef, b_exps, b_offsets, keep)
+    if a_exps.dtype != b_exps.dtype or a_exps.shape[1] != b_exps.shape[1]:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share dtype and variable space (PAPER.md:175)")
+    if aoff.shape[0] - 1 != m * k or boff.shape[0] - 1 != k * n:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "A needs m*k entries and B k*n entries (row-major)")
+    na_e, nb_e = np.diff(aoff).reshape(m, k), np.diff(boff).reshape(k, n)
+    nprod = int((na_e.astype(np.int64) @ nb_e.astype(np.int64)).sum())
+    nvars = int(a_exps.shape[1])
+    cap = nprod if out_capacity is None else int(out_capacity)
+    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], None, flags=flags, keep=keep)
+    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=a_coef.device)
+    out_exps = torch.empty((max(cap, 1), nvars), dtype=a_exps.dtype, device=a_coef.device)
+    out_off = np.zeros(m * n + 1, dtype=np.int64)
+    wsb = int(lib().polylab_matmul_simplify_workspace_bytes(nprod, int(aoff[-1]), int(boff[-1]), m, k, n, nvars, ctypes.byref(o)))
+    if wsb == 0:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "the matrix product has 2^30 or more term products")
+    ws = _ws(a_coef.device, workspace).get(max(wsb, 256))
+    with torch.cuda.device(a_coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_matmul_simplify(ctypes.byref(ba), m, k, ctypes.byref(bb), n, float(tol), ctypes.byref(o), out_coef.data_ptr(),
+                                           out_exps.data_ptr(), cap, out_off.ctypes.data, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    kk = int(out_off[-1])
+    res = (out_coef[:kk], out_exps[:kk], out_off)
     return (*res, _stats(st)) if return_stats else res
 
 

@@ -3,6 +3,7 @@
 // No step of the path runs on the host; the host only sizes and launches.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "kernels.h"
@@ -365,10 +366,13 @@ static bool small_eligible(int64_t n, const Plan& plan, const Opts& o)
     return !(o.flags & (POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE | (0xfu << POLYLAB_FLAG_DEBUG_NFAST_SHIFT)));
 }
 
+// Batched calls (batch.cu): after the segmented sum, count the survivors of every entry (the key's top field).
+struct BatchOut { int entry_shift; uint32_t* counts; };
+
 static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
-                            const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr)
+                            const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr, const BatchOut* batch = nullptr)
 {
     if (k_bucket > 0)
         return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
@@ -382,6 +386,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     if (small) {
         tm.mark(POLYLAB_STAGE_SORT);
         *launches += launch_block_sort_reduce(plan, kbuf[0], coef0, nullptr, (uint32_t)n, kbuf[1], cbuf[1], ctl, stream);
+        if (batch) *launches += launch_entry_count(plan.key_bytes, n, kbuf[1], cbuf[1], ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, kbuf[1], cbuf[1], tol, out_coef, out_exps, o.exp_bytes, out_capacity,
                                          (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
@@ -405,6 +410,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
         sc.tile_frag = (double*)(ws + L.red_frag);
         sc.tile_cont = (uint8_t*)(ws + L.red_cont);
         *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
+        if (batch) *launches += launch_entry_count(plan.key_bytes, n, ukeys, usums, ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
                                          (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
@@ -775,6 +781,207 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
         return mul_simplify_once(a, b, tol, opts, out_coef, out_exps, out_capacity, out_nterms, workspace, workspace_bytes,
                                  cuda_stream, at);
     });
+}
+
+// ------------------------------------------------------------------------------- batched (N3)
+
+// Plan of a batched call: make_plan over (entry, variables) -- the entry index is "variable -1", the most significant field --
+// then the entry field is dropped from the variable tables (S5 unpacks variables only).
+static int make_batched_plan(int nvars, const uint64_t* m, const uint32_t* bound, int64_t nentries, Plan* plan, int* entry_shift)
+{
+    uint64_t m2[kMaxVars];
+    uint32_t b2[kMaxVars];
+    m2[0] = nentries > 1 ? (uint64_t)(nentries - 1) : 1u;        // at least one bit, so that shifting by entry_shift is defined
+    b2[0] = (uint32_t)m2[0];
+    for (int v = 0; v < nvars; ++v) { m2[v + 1] = m[v]; b2[v + 1] = bound[v]; }
+    Plan full;
+    const int rc = make_plan(nvars + 1, m2, b2, &full);
+    if (rc != POLYLAB_OK) return rc;
+    *plan = full;
+    plan->nvars = nvars;
+    for (int v = 0; v < nvars; ++v) { plan->shift[v] = full.shift[v + 1]; plan->width[v] = full.width[v + 1]; plan->bound[v] = full.bound[v + 1]; }
+    plan->shift[nvars] = 0; plan->width[nvars] = 0; plan->bound[nvars] = 0;
+    *entry_shift = full.shift[0];
+    return POLYLAB_OK;
+}
+
+static int batch_args_ok(const polylab_batch* p, const polylab_opts* opts)
+{
+    if (!p || p->nvars < 1 || p->nvars > POLYLAB_MAX_NVARS - 1 || p->nentries < 0 || p->nentries >= POLYLAB_MAX_TERMS) return 0;
+    if (p->nentries > 0 && !p->offsets_host) return 0;
+    if (opts && (opts->max_exp_host || (opts->flags & POLYLAB_FLAG_DEVICE_COUNT) || opts->term_stride != 0 || opts->var_stride != 0)) return 0;
+    int64_t prev = 0;
+    for (int64_t e = 0; e <= p->nentries && p->nentries > 0; ++e) {
+        if (p->offsets_host[e] < prev || (e == 0 && p->offsets_host[0] != 0)) return 0;
+        prev = p->offsets_host[e];
+    }
+    if (prev >= POLYLAB_MAX_TERMS) return 0;
+    if (prev > 0 && (!p->coef || !p->exps)) return 0;
+    return 1;
+}
+
+struct BatchLayout { size_t inner_bytes, segs, counts, total; };
+static BatchLayout batch_layout(int64_t n, int64_t na, int64_t nb, int64_t nseg, int64_t nentries)
+{
+    BatchLayout B;
+    B.inner_bytes = worst_layout_bytes(n, na, nb);
+    size_t off = align_up(B.inner_bytes);
+    B.segs = off; off = align_up(off + (size_t)(nseg + 1) * sizeof(BatchSeg));
+    B.counts = off; off = align_up(off + (size_t)(nentries + 1) * sizeof(uint32_t));
+    B.total = off + 256;
+    return B;
+}
+
+// The shared body: operands a (and b for products) are packed with one plan, the segments' records are materialised with
+// the entry index on top, and the ordinary tail (one-block path or LSD passes, segmented sum, prune, unpack) runs once.
+static int batched_run(const polylab_batch* a, const polylab_batch* b, const BatchSeg* segs_host, int64_t nseg, int64_t n,
+                       int64_t nentries, double tol, const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                       int64_t* out_offsets_host, void* workspace, size_t workspace_bytes, void* cuda_stream, const Attempt& at)
+{
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const int nvars = a->nvars;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    for (int64_t e = 0; e <= nentries; ++e) out_offsets_host[e] = 0;
+    if (n == 0) { if (o.stats) memset(o.stats, 0, sizeof *o.stats); return POLYLAB_OK; }
+    if (!workspace || (out_capacity > 0 && (!out_coef || !out_exps))) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int64_t na = a->nentries ? a->offsets_host[a->nentries] : 0, nb = b ? (b->nentries ? b->offsets_host[b->nentries] : 0) : 0;
+    unsigned char* ws = align_ptr(workspace);
+    const size_t avail = workspace_bytes >= (size_t)(ws - (unsigned char*)workspace) ? workspace_bytes - (ws - (unsigned char*)workspace) : 0;
+    const BatchLayout BL = batch_layout(n, na, nb, nseg, nentries);
+    if (avail < BL.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    int launches = 0;
+    Control* ctl = (Control*)ws;
+    Timing tm;
+    tm.begin((o.flags & POLYLAB_FLAG_TIMING) && o.stats, stream);
+    const ExpView eva = make_view(a->exps, o, nvars);
+    ExpView evb = eva;
+    if (b) evb = make_view(b->exps, o, nvars);
+
+    // ---- S0 over all terms of the operand(s); for products the fields are sized for max_a + max_b
+    PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
+    launches += launch_bounds(eva, na, nvars, ctl, 0, stream);
+    if (b) launches += launch_bounds(evb, nb, nvars, ctl, 1, stream);
+    uint32_t mh[2][kMaxVars];
+    PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp, sizeof mh, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    uint64_t m[kMaxVars];
+    uint32_t ba[kMaxVars], bb[kMaxVars];
+    const uint32_t emax = exp_max_of(o.exp_bytes);
+    for (int v = 0; v < nvars; ++v) {
+        ba[v] = mh[0][v]; bb[v] = b ? mh[1][v] : 0u;
+        m[v] = (uint64_t)ba[v] + bb[v];
+        if (m[v] > emax) return POLYLAB_ERR_EXPONENT_RANGE;           // a product's exponent sums must fit exp_type (A8)
+    }
+    tm.mark(POLYLAB_STAGE_BOUNDS);
+    Plan plan_a, plan_b;
+    int entry_shift = 0;
+    rc = make_batched_plan(nvars, m, ba, nentries, &plan_a, &entry_shift);
+    if (rc != POLYLAB_OK) return rc;
+    make_batched_plan(nvars, m, bb, nentries, &plan_b, &entry_shift);
+    fill_stats(o.stats, plan_a, n);
+
+    const Layout L = make_layout(n, plan_a.key_bytes, na, nb);
+    if (L.total > BL.inner_bytes) return POLYLAB_ERR_INTERNAL;
+    PL_CUDA(cudaMemsetAsync(ws, 0, L.zero_end, stream));
+    BatchSeg* segs = (BatchSeg*)(ws + BL.segs);
+    uint32_t* counts = (uint32_t*)(ws + BL.counts);
+    PL_CUDA(cudaMemcpyAsync(segs, segs_host, (size_t)nseg * sizeof(BatchSeg), cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemsetAsync(counts, 0, (size_t)(nentries + 1) * sizeof(uint32_t), stream));
+
+    // ---- S1 on the operands (monomial fields only), then the records with the entry index on top (+ X1 for products)
+    launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, -1, stream);
+    if (b) launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, -1, stream);
+    launches += launch_batched_expand(plan_a, segs, (uint32_t)nseg, n, ws + L.ka, a->coef, b ? ws + L.kb : nullptr, b ? b->coef : nullptr,
+                                      entry_shift, ws + L.keys[0], (double*)(ws + L.coefs[0]), ctl, stream);
+    tm.mark(POLYLAB_STAGE_PACK);
+    const BatchOut bo = {entry_shift, counts};
+    Opts o2 = o;
+    o2.flags |= POLYLAB_FLAG_NO_BUCKET | POLYLAB_FLAG_NO_TABLE;
+    int64_t total = 0;
+    rc = sort_reduce_emit(plan_a, 0, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o2, out_coef, out_exps, out_capacity, &total,
+                          &launches, tm, at.safe_rank, stream, nullptr, nullptr, &bo);
+    if (rc != POLYLAB_OK && rc != POLYLAB_ERR_OUTPUT_TOO_SMALL) return rc;
+    // ---- offsets: prefix sums of the entries' survivor counts (nentries values, on the host)
+    uint32_t* hc = (uint32_t*)malloc((size_t)(nentries + 1) * sizeof(uint32_t));
+    if (!hc) return POLYLAB_ERR_INTERNAL;
+    if (cuda_failed(cudaMemcpyAsync(hc, counts, (size_t)nentries * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream), "copy of the entry counts") ||
+        cuda_failed(cudaStreamSynchronize(stream), "cudaStreamSynchronize")) { free(hc); return POLYLAB_ERR_CUDA; }
+    int64_t run = 0;
+    for (int64_t e = 0; e < nentries; ++e) { out_offsets_host[e] = run; run += hc[e]; }
+    out_offsets_host[nentries] = run;
+    free(hc);
+    if (run != total) return POLYLAB_ERR_INTERNAL;
+    return rc;
+}
+
+size_t polylab_simplify_batched_workspace_bytes(int64_t nterms, int64_t nentries, int32_t nvars, const polylab_opts* opts)
+{
+    (void)nvars; (void)opts;
+    if (nterms < 0 || nentries < 0 || nterms >= POLYLAB_MAX_TERMS) return 0;
+    return batch_layout(nterms, nterms, 0, nentries, nentries).total;
+}
+
+int polylab_simplify_batched(const polylab_batch* p, double tol, const polylab_opts* opts, double* out_coef, void* out_exps,
+                             int64_t out_capacity, int64_t* out_offsets_host, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!batch_args_ok(p, opts) || !(tol >= 0.0) || isinf(tol) || !out_offsets_host || out_capacity < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int64_t ne = p->nentries, n = ne ? p->offsets_host[ne] : 0;
+    BatchSeg* segs = (BatchSeg*)malloc((size_t)(ne + 1) * sizeof(BatchSeg));
+    if (!segs) return POLYLAB_ERR_INTERNAL;
+    int64_t nseg = 0;
+    for (int64_t e = 0; e < ne; ++e) {                               // one segment per non-empty entry: its raw terms
+        const int64_t t0 = p->offsets_host[e], t1 = p->offsets_host[e + 1];
+        if (t1 > t0) { const BatchSeg s = {(uint32_t)t0, (uint32_t)t0, (uint32_t)(t1 - t0), 0u, 0u, (uint32_t)e}; segs[nseg++] = s; }
+    }
+    const int rc = run_attempts(opts, [&](const Attempt& at) {
+        return batched_run(p, nullptr, segs, nseg, n, ne, tol, opts, out_coef, out_exps, out_capacity, out_offsets_host, workspace,
+                           workspace_bytes, cuda_stream, at);
+    });
+    free(segs);
+    return rc;
+}
+
+size_t polylab_matmul_simplify_workspace_bytes(int64_t nproducts, int64_t a_nterms, int64_t b_nterms, int64_t m, int64_t k, int64_t n,
+                                               int32_t nvars, const polylab_opts* opts)
+{
+    (void)nvars; (void)opts;
+    if (nproducts < 0 || nproducts >= POLYLAB_MAX_TERMS || a_nterms < 0 || b_nterms < 0 || m < 0 || k < 0 || n < 0) return 0;
+    if (m * n >= POLYLAB_MAX_TERMS || (k > 0 && m * n > POLYLAB_MAX_TERMS / k)) return 0;
+    return batch_layout(nproducts, a_nterms, b_nterms, m * n * k, m * n).total;
+}
+
+int polylab_matmul_simplify(const polylab_batch* a, int32_t m, int32_t k, const polylab_batch* b, int32_t n, double tol,
+                            const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_offsets_host,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!batch_args_ok(a, opts) || !batch_args_ok(b, opts) || a->nvars != b->nvars || m < 0 || k < 0 || n < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (a->nentries != (int64_t)m * k || b->nentries != (int64_t)k * n) return POLYLAB_ERR_INVALID_ARGUMENT;
+    if (!(tol >= 0.0) || isinf(tol) || !out_offsets_host || out_capacity < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
+    const int64_t ne = (int64_t)m * n;
+    if (ne >= POLYLAB_MAX_TERMS || (k > 0 && ne > POLYLAB_MAX_TERMS / k)) return POLYLAB_ERR_INVALID_ARGUMENT;
+    BatchSeg* segs = (BatchSeg*)malloc((size_t)(ne * k + 1) * sizeof(BatchSeg));
+    if (!segs) return POLYLAB_ERR_INTERNAL;
+    int64_t nseg = 0, nprod = 0;
+    for (int i = 0; i < m; ++i)
+        for (int j = 0; j < n; ++j)
+            for (int l = 0; l < k; ++l) {                            // C(i,j) += A(i,l) * B(l,j): one segment of products
+                const int64_t a0 = a->offsets_host[(int64_t)i * k + l], a1 = a->offsets_host[(int64_t)i * k + l + 1];
+                const int64_t b0 = b->offsets_host[(int64_t)l * n + j], b1 = b->offsets_host[(int64_t)l * n + j + 1];
+                const int64_t cnt = (a1 - a0) * (b1 - b0);
+                if (cnt == 0) continue;
+                if (nprod + cnt >= POLYLAB_MAX_TERMS) { free(segs); return POLYLAB_ERR_INVALID_ARGUMENT; }
+                const BatchSeg s = {(uint32_t)nprod, (uint32_t)a0, (uint32_t)(a1 - a0), (uint32_t)b0, (uint32_t)(b1 - b0), (uint32_t)((int64_t)i * n + j)};
+                segs[nseg++] = s;
+                nprod += cnt;
+            }
+    const int rc = run_attempts(opts, [&](const Attempt& at) {
+        return batched_run(a, b, segs, nseg, nprod, ne, tol, opts, out_coef, out_exps, out_capacity, out_offsets_host, workspace,
+                           workspace_bytes, cuda_stream, at);
+    });
+    free(segs);
+    return rc;
 }
 
 // ------------------------------------------------------------------------------- powers (N2)

@@ -147,6 +147,18 @@ inline int small_cap(int key_bytes) { return key_bytes == 8 ? kSmallCap : kSmall
 int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
                              void* ukeys, double* usums, Control* ctl, cudaStream_t stream);
 
+// Batched simplify (batch.cu): the records of all entries, keyed (entry, monomial).
+struct BatchSeg {
+    uint32_t start;         // number of the segment's first record
+    uint32_t a0, na;        // terms [a0, a0 + na) of the packed operand A (or of the packed polynomial when nb == 0)
+    uint32_t b0, nb;        // terms [b0, b0 + nb) of B: the segment holds the na * nb products; nb == 0: the na raw terms
+    uint32_t entry;         // the polynomial (matrix entry) the segment's records belong to
+};
+int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, const double* ca,
+                          const void* kb, const double* cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
+int launch_entry_count(int key_bytes, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
+                       int entry_shift, uint32_t* counts, cudaStream_t stream);
+
 // Table path (table.cu): merge like terms in a dense or hash table before any sort.
 struct __align__(16) TableSlot {
     uint64_t key1;          // packed key + 1; 0 = empty

@@ -29,7 +29,9 @@ def test_header_symbols_exported(L):
     names = _declared_functions()
     assert {"polylab_simplify", "polylab_mul_simplify", "polylab_expand", "polylab_pack_keys", "polylab_simplify_host",
             "polylab_mul_simplify_host", "polylab_simplify_workspace_bytes", "polylab_mul_simplify_workspace_bytes",
-            "polylab_status_string", "polylab_version", "polylab_pow_simplify", "polylab_pow_simplify_workspace_bytes"} <= set(names)
+            "polylab_status_string", "polylab_version", "polylab_pow_simplify", "polylab_pow_simplify_workspace_bytes",
+            "polylab_simplify_batched", "polylab_simplify_batched_workspace_bytes", "polylab_matmul_simplify",
+            "polylab_matmul_simplify_workspace_bytes"} <= set(names)
     for n in names:
         assert hasattr(L, n), f"{n} declared in include/polylab.h but not exported"
 
@@ -117,6 +119,27 @@ def test_host_side_argument_errors(L):
     cnt.value = -7
     assert g(ctypes.byref(pa), ctypes.byref(pb), 0.0, None, one, one, 25, ctypes.addressof(cnt), one, 1 << 20, None) == B.OK
     assert cnt.value == 0
+
+
+def test_batched_host_side_checks(L):
+    """Batched entry points: argument errors are found on the host (no GPU needed); an all-empty batch returns zero offsets."""
+    from paper_2604_06575_b200 import binding as B
+    off = (ctypes.c_int64 * 4)(0, 0, 0, 0)
+    out_off = (ctypes.c_int64 * 4)(7, 7, 7, 7)
+    b = B._Batch(None, None, off, 3, 2)
+    assert L.polylab_simplify_batched(ctypes.byref(b), 0.0, None, None, None, 0, out_off, None, 0, None) == B.OK
+    assert list(out_off) == [0, 0, 0, 0]
+    assert L.polylab_simplify_batched(ctypes.byref(b), -1.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
+    bad = (ctypes.c_int64 * 4)(0, 2, 1, 3)                       # decreasing offsets
+    b2 = B._Batch(1, 1, bad, 3, 2)
+    assert L.polylab_simplify_batched(ctypes.byref(b2), 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
+    b3 = B._Batch(None, None, off, 3, 128)                       # the entry index needs a field of its own: nvars <= 127
+    assert L.polylab_simplify_batched(ctypes.byref(b3), 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
+    # matrix product: A must have m*k entries, B k*n
+    assert L.polylab_matmul_simplify(ctypes.byref(b), 2, 2, ctypes.byref(b), 2, 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
+    assert L.polylab_matmul_simplify(ctypes.byref(b), 1, 3, ctypes.byref(b), 1, 0.0, None, None, None, 0, out_off, None, 0, None) == B.OK
+    assert L.polylab_simplify_batched_workspace_bytes(1000, 9, 3, None) > L.polylab_simplify_workspace_bytes(1000, 3, None)
+    assert L.polylab_matmul_simplify_workspace_bytes(1 << 30, 10, 10, 3, 3, 3, 3, None) == 0
 
 
 def test_pow_simplify_host_side_checks(L):
