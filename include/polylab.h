@@ -42,16 +42,16 @@ extern "C" {
 #pragma GCC visibility push(default)
 #endif
 
-#define POLYLAB_VERSION 100          /* 0.1.0 */
-#define POLYLAB_MAX_NVARS 128        /* packed keys hold at most 128 bits (reading A9) */
+#define POLYLAB_VERSION 110          /* 0.1.1 */
+#define POLYLAB_MAX_NVARS 256        /* packed keys hold at most 256 bits (reading A9) */
 #define POLYLAB_MAX_TERMS ((int64_t)1 << 30)   /* exclusive bound on nterms and on na*nb */
-#define POLYLAB_SMALL_WORKSPACE_BYTES 32768    /* workspace of polylab_expand and polylab_pack_keys */
+#define POLYLAB_SMALL_WORKSPACE_BYTES 65536    /* workspace of polylab_expand and polylab_pack_keys */
 
 typedef enum {
     POLYLAB_OK = 0,
     POLYLAB_ERR_INVALID_ARGUMENT = 1,   /* null pointer with work to do, nvars < 1 or > MAX_NVARS, nterms < 0 or
                                            >= MAX_TERMS, tol NaN or < 0, unknown exp_type, nvars mismatch */
-    POLYLAB_ERR_KEY_TOO_WIDE = 2,       /* sum over variables of bitlen(max exponent) > 128 */
+    POLYLAB_ERR_KEY_TOO_WIDE = 2,       /* sum over variables of bitlen(max exponent) > 256 (polylab_pack_keys: > 128) */
     POLYLAB_ERR_EXPONENT_RANGE = 3,     /* an exponent exceeds the caller's max_exp_host bound, or a product's
                                            exponent sum does not fit exp_type */
     POLYLAB_ERR_WORKSPACE_TOO_SMALL = 4,
@@ -122,9 +122,9 @@ enum { POLYLAB_STAGE_BOUNDS = 0, POLYLAB_STAGE_PACK = 1, POLYLAB_STAGE_SORT = 2,
 /* Per-call statistics (HOST, optional): the plan that was chosen and what the pipeline saw. */
 typedef struct polylab_stats {
     int32_t key_bits;        /* B = sum of field widths                                  */
-    int32_t key_bytes;       /* W = 8 or 16                                              */
+    int32_t key_bytes;       /* W = 8, 16 or 32 (one, two or four 64-bit words)           */
     int32_t sort_passes;     /* P radix passes executed                                  */
-    int32_t digit_bits[16];  /* width of each digit of the key, least significant first   */
+    int32_t digit_bits[32];  /* width of each digit of the key, least significant first   */
     int64_t sort_terms;      /* N = terms that entered the sort (na*nb for a product)    */
     int64_t distinct;        /* U = distinct monomials before pruning (-1 with DEVICE_COUNT) */
     int64_t survivors;       /* U' (-1 with DEVICE_COUNT)                                */
@@ -226,7 +226,7 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
  * canonical monomial order, in out_coef[out_capacity] / out_exps[out_capacity x nvars] (DEVICE); out_offsets_host (HOST,
  * nentries + 1 values) receives where each entry starts (out_offsets_host[nentries] = total number of terms).  Survivors
  * beyond out_capacity -> POLYLAB_ERR_OUTPUT_TOO_SMALL with out_offsets_host filled in.  Exponents: row-major, opts->exp_type;
- * opts->max_exp_host, strides and POLYLAB_FLAG_DEVICE_COUNT are not supported (POLYLAB_ERR_INVALID_ARGUMENT); nvars <= 127.
+ * opts->max_exp_host, strides and POLYLAB_FLAG_DEVICE_COUNT are not supported (POLYLAB_ERR_INVALID_ARGUMENT); nvars <= 255.
  * The calls synchronise the stream.
  */
 typedef struct polylab_batch {

@@ -37,9 +37,9 @@ FLAG_DEBUG_FORCE_BUCKET = 0x20000000
 FLAG_DEBUG_UNSTABLE = 0x40000000
 FLAG_DEBUG_NFAST_SHIFT = 8
 STAGES = ("bounds", "pack", "sort", "reduce", "prune")
-MAX_NVARS = 128
+MAX_NVARS = 256
 MAX_TERMS = 1 << 30
-SMALL_WORKSPACE_BYTES = 32768
+SMALL_WORKSPACE_BYTES = 65536
 
 
 class PolylabError(RuntimeError):
@@ -50,7 +50,7 @@ class PolylabError(RuntimeError):
 
 class _Stats(ctypes.Structure):
     _fields_ = [("key_bits", ctypes.c_int32), ("key_bytes", ctypes.c_int32), ("sort_passes", ctypes.c_int32),
-                ("digit_bits", ctypes.c_int32 * 16), ("sort_terms", ctypes.c_int64), ("distinct", ctypes.c_int64),
+                ("digit_bits", ctypes.c_int32 * 32), ("sort_terms", ctypes.c_int64), ("distinct", ctypes.c_int64),
                 ("survivors", ctypes.c_int64), ("kernel_launches", ctypes.c_int32), ("rank_fallback", ctypes.c_int32),
                 ("stage_ms", ctypes.c_float * 8), ("prefix_passes", ctypes.c_int32), ("bucket_fallback", ctypes.c_int32),
                 ("refinish_tiles", ctypes.c_int32), ("plan_digits", ctypes.c_int32), ("bounds_sampled", ctypes.c_int32),

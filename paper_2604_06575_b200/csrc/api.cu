@@ -95,14 +95,14 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
     for (int v = nvars - 1; v >= 0; --v) {
         const int w = bitlen(m[v]);
         if (w > 32) return POLYLAB_ERR_EXPONENT_RANGE;
-        if (bits + w > 128) return POLYLAB_ERR_KEY_TOO_WIDE;
+        if (bits + w > 256) return POLYLAB_ERR_KEY_TOO_WIDE;
         plan->shift[v] = (uint8_t)(w ? bits : 0);
         plan->width[v] = (uint8_t)w;
         plan->bound[v] = bound[v];
         bits += w;
     }
     plan->key_bits = bits;
-    plan->key_bytes = bits <= 64 ? 8 : 16;
+    plan->key_bytes = bits <= 64 ? 8 : bits <= 128 ? 16 : 32;
     // Digits: each 32-bit word of the key is split into ceil(bits_in_word / 8) digits of balanced width, so no digit
     // straddles a word (one shift + mask per digit) and the pass count is still ceil(B / 8).
     int P = 0;
@@ -195,10 +195,23 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     return L;
 }
 
-static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb)
+// Widest key a call can need: every variable's field is at most as wide as its exponent type (a product's sums must fit
+// that type too), plus `extra_bits` (the entry field of a batched call).
+static int max_key_bytes(int nvars, const polylab_opts* opts, int extra_bits = 0)
 {
-    const size_t a = make_layout(n, 8, na, nb).total, b = make_layout(n, 16, na, nb).total;
-    return (a > b ? a : b) + 256;                       // + slack to align the caller's base pointer
+    const int es = (opts && opts->exp_type) ? opts->exp_type : 4;
+    const int64_t bits = (int64_t)nvars * 8 * es + extra_bits;
+    return bits <= 64 ? 8 : bits <= 128 ? 16 : 32;
+}
+
+static size_t worst_layout_bytes(int64_t n, int64_t na, int64_t nb, int widest_key_bytes = 32)
+{
+    size_t best = 0;
+    for (int kb = 8; kb <= widest_key_bytes; kb *= 2) {
+        const size_t t = make_layout(n, kb, na, nb).total;
+        best = t > best ? t : best;
+    }
+    return best + 256;                                  // + slack to align the caller's base pointer
 }
 
 static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
@@ -261,6 +274,7 @@ static int choose_prefix_passes(const Plan& plan, int64_t n, const Opts& o, cons
     const bool force = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET) != 0;
     if (!at.allow_bucket || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_BUCKET | POLYLAB_FLAG_DEVICE_COUNT))) return 0;
     const int P = plan.npasses;
+    if (plan.key_bytes > 16) return 0;                  // finish.cu handles one- and two-word keys
     if (P < 1 || (!force && (P < 4 || n < (1 << 20)))) return 0;
     for (int k = 1; k <= P; ++k) {
         const int T = plan.key_bits - plan.digit_pos[P - k];
@@ -386,7 +400,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     if (small) {
         tm.mark(POLYLAB_STAGE_SORT);
         *launches += launch_block_sort_reduce(plan, kbuf[0], coef0, nullptr, (uint32_t)n, kbuf[1], cbuf[1], ctl, stream);
-        if (batch) *launches += launch_entry_count(plan.key_bytes, n, kbuf[1], cbuf[1], ctl, tol, batch->entry_shift, batch->counts, stream);
+        if (batch) *launches += launch_entry_count(plan.key_bytes, plan.key_bits, n, kbuf[1], cbuf[1], ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, kbuf[1], cbuf[1], tol, out_coef, out_exps, o.exp_bytes, out_capacity,
                                          (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
@@ -410,7 +424,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
         sc.tile_frag = (double*)(ws + L.red_frag);
         sc.tile_cont = (uint8_t*)(ws + L.red_cont);
         *launches += launch_reduce(plan.key_bytes, n, skeys, scoef, ukeys, usums, sc, ctl, stream);
-        if (batch) *launches += launch_entry_count(plan.key_bytes, n, ukeys, usums, ctl, tol, batch->entry_shift, batch->counts, stream);
+        if (batch) *launches += launch_entry_count(plan.key_bytes, plan.key_bits, n, ukeys, usums, ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
                                          (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
@@ -549,17 +563,15 @@ static int opts_exp_bytes(const polylab_opts* opts) { return (opts && opts->exp_
 
 size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
 {
-    (void)nvars; (void)opts;
-    if (nterms < 0) return 0;
-    return worst_layout_bytes(nterms, 0, 0);
+    if (nterms < 0 || nvars < 1) return 0;
+    return worst_layout_bytes(nterms, 0, 0, max_key_bytes(nvars, opts));
 }
 
 size_t polylab_mul_simplify_workspace_bytes(int64_t na, int64_t nb, int32_t nvars, const polylab_opts* opts)
 {
-    (void)nvars; (void)opts;
-    if (na < 0 || nb < 0) return 0;
+    if (na < 0 || nb < 0 || nvars < 1) return 0;
     if (na > 0 && nb > 0 && na >= POLYLAB_MAX_TERMS / nb + 1) return 0;
-    return worst_layout_bytes(na * nb, na, nb);
+    return worst_layout_bytes(na * nb, na, nb, max_key_bytes(nvars, opts));
 }
 
 static int simplify_once(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
@@ -821,10 +833,10 @@ static int batch_args_ok(const polylab_batch* p, const polylab_opts* opts)
 }
 
 struct BatchLayout { size_t inner_bytes, segs, counts, total; };
-static BatchLayout batch_layout(int64_t n, int64_t na, int64_t nb, int64_t nseg, int64_t nentries)
+static BatchLayout batch_layout(int64_t n, int64_t na, int64_t nb, int64_t nseg, int64_t nentries, int widest_key_bytes)
 {
     BatchLayout B;
-    B.inner_bytes = worst_layout_bytes(n, na, nb);
+    B.inner_bytes = worst_layout_bytes(n, na, nb, widest_key_bytes);
     size_t off = align_up(B.inner_bytes);
     B.segs = off; off = align_up(off + (size_t)(nseg + 1) * sizeof(BatchSeg));
     B.counts = off; off = align_up(off + (size_t)(nentries + 1) * sizeof(uint32_t));
@@ -849,7 +861,7 @@ static int batched_run(const polylab_batch* a, const polylab_batch* b, const Bat
     const int64_t na = a->nentries ? a->offsets_host[a->nentries] : 0, nb = b ? (b->nentries ? b->offsets_host[b->nentries] : 0) : 0;
     unsigned char* ws = align_ptr(workspace);
     const size_t avail = workspace_bytes >= (size_t)(ws - (unsigned char*)workspace) ? workspace_bytes - (ws - (unsigned char*)workspace) : 0;
-    const BatchLayout BL = batch_layout(n, na, nb, nseg, nentries);
+    const BatchLayout BL = batch_layout(n, na, nb, nseg, nentries, max_key_bytes(nvars, opts, 30));
     if (avail < BL.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     int launches = 0;
     Control* ctl = (Control*)ws;
@@ -918,9 +930,8 @@ static int batched_run(const polylab_batch* a, const polylab_batch* b, const Bat
 
 size_t polylab_simplify_batched_workspace_bytes(int64_t nterms, int64_t nentries, int32_t nvars, const polylab_opts* opts)
 {
-    (void)nvars; (void)opts;
-    if (nterms < 0 || nentries < 0 || nterms >= POLYLAB_MAX_TERMS) return 0;
-    return batch_layout(nterms, nterms, 0, nentries, nentries).total;
+    if (nterms < 0 || nentries < 0 || nterms >= POLYLAB_MAX_TERMS || nvars < 1) return 0;
+    return batch_layout(nterms, nterms, 0, nentries, nentries, max_key_bytes(nvars, opts, 30)).total;
 }
 
 int polylab_simplify_batched(const polylab_batch* p, double tol, const polylab_opts* opts, double* out_coef, void* out_exps,
@@ -946,10 +957,9 @@ int polylab_simplify_batched(const polylab_batch* p, double tol, const polylab_o
 size_t polylab_matmul_simplify_workspace_bytes(int64_t nproducts, int64_t a_nterms, int64_t b_nterms, int64_t m, int64_t k, int64_t n,
                                                int32_t nvars, const polylab_opts* opts)
 {
-    (void)nvars; (void)opts;
-    if (nproducts < 0 || nproducts >= POLYLAB_MAX_TERMS || a_nterms < 0 || b_nterms < 0 || m < 0 || k < 0 || n < 0) return 0;
+    if (nproducts < 0 || nproducts >= POLYLAB_MAX_TERMS || a_nterms < 0 || b_nterms < 0 || m < 0 || k < 0 || n < 0 || nvars < 1) return 0;
     if (m * n >= POLYLAB_MAX_TERMS || (k > 0 && m * n > POLYLAB_MAX_TERMS / k)) return 0;
-    return batch_layout(nproducts, a_nterms, b_nterms, m * n * k, m * n).total;
+    return batch_layout(nproducts, a_nterms, b_nterms, m * n * k, m * n, max_key_bytes(nvars, opts, 30)).total;
 }
 
 int polylab_matmul_simplify(const polylab_batch* a, int32_t m, int32_t k, const polylab_batch* b, int32_t n, double tol,
@@ -1121,6 +1131,8 @@ int polylab_pack_keys(const void* exps, int64_t nterms, int32_t nvars, const pol
     rc = make_plan(nvars, m, bound, &plan);
     if (rc != POLYLAB_OK) return rc;
     if (key_bits_host) *key_bits_host = plan.key_bits;
+    if (plan.key_bits > 128) return POLYLAB_ERR_KEY_TOO_WIDE;          // this entry point's output format is (hi, lo)
+    plan.key_bytes = 16;
     launch_pack_hilo(ev, nterms, plan, out_keys, ctl, stream);
     PL_CUDA(cudaGetLastError());
     int32_t status = 0;
@@ -1249,7 +1261,7 @@ const char* polylab_status_string(int status)
     switch (status) {
     case POLYLAB_OK: return "ok";
     case POLYLAB_ERR_INVALID_ARGUMENT: return "invalid argument";
-    case POLYLAB_ERR_KEY_TOO_WIDE: return "packed key wider than 128 bits";
+    case POLYLAB_ERR_KEY_TOO_WIDE: return "packed key wider than 256 bits";
     case POLYLAB_ERR_EXPONENT_RANGE: return "exponent out of range";
     case POLYLAB_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case POLYLAB_ERR_OUTPUT_TOO_SMALL: return "output capacity too small";

@@ -14,22 +14,9 @@
 
 namespace polylab {
 
-__device__ __forceinline__ uint64_t entry_key(uint64_t k, uint32_t entry, int shift) { return k | ((uint64_t)entry << shift); }
-__device__ __forceinline__ Key128 entry_key(Key128 k, uint32_t entry, int shift)
-{
-    if (shift >= 64) k.hi |= (uint64_t)entry << (shift - 64);
-    else {
-        k.lo |= (uint64_t)entry << shift;
-        if (shift > 32) k.hi |= (uint64_t)entry >> (64 - shift);
-    }
-    return k;
-}
-__device__ __forceinline__ uint32_t key_entry(uint64_t k, int shift) { return (uint32_t)(k >> shift); }
-__device__ __forceinline__ uint32_t key_entry(const Key128& k, int shift)
-{
-    if (shift >= 64) return (uint32_t)(k.hi >> (shift - 64));
-    return (uint32_t)((k.lo >> shift) | (shift ? (k.hi << (64 - shift)) : 0ull));
-}
+// the entry index is one more field of the key, above variable 0 (at most 30 bits: nentries < 2^30)
+template <typename K> __device__ __forceinline__ K entry_key(K k, uint32_t entry, int shift) { key_or_field(k, entry, shift); return k; }
+template <typename K> __device__ __forceinline__ uint32_t key_entry(const K& k, int shift, int width) { return key_get_field(k, shift, width); }
 
 template <typename K>
 __global__ void __launch_bounds__(256) batched_expand_kernel(const BatchSeg* __restrict__ segs, uint32_t nseg, uint32_t n,
@@ -81,30 +68,35 @@ int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg,
     if (plan.key_bytes == 8)
         batched_expand_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>(segs, nseg, (uint32_t)n, (const uint64_t*)ka, ca, (const uint64_t*)kb,
                                                                             cb, entry_shift, (uint64_t*)keys, coefs, dpos, dmask, ctl->hist[0]);
-    else
+    else if (plan.key_bytes == 16)
         batched_expand_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>(segs, nseg, (uint32_t)n, (const Key128*)ka, ca, (const Key128*)kb, cb,
                                                                           entry_shift, (Key128*)keys, coefs, dpos, dmask, ctl->hist[0]);
+    else
+        batched_expand_kernel<Key256><<<(unsigned)blocks, 256, 0, stream>>>(segs, nseg, (uint32_t)n, (const Key256*)ka, ca, (const Key256*)kb, cb,
+                                                                          entry_shift, (Key256*)keys, coefs, dpos, dmask, ctl->hist[0]);
     return 1;
 }
 
 // survivors per entry, from the merged (key, sum) list (the prune predicate of S4, reading A2)
 template <typename K>
 __global__ void __launch_bounds__(256) entry_count_kernel(const K* __restrict__ ukeys, const double* __restrict__ usums, const Control* ctl,
-                                                          double tol, int entry_shift, uint32_t* __restrict__ counts)
+                                                          double tol, int entry_shift, int entry_bits, uint32_t* __restrict__ counts)
 {
     const uint32_t U = ctl->distinct;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < U; i += gridDim.x * blockDim.x)
-        if (fabs(usums[i]) > tol) atomicAdd(&counts[key_entry(ukeys[i], entry_shift)], 1u);
+        if (fabs(usums[i]) > tol) atomicAdd(&counts[key_entry(ukeys[i], entry_shift, entry_bits)], 1u);
 }
 
-int launch_entry_count(int key_bytes, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
+int launch_entry_count(int key_bytes, int key_bits, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
                        int entry_shift, uint32_t* counts, cudaStream_t stream)
 {
     if (max_units <= 0) return 0;
     int64_t blocks = (max_units + 1023) / 1024;
     if (blocks > sm_count() * 8) blocks = sm_count() * 8;
-    if (key_bytes == 8) entry_count_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)ukeys, usums, ctl, tol, entry_shift, counts);
-    else entry_count_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)ukeys, usums, ctl, tol, entry_shift, counts);
+    const int eb = key_bits - entry_shift;
+    if (key_bytes == 8) entry_count_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)ukeys, usums, ctl, tol, entry_shift, eb, counts);
+    else if (key_bytes == 16) entry_count_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)ukeys, usums, ctl, tol, entry_shift, eb, counts);
+    else entry_count_kernel<Key256><<<(unsigned)blocks, 256, 0, stream>>>((const Key256*)ukeys, usums, ctl, tol, entry_shift, eb, counts);
     return 1;
 }
 

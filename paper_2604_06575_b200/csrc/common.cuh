@@ -15,7 +15,7 @@
 namespace polylab {
 
 constexpr int kMaxVars = POLYLAB_MAX_NVARS;
-constexpr int kMaxPasses = 16;          // 128 bits / 8-bit digits
+constexpr int kMaxPasses = 32;          // 256 bits / 8-bit digits
 constexpr int kRadixBits = 8;           // widest digit
 constexpr int kRadix = 1 << kRadixBits; // bins per pass
 constexpr unsigned kFullMask = 0xffffffffu;
@@ -27,10 +27,77 @@ struct __align__(16) Key128 {
     uint64_t hi, lo;     // memory order (hi, lo): the layout polylab_pack_keys exposes
 };
 
+// 256-bit key for wide variable sets ("multi-word for wide variable sets"; the 500-variable sparse quartics
+// of PAPER.md:546 are the paper's own wide case): four 64-bit limbs, most significant first, like Key128's (hi, lo).
+struct __align__(32) Key256 {
+    uint64_t q[4];       // q[0] most significant
+};
+
 __host__ __device__ inline bool key_eq(uint64_t a, uint64_t b) { return a == b; }
 __host__ __device__ inline bool key_eq(const Key128& a, const Key128& b) { return a.lo == b.lo && a.hi == b.hi; }
 __host__ __device__ inline bool key_lt(uint64_t a, uint64_t b) { return a < b; }
 __host__ __device__ inline bool key_lt(const Key128& a, const Key128& b) { return a.hi < b.hi || (a.hi == b.hi && a.lo < b.lo); }
+
+__host__ __device__ inline bool key_eq(const Key256& a, const Key256& b) { return a.q[0] == b.q[0] && a.q[1] == b.q[1] && a.q[2] == b.q[2] && a.q[3] == b.q[3]; }
+__host__ __device__ inline bool key_lt(const Key256& a, const Key256& b)
+{
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+        if (a.q[i] != b.q[i]) return a.q[i] < b.q[i];
+    return a.q[3] < b.q[3];
+}
+__device__ __forceinline__ uint32_t key_word(const Key256& k, int wi)
+{
+    const int l = wi >> 1;                               // 64-bit limb, 0 = least significant
+    const uint64_t h = l == 0 ? k.q[3] : l == 1 ? k.q[2] : l == 2 ? k.q[1] : k.q[0];
+    return (wi & 1) ? (uint32_t)(h >> 32) : (uint32_t)h;
+}
+__device__ __forceinline__ Key256 key_add(const Key256& a, const Key256& b)
+{
+    Key256 r;
+    uint64_t carry = 0;
+#pragma unroll
+    for (int i = 3; i >= 0; --i) {                       // fields never carry into each other, limbs may
+        const uint64_t s = a.q[i] + b.q[i], t = s + carry;
+        carry = (s < a.q[i]) || (t < s) ? 1ull : 0ull;
+        r.q[i] = t;
+    }
+    return r;
+}
+__host__ __device__ inline bool same_prefix(const Key256& a, const Key256& b, int pos)
+{
+#pragma unroll
+    for (int l = 3; l >= 0; --l) {                       // limb l holds bits [64 l, 64 l + 64)
+        const uint64_t x = a.q[3 - l] ^ b.q[3 - l];
+        if (pos >= 64 * (l + 1)) break;
+        if (pos <= 64 * l) { if (x) return false; }
+        else return (x >> (pos - 64 * l)) == 0;
+    }
+    return true;
+}
+__device__ __forceinline__ void key_or_field(Key256& k, uint32_t e, int shift)
+{
+    const int l = shift >> 6, sh = shift & 63;
+    const uint64_t lo = (uint64_t)e << sh, hi = sh > 32 ? (uint64_t)e >> (64 - sh) : 0ull;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {                        // selects, not dynamically indexed registers
+        if (3 - i == l) k.q[i] |= lo;
+        if (3 - i == l + 1) k.q[i] |= hi;
+    }
+}
+__device__ __forceinline__ uint32_t key_get_field(const Key256& k, int shift, int width)
+{
+    if (width == 0) return 0u;
+    const int l = shift >> 6, sh = shift & 63;
+    uint64_t a = 0, b = 0;                               // limb l and the one above it
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (3 - i == l) a = k.q[i];
+        if (3 - i == l + 1) b = k.q[i];
+    }
+    const uint64_t w = sh == 0 ? a : ((a >> sh) | (b << (64 - sh)));
+    return (uint32_t)(w & ((width == 32) ? 0xffffffffull : ((1ull << width) - 1)));
+}
 
 // 32-bit word `wi` of a key (0 = least significant).  wi is uniform across a kernel: the selects cost 1-3 instructions.
 __device__ __forceinline__ uint32_t key_word(uint64_t k, int wi) { return wi ? (uint32_t)(k >> 32) : (uint32_t)k; }
@@ -43,6 +110,7 @@ __device__ __forceinline__ uint32_t key_word(const Key128& k, int wi)
 template <typename K> __host__ __device__ inline int key_word_byte_offset(int wi);
 template <> __host__ __device__ inline int key_word_byte_offset<uint64_t>(int wi) { return wi * 4; }
 template <> __host__ __device__ inline int key_word_byte_offset<Key128>(int wi) { return (wi ^ 2) * 4; }
+template <> __host__ __device__ inline int key_word_byte_offset<Key256>(int wi) { return (wi ^ 6) * 4; }
 
 // The digit of `mask`'s width at bit `pos` (0 = least significant).  The plan never lets a digit straddle a
 // 32-bit word (make_plan), so a digit is one shift and one mask of one word.
@@ -69,6 +137,7 @@ __host__ __device__ inline bool same_prefix(const Key128& a, const Key128& b, in
 template <typename K> __device__ __forceinline__ K key_max();
 template <> __device__ __forceinline__ uint64_t key_max<uint64_t>() { return ~0ull; }
 template <> __device__ __forceinline__ Key128 key_max<Key128>() { Key128 k; k.lo = ~0ull; k.hi = ~0ull; return k; }
+template <> __device__ __forceinline__ Key256 key_max<Key256>() { Key256 k; k.q[0] = k.q[1] = k.q[2] = k.q[3] = ~0ull; return k; }
 
 // OR `e << shift` into a key (shift + width <= key bits by construction of the plan)
 __device__ __forceinline__ void key_or_field(uint64_t& k, uint32_t e, int shift) { k |= (uint64_t)e << shift; }
@@ -100,6 +169,9 @@ __device__ __forceinline__ uint64_t key_top64(uint64_t k) { return k; }         
 __device__ __forceinline__ uint64_t key_top64(const Key128& k) { return k.hi; }
 __device__ __forceinline__ void key_zero(uint64_t& k) { k = 0; }
 __device__ __forceinline__ void key_zero(Key128& k) { k.lo = 0; k.hi = 0; }
+__device__ __forceinline__ void key_zero(Key256& k) { k.q[0] = k.q[1] = k.q[2] = k.q[3] = 0; }
+__device__ __forceinline__ void key_from_halves(Key256& k, uint64_t hi, uint64_t lo) { k.q[0] = hi; k.q[1] = 0; k.q[2] = 0; k.q[3] = lo; }   // (never used: no fused pack for 256-bit keys)
+__device__ __forceinline__ uint64_t key_top64(const Key256& k) { return k.q[0]; }
 
 // ------------------------------------------------------------------------------------ plan
 
@@ -108,7 +180,7 @@ __device__ __forceinline__ void key_zero(Key128& k) { k.lo = 0; k.hi = 0; }
 struct Plan {
     int32_t nvars;
     int32_t key_bits;                  // B
-    int32_t key_bytes;                 // W: 8 or 16
+    int32_t key_bytes;                 // W: 8, 16 or 32
     int32_t npasses;                   // P
     uint8_t shift[kMaxVars];           // bit position of field v
     uint8_t width[kMaxVars];           // w_v

@@ -11,6 +11,8 @@ namespace polylab {
 constexpr int kSortThreads64 = 256;
 constexpr int kSortThreads128 = 256;
 constexpr int kSortItems64 = 16;    // 4096-record tiles of (u64 key, f64 coef)
+constexpr int kSortThreads256 = 256;
+constexpr int kSortItems256 = 8;    // 2048-record tiles of (256-bit key, f64 coef): 64 KB of staging, three blocks per SM
 constexpr int kSortItems128 = 20;   // 5120-record tiles of (u128 key, f64 coef), two blocks per SM (swept on B200: 12x3 4.26, 16x2 4.08, 20x2 4.04, 24x2 4.74 ms for two passes of config 5)
 constexpr int kReduceThreads = 256;
 constexpr int kReduceItems = 9;     // odd: conflict-free blocked reads from shared memory
@@ -41,7 +43,10 @@ inline int sm_count()
     return cached[dev];
 }
 
-inline int sort_tile(int key_bytes) { return key_bytes == 8 ? kSortThreads64 * kSortItems64 : kSortThreads128 * kSortItems128; }
+inline int sort_tile(int key_bytes)
+{
+    return key_bytes == 8 ? kSortThreads64 * kSortItems64 : key_bytes == 16 ? kSortThreads128 * kSortItems128 : kSortThreads256 * kSortItems256;
+}
 constexpr int kReduceTile = kReduceThreads * kReduceItems;
 constexpr int kPruneTile = kPruneThreads * kPruneItems;
 
@@ -142,8 +147,8 @@ int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, 
 // in shared memory, segmented sum; (ukeys, usums)[U] ascending and ctl->distinct = U as launch_reduce leaves them (then
 // launch_prune_unpack).  Sets ctl->unsorted if its atomic ranking turned out unstable.
 // n_device (optional, DEVICE): the pair count is read on the device (clamped) instead of `n`.
-constexpr int kSmallCap = 8192;          // 64-bit keys; half of it for 128-bit keys
-inline int small_cap(int key_bytes) { return key_bytes == 8 ? kSmallCap : kSmallCap / 2; }
+constexpr int kSmallCap = 8192;          // 64-bit keys; 4096 for 128-bit keys, 2048 for 256-bit keys
+inline int small_cap(int key_bytes) { return kSmallCap * 8 / key_bytes; }
 int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
                              void* ukeys, double* usums, Control* ctl, cudaStream_t stream);
 
@@ -156,7 +161,7 @@ struct BatchSeg {
 };
 int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, const double* ca,
                           const void* kb, const double* cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
-int launch_entry_count(int key_bytes, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
+int launch_entry_count(int key_bytes, int key_bits, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
                        int entry_shift, uint32_t* counts, cudaStream_t stream);
 
 // Table path (table.cu): merge like terms in a dense or hash table before any sort.

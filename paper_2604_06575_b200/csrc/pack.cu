@@ -359,7 +359,8 @@ int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys,
                 cudaStream_t stream)
 {
     if (plan.key_bytes == 8) return launch_pack_t<uint64_t>(ev, nterms, plan, (uint64_t*)keys, ctl, hd, stream);
-    return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)keys, ctl, hd, stream);
+    if (plan.key_bytes == 16) return launch_pack_t<Key128>(ev, nterms, plan, (Key128*)keys, ctl, hd, stream);
+    return launch_pack_t<Key256>(ev, nterms, plan, (Key256*)keys, ctl, hd, stream);
 }
 
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
@@ -392,7 +393,8 @@ int launch_key_hist(const Plan& plan, int hd, int64_t n, const void* keys, Contr
     const int dpos = plan.digit_pos[hd];
     const uint32_t dmask = (1u << plan.digit_bits[hd]) - 1u;
     if (plan.key_bytes == 8) key_hist_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)keys, n, dpos, dmask, ctl->hist[hd]);
-    else key_hist_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)keys, n, dpos, dmask, ctl->hist[hd]);
+    else if (plan.key_bytes == 16) key_hist_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)keys, n, dpos, dmask, ctl->hist[hd]);
+    else key_hist_kernel<Key256><<<(unsigned)blocks, 256, 0, stream>>>((const Key256*)keys, n, dpos, dmask, ctl->hist[hd]);
     return 1;
 }
 
@@ -534,9 +536,12 @@ int launch_expand_packed(const void* ka, const double* ca, int64_t na, const voi
     if (plan.key_bytes == 8)
         expand_packed_kernel<uint64_t><<<blocks, 256, 0, stream>>>((const uint64_t*)ka, ca, (uint32_t)na, (const uint64_t*)kb,
                                                                    cb, (uint32_t)nb, (uint64_t*)keys, coefs, dpos, dmask, ctl->hist[hd]);
-    else
+    else if (plan.key_bytes == 16)
         expand_packed_kernel<Key128><<<blocks, 256, 0, stream>>>((const Key128*)ka, ca, (uint32_t)na, (const Key128*)kb, cb,
                                                                  (uint32_t)nb, (Key128*)keys, coefs, dpos, dmask, ctl->hist[hd]);
+    else
+        expand_packed_kernel<Key256><<<blocks, 256, 0, stream>>>((const Key256*)ka, ca, (uint32_t)na, (const Key256*)kb, cb,
+                                                                 (uint32_t)nb, (Key256*)keys, coefs, dpos, dmask, ctl->hist[hd]);
     return 1;
 }
 
@@ -569,8 +574,11 @@ int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hd, Control* c
     if (plan.key_bytes == 8)
         expand_hist_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>((const uint64_t*)xs.ka, (uint32_t)xs.na, (const uint64_t*)xs.kb,
                                                                           (uint32_t)xs.nb, dpos, dmask, ctl->hist[hd]);
-    else
+    else if (plan.key_bytes == 16)
         expand_hist_kernel<Key128><<<(unsigned)blocks, 256, 0, stream>>>((const Key128*)xs.ka, (uint32_t)xs.na, (const Key128*)xs.kb,
+                                                                        (uint32_t)xs.nb, dpos, dmask, ctl->hist[hd]);
+    else
+        expand_hist_kernel<Key256><<<(unsigned)blocks, 256, 0, stream>>>((const Key256*)xs.ka, (uint32_t)xs.na, (const Key256*)xs.kb,
                                                                         (uint32_t)xs.nb, dpos, dmask, ctl->hist[hd]);
     return 1;
 }

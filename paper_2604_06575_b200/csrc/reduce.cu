@@ -220,7 +220,8 @@ int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coef
 {
     if (n <= 0) return 0;
     if (key_bytes == 8) return launch_reduce_t<uint64_t>(n, keys, coefs, ukeys, usums, sc, ctl, stream);
-    return launch_reduce_t<Key128>(n, keys, coefs, ukeys, usums, sc, ctl, stream);
+    if (key_bytes == 16) return launch_reduce_t<Key128>(n, keys, coefs, ukeys, usums, sc, ctl, stream);
+    return launch_reduce_t<Key256>(n, keys, coefs, ukeys, usums, sc, ctl, stream);
 }
 
 // ------------------------------------------------------------------------------------------ S4 + S5
@@ -315,9 +316,13 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
         prune_unpack_kernel<uint64_t, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const uint64_t*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
             out_capacity, tile_state, ctl, out_count_device);
-    else
+    else if (plan.key_bytes == 16)
         prune_unpack_kernel<Key128, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const Key128*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
+            out_capacity, tile_state, ctl, out_count_device);
+    else
+        prune_unpack_kernel<Key256, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
+            (const Key256*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
             out_capacity, tile_state, ctl, out_count_device);
     return 1;
 }

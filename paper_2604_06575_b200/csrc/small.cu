@@ -19,7 +19,7 @@ constexpr int kSmallThreads = 1024;
 // coefficients) + two permutations + the (digit, warp) counters must fit 227 KB of shared memory.
 template <typename K>
 struct SmallSmem {
-    static constexpr int CAP = sizeof(K) == 8 ? kSmallCap : kSmallCap / 2;
+    static constexpr int CAP = kSmallCap * 8 / (int)sizeof(K);
     static constexpr int HROW = 33;                                          // counters of one digit: 32 warps + 1 pad (bank spread)
     static constexpr size_t off_a = 0;                                       // keys by original index, then sorted coefficients
     static constexpr size_t off_b = off_a + (size_t)CAP * sizeof(K);         // sorted keys
@@ -214,7 +214,8 @@ int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* c
                              void* ukeys, double* usums, Control* ctl, cudaStream_t stream)
 {
     if (plan.key_bytes == 8) return launch_block_sort_reduce_t<uint64_t>(plan, keys, coefs, n_device, n, ukeys, usums, ctl, stream);
-    return launch_block_sort_reduce_t<Key128>(plan, keys, coefs, n_device, n, ukeys, usums, ctl, stream);
+    if (plan.key_bytes == 16) return launch_block_sort_reduce_t<Key128>(plan, keys, coefs, n_device, n, ukeys, usums, ctl, stream);
+    return launch_block_sort_reduce_t<Key256>(plan, keys, coefs, n_device, n, ukeys, usums, ctl, stream);
 }
 
 }  // namespace polylab

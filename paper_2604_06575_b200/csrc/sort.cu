@@ -387,8 +387,11 @@ int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, c
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortThreads64, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
                                                              tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
-    return launch_sort_pass_t<Key128, kSortThreads128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                        tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
+    if (plan.key_bytes == 16)
+        return launch_sort_pass_t<Key128, kSortThreads128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+                                                            tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
+    return launch_sort_pass_t<Key256, kSortThreads256, kSortItems256, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
+                                                        tile_state, ctl, safe_rank, debug_unstable, nullptr, xs, stream);
 }
 
 }  // namespace polylab

@@ -59,7 +59,7 @@ def test_struct_layouts_match(L, tmp_path):
 
 
 def test_version_and_status_strings(L):
-    assert L.polylab_version() == 100
+    assert L.polylab_version() == 110
     seen = {L.polylab_status_string(i).decode() for i in range(7)}
     assert len(seen) == 7 and "ok" in seen
     assert L.polylab_status_string(99).decode() == "unknown status"
@@ -133,7 +133,7 @@ def test_batched_host_side_checks(L):
     bad = (ctypes.c_int64 * 4)(0, 2, 1, 3)                       # decreasing offsets
     b2 = B._Batch(1, 1, bad, 3, 2)
     assert L.polylab_simplify_batched(ctypes.byref(b2), 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
-    b3 = B._Batch(None, None, off, 3, 128)                       # the entry index needs a field of its own: nvars <= 127
+    b3 = B._Batch(None, None, off, 3, 256)                       # the entry index needs a field of its own: nvars <= 255
     assert L.polylab_simplify_batched(ctypes.byref(b3), 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT
     # matrix product: A must have m*k entries, B k*n
     assert L.polylab_matmul_simplify(ctypes.byref(b), 2, 2, ctypes.byref(b), 2, 0.0, None, None, None, 0, out_off, None, 0, None) == B.ERR_INVALID_ARGUMENT

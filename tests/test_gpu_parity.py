@@ -321,7 +321,7 @@ def test_caller_bounds_and_errors():
     with pytest.raises(B.PolylabError) as ei:
         B.simplify(dev(p.coef), dev(p.exps), tol, max_exp=[3, 3, 2, 3])
     assert ei.value.status == B.ERR_EXPONENT_RANGE
-    wide = np.full((10, 17), 255, np.uint8)
+    wide = np.full((10, 33), 255, np.uint8)                # 264 bits: one more than four words hold
     with pytest.raises(B.PolylabError) as ei:
         B.simplify(dev(np.ones(10)), dev(wide))
     assert ei.value.status == B.ERR_KEY_TOO_WIDE
