@@ -243,19 +243,19 @@ def measure_other_config(B, torch, cfg, variant, steps, warmup, peak, ws):
     d = [(dev(p.coef), dev(p.exps)) for p in polys]
     last = {}
 
-    def step():
+    def step(timing=False):
         if kind == "simplify":
-            c, e, st = B.simplify(*d[0], tol, workspace=ws, return_stats=True, timing=True)
+            c, e, st = B.simplify(*d[0], tol, workspace=ws, return_stats=True, timing=timing)
         elif kind == "mul":
-            c, e, st = B.mul_simplify(*d[0], *d[1], tol, workspace=ws, return_stats=True, timing=True)
+            c, e, st = B.mul_simplify(*d[0], *d[1], tol, workspace=ws, return_stats=True, timing=timing)
         elif variant == "A":                      # config 4, two chained mul+simplify passes (reading A16)
-            qc, qe, st0 = B.mul_simplify(*d[0], *d[0], tol, workspace=ws, return_stats=True, timing=True)
-            c, e, st = B.mul_simplify(qc, qe, *d[0], tol, workspace=ws, return_stats=True, timing=True)
+            qc, qe, st0 = B.mul_simplify(*d[0], *d[0], tol, workspace=ws, return_stats=True, timing=timing)
+            c, e, st = B.mul_simplify(qc, qe, *d[0], tol, workspace=ws, return_stats=True, timing=timing)
             last["n_sort"] = st0.sort_terms + st.sort_terms
             last["launches"] = st0.kernel_launches + st.kernel_launches
         else:                                     # raw p*p, then (p*p)*p merged in one sort
             rc, re_ = B.expand(*d[0], *d[0])
-            c, e, st = B.mul_simplify(rc, re_, *d[0], tol, workspace=ws, return_stats=True, timing=True)
+            c, e, st = B.mul_simplify(rc, re_, *d[0], tol, workspace=ws, return_stats=True, timing=timing)
             last["n_sort"] = rc.shape[0] + st.sort_terms
             last["launches"] = 1 + st.kernel_launches
         last["out"], last["st"] = (c, e), st
@@ -265,10 +265,12 @@ def measure_other_config(B, torch, cfg, variant, steps, warmup, peak, ws):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(steps):
-        step()
+        step()                                    # (the library's stage events cost ~40 us per call: not in this loop)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
+    step(timing=True)                             # one more call, with POLYLAB_FLAG_TIMING, for the stage times
+    torch.cuda.synchronize()
     st = last["st"]
     n_sort = last.get("n_sort", st.sort_terms)
     c, e = last["out"]
@@ -560,6 +562,7 @@ def main():
                                     "frac_of_nominal_8TBs": lsd_bytes / (sr_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
                                     "note": "above 1.0 means the call beats the roofline of the LSD method by moving fewer bytes "
                                             "(bucket path: %d passes over HBM instead of %d)" % (P, lsd_digits)}
+    roofline["traffic_capture"] = json.load(open(tpath)).get("capture") if os.path.exists(tpath) else None
     roofline["stage_ms"] = stage_ms
     roofline["path"] = path_name(st)
 

@@ -200,14 +200,16 @@ int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double to
 
 /*
  * simplify(p^power) -- the paper's mpower on a scalar polynomial (Table 1; the heavy workload
- * simplify(p_d^3)) -- by repeated products q <- simplify(q * p), left to right.  The intermediate
- * powers stay on the device inside the workspace (no unpack to the caller, no re-upload); they are merged with
- * tolerance 0 (exact zeros dropped, reading A2) and only the final power is pruned with `tol`.  Every intermediate
- * power must fit out_capacity terms, else POLYLAB_ERR_OUTPUT_TOO_SMALL with *out_nterms = the size that was needed.
- * power >= 0: power 0 gives the constant polynomial 1, power 1 is polylab_simplify.  p: DEVICE, row-major exponents
- * (strides in opts are not supported here); opts->max_exp_host and POLYLAB_FLAG_DEVICE_COUNT are not supported
- * (POLYLAB_ERR_INVALID_ARGUMENT).  An exponent of any power that does not fit exp_type -> POLYLAB_ERR_EXPONENT_RANGE.
- * opts->stats describes the last product.  The call synchronises the stream once per product.
+ * simplify(p_d^3)) -- by repeated products q <- simplify(q * p), left to right.  The bounds step runs
+ * once on p, ONE key layout is sized for the final degree (field v holds power * max_v), p is packed once, and the
+ * intermediate powers stay on the device as packed (key, sum) pairs inside the workspace: no unpack, no re-pack, no
+ * re-upload between products.  Intermediates are merged with tolerance 0 (exact zeros dropped, reading A2); only the final
+ * power is pruned with `tol`.  Every intermediate power must fit out_capacity terms, else POLYLAB_ERR_OUTPUT_TOO_SMALL with
+ * *out_nterms = the size that was needed.  power >= 0: power 0 gives the constant polynomial 1, power 1 is
+ * polylab_simplify.  p: DEVICE, row-major exponents (strides in opts are not supported here); opts->max_exp_host and
+ * POLYLAB_FLAG_DEVICE_COUNT are not supported (POLYLAB_ERR_INVALID_ARGUMENT).  power * (largest exponent of a variable in
+ * p) must fit exp_type, else POLYLAB_ERR_EXPONENT_RANGE.  opts->stats describes the last product.  The call synchronises
+ * the stream once for the bounds and once per product (for the term count that sizes the next product's launches).
  */
 size_t polylab_pow_simplify_workspace_bytes(int64_t nterms, int32_t nvars, int32_t power, int64_t out_capacity,
                                             const polylab_opts* opts);

@@ -386,7 +386,8 @@ struct BatchOut { int entry_shift; uint32_t* counts; };
 static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
                             double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
-                            const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr, const BatchOut* batch = nullptr)
+                            const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr, const BatchOut* batch = nullptr,
+                            void* packed_keys = nullptr)
 {
     if (k_bucket > 0)
         return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
@@ -403,7 +404,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
         if (batch) *launches += launch_entry_count(plan.key_bytes, plan.key_bits, n, kbuf[1], cbuf[1], ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, kbuf[1], cbuf[1], tol, out_coef, out_exps, o.exp_bytes, out_capacity,
-                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream, packed_keys);
         if (o.stats) { o.stats->small_path = 1; o.stats->sort_passes = 0; }
     } else {
         for (int p = 0; p < P; ++p) {
@@ -427,7 +428,7 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
         if (batch) *launches += launch_entry_count(plan.key_bytes, plan.key_bits, n, ukeys, usums, ctl, tol, batch->entry_shift, batch->counts, stream);
         tm.mark(POLYLAB_STAGE_REDUCE);
         *launches += launch_prune_unpack(plan, n, ukeys, usums, tol, out_coef, out_exps, o.exp_bytes, out_capacity,
-                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream);
+                                         (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream, packed_keys);
     }
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
@@ -465,12 +466,13 @@ static bool table_eligible(const Plan& plan, int64_t n, const Opts& o, const Att
 // (too many distinct monomials) and nothing was emitted -- the caller continues on the sort path.
 static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, TableSrc src, double tol, const Opts& o,
                       double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
-                      cudaStream_t stream, bool* done)
+                      cudaStream_t stream, bool* done, void* packed_keys = nullptr)
 {
     *done = false;
     Control* ctl = (Control*)(ws + L.control);
     const bool forced = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_TABLE) != 0;
-    const bool dense = !(o.flags & POLYLAB_FLAG_DEBUG_FORCE_HASH) && plan.key_bits <= kTableDenseMaxBits &&
+    // (packed output -- an intermediate power -- goes through the hash table: its tail is the prune kernel, which can keep keys)
+    const bool dense = !packed_keys && !(o.flags & POLYLAB_FLAG_DEBUG_FORCE_HASH) && plan.key_bits <= kTableDenseMaxBits &&
                        ((int64_t)1 << plan.key_bits) <= table_max_dense_slots(n);
     src.n = (uint32_t)n;
     TableArgs t;
@@ -520,7 +522,7 @@ static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layo
         }
         if (o.stats) { o.stats->table_path = 2; o.stats->sort_terms = n; }
         const int rc = sort_reduce_emit(plan, 0, U, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                                        out_nterms, launches, tm, false, stream);
+                                        out_nterms, launches, tm, false, stream, nullptr, nullptr, nullptr, packed_keys);
         return rc == kRetrySafeRank ? kRetrySafeRank : rc;
     }
     tm.mark(POLYLAB_STAGE_SORT);
@@ -695,6 +697,39 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
     });
 }
 
+// X1 + S2..S5 of a product whose operands are PACKED (keys with the product's field layout + coefficients): table path, or
+// X1 fused into the first radix pass, or materialised products for the one-block / ballot paths.  packed_keys != nullptr:
+// the result stays packed -- keys to packed_keys[], sums to out_coef[] -- for the next product of a power.
+static int product_tail(const Plan& plan, const ExpandSrc& xs, int k, unsigned char* ws, const Layout& L, double tol, const Opts& o,
+                        double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
+                        const Attempt& at, cudaStream_t stream, void* packed_keys)
+{
+    Control* ctl = (Control*)(ws + L.control);
+    const int64_t n = xs.na * xs.nb;
+    int rc;
+    if (packed_keys) k = 0;                              // (the bucket path's emit kernel unpacks)
+    if (table_eligible(plan, n, o, at)) {
+        tm.mark(POLYLAB_STAGE_PACK);
+        TableSrc src;
+        memset(&src, 0, sizeof src);
+        src.ka = xs.ka; src.ca = xs.ca; src.kb = xs.kb; src.cb = xs.cb; src.nb = (uint32_t)xs.nb;
+        bool done = false;
+        rc = table_path(plan, n, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches, tm, stream, &done, packed_keys);
+        if (done || rc != POLYLAB_OK) return rc;
+    }
+    // X1 runs inside the first radix pass (the products are formed in registers and never stored) unless the ballot
+    // ranking kernel or the one-block path is taken or there is no pass at all; only the first digit's histogram is built up front
+    const bool fuse = plan.npasses > 0 && !at.safe_rank && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK) && !small_eligible(n, plan, o);
+    if (fuse) *launches += launch_expand_hist(xs, plan, k ? plan.npasses - k : 0, ctl, stream);
+    else *launches += launch_expand_packed(xs.ka, xs.ca, xs.na, xs.kb, xs.cb, xs.nb, plan, ws + L.keys[0],
+                                           (double*)(ws + L.coefs[0]), ctl, k ? plan.npasses - k : 0, stream);
+    rc = bucket_precheck(plan, &k, n, ws, L, o, launches, stream, nullptr, fuse ? &xs : nullptr);
+    if (rc != POLYLAB_OK) return rc;
+    tm.mark(POLYLAB_STAGE_PACK);
+    return sort_reduce_emit(plan, k, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
+                            out_nterms, launches, tm, at.safe_rank, stream, nullptr, fuse ? &xs : nullptr, nullptr, packed_keys);
+}
+
 static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
                              double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms,
                              void* workspace, size_t workspace_bytes, void* cuda_stream, const Attempt& at)
@@ -765,24 +800,7 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     // X1 runs inside the first radix pass (the products are formed in registers and never stored) unless the ballot
     // ranking kernel is asked for or there is no pass at all; only the first digit's histogram is built up front
     const ExpandSrc xs = {ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb};
-    if (table_eligible(plan_a, n, o, at)) {
-        tm.mark(POLYLAB_STAGE_PACK);
-        TableSrc src;
-        memset(&src, 0, sizeof src);
-        src.ka = ws + L.ka; src.ca = a->coef; src.kb = ws + L.kb; src.cb = b->coef; src.nb = (uint32_t)nb;
-        bool done = false;
-        rc = table_path(plan_a, n, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
-        if (done || rc != POLYLAB_OK) return rc;
-    }
-    const bool fuse = plan_a.npasses > 0 && !at.safe_rank && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK) && !small_eligible(n, plan_a, o);      // (at.safe_rank already excludes fusing)
-    if (fuse) launches += launch_expand_hist(xs, plan_a, k ? plan_a.npasses - k : 0, ctl, stream);
-    else launches += launch_expand_packed(ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb, plan_a, ws + L.keys[0],
-                                          (double*)(ws + L.coefs[0]), ctl, k ? plan_a.npasses - k : 0, stream);
-    rc = bucket_precheck(plan_a, &k, n, ws, L, o, &launches, stream, nullptr, fuse ? &xs : nullptr);
-    if (rc != POLYLAB_OK) return rc;
-    tm.mark(POLYLAB_STAGE_PACK);
-    return sort_reduce_emit(plan_a, k, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o, out_coef, out_exps, out_capacity,
-                            out_nterms, &launches, tm, at.safe_rank, stream, nullptr, fuse ? &xs : nullptr);
+    return product_tail(plan_a, xs, k, ws, L, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, at, stream, nullptr);
 }
 
 int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
@@ -996,15 +1014,22 @@ int polylab_matmul_simplify(const polylab_batch* a, int32_t m, int32_t k, const 
 
 // ------------------------------------------------------------------------------- powers (N2)
 
-struct PowLayout { size_t coef[2], exps[2], inner, inner_bytes, total; };
+// The powers stay PACKED between the products: S0 runs once on p, ONE key layout is sized for the final
+// degree (field v holds power * max_v), p is packed once, and every intermediate power lives in the workspace as
+// (keys, sums) -- no S5 -> S0 -> S1 round trip between products.  Products go left to right (q <- q * p): for the paper's
+// dense p_d family binary powering forms MORE term products (p_4^4: 126^2 + 1287^2 = 1.67e6 against 126^2 + 1287*126 +
+// 6188*126 = 0.96e6), and the product count, not the number of calls, is what the time follows.
+struct PowLayout { size_t keys[2], coef[2], kp, inner, inner_bytes, total; };
 
-static PowLayout pow_layout(int64_t np, int nvars, int es, int64_t cap, const polylab_opts* opts)
+static PowLayout pow_layout(int64_t np, int nvars, int64_t cap, const polylab_opts* opts)
 {
     PowLayout P;
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
-    for (int i = 0; i < 2; ++i) { P.coef[i] = take((size_t)cap * sizeof(double)); P.exps[i] = take((size_t)cap * nvars * es); }
-    P.inner_bytes = polylab_mul_simplify_workspace_bytes(cap, np, nvars, opts);
+    const int kb = max_key_bytes(nvars, opts);
+    for (int i = 0; i < 2; ++i) { P.keys[i] = take((size_t)cap * kb); P.coef[i] = take((size_t)cap * sizeof(double)); }
+    P.kp = take((size_t)np * kb);
+    P.inner_bytes = worst_layout_bytes(cap * np, 0, 0, kb);
     P.inner = take(P.inner_bytes);
     P.total = off + 256;
     return P;
@@ -1017,8 +1042,7 @@ size_t polylab_pow_simplify_workspace_bytes(int64_t nterms, int32_t nvars, int32
     if (power <= 1) return polylab_simplify_workspace_bytes(nterms, nvars, opts);
     const int64_t cap = out_capacity > nterms ? out_capacity : nterms;
     if (nterms > 0 && cap >= POLYLAB_MAX_TERMS / nterms) return 0;              // a product could exceed the term limit
-    const PowLayout P = pow_layout(nterms, nvars, opts_exp_bytes(opts), cap, opts);
-    return P.inner_bytes ? P.total : 0;
+    return pow_layout(nterms, nvars, cap, opts).total;
 }
 
 int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const polylab_opts* opts,
@@ -1050,24 +1074,64 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
     if (!p->coef || !p->exps || !workspace || (out_capacity > 0 && (!out_coef || !out_exps))) return POLYLAB_ERR_INVALID_ARGUMENT;
     const int64_t cap = out_capacity > np ? out_capacity : np;
     if (cap >= POLYLAB_MAX_TERMS / np) return POLYLAB_ERR_INVALID_ARGUMENT;
-    const PowLayout P = pow_layout(np, nvars, es, cap, opts);
+    const PowLayout P = pow_layout(np, nvars, cap, opts);
     unsigned char* ws = align_ptr(workspace);
-    if (!P.inner_bytes || workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + P.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    if (workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + P.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
+    Opts o;
+    int rc = parse_opts(opts, nvars, &o);
+    if (rc != POLYLAB_OK) return rc;
+    unsigned char* iws = ws + P.inner;                   // the products' own workspace (256-byte aligned: every region is)
+    Control* ctl = (Control*)iws;
 
-    polylab_poly cur = *p;
-    int64_t count = 0;
+    // ---- S0 once; the key layout of p^power: field v is sized for power * max_v, which must fit exp_type (reading A8)
+    const ExpView ev = make_view(p->exps, o, nvars);
+    PL_CUDA(cudaMemsetAsync(ctl, 0, sizeof(Control), stream));
+    int launches0 = launch_bounds(ev, np, nvars, ctl, 0, stream);
+    uint32_t mh[kMaxVars];
+    PL_CUDA(cudaMemcpyAsync(mh, ctl->max_exp[0], sizeof(uint32_t) * nvars, cudaMemcpyDeviceToHost, stream));
+    PL_CUDA(cudaStreamSynchronize(stream));
+    uint64_t m[kMaxVars];
+    const uint32_t emax = exp_max_of(es);
+    for (int v = 0; v < nvars; ++v) {
+        m[v] = (uint64_t)mh[v] * (uint64_t)power;
+        if (m[v] > emax) return POLYLAB_ERR_EXPONENT_RANGE;
+    }
+    Plan plan;
+    rc = make_plan(nvars, m, mh, &plan);
+    if (rc != POLYLAB_OK) return rc;
+    // ---- S1 once: p's keys in the final layout
+    launches0 += launch_pack(ev, np, plan, ws + P.kp, ctl, -1, stream);
+
+    const void* ak = ws + P.kp;                          // the running power q (packed): starts as p itself
+    const double* ac = p->coef;
+    int64_t count = np;
     for (int step = 2; step <= power; ++step) {
         const bool last = step == power;
-        double* dc = last ? out_coef : (double*)(ws + P.coef[step & 1]);
-        void* de = last ? out_exps : (void*)(ws + P.exps[step & 1]);
-        const int rc = polylab_mul_simplify(&cur, p, last ? tol : 0.0, opts, dc, de, last ? out_capacity : cap, &count, ws + P.inner,
-                                            P.inner_bytes, cuda_stream);
+        const int64_t n = count * np;
+        const Layout L = make_layout(n, plan.key_bytes, 0, 0);
+        if (L.total > P.inner_bytes) return POLYLAB_ERR_INTERNAL;
+        const ExpandSrc xs = {ak, ac, count, ws + P.kp, p->coef, np};
+        void* pk = last ? nullptr : (void*)(ws + P.keys[step & 1]);
+        double* oc = last ? out_coef : (double*)(ws + P.coef[step & 1]);
+        int64_t produced = 0;
+        rc = run_attempts(opts, [&](const Attempt& at) {
+            cudaError_t e = cudaMemsetAsync(iws, 0, L.zero_end, stream);
+            if (cuda_failed(e, "cudaMemsetAsync")) return (int)POLYLAB_ERR_CUDA;
+            fill_stats(o.stats, plan, n);
+            int launches = step == 2 ? launches0 : 0;
+            Timing tm;
+            tm.begin((o.flags & POLYLAB_FLAG_TIMING) && o.stats, stream);
+            tm.mark(POLYLAB_STAGE_BOUNDS);
+            return product_tail(plan, xs, choose_prefix_passes(plan, n, o, at), iws, L, last ? tol : 0.0, o, oc, last ? out_exps : nullptr,
+                                last ? out_capacity : cap, &produced, &launches, tm, at, stream, pk);
+        });
         if (rc != POLYLAB_OK) {
-            if (rc == POLYLAB_ERR_OUTPUT_TOO_SMALL) *out_nterms = count;
+            if (rc == POLYLAB_ERR_OUTPUT_TOO_SMALL) *out_nterms = produced;
             return rc;
         }
-        if (!last && count > out_capacity) { *out_nterms = count; return POLYLAB_ERR_OUTPUT_TOO_SMALL; }
-        cur.coef = dc; cur.exps = de; cur.nterms = count;
+        if (!last && produced > out_capacity) { *out_nterms = produced; return POLYLAB_ERR_OUTPUT_TOO_SMALL; }
+        count = produced;
+        ak = pk; ac = oc;
         if (count == 0) break;                           // the zero polynomial stays zero
     }
     *out_nterms = count;

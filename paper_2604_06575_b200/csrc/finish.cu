@@ -409,7 +409,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         uint32_t nbuckets = 1;
         int ob = 0, fb = 0, pre = 0;
         if (one_bucket) {
-            fb = min(min(27, rbits), a.fast_bits);
+            fb = min(min(kFinFastBits, rbits), a.fast_bits);
             pre = rbits - fb;
         } else {
             uint32_t cnt = 0;
@@ -417,7 +417,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
                 if (first + j < n_loc) cnt += py[first + j];
             uint32_t o = block_exclusive_scan<THREADS>(cnt, scratch, &nbuckets);
             while (nbuckets > 1 && ((nbuckets - 1u) >> ob) != 0u) ++ob;
-            fb = min(min(27 - ob, rbits), a.fast_bits);
+            fb = min(min(kFinFastBits - ob, rbits), a.fast_bits);
             for (uint32_t j = 0; j < itn; ++j) {
                 if (first + j < n_loc) {
                     o += py[first + j];

@@ -26,6 +26,7 @@ constexpr int kFinCap = 4608;       // most records a finish tile can own (10 by
                                     // as long as kFinCap - fin_tile
 constexpr int kFinDigit = 9;         // local sort: 9-bit digits, 512 bins
 constexpr int kFinBins = 1 << kFinDigit;
+constexpr int kFinFastBits = kFinDigit == 9 ? 27 : 2 * kFinDigit;   // sort bits of the first attempt
 constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^T is below this
 constexpr int kFinMinTile = 512;    // smallest fin_tile the planner picks (workspace sizing)
 
@@ -131,7 +132,8 @@ int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coef
 // ctl->survivors = U'.  max_units bounds U (grid sizing); tile_state: ceil(max_units/kPruneTile) words, zeroed.
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
                         double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
-                        Control* ctl, int64_t* out_count_device, cudaStream_t stream);
+                        Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys = nullptr);
+// (out_keys != nullptr: packed output -- the survivors' KEYS go to out_keys[U'] instead of unpacked rows to out_exps)
 
 // Bucket path (finish.cu): the pairs are sorted by their top `prefix_passes` plan digits; finish every bucket in
 // shared memory and emit the simplified polynomial (S2 rest + S3 + S4 + S5).  (ukeys, usums): scratch for n pairs.

@@ -230,7 +230,8 @@ template <typename K, int THREADS, int ITEMS>
 __global__ void __launch_bounds__(THREADS)
 prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usums, double tol,
                     const __grid_constant__ Plan plan, double* __restrict__ out_coef, void* out_exps, int exp_bytes,
-                    int wpr, int64_t out_capacity, uint32_t* tile_state, Control* ctl, int64_t* out_count_device)
+                    int wpr, int64_t out_capacity, uint32_t* tile_state, Control* ctl, int64_t* out_count_device,
+                    K* __restrict__ out_keys)
 {
     constexpr int TILE = THREADS * ITEMS, NW = THREADS / 32;
     __shared__ uint32_t scratch[NW + 2];
@@ -282,7 +283,11 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
         const uint64_t obase = sm_base;
         for (uint32_t i = tid; i < total; i += THREADS)
             if ((int64_t)(obase + i) < out_capacity) out_coef[obase + i] = usums[tile_base + sel[i]];
-        if (wpr > 0) {
+        if (out_keys) {
+            // packed output (the intermediate powers of polylab_pow_simplify): the survivors' keys stay keys
+            for (uint32_t i = tid; i < total; i += THREADS)
+                if ((int64_t)(obase + i) < out_capacity) out_keys[obase + i] = ukeys[tile_base + sel[i]];
+        } else if (wpr > 0) {
             uint32_t* __restrict__ ow = (uint32_t*)out_exps;
             for (uint32_t f = tid; f < total * (uint32_t)wpr; f += THREADS) {
                 const uint32_t i = f / (uint32_t)wpr, w = f - i * (uint32_t)wpr;
@@ -307,7 +312,7 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
 
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
                         double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
-                        Control* ctl, int64_t* out_count_device, cudaStream_t stream)
+                        Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys)
 {
     if (max_units <= 0) return 0;
     int64_t blocks = (max_units + kPruneTile - 1) / kPruneTile;
@@ -315,15 +320,15 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
     if (plan.key_bytes == 8)
         prune_unpack_kernel<uint64_t, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const uint64_t*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
-            out_capacity, tile_state, ctl, out_count_device);
+            out_capacity, tile_state, ctl, out_count_device, (uint64_t*)out_keys);
     else if (plan.key_bytes == 16)
         prune_unpack_kernel<Key128, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const Key128*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
-            out_capacity, tile_state, ctl, out_count_device);
+            out_capacity, tile_state, ctl, out_count_device, (Key128*)out_keys);
     else
         prune_unpack_kernel<Key256, kPruneThreads, kPruneItems><<<(unsigned)blocks, kPruneThreads, 0, stream>>>(
             (const Key256*)ukeys, usums, tol, plan, out_coef, out_exps, exp_bytes, row_words(plan.nvars, exp_bytes, out_exps),
-            out_capacity, tile_state, ctl, out_count_device);
+            out_capacity, tile_state, ctl, out_count_device, (Key256*)out_keys);
     return 1;
 }
 

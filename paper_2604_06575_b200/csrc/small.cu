@@ -1,14 +1,17 @@
 // small.cu -- steps S2 and S3 of a SMALL input in one thread block: sort and segmented sum without a single trip through
 // global memory in between; the runs then go through the ordinary prune / unpack kernel (S4, S5: reduce.cu), whose many
-// blocks write the output rows far faster than one SM can (measured: 58 us of 104 for 7,680 rows of 10 bytes).  Used (a) for inputs of at most kSmallCap terms, where the multi-kernel radix
-// path is all launch latency (the paper's lightweight-operator regime, Table 7), and (b) as the tail of
-// the table path (table.cu) when at most kSmallCap distinct monomials are left to put in canonical order.
+// blocks write the output rows far faster than one SM can (measured: 58 us of 104 for 7,680 rows of 10 bytes).  Used
+// (a) for inputs of at most small_cap() terms, where the multi-kernel radix path is all launch latency (the paper's
+// lightweight-operator regime, Table 7), and (b) as the tail of the table path (table.cu) when at most
+// that many distinct monomials are left to put in canonical order.
 //
 // The block keeps the keys in shared memory and sorts a PERMUTATION of them, least significant plan digit first: warp w
-// ranks the 1/32 of the positions it owns (one shared-memory atomic per record, order verified afterwards), a 256-bin scan over (warp, digit) counts gives every record its slot, and only 16-bit indices move.  A stable
-// sort sums equal monomials in input order -- left to right inside a thread, by a fixed shuffle tree across threads
-// (reading A6): a function of the layout only, bit-reproducible.  (A bitonic network over 8192 pairs was measured first:
-// 91 stages * 164 KB of shared-memory traffic on ONE SM = 183 us; the radix passes move 100 KB each.)
+// ranks the 1/32 of the positions it owns (one shared-memory atomic per record, order verified afterwards), a 256-bin
+// scan over (warp, digit) counts gives every record its slot, and only 16-bit indices move.  A stable sort sums equal
+// monomials in input order -- left to right inside a thread, by a fixed shuffle tree across threads (reading A6): a
+// function of the layout only, bit-reproducible.  Measured and rejected: a bitonic network over 8192 pairs (91 stages *
+// 164 KB of shared-memory traffic on ONE SM = 183 us); ballot-matching ranks (3x the instructions, and one block has one
+// SM's four issue slots: 15k cycles per pass).
 #include "kernels.h"
 
 namespace polylab {

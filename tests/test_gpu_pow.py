@@ -79,3 +79,30 @@ def test_small_powers_errors_and_zero():
     assert ei.value.status == B.ERR_EXPONENT_RANGE
     c, e = gpu_pow(W.Poly(np.array([2.0]), np.array([[100]], np.uint16)), 3)
     assert c.tolist() == [8.0] and e.tolist() == [[300]]
+
+
+@pytest.mark.parametrize("k", [4, 6, 8])
+def test_higher_powers_match_the_oracle_chain(k):
+    """The powers stay packed between the products (one key layout sized for degree k * max): k - 1 products, each against
+    the oracle's chain; the last product's output is unpacked and pruned with tol."""
+    r = np.random.default_rng(k)
+    p = W.Poly(r.uniform(-1.0, 1.0, 12), r.integers(0, 3, size=(12, 4)).astype(np.uint8))
+    tol = [0.0, 1e-9][k % 2 == 0 and k > 4]
+    c, e, st = B.pow_simplify(dev(p.coef), dev(p.exps), k, tol, return_stats=True)
+    assert st.key_bits == sum(int(k * int(mx)).bit_length() for mx in p.exps.max(axis=0))
+    assert_parity(oracle_pow(p, k, tol), c.cpu().numpy(), e.cpu().numpy())
+
+
+def test_power_of_a_wide_polynomial_and_the_table_path():
+    """30 variables (p^3 needs 2 bits each... up to 8 bits: 240-bit keys): the packed intermediates are 256-bit keys; and a
+    p_3^4 whose products (up to 6188 * 56 = 346,528) take the table path with packed output."""
+    r = np.random.default_rng(5)
+    p = W.Poly(r.standard_normal(40), r.integers(0, 80, size=(40, 30)).astype(np.uint8))
+    c, e, st = B.pow_simplify(dev(p.coef), dev(p.exps), 3, 0.0, return_stats=True)
+    assert st.key_bytes == 32
+    assert_parity(oracle_pow(p, 3), c.cpu().numpy(), e.cpu().numpy())
+    q = W.p_d(3)
+    c, e, st = B.pow_simplify(dev(q.coef), dev(q.exps), 4, 0.0, return_stats=True, out_capacity=100_000)
+    c, e = c.cpu().numpy(), e.cpu().numpy()
+    assert len(c) == math.comb(5 + 12, 5) and c.sum() == float(56 ** 4) and (c == np.round(c)).all()
+    assert st.table_path in (1, 2)

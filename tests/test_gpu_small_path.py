@@ -1,6 +1,7 @@
-"""-m gpu: the one-block path (csrc/small.cu): at most 8192 (key, coefficient) pairs are sorted (stable bitonic network in
-shared memory), summed, pruned and unpacked by a single thread block -- the paper's lightweight-operator regime
-(Table 7), where the multi-kernel path is all launch latency -- against the CPU oracle."""
+"""-m gpu: the one-block path (csrc/small.cu): at most 8192 (key, coefficient) pairs (4096 with 128-bit keys) are sorted
+(radix sort of a permutation in shared memory) and summed by a single thread block, then pruned and unpacked -- the paper's
+lightweight-operator regime (Table 7), where the multi-kernel path is all launch latency -- against the
+CPU oracle."""
 import numpy as np
 import pytest
 import torch
