@@ -596,6 +596,31 @@ def main():
                "d2h_bytes_per_step": int(d2h) + 8, "steps": k2, "ms_per_step": ms2 / k2}
         del hp
 
+    # ---- the same step without any host synchronisation (POLYLAB_FLAG_DEVICE_COUNT + caller bounds): count and status stay
+    # on the device; the fast kernels (atomic ranking, fused pack, bucket path) report their self-checks through status_device
+    async_info = None
+    if kind == "simplify" and rank == 0:
+        bound = [int(x) for x in np.asarray(polys[0].exps[: 1 << 16]).max(axis=0)]
+        emax = int(np.iinfo(polys[0].exps.dtype).max)
+        bound = [emax if args.config == 5 else b for b in bound]      # config 5 draws the full range; others: probed, may RETRY
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        stat = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+        try:
+            for _ in range(2):
+                B.simplify_async(*dpolys[0], tol, bound, outbuf[0], outbuf[1], cnt, stat, workspace=ws)
+            barrier()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            for _ in range(steps):
+                ast = B.simplify_async(*dpolys[0], tol, bound, outbuf[0], outbuf[1], cnt, stat, workspace=ws)
+            a1.record()
+            barrier()
+            async_info = {"ms_per_step": a0.elapsed_time(a1) / steps, "status_device": int(stat.item()), "count_device": int(cnt.item()),
+                          "prefix_passes": ast.prefix_passes, "host_synchronisations": 0,
+                          "ratio_to_synchronous": (a0.elapsed_time(a1) / steps) / ms_per_step}
+        except B.PolylabError as ex:
+            async_info = {"error": str(ex)}
+
     # ---- parity of the timed output against the oracle (outside the timed region): every monomial for the configs of at most
     # 1e7 terms, an oracle key slice (1/256 of the monomials, all their contributions) for config 5
     par = None
@@ -644,7 +669,7 @@ def main():
                        "l2": "inputs and workspace are far larger than the 126 MB L2" if n_sort * (Wb + 8) > 4e8 else
                              "working set fits L2 (no flush between steps; launch-latency bound)"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "parity": par, "other_configs": others,
+            "parity": par, "async": async_info, "other_configs": others,
         }))
     if dist is not None:
         dist.destroy_process_group()

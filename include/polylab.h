@@ -58,15 +58,23 @@ typedef enum {
     POLYLAB_ERR_OUTPUT_TOO_SMALL = 5,   /* survivors > out_capacity: *out_nterms = required size, the first
                                            out_capacity terms are written */
     POLYLAB_ERR_CUDA = 6,               /* a CUDA runtime call failed (see polylab_last_cuda_error) */
-    POLYLAB_ERR_INTERNAL = 7            /* the sorted-order self-check failed even with the ballot-ranking kernel */
+    POLYLAB_ERR_INTERNAL = 7,           /* the sorted-order self-check failed even with the ballot-ranking kernel */
+    POLYLAB_ERR_RETRY = 8               /* only ever written to opts->status_device by a POLYLAB_FLAG_DEVICE_COUNT call: a
+                                           self-check of the fast path failed (ranking order, bucket length), nothing valid
+                                           was emitted and the device count is 0 -- call again with POLYLAB_FLAG_SAFE_RANK |
+                                           POLYLAB_FLAG_NO_BUCKET (or without POLYLAB_FLAG_DEVICE_COUNT, which retries itself) */
 } polylab_status;
 
 typedef enum { POLYLAB_EXP_U8 = 1, POLYLAB_EXP_U16 = 2, POLYLAB_EXP_U32 = 4 } polylab_exp_type;
 
 enum {
     POLYLAB_FLAG_DEVICE_COUNT = 1u,  /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
-                                        Requires max_exp_host (no bounds read-back).  Data errors are then
-                                        reported only through the device status word, see polylab_opts. */
+                                        Requires max_exp_host (no bounds read-back).  Data errors and failed self-checks
+                                        are then reported only through the device status word opts->status_device
+                                        (POLYLAB_ERR_EXPONENT_RANGE, POLYLAB_ERR_RETRY).  With a status word the call takes
+                                        the same fast kernels as a synchronous one (atomic ranking, one-block path, bucket
+                                        path; not the table path, which needs a read-back); without one it ranks by
+                                        ballot matching, whose order needs no check. */
     POLYLAB_FLAG_TIMING = 2u,        /* record CUDA events between the steps and fill stats->stage_ms
                                         (needs stats; ignored with POLYLAB_FLAG_DEVICE_COUNT) */
     POLYLAB_FLAG_SAFE_RANK = 4u,     /* rank records inside a radix pass by warp ballot matching (stable by
@@ -75,15 +83,15 @@ enum {
                                         one warp instruction's same-address atomics in lane order (measured, not
                                         documented); therefore the default path verifies the sorted order in the
                                         segmented-sum step and re-runs the call with this flag if the check
-                                        fails (stats->rank_fallback = 1).  Implied by POLYLAB_FLAG_DEVICE_COUNT,
-                                        which cannot read the check back. */
+                                        fails (stats->rank_fallback = 1).  Implied by POLYLAB_FLAG_DEVICE_COUNT without
+                                        opts->status_device, which could not report the check. */
     POLYLAB_FLAG_NO_BUCKET = 8u,     /* never take the bucket path: always sort with ceil(B/8) LSD passes.  By default a
                                         call with >= 2^20 terms and >= 4 digits first partitions the pairs on their
                                         most significant digit(s) and, if those spread the keys evenly enough for every
                                         bucket to fit shared memory, finishes sort + sum + prune + unpack on chip
                                         (stats->prefix_passes > 0); otherwise (stats->bucket_fallback = 1) it runs the
                                         LSD passes.  Both paths give the same result up to summation order.  Not
-                                        taken with POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
+                                        taken with POLYLAB_FLAG_SAFE_RANK. */
     POLYLAB_FLAG_NO_FUSED_PACK = 16u, /* always run S1 (pack) and X1 (expand) as kernels of their own.  By default the first
                                         radix pass forms its keys in registers: from the exponent rows on the bucket path
                                         (contiguous rows of 8 or 16 bytes), from the packed operands for a product

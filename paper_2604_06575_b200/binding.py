@@ -22,7 +22,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpolylab.so")
 
 (OK, ERR_INVALID_ARGUMENT, ERR_KEY_TOO_WIDE, ERR_EXPONENT_RANGE, ERR_WORKSPACE_TOO_SMALL, ERR_OUTPUT_TOO_SMALL, ERR_CUDA,
- ERR_INTERNAL) = range(8)
+ ERR_INTERNAL, ERR_RETRY) = range(9)
 FLAG_DEVICE_COUNT = 1
 FLAG_TIMING = 2
 FLAG_SAFE_RANK = 4
@@ -272,13 +272,15 @@ def simplify(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_ex
 
 
 def simplify_async(coef: torch.Tensor, exps: torch.Tensor, tol: float, max_exp: Sequence[int], out_coef: torch.Tensor,
-                   out_exps: torch.Tensor, out_count: torch.Tensor, status: torch.Tensor,
-                   workspace: Optional[Workspace] = None, stream=None) -> Stats:
-    """polylab_simplify with POLYLAB_FLAG_DEVICE_COUNT: no host synchronisation; count/status stay on the device."""
+                   out_exps: torch.Tensor, out_count: torch.Tensor, status: Optional[torch.Tensor],
+                   workspace: Optional[Workspace] = None, stream=None, flags: int = 0) -> Stats:
+    """polylab_simplify with POLYLAB_FLAG_DEVICE_COUNT: no host synchronisation; count/status stay on the device.
+    `status` may come back as ERR_RETRY (a self-check of the fast path failed): call again with
+    flags=FLAG_SAFE_RANK | FLAG_NO_BUCKET."""
     coef, exps, strides = _dev_poly(coef, exps)
     n, nvars = int(exps.shape[0]), int(exps.shape[1])
     keep = []
-    o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=FLAG_DEVICE_COUNT, strides=strides, status_device=status, keep=keep)
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=FLAG_DEVICE_COUNT | flags, strides=strides, status_device=status, keep=keep)
     wsb = simplify_workspace_bytes(n, nvars)
     ws = _ws(coef.device, workspace).get(max(wsb, 256))
     with torch.cuda.device(coef.device):     # the library launches on the CURRENT device

@@ -272,7 +272,7 @@ struct Timing {
 static int choose_prefix_passes(const Plan& plan, int64_t n, const Opts& o, const Attempt& at)
 {
     const bool force = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET) != 0;
-    if (!at.allow_bucket || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_BUCKET | POLYLAB_FLAG_DEVICE_COUNT))) return 0;
+    if (!at.allow_bucket || at.safe_rank || (o.flags & POLYLAB_FLAG_NO_BUCKET)) return 0;
     const int P = plan.npasses;
     if (plan.key_bytes > 16) return 0;                  // finish.cu handles one- and two-word keys
     if (P < 1 || (!force && (P < 4 || n < (1 << 20)))) return 0;
@@ -306,7 +306,8 @@ static int fast_digits(const Opts& o)
 static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* ws, const Layout& L, const Opts& o,
                            int* launches, cudaStream_t stream, const ExpView* unpacked = nullptr, const ExpandSrc* xs = nullptr)
 {
-    if (*k == 0 || (o.flags & POLYLAB_FLAG_DEBUG_FORCE_BUCKET)) return POLYLAB_OK;
+    // (an asynchronous call cannot read the histogram back: tile_bounds_kernel alone decides, through status_device)
+    if (*k == 0 || (o.flags & (POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEVICE_COUNT))) return POLYLAB_OK;
     // (the rejection branch below is the only one that needs `unpacked`)
     Control* ctl = (Control*)(ws + L.control);
     const int P = plan.npasses, d = P - *k;
@@ -352,10 +353,16 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
                                kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes, out_capacity,
-                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint32_t*)(ws + L.fin_chunks), ctl, nullptr,
+                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint32_t*)(ws + L.fin_chunks), ctl,
+                               (o.flags & POLYLAB_FLAG_DEVICE_COUNT) ? out_nterms : nullptr,
                                tm.on ? tm.ev[POLYLAB_STAGE_REDUCE + 1] : nullptr, stream);      // REDUCE = tiles, PRUNE = scan + emit
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
+    if (o.flags & POLYLAB_FLAG_DEVICE_COUNT) {             // no read-back: the self-checks report through status_device
+        *launches += launch_async_status(ctl, o.status_device, out_nterms, stream);
+        if (o.stats) { o.stats->kernel_launches += *launches; o.stats->prefix_passes = k; o.stats->sort_passes = k; }
+        return POLYLAB_OK;
+    }
     if (o.stats) o.stats->kernel_launches += *launches;
     Readback res;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
@@ -434,8 +441,8 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
     PL_CUDA(cudaGetLastError());
     if (o.stats) o.stats->kernel_launches += *launches;
     if (dev_count) {
-        if (o.status_device)
-            PL_CUDA(cudaMemcpyAsync(o.status_device, &ctl->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+        *launches += launch_async_status(ctl, o.status_device, out_nterms, stream);
+        if (o.stats) o.stats->kernel_launches += 1;
         return POLYLAB_OK;
     }
     struct { int32_t status; uint32_t distinct, survivors, unsorted; } res;
@@ -655,7 +662,8 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
 
 static bool wants_safe_rank(const polylab_opts* opts)
 {
-    return opts && (opts->flags & (POLYLAB_FLAG_SAFE_RANK | POLYLAB_FLAG_DEVICE_COUNT)) != 0;
+    // an asynchronous call without a status word could not report a failed self-check: it gets the ranking that needs none
+    return opts && ((opts->flags & POLYLAB_FLAG_SAFE_RANK) || ((opts->flags & POLYLAB_FLAG_DEVICE_COUNT) && !opts->status_device));
 }
 
 // Runs `once(attempt)`; a failed self-check re-runs the call on a more conservative path (at most twice).
@@ -1331,6 +1339,7 @@ const char* polylab_status_string(int status)
     case POLYLAB_ERR_OUTPUT_TOO_SMALL: return "output capacity too small";
     case POLYLAB_ERR_CUDA: return "CUDA error";
     case POLYLAB_ERR_INTERNAL: return "internal error: sorted-order self-check failed";
+    case POLYLAB_ERR_RETRY: return "asynchronous call: a self-check of the fast path failed, call again with POLYLAB_FLAG_SAFE_RANK";
     default: return "unknown status";
     }
 }

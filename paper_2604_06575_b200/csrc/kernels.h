@@ -135,6 +135,9 @@ int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, 
                         Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys = nullptr);
 // (out_keys != nullptr: packed output -- the survivors' KEYS go to out_keys[U'] instead of unpacked rows to out_exps)
 
+// DEVICE_COUNT calls: *status_device = ctl->status, or POLYLAB_ERR_RETRY (and a zero count) when a self-check failed.
+int launch_async_status(const Control* ctl, int32_t* status_device, int64_t* out_count_device, cudaStream_t stream);
+
 // Bucket path (finish.cu): the pairs are sorted by their top `prefix_passes` plan digits; finish every bucket in
 // shared memory and emit the simplified polynomial (S2 rest + S3 + S4 + S5).  (ukeys, usums): scratch for n pairs.
 // tile_start, tile_state: ceil(n/fin_tile)+1 words each, tile_state zeroed; worklist: as many uint4; chunk_sum: ceil(tiles/4096) words.  after_tiles (optional): recorded

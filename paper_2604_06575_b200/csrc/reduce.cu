@@ -310,6 +310,21 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
     }
 }
 
+// Asynchronous calls (POLYLAB_FLAG_DEVICE_COUNT): the status the host would have read back, on the device.  A failed
+// self-check (unstable ranking, a bucket too long for a tile) is POLYLAB_ERR_RETRY: nothing valid was emitted.
+__global__ void async_status_kernel(const Control* ctl, int32_t* status_device, int64_t* out_count_device)
+{
+    const int32_t st = ctl->status != POLYLAB_OK ? ctl->status : (ctl->unsorted || ctl->overflow) ? (int32_t)POLYLAB_ERR_RETRY : (int32_t)POLYLAB_OK;
+    if (status_device) *status_device = st;
+    if (st == POLYLAB_ERR_RETRY && out_count_device) *out_count_device = 0;
+}
+
+int launch_async_status(const Control* ctl, int32_t* status_device, int64_t* out_count_device, cudaStream_t stream)
+{
+    async_status_kernel<<<1, 1, 0, stream>>>(ctl, status_device, out_count_device);
+    return 1;
+}
+
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
                         double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
                         Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys)

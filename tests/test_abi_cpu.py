@@ -60,8 +60,8 @@ def test_struct_layouts_match(L, tmp_path):
 
 def test_version_and_status_strings(L):
     assert L.polylab_version() == 110
-    seen = {L.polylab_status_string(i).decode() for i in range(7)}
-    assert len(seen) == 7 and "ok" in seen
+    seen = {L.polylab_status_string(i).decode() for i in range(9)}
+    assert len(seen) == 9 and "ok" in seen
     assert L.polylab_status_string(99).decode() == "unknown status"
 
 

@@ -267,3 +267,48 @@ def test_sampled_bounds_retry_on_the_bucket_path_with_fused_pack():
     c, e, st = run(p, 0.0)
     assert st.bounds_retry == 1 and st.key_bits == 68 and st.prefix_passes == 2
     assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+
+
+# ------------------------------------------------------------------ asynchronous calls on the fast path
+
+def _async(p, tol, flags=0, with_status=True):
+    n = p.nterms
+    oc = torch.empty(n, dtype=torch.float64, device="cuda")
+    oe = torch.empty((n, p.nvars), dtype=torch.uint8, device="cuda")
+    cnt = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    status = torch.full((1,), -1, dtype=torch.int32, device="cuda") if with_status else None
+    st = B.simplify_async(dev(p.coef), dev(p.exps), tol, [255] * p.nvars, oc, oe, cnt, status, flags=flags)
+    torch.cuda.synchronize()
+    k = int(cnt.item())
+    return oc[:k].cpu().numpy(), oe[:k].cpu().numpy(), (int(status.item()) if with_status else None), st
+
+
+def test_async_call_takes_the_bucket_path():
+    """POLYLAB_FLAG_DEVICE_COUNT with a status word: no host synchronisation, yet atomic ranking, fused pack and the bucket
+    path -- the self-checks report through status_device (POLYLAB_ERR_RETRY) instead of a read-back."""
+    p, tol = W.config5(2_000_000)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, status, st = _async(p, tol)
+    assert status == B.OK and st.prefix_passes == 2 and len(c) == 100_000
+    assert_parity(res, c, e)
+    c0, e0, _ = run(p, tol)                                       # the synchronous call: same kernels, same bits
+    assert (e0 == e).all() and (c0.view(np.uint64) == c.view(np.uint64)).all()
+    # an unstable ranking (test hook) is reported, not hidden: status RETRY, count 0
+    c, e, status, st = _async(p, tol, flags=B.FLAG_DEBUG_UNSTABLE)
+    assert status == B.ERR_RETRY and len(c) == 0
+    # the retry the header prescribes
+    c, e, status, st = _async(p, tol, flags=B.FLAG_SAFE_RANK | B.FLAG_NO_BUCKET)
+    assert status == B.OK and st.prefix_passes == 0
+    assert_parity(res, c, e)
+    # without a status word the call must not depend on a check nobody could read: ballot ranking, LSD passes
+    c, e, status, st = _async(p, tol, with_status=False)
+    assert st.prefix_passes == 0 and st.sort_passes == 16
+    assert_parity(res, c, e)
+    # a skewed prefix (one huge bucket): tile_bounds_kernel raises overflow -> RETRY
+    q = pooled(300_000, 16, 10, seed=3)
+    q.exps[:, :2] = 7
+    c, e, status, st = _async(q, 0.0, flags=FORCE)
+    assert status == B.ERR_RETRY and len(c) == 0
+    c, e, status, st = _async(q, 0.0, flags=B.FLAG_SAFE_RANK | B.FLAG_NO_BUCKET)
+    assert status == B.OK
+    assert_parity(oracle.simplify(q.coef, q.exps, 0.0), c, e)
