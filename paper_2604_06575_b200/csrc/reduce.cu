@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(256) reduce_fixup_kernel(uint32_t ntiles, doub
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) f = __dadd_rn(f, __shfl_xor_sync(kFullMask, f, o));
         if (last >= 0) s = __dadd_rn(s, f);
-        if (last < 31) break;
+        if (stop_before | stop_after) break;                                 // the chain ended in this window (maybe in its last lane)
         u0 += 32u;
     }
     if (lane == 0) usums[slot] = s;

@@ -135,3 +135,19 @@ def test_one_run_of_1e7_equal_keys(n):
     c2, e2, _ = run(W.Poly(coef, exps2), 0.0)
     assert_parity(res, c2, e2)
     assert len(c2) == 3
+
+
+@pytest.mark.parametrize("first", [2304 * 32 + 100, 2304 * 33, 2304 * 31 + 7, 2304 * 64 + 1, 75_000])
+def test_runs_whose_cross_tile_chain_ends_on_a_window_boundary(first):
+    """The cross-tile fix-up walks a run's tile fragments 32 tiles at a time: a run whose last tile is the LAST of a window
+    (found by the round-2 fuzzer: four runs of 75,000 records) must not swallow the next run's fragments."""
+    r = np.random.default_rng(first)
+    lens = [first, 2304 * 40 + 11, 5, first, 2304 * 32]
+    exps = np.concatenate([np.full((n, 1), i, np.uint8) for i, n in enumerate(lens)])
+    coef = r.standard_normal(len(exps))
+    c, e, st = run(W.Poly(coef, exps), 0.0, flags=B.FLAG_NO_TABLE | B.FLAG_NO_SMALL)
+    assert st.table_path == 0 and len(c) == len(lens)
+    assert_parity(oracle.simplify(coef, exps, 0.0), c, e)
+    for sh in (1, 1000, 2303):                                      # the same runs shifted against the tile grid
+        c, e, _ = run(W.Poly(coef[sh:], exps[sh:]), 0.0, flags=B.FLAG_NO_TABLE)
+        assert_parity(oracle.simplify(coef[sh:], exps[sh:], 0.0), c, e)
