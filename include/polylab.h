@@ -73,7 +73,7 @@ enum {
                                         are then reported only through the device status word opts->status_device
                                         (POLYLAB_ERR_EXPONENT_RANGE, POLYLAB_ERR_RETRY).  With a status word the call takes
                                         the same fast kernels as a synchronous one (atomic ranking, one-block path, bucket
-                                        path; not the table path, which needs a read-back); without one it ranks by
+                                        path, dense table; not the hash table, which needs a read-back); without one it ranks by
                                         ballot matching, whose order needs no check. */
     POLYLAB_FLAG_TIMING = 2u,        /* record CUDA events between the steps and fill stats->stage_ms
                                         (needs stats; ignored with POLYLAB_FLAG_DEVICE_COUNT) */
@@ -107,11 +107,11 @@ enum {
                                         more than min(N/4, 2^20) distinct monomials turn up the call continues on the sort
                                         path (stats->table_fallback = 1).  Results obey the same parity rule; on this path
                                         they are also invariant under permutations of the input terms.  Not taken with
-                                        POLYLAB_FLAG_DEVICE_COUNT or POLYLAB_FLAG_SAFE_RANK. */
+                                        POLYLAB_FLAG_SAFE_RANK; with POLYLAB_FLAG_DEVICE_COUNT only the dense table. */
     POLYLAB_FLAG_NO_SMALL = 128u,     /* never take the one-block path.  By default at most 8192 terms (or products, or distinct
                                         monomials left by the table path; 4096 with 128-bit keys) are sorted and summed by a
                                         single thread block in shared memory (stats->small_path = 1): two launches instead of
-                                        a dozen.  Not taken with POLYLAB_FLAG_SAFE_RANK / POLYLAB_FLAG_DEVICE_COUNT. */
+                                        a dozen.  Not taken with POLYLAB_FLAG_SAFE_RANK. */
     POLYLAB_FLAG_DEBUG_FORCE_TABLE = 0x10000000u,  /* test hook: take the table path at any size up to 2^20 terms (abandoned only beyond 16384 distinct monomials) */
     POLYLAB_FLAG_DEBUG_FORCE_HASH = 0x08000000u,   /* test hook: use the hash table even where the dense table applies */
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no

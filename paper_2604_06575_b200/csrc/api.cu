@@ -459,9 +459,17 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
 
 // ---------------------------------------------------------------------------------------- table path
 
+static bool table_dense(const Plan& plan, int64_t n, const Opts& o)
+{
+    return !(o.flags & POLYLAB_FLAG_DEBUG_FORCE_HASH) && plan.key_bits <= kTableDenseMaxBits &&
+           ((int64_t)1 << plan.key_bits) <= table_max_dense_slots(n);
+}
+
 static bool table_eligible(const Plan& plan, int64_t n, const Opts& o, const Attempt& at)
 {
-    if (!at.allow_table || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_TABLE | POLYLAB_FLAG_DEVICE_COUNT | POLYLAB_FLAG_SAFE_RANK))) return false;
+    if (!at.allow_table || at.safe_rank || (o.flags & (POLYLAB_FLAG_NO_TABLE | POLYLAB_FLAG_SAFE_RANK))) return false;
+    // an asynchronous call cannot read the hash table's distinct count back; the dense table needs no read-back
+    if ((o.flags & POLYLAB_FLAG_DEVICE_COUNT) && !table_dense(plan, n, o)) return false;
     // the sort path's test hooks mean the sort path
     if (o.flags & (POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE | (0xfu << POLYLAB_FLAG_DEBUG_NFAST_SHIFT))) return false;
     if (plan.key_bytes != 8 || plan.key_bits > 63 || plan.npasses < 1 || n > kTableMaxTerms) return false;
@@ -479,8 +487,7 @@ static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layo
     Control* ctl = (Control*)(ws + L.control);
     const bool forced = (o.flags & POLYLAB_FLAG_DEBUG_FORCE_TABLE) != 0;
     // (packed output -- an intermediate power -- goes through the hash table: its tail is the prune kernel, which can keep keys)
-    const bool dense = !packed_keys && !(o.flags & POLYLAB_FLAG_DEBUG_FORCE_HASH) && plan.key_bits <= kTableDenseMaxBits &&
-                       ((int64_t)1 << plan.key_bits) <= table_max_dense_slots(n);
+    const bool dense = !packed_keys && table_dense(plan, n, o);
     src.n = (uint32_t)n;
     TableArgs t;
     memset(&t, 0, sizeof t);
@@ -534,9 +541,16 @@ static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layo
     }
     tm.mark(POLYLAB_STAGE_SORT);
     tm.mark(POLYLAB_STAGE_REDUCE);
-    *launches += launch_table_dense_emit(t, plan, tol, out_coef, out_exps, o.exp_bytes, out_capacity, (uint32_t*)(ws + L.tab_state), stream);
+    const bool dev_count = (o.flags & POLYLAB_FLAG_DEVICE_COUNT) != 0;
+    *launches += launch_table_dense_emit(t, plan, tol, out_coef, out_exps, o.exp_bytes, out_capacity, (uint32_t*)(ws + L.tab_state),
+                                         dev_count ? out_nterms : nullptr, stream);
     tm.mark(POLYLAB_STAGE_PRUNE);
     PL_CUDA(cudaGetLastError());
+    if (dev_count) {
+        *launches += launch_async_status(ctl, o.status_device, out_nterms, stream);
+        if (o.stats) { o.stats->kernel_launches += *launches; o.stats->table_path = 1; o.stats->sort_passes = 0; }
+        return POLYLAB_OK;
+    }
     if (o.stats) o.stats->kernel_launches += *launches;
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));

@@ -206,6 +206,6 @@ int launch_table_insert(const TableSrc& src, const TableArgs& t, bool dense, cud
 int launch_table_accum(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
 int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cudaStream_t stream);
 int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, double* out_coef, void* out_exps, int exp_bytes,
-                            int64_t out_capacity, uint32_t* tile_state, cudaStream_t stream);
+                            int64_t out_capacity, uint32_t* tile_state, int64_t* out_count_device, cudaStream_t stream);
 
 }  // namespace polylab

@@ -253,7 +253,8 @@ constexpr int kDenseTile = kDenseThreads * kDenseItems;
 
 __global__ void __launch_bounds__(kDenseThreads) table_dense_emit_kernel(const __grid_constant__ TableArgs t, const __grid_constant__ Plan plan,
                                                                          double tol, double* __restrict__ out_coef, void* out_exps,
-                                                                         int exp_bytes, int wpr, int64_t out_capacity, uint32_t* tile_state)
+                                                                         int exp_bytes, int wpr, int64_t out_capacity, uint32_t* tile_state,
+                                                                         int64_t* out_count_device)
 {
     constexpr int NW = kDenseThreads / 32;
     __shared__ uint32_t scratch[NW + 2];
@@ -310,7 +311,10 @@ __global__ void __launch_bounds__(kDenseThreads) table_dense_emit_kernel(const _
         }
         if (tid == 0) {
             if (total >> 16) atomicAdd(&t.ctl->distinct, total >> 16);
-            if (tile == ntiles - 1) t.ctl->survivors = sm_base + (total & 0xffffu);
+            if (tile == ntiles - 1) {
+                t.ctl->survivors = sm_base + (total & 0xffffu);
+                if (out_count_device) *out_count_device = (int64_t)(sm_base + (total & 0xffffu));
+            }
         }
     }
 }
@@ -362,13 +366,14 @@ int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cu
 }
 
 int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, double* out_coef, void* out_exps, int exp_bytes,
-                            int64_t out_capacity, uint32_t* tile_state, cudaStream_t stream)
+                            int64_t out_capacity, uint32_t* tile_state, int64_t* out_count_device, cudaStream_t stream)
 {
     int64_t blocks = ((int64_t)t.nord + kDenseTile - 1) / kDenseTile;
     if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     if (blocks < 1) blocks = 1;
     table_dense_emit_kernel<<<(unsigned)blocks, kDenseThreads, 0, stream>>>(t, plan, tol, out_coef, out_exps, exp_bytes,
-                                                                          row_words(plan.nvars, exp_bytes, out_exps), out_capacity, tile_state);
+                                                                          row_words(plan.nvars, exp_bytes, out_exps), out_capacity, tile_state,
+                                                                          out_count_device);
     return 1;
 }
 
