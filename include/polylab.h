@@ -67,6 +67,14 @@ typedef enum {
 
 typedef enum { POLYLAB_EXP_U8 = 1, POLYLAB_EXP_U16 = 2, POLYLAB_EXP_U32 = 4 } polylab_exp_type;
 
+/* Coefficient STORAGE type of every coefficient array a call is given or fills (coef, out_coef, polylab_poly.coef,
+ * polylab_batch.coef; the prototypes say double*): POLYLAB_COEF_F32 is the paper's polylab_precision('set','single')
+ * (Table 10) -- pass float arrays cast to the prototype's pointer type.  fp32 values
+ * are widened when first loaded; products, sums and the prune comparison are fp64; a result is rounded to fp32 once,
+ * when stored (so |stored - exact| <= 2^-24 |s| + the fp64 bound).  The prune predicate |s| > tol is applied to the fp64
+ * sum, before that rounding. */
+typedef enum { POLYLAB_COEF_F64 = 0, POLYLAB_COEF_F32 = 1 } polylab_coef_type;
+
 enum {
     POLYLAB_FLAG_DEVICE_COUNT = 1u,  /* out_nterms is a DEVICE int64_t*; the call does not synchronise.
                                         Requires max_exp_host (no bounds read-back).  Data errors and failed self-checks
@@ -169,6 +177,7 @@ typedef struct polylab_opts {
     int32_t* status_device;       /* DEVICE, optional: receives the polylab_status of data-dependent      */
                                   /*   checks (used with POLYLAB_FLAG_DEVICE_COUNT)                      */
     polylab_stats* stats;         /* HOST, optional                                                      */
+    int32_t coef_type;            /* polylab_coef_type of every coefficient array of the call; 0 = fp64   */
 } polylab_opts;
 
 /* A read-only view of a polynomial: coef[nterms], exps[nterms x nvars] (strides from polylab_opts). */

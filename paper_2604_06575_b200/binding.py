@@ -61,7 +61,7 @@ class _Stats(ctypes.Structure):
 class _Opts(ctypes.Structure):
     _fields_ = [("exp_type", ctypes.c_int32), ("flags", ctypes.c_uint32), ("term_stride", ctypes.c_int64),
                 ("var_stride", ctypes.c_int64), ("max_exp_host", ctypes.POINTER(ctypes.c_uint32)),
-                ("status_device", ctypes.c_void_p), ("stats", ctypes.POINTER(_Stats))]
+                ("status_device", ctypes.c_void_p), ("stats", ctypes.POINTER(_Stats)), ("coef_type", ctypes.c_int32)]
 
 
 class _Batch(ctypes.Structure):
@@ -192,9 +192,13 @@ def _stream_ptr(stream) -> int:
     return int(s.cuda_stream)
 
 
-def _make_opts(exp_bytes: int, max_exp, flags: int = 0, strides=None, status_device=None, keep=None):
+_COEF_TYPE = {torch.float64: 0, torch.float32: 1}      # polylab_coef_type
+
+
+def _make_opts(exp_bytes: int, max_exp, flags: int = 0, strides=None, status_device=None, keep=None, coef_dtype=torch.float64):
     o = _Opts()
     o.exp_type = exp_bytes
+    o.coef_type = _COEF_TYPE[coef_dtype]
     o.flags = flags
     if strides is not None:
         o.term_stride, o.var_stride = int(strides[0]), int(strides[1])
@@ -220,8 +224,8 @@ def _stats(st: _Stats) -> Stats:
 def _dev_poly(coef: torch.Tensor, exps: torch.Tensor, strides=None):
     if not (coef.is_cuda and exps.is_cuda):
         raise PolylabError(ERR_INVALID_ARGUMENT, "coef and exps must be CUDA tensors (use simplify_host for host data)")
-    if coef.dtype != torch.float64 or exps.dtype not in _EXP_TYPE:
-        raise PolylabError(ERR_INVALID_ARGUMENT, "coef must be float64, exps uint8/uint16/uint32")
+    if coef.dtype not in _COEF_TYPE or exps.dtype not in _EXP_TYPE:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "coef must be float64 (or float32: single-precision storage), exps uint8/uint16/uint32")
     if exps.dim() != 2 or coef.dim() != 1:
         raise PolylabError(ERR_INVALID_ARGUMENT, "coef [nterms], exps [nterms, nvars] (PAPER.md:80)")
     if strides is None:
@@ -252,9 +256,9 @@ def simplify(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_ex
     eb = _EXP_TYPE[exps.dtype]
     cap = n if out_capacity is None else int(out_capacity)
     keep = []
-    o, st = _make_opts(eb, max_exp, flags=(FLAG_TIMING if timing else 0) | flags, strides=strides, keep=keep)
+    o, st = _make_opts(eb, max_exp, flags=(FLAG_TIMING if timing else 0) | flags, strides=strides, keep=keep, coef_dtype=coef.dtype)
     if out is None:
-        out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
+        out_coef = torch.empty(max(cap, 1), dtype=coef.dtype, device=coef.device)
         out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
     else:
         out_coef, out_exps = out
@@ -280,7 +284,8 @@ def simplify_async(coef: torch.Tensor, exps: torch.Tensor, tol: float, max_exp: 
     coef, exps, strides = _dev_poly(coef, exps)
     n, nvars = int(exps.shape[0]), int(exps.shape[1])
     keep = []
-    o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=FLAG_DEVICE_COUNT | flags, strides=strides, status_device=status, keep=keep)
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=FLAG_DEVICE_COUNT | flags, strides=strides, status_device=status, keep=keep,
+                       coef_dtype=coef.dtype)
     wsb = simplify_workspace_bytes(n, nvars)
     ws = _ws(coef.device, workspace).get(max(wsb, 256))
     with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
@@ -300,16 +305,16 @@ def mul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tenso
     b_coef, b_exps, sb = _dev_poly(b_coef, b_exps)
     if sa is not None or sb is not None:
         a_exps, b_exps = a_exps.contiguous(), b_exps.contiguous()
-    if a_exps.dtype != b_exps.dtype or a_exps.shape[1] != b_exps.shape[1]:
-        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share dtype and variable space (PAPER.md:175)")
+    if a_exps.dtype != b_exps.dtype or a_exps.shape[1] != b_exps.shape[1] or a_coef.dtype != b_coef.dtype:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share dtypes and variable space (PAPER.md:175)")
     na, nb, nvars = int(a_exps.shape[0]), int(b_exps.shape[0]), int(a_exps.shape[1])
     n = na * nb
     if n >= MAX_TERMS:
         raise PolylabError(ERR_INVALID_ARGUMENT, "na*nb must be < 2^30")
     cap = n if out_capacity is None else int(out_capacity)
     keep = []
-    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], max_exp, flags=(FLAG_TIMING if timing else 0) | flags, keep=keep)
-    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=a_coef.device)
+    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], max_exp, flags=(FLAG_TIMING if timing else 0) | flags, keep=keep, coef_dtype=a_coef.dtype)
+    out_coef = torch.empty(max(cap, 1), dtype=a_coef.dtype, device=a_coef.device)
     out_exps = torch.empty((max(cap, 1), nvars), dtype=a_exps.dtype, device=a_coef.device)
     wsb = mul_simplify_workspace_bytes(na, nb, nvars)
     ws = _ws(a_coef.device, workspace).get(max(wsb, 256))
@@ -336,8 +341,8 @@ def pow_simplify(coef: torch.Tensor, exps: torch.Tensor, power: int, tol: float 
     n, nvars = int(exps.shape[0]), int(exps.shape[1])
     cap = int(out_capacity) if out_capacity is not None else max(1, min(max(n, 1) ** max(int(power), 1), 1 << 22))
     keep = []
-    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep)
-    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep, coef_dtype=coef.dtype)
+    out_coef = torch.empty(max(cap, 1), dtype=coef.dtype, device=coef.device)
     out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
     wsb = int(lib().polylab_pow_simplify_workspace_bytes(n, nvars, int(power), cap, ctypes.byref(o)))
     if wsb == 0 and n > 0 and power > 1:
@@ -374,8 +379,8 @@ def simplify_batched(coef: torch.Tensor, exps: torch.Tensor, offsets, tol: float
     bt, coef, exps, off = _batch(coef, exps, offsets, keep)
     n, ne, nvars = int(coef.shape[0]), int(off.shape[0] - 1), int(exps.shape[1])
     cap = n if out_capacity is None else int(out_capacity)
-    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep)
-    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=coef.device)
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], None, flags=flags, keep=keep, coef_dtype=coef.dtype)
+    out_coef = torch.empty(max(cap, 1), dtype=coef.dtype, device=coef.device)
     out_exps = torch.empty((max(cap, 1), nvars), dtype=exps.dtype, device=coef.device)
     out_off = np.zeros(ne + 1, dtype=np.int64)
     wsb = int(lib().polylab_simplify_batched_workspace_bytes(n, ne, nvars, ctypes.byref(o)))
@@ -397,16 +402,16 @@ def matmul_simplify(a_coef: torch.Tensor, a_exps: torch.Tensor, a_offsets, b_coe
     keep = []
     ba, a_coef, a_exps, aoff = _batch(a_coef, a_exps, a_offsets, keep)
     bb, b_coef, b_exps, boff = _batch(b_coef, b_exps, b_offsets, keep)
-    if a_exps.dtype != b_exps.dtype or a_exps.shape[1] != b_exps.shape[1]:
-        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share dtype and variable space (PAPER.md:175)")
+    if a_exps.dtype != b_exps.dtype or a_exps.shape[1] != b_exps.shape[1] or a_coef.dtype != b_coef.dtype:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share dtypes and variable space (PAPER.md:175)")
     if aoff.shape[0] - 1 != m * k or boff.shape[0] - 1 != k * n:
         raise PolylabError(ERR_INVALID_ARGUMENT, "A needs m*k entries and B k*n entries (row-major)")
     na_e, nb_e = np.diff(aoff).reshape(m, k), np.diff(boff).reshape(k, n)
     nprod = int((na_e.astype(np.int64) @ nb_e.astype(np.int64)).sum())
     nvars = int(a_exps.shape[1])
     cap = nprod if out_capacity is None else int(out_capacity)
-    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], None, flags=flags, keep=keep)
-    out_coef = torch.empty(max(cap, 1), dtype=torch.float64, device=a_coef.device)
+    o, st = _make_opts(_EXP_TYPE[a_exps.dtype], None, flags=flags, keep=keep, coef_dtype=a_coef.dtype)
+    out_coef = torch.empty(max(cap, 1), dtype=a_coef.dtype, device=a_coef.device)
     out_exps = torch.empty((max(cap, 1), nvars), dtype=a_exps.dtype, device=a_coef.device)
     out_off = np.zeros(m * n + 1, dtype=np.int64)
     wsb = int(lib().polylab_matmul_simplify_workspace_bytes(nprod, int(aoff[-1]), int(boff[-1]), m, k, n, nvars, ctypes.byref(o)))
@@ -429,8 +434,10 @@ def expand(a_coef: torch.Tensor, a_exps: torch.Tensor, b_coef: torch.Tensor, b_e
     na, nb, nvars = int(a_exps.shape[0]), int(b_exps.shape[0]), int(a_exps.shape[1])
     n = na * nb
     keep = []
-    o, _ = _make_opts(_EXP_TYPE[a_exps.dtype], None, keep=keep)
-    out_coef = torch.empty(max(n, 1), dtype=torch.float64, device=a_coef.device)
+    if a_coef.dtype != b_coef.dtype:
+        raise PolylabError(ERR_INVALID_ARGUMENT, "operands must share the coefficient dtype")
+    o, _ = _make_opts(_EXP_TYPE[a_exps.dtype], None, keep=keep, coef_dtype=a_coef.dtype)
+    out_coef = torch.empty(max(n, 1), dtype=a_coef.dtype, device=a_coef.device)
     out_exps = torch.empty((max(n, 1), nvars), dtype=a_exps.dtype, device=a_coef.device)
     ws = torch.empty(SMALL_WORKSPACE_BYTES, dtype=torch.uint8, device=a_coef.device)
     pa = _Poly(a_coef.data_ptr(), a_exps.data_ptr(), na, nvars)

@@ -44,6 +44,7 @@ static inline uint32_t exp_max_of(int exp_bytes) { return exp_bytes == 1 ? 0xffu
 
 struct Opts {
     int exp_bytes;
+    int coef_f32;          // coefficient arrays of the caller are fp32 (opts->coef_type)
     uint32_t flags;
     int64_t term_stride, var_stride;
     const uint32_t* max_exp_host;
@@ -54,7 +55,7 @@ struct Opts {
 static int parse_opts(const polylab_opts* o, int nvars, Opts* out)
 {
     Opts r;
-    r.exp_bytes = 4; r.flags = 0; r.term_stride = nvars; r.var_stride = 1;
+    r.exp_bytes = 4; r.coef_f32 = 0; r.flags = 0; r.term_stride = nvars; r.var_stride = 1;
     r.max_exp_host = nullptr; r.status_device = nullptr; r.stats = nullptr;
     if (o) {
         if (o->exp_type != 0) {
@@ -63,6 +64,8 @@ static int parse_opts(const polylab_opts* o, int nvars, Opts* out)
             r.exp_bytes = o->exp_type;
         }
         r.flags = o->flags;
+        if (o->coef_type != POLYLAB_COEF_F64 && o->coef_type != POLYLAB_COEF_F32) return POLYLAB_ERR_INVALID_ARGUMENT;
+        r.coef_f32 = o->coef_type == POLYLAB_COEF_F32;
         if (o->term_stride != 0 || o->var_stride != 0) { r.term_stride = o->term_stride; r.var_stride = o->var_stride; }
         if (r.term_stride < 0 || r.var_stride < 0) return POLYLAB_ERR_INVALID_ARGUMENT;
         r.max_exp_host = o->max_exp_host;
@@ -127,7 +130,7 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 struct Layout {
     size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
     size_t tab_state, tab, tab_bytes;
-    size_t keys[2], coefs[2], ka, kb, total;
+    size_t keys[2], coefs[2], ka, kb, ca, cb, total;      // ca, cb: fp32 operand coefficients of a product, widened to fp64
 };
 
 // Table path (table.cu): the dense table indexes 2^B slots with the key itself (B <= 22 and no more slots than
@@ -191,6 +194,8 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     for (int i = 0; i < 2; ++i) L.coefs[i] = take((size_t)n * sizeof(double));
     L.ka = take((size_t)na * key_bytes);
     L.kb = take((size_t)nb * key_bytes);
+    L.ca = take((size_t)na * sizeof(double));
+    L.cb = take((size_t)nb * sizeof(double));
     L.total = off;
     return L;
 }
@@ -334,8 +339,8 @@ struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overfl
 
 // Bucket path: k stable passes over the top k digits, then finish.cu.  The pairs are in (L.keys[0], coef0) and the
 // histogram of digit P-k is in ctl->hist[P-k].
-static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
-                            double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
+static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, CoefIn coef0,
+                            double tol, const Opts& o, CoefOut out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream, const ExpView* rows,
                             const ExpandSrc* xs)
 {
@@ -343,8 +348,12 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
     const int P = plan.npasses;
+    if (coef0.f32) {                                     // the radix passes take fp64: widen into the buffer the first pass does not write
+        *launches += launch_widen(coef0.p, cbuf[0], n, stream);
+        coef0 = CoefIn(cbuf[0]);
+    }
     for (int s = 0; s < k; ++s) {
-        const double* cin = (s == 0) ? coef0 : cbuf[s & 1];
+        const double* cin = (s == 0) ? (const double*)coef0.p : cbuf[s & 1];
         *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
                                       cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr,
@@ -390,8 +399,8 @@ static bool small_eligible(int64_t n, const Plan& plan, const Opts& o)
 // Batched calls (batch.cu): after the segmented sum, count the survivors of every entry (the key's top field).
 struct BatchOut { int entry_shift; uint32_t* counts; };
 
-static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, const double* coef0,
-                            double tol, const Opts& o, double* out_coef, void* out_exps, int64_t out_capacity,
+static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned char* ws, const Layout& L, CoefIn coef0,
+                            double tol, const Opts& o, CoefOut out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
                             const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr, const BatchOut* batch = nullptr,
                             void* packed_keys = nullptr)
@@ -414,15 +423,19 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
                                          (uint32_t*)(ws + L.prune_state), ctl, dev_count ? out_nterms : nullptr, stream, packed_keys);
         if (o.stats) { o.stats->small_path = 1; o.stats->sort_passes = 0; }
     } else {
+        if (coef0.f32 && P > 0) {                        // the radix passes take fp64: widen into the buffer the first pass does not write
+            *launches += launch_widen(coef0.p, cbuf[0], n, stream);
+            coef0 = CoefIn(cbuf[0]);
+        }
         for (int p = 0; p < P; ++p) {
-            const double* cin = (p == 0) ? coef0 : cbuf[p & 1];
+            const double* cin = (p == 0) ? (const double*)coef0.p : cbuf[p & 1];
             *launches += launch_sort_pass(plan, p, p + 1 < P ? p + 1 : -1, p, n, kbuf[p & 1], cin, kbuf[(p + 1) & 1],
                                           cbuf[(p + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, safe_rank,
                                           (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, nullptr, p == 0 ? xs : nullptr);
         }
         tm.mark(POLYLAB_STAGE_SORT);
         const void* skeys = kbuf[P & 1];
-        const double* scoef = (P == 0) ? coef0 : cbuf[P & 1];
+        const CoefIn scoef = (P == 0) ? coef0 : CoefIn(cbuf[P & 1]);
         void* ukeys = kbuf[(P + 1) & 1];
         double* usums = cbuf[(P + 1) & 1];
         ReduceScratch sc;
@@ -480,7 +493,7 @@ static bool table_eligible(const Plan& plan, int64_t n, const Opts& o, const Att
 // Merges the N records of `src` in a table and emits the simplified polynomial.  *done = false: the table was abandoned
 // (too many distinct monomials) and nothing was emitted -- the caller continues on the sort path.
 static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, TableSrc src, double tol, const Opts& o,
-                      double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
+                      CoefOut out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
                       cudaStream_t stream, bool* done, void* packed_keys = nullptr)
 {
     *done = false;
@@ -583,6 +596,7 @@ using namespace polylab;
 extern "C" {
 
 static int opts_exp_bytes(const polylab_opts* opts) { return (opts && opts->exp_type) ? opts->exp_type : 4; }
+static size_t opts_coef_bytes(const polylab_opts* opts) { return (opts && opts->coef_type == POLYLAB_COEF_F32) ? 4 : 8; }
 
 size_t polylab_simplify_workspace_bytes(int64_t nterms, int32_t nvars, const polylab_opts* opts)
 {
@@ -659,17 +673,16 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     else launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
     if (try_table) {
         tm.mark(POLYLAB_STAGE_PACK);
-        TableSrc src;
-        memset(&src, 0, sizeof src);
-        src.keys = (const uint64_t*)(ws + L.keys[0]); src.coef = coef;
+        TableSrc src = TableSrc();
+        src.keys = (const uint64_t*)(ws + L.keys[0]); src.coef = CoefIn(coef, o.coef_f32);
         bool done = false;
-        rc = table_path(plan, nterms, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
+        rc = table_path(plan, nterms, ws, L, src, tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
         if (done || rc != POLYLAB_OK) return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
     }
     rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
     if (rc != POLYLAB_OK) return rc;
     tm.mark(POLYLAB_STAGE_PACK);
-    rc = sort_reduce_emit(plan, k, nterms, ws, L, coef, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm,
+    rc = sort_reduce_emit(plan, k, nterms, ws, L, CoefIn(coef, o.coef_f32), tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm,
                           at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr);
     return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
 }
@@ -723,7 +736,7 @@ int polylab_simplify(const double* coef, const void* exps, int64_t nterms, int32
 // X1 fused into the first radix pass, or materialised products for the one-block / ballot paths.  packed_keys != nullptr:
 // the result stays packed -- keys to packed_keys[], sums to out_coef[] -- for the next product of a power.
 static int product_tail(const Plan& plan, const ExpandSrc& xs, int k, unsigned char* ws, const Layout& L, double tol, const Opts& o,
-                        double* out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
+                        CoefOut out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
                         const Attempt& at, cudaStream_t stream, void* packed_keys)
 {
     Control* ctl = (Control*)(ws + L.control);
@@ -732,8 +745,7 @@ static int product_tail(const Plan& plan, const ExpandSrc& xs, int k, unsigned c
     if (packed_keys) k = 0;                              // (the bucket path's emit kernel unpacks)
     if (table_eligible(plan, n, o, at)) {
         tm.mark(POLYLAB_STAGE_PACK);
-        TableSrc src;
-        memset(&src, 0, sizeof src);
+        TableSrc src = TableSrc();
         src.ka = xs.ka; src.ca = xs.ca; src.kb = xs.kb; src.cb = xs.cb; src.nb = (uint32_t)xs.nb;
         bool done = false;
         rc = table_path(plan, n, ws, L, src, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches, tm, stream, &done, packed_keys);
@@ -821,8 +833,14 @@ static int mul_simplify_once(const polylab_poly* a, const polylab_poly* b, doubl
     launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, -1, stream);
     // X1 runs inside the first radix pass (the products are formed in registers and never stored) unless the ballot
     // ranking kernel is asked for or there is no pass at all; only the first digit's histogram is built up front
-    const ExpandSrc xs = {ws + L.ka, a->coef, na, ws + L.kb, b->coef, nb};
-    return product_tail(plan_a, xs, k, ws, L, tol, o, out_coef, out_exps, out_capacity, out_nterms, &launches, tm, at, stream, nullptr);
+    CoefIn ca(a->coef, o.coef_f32), cb(b->coef, o.coef_f32);
+    if (o.coef_f32) {                                    // two small arrays: every kernel downstream sees fp64 operands
+        launches += launch_widen(a->coef, (double*)(ws + L.ca), na, stream) + launch_widen(b->coef, (double*)(ws + L.cb), nb, stream);
+        ca = CoefIn((const double*)(ws + L.ca));
+        cb = CoefIn((const double*)(ws + L.cb));
+    }
+    const ExpandSrc xs = {ws + L.ka, ca, na, ws + L.kb, cb, nb};
+    return product_tail(plan_a, xs, k, ws, L, tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm, at, stream, nullptr);
 }
 
 int polylab_mul_simplify(const polylab_poly* a, const polylab_poly* b, double tol, const polylab_opts* opts,
@@ -945,14 +963,14 @@ static int batched_run(const polylab_batch* a, const polylab_batch* b, const Bat
     // ---- S1 on the operands (monomial fields only), then the records with the entry index on top (+ X1 for products)
     launches += launch_pack(eva, na, plan_a, ws + L.ka, ctl, -1, stream);
     if (b) launches += launch_pack(evb, nb, plan_b, ws + L.kb, ctl, -1, stream);
-    launches += launch_batched_expand(plan_a, segs, (uint32_t)nseg, n, ws + L.ka, a->coef, b ? ws + L.kb : nullptr, b ? b->coef : nullptr,
+    launches += launch_batched_expand(plan_a, segs, (uint32_t)nseg, n, ws + L.ka, CoefIn(a->coef, o.coef_f32), b ? ws + L.kb : nullptr, b ? CoefIn(b->coef, o.coef_f32) : CoefIn(),
                                       entry_shift, ws + L.keys[0], (double*)(ws + L.coefs[0]), ctl, stream);
     tm.mark(POLYLAB_STAGE_PACK);
     const BatchOut bo = {entry_shift, counts};
     Opts o2 = o;
     o2.flags |= POLYLAB_FLAG_NO_BUCKET | POLYLAB_FLAG_NO_TABLE;
     int64_t total = 0;
-    rc = sort_reduce_emit(plan_a, 0, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o2, out_coef, out_exps, out_capacity, &total,
+    rc = sort_reduce_emit(plan_a, 0, n, ws, L, (const double*)(ws + L.coefs[0]), tol, o2, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, &total,
                           &launches, tm, at.safe_rank, stream, nullptr, nullptr, &bo);
     if (rc != POLYLAB_OK && rc != POLYLAB_ERR_OUTPUT_TOO_SMALL) return rc;
     // ---- offsets: prefix sums of the entries' survivor counts (nentries values, on the host)
@@ -1041,7 +1059,7 @@ int polylab_matmul_simplify(const polylab_batch* a, int32_t m, int32_t k, const 
 // (keys, sums) -- no S5 -> S0 -> S1 round trip between products.  Products go left to right (q <- q * p): for the paper's
 // dense p_d family binary powering forms MORE term products (p_4^4: 126^2 + 1287^2 = 1.67e6 against 126^2 + 1287*126 +
 // 6188*126 = 0.96e6), and the product count, not the number of calls, is what the time follows.
-struct PowLayout { size_t keys[2], coef[2], kp, inner, inner_bytes, total; };
+struct PowLayout { size_t keys[2], coef[2], kp, cp, inner, inner_bytes, total; };
 
 static PowLayout pow_layout(int64_t np, int nvars, int64_t cap, const polylab_opts* opts)
 {
@@ -1051,6 +1069,7 @@ static PowLayout pow_layout(int64_t np, int nvars, int64_t cap, const polylab_op
     const int kb = max_key_bytes(nvars, opts);
     for (int i = 0; i < 2; ++i) { P.keys[i] = take((size_t)cap * kb); P.coef[i] = take((size_t)cap * sizeof(double)); }
     P.kp = take((size_t)np * kb);
+    P.cp = take((size_t)np * sizeof(double));
     P.inner_bytes = worst_layout_bytes(cap * np, 0, 0, kb);
     P.inner = take(P.inner_bytes);
     P.total = off + 256;
@@ -1085,7 +1104,9 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
         if (out_capacity < 1) return POLYLAB_ERR_OUTPUT_TOO_SMALL;
         if (!out_coef || !out_exps) return POLYLAB_ERR_INVALID_ARGUMENT;
         const double one = 1.0;
-        PL_CUDA(cudaMemcpyAsync(out_coef, &one, sizeof one, cudaMemcpyHostToDevice, stream));
+        const float onef = 1.0f;
+        const bool f32 = opts && opts->coef_type == POLYLAB_COEF_F32;
+        PL_CUDA(cudaMemcpyAsync(out_coef, f32 ? (const void*)&onef : (const void*)&one, f32 ? sizeof onef : sizeof one, cudaMemcpyHostToDevice, stream));
         PL_CUDA(cudaMemsetAsync(out_exps, 0, (size_t)nvars * es, stream));
         PL_CUDA(cudaStreamSynchronize(stream));
         return POLYLAB_OK;
@@ -1125,16 +1146,21 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
     launches0 += launch_pack(ev, np, plan, ws + P.kp, ctl, -1, stream);
 
     const void* ak = ws + P.kp;                          // the running power q (packed): starts as p itself
-    const double* ac = p->coef;
+    CoefIn pc(p->coef, o.coef_f32);
+    if (o.coef_f32) {                                    // p's coefficients widened once; the powers' sums are fp64 anyway
+        launches0 += launch_widen(p->coef, (double*)(ws + P.cp), np, stream);
+        pc = CoefIn((const double*)(ws + P.cp));
+    }
+    CoefIn ac = pc;
     int64_t count = np;
     for (int step = 2; step <= power; ++step) {
         const bool last = step == power;
         const int64_t n = count * np;
         const Layout L = make_layout(n, plan.key_bytes, 0, 0);
         if (L.total > P.inner_bytes) return POLYLAB_ERR_INTERNAL;
-        const ExpandSrc xs = {ak, ac, count, ws + P.kp, p->coef, np};
+        const ExpandSrc xs = {ak, ac, count, ws + P.kp, pc, np};
         void* pk = last ? nullptr : (void*)(ws + P.keys[step & 1]);
-        double* oc = last ? out_coef : (double*)(ws + P.coef[step & 1]);
+        const CoefOut oc = last ? CoefOut(out_coef, o.coef_f32) : CoefOut((double*)(ws + P.coef[step & 1]));
         int64_t produced = 0;
         rc = run_attempts(opts, [&](const Attempt& at) {
             cudaError_t e = cudaMemsetAsync(iws, 0, L.zero_end, stream);
@@ -1153,7 +1179,7 @@ int polylab_pow_simplify(const polylab_poly* p, int32_t power, double tol, const
         }
         if (!last && produced > out_capacity) { *out_nterms = produced; return POLYLAB_ERR_OUTPUT_TOO_SMALL; }
         count = produced;
-        ak = pk; ac = oc;
+        ak = pk; ac = CoefIn((const double*)oc.p);
         if (count == 0) break;                           // the zero polynomial stays zero
     }
     *out_nterms = count;
@@ -1178,7 +1204,7 @@ int polylab_expand(const polylab_poly* a, const polylab_poly* b, const polylab_o
     if (workspace_bytes < (size_t)(ws - (unsigned char*)workspace) + sizeof(Control)) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     Control* ctl = (Control*)ws;
     PL_CUDA(cudaMemsetAsync(&ctl->status, 0, sizeof(int32_t), stream));
-    launch_expand_raw(make_view(a->exps, o, nvars), a->coef, na, make_view(b->exps, o, nvars), b->coef, nb, nvars, out_coef,
+    launch_expand_raw(make_view(a->exps, o, nvars), CoefIn(a->coef, o.coef_f32), na, make_view(b->exps, o, nvars), CoefIn(b->coef, o.coef_f32), nb, nvars, CoefOut(out_coef, o.coef_f32),
                       out_exps, ctl, stream);
     PL_CUDA(cudaGetLastError());
     int32_t status = 0;
@@ -1280,7 +1306,8 @@ int polylab_simplify_host(const double* coef_host, const void* exps_host, int64_
     const HostLayout H = host_layout(nterms, nterms, nvars, es, inner);
     unsigned char* ws = align_ptr(device_workspace);
     if (workspace_bytes < (size_t)(ws - (unsigned char*)device_workspace) + H.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
-    PL_CUDA(cudaMemcpyAsync(ws + H.coef, coef_host, (size_t)nterms * sizeof(double), cudaMemcpyHostToDevice, stream));
+    const size_t cbytes = opts_coef_bytes(opts);
+    PL_CUDA(cudaMemcpyAsync(ws + H.coef, coef_host, (size_t)nterms * cbytes, cudaMemcpyHostToDevice, stream));
     PL_CUDA(cudaMemcpyAsync(ws + H.exps, exps_host, (size_t)nterms * nvars * es, cudaMemcpyHostToDevice, stream));
     int64_t count = 0;
     const int rc = polylab_simplify((const double*)(ws + H.coef), ws + H.exps, nterms, nvars, tol, opts, (double*)(ws + H.out_coef),
@@ -1290,7 +1317,7 @@ int polylab_simplify_host(const double* coef_host, const void* exps_host, int64_
     const int64_t ncopy = count < out_capacity ? count : out_capacity;
     if (ncopy > 0) {
         if (!out_coef_host || !out_exps_host) return POLYLAB_ERR_INVALID_ARGUMENT;
-        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * cbytes, cudaMemcpyDeviceToHost, stream));
         PL_CUDA(cudaMemcpyAsync(out_exps_host, ws + H.out_exps, (size_t)ncopy * nvars * es, cudaMemcpyDeviceToHost, stream));
     }
     PL_CUDA(cudaStreamSynchronize(stream));
@@ -1318,12 +1345,13 @@ int polylab_mul_simplify_host(const polylab_poly* a_host, const polylab_poly* b_
     if (workspace_bytes < (size_t)(ws - (unsigned char*)device_workspace) + H.total - 256) return POLYLAB_ERR_WORKSPACE_TOO_SMALL;
     // operand b sits behind operand a in the input slices, each 32-term aligned
     const int64_t nb_off = (na + 31) / 32 * 32;
+    const size_t cbytes = opts_coef_bytes(opts);
     double* dca = (double*)(ws + H.coef);
-    double* dcb = dca + nb_off;
+    double* dcb = dca + nb_off;                          // (8-byte slots also when the coefficients are fp32)
     unsigned char* dea = ws + H.exps;
     unsigned char* deb = dea + (size_t)nb_off * nvars * es;
-    PL_CUDA(cudaMemcpyAsync(dca, a_host->coef, (size_t)na * sizeof(double), cudaMemcpyHostToDevice, stream));
-    PL_CUDA(cudaMemcpyAsync(dcb, b_host->coef, (size_t)nb * sizeof(double), cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(dca, a_host->coef, (size_t)na * cbytes, cudaMemcpyHostToDevice, stream));
+    PL_CUDA(cudaMemcpyAsync(dcb, b_host->coef, (size_t)nb * cbytes, cudaMemcpyHostToDevice, stream));
     PL_CUDA(cudaMemcpyAsync(dea, a_host->exps, (size_t)na * nvars * es, cudaMemcpyHostToDevice, stream));
     PL_CUDA(cudaMemcpyAsync(deb, b_host->exps, (size_t)nb * nvars * es, cudaMemcpyHostToDevice, stream));
     polylab_poly da = {dca, dea, na, nvars}, db = {dcb, deb, nb, nvars};
@@ -1335,7 +1363,7 @@ int polylab_mul_simplify_host(const polylab_poly* a_host, const polylab_poly* b_
     const int64_t ncopy = count < out_capacity ? count : out_capacity;
     if (ncopy > 0) {
         if (!out_coef_host || !out_exps_host) return POLYLAB_ERR_INVALID_ARGUMENT;
-        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaMemcpyAsync(out_coef_host, ws + H.out_coef, (size_t)ncopy * cbytes, cudaMemcpyDeviceToHost, stream));
         PL_CUDA(cudaMemcpyAsync(out_exps_host, ws + H.out_exps, (size_t)ncopy * nvars * es, cudaMemcpyDeviceToHost, stream));
     }
     PL_CUDA(cudaStreamSynchronize(stream));

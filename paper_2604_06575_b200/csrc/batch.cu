@@ -20,8 +20,8 @@ template <typename K> __device__ __forceinline__ uint32_t key_entry(const K& k, 
 
 template <typename K>
 __global__ void __launch_bounds__(256) batched_expand_kernel(const BatchSeg* __restrict__ segs, uint32_t nseg, uint32_t n,
-                                                             const K* __restrict__ ka, const double* __restrict__ ca,
-                                                             const K* __restrict__ kb, const double* __restrict__ cb,
+                                                             const K* __restrict__ ka, CoefIn ca,
+                                                             const K* __restrict__ kb, CoefIn cb,
                                                              int entry_shift, K* __restrict__ keys, double* __restrict__ coefs,
                                                              int dpos, uint32_t dmask, uint32_t* hist)
 {
@@ -57,8 +57,8 @@ __global__ void __launch_bounds__(256) batched_expand_kernel(const BatchSeg* __r
             if (sh[b]) atomicAdd(&hist[b], sh[b]);
 }
 
-int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, const double* ca,
-                          const void* kb, const double* cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream)
+int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, CoefIn ca,
+                          const void* kb, CoefIn cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream)
 {
     if (n <= 0 || nseg == 0) return 0;
     int64_t blocks = (n + 1023) / 1024;

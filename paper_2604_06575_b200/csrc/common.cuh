@@ -173,6 +173,38 @@ __device__ __forceinline__ void key_zero(Key256& k) { k.q[0] = k.q[1] = k.q[2] =
 __device__ __forceinline__ void key_from_halves(Key256& k, uint64_t hi, uint64_t lo) { k.q[0] = hi; k.q[1] = 0; k.q[2] = 0; k.q[3] = lo; }   // (never used: no fused pack for 256-bit keys)
 __device__ __forceinline__ uint64_t key_top64(const Key256& k) { return k.q[0]; }
 
+// --------------------------------------------------------------------------------- coefficients
+
+// Coefficient arrays at the ABI are fp64, or fp32 with opts->coef_type = POLYLAB_COEF_F32 (the paper's
+// polylab_precision('set','single')): single-precision STORAGE.  Every fp32 value is widened on its first
+// load, all arithmetic of the path (products, sums, the prune comparison) stays fp64, and a result is rounded to fp32 once,
+// when it is stored.  Workspace intermediates are always fp64.  CoefIn / CoefOut carry the pointer with its type so that
+// kernels index them like plain arrays.
+struct CoefIn {
+    const void* p;
+    int f32;
+    CoefIn() : p(nullptr), f32(0) {}
+    CoefIn(const double* d) : p(d), f32(0) {}
+    CoefIn(const void* q, int is_f32) : p(q), f32(is_f32) {}
+    __device__ __forceinline__ double operator[](size_t i) const
+    {
+        return f32 ? (double)__ldg((const float*)p + i) : __ldg((const double*)p + i);
+    }
+    __host__ __device__ CoefIn operator+(size_t off) const { return CoefIn((const char*)p + off * (f32 ? 4 : 8), f32); }
+};
+struct CoefOut {
+    void* p;
+    int f32;
+    CoefOut() : p(nullptr), f32(0) {}
+    CoefOut(double* d) : p(d), f32(0) {}
+    CoefOut(void* q, int is_f32) : p(q), f32(is_f32) {}
+    __device__ __forceinline__ void store(size_t i, double v) const
+    {
+        if (f32) ((float*)p)[i] = __double2float_rn(v);
+        else ((double*)p)[i] = v;
+    }
+};
+
 // ------------------------------------------------------------------------------------ plan
 
 // Key layout and pass table, computed on the host from the per-variable maxima (step S0) and passed

@@ -259,7 +259,7 @@ struct EmitArgs {
     uint32_t ntiles;
     const uint32_t* tile_start;     // [ntiles + 1]
     const uint32_t* tile_off;       // [ntiles + 1] exclusive scan of the tiles' survivor counts; [ntiles] = U'
-    double* out_coef;
+    CoefOut out_coef;
     void* out_exps;
     int exp_bytes;
     int wpr;                        // > 0: rows are written as this many 32-bit words (common.cuh, row_words)
@@ -272,7 +272,7 @@ struct EmitArgs {
 template <typename K>
 __device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, uint64_t o, double s, const K& kk)
 {
-    a.out_coef[o] = s;
+    a.out_coef.store(o, s);
     if (a.wpr > 0) {
         uint32_t* row = (uint32_t*)a.out_exps + o * (uint64_t)a.wpr;
         for (int w = 0; w < a.wpr; ++w) row[w] = unpack_row_word(plan, kk, w, a.exp_bytes);
@@ -673,7 +673,7 @@ __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitA
 
 template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
-                           const double* coefs, double tol, void* ukeys, double* usums, double* out_coef, void* out_exps,
+                           const double* coefs, double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps,
                            int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint4* worklist,
                            uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
@@ -711,7 +711,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
 }
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
-                  double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
+                  double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
                   uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
                   int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {

@@ -63,6 +63,9 @@ int launch_bounds_sample(const ExpView& ev, int64_t nterms, int nvars, Control* 
 int launch_sum_range_check(const ExpView& ea, int64_t na, const ExpView& eb, int64_t nb, int nvars, uint32_t emax, Control* ctl,
                            cudaStream_t stream);
 
+// fp32 -> fp64: out[i] = in[i] (the radix passes take fp64 coefficients only; see CoefIn in common.cuh).
+int launch_widen(const void* in_f32, double* out, int64_t n, cudaStream_t stream);
+
 // S1: pack rows into keys (key_bytes from the plan), check e <= plan.bound (-> ctl->status), and, when
 // hist_digit >= 0, accumulate the histogram of that plan digit into ctl->hist[hist_digit] (the first pass's digit).
 int launch_pack(const ExpView& ev, int64_t nterms, const Plan& plan, void* keys, Control* ctl, int hist_digit,
@@ -83,12 +86,12 @@ int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64
 
 // X1: all products of packed operands: key = ka_i + kb_j, coef = fl(ca_i * cb_j); N = na*nb pairs written
 // to keys/coefs (emission order: i*nb + j); histogram of plan digit `hist_digit` into ctl->hist[hist_digit].
-int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
+int launch_expand_packed(const void* ka, CoefIn ca, int64_t na, const void* kb, CoefIn cb, int64_t nb,
                          const Plan& plan, void* keys, double* coefs, Control* ctl, int hist_digit, cudaStream_t stream);
 
 // Raw product without keys (polylab_expand): rows a_i + b_j, coefficients fl(ca_i*cb_j).
-int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const ExpView& eb, const double* cb, int64_t nb,
-                      int nvars, double* out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream);
+int launch_expand_raw(const ExpView& ea, CoefIn ca, int64_t na, const ExpView& eb, CoefIn cb, int64_t nb,
+                      int nvars, CoefOut out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream);
 
 // S2: one stable radix pass on plan digit `pass` of n (key, coef) pairs from (keys_in, coef_in) to (keys_out,
 // coef_out); needs ctl->hist[pass].  `next` >= 0: also accumulate the histogram of plan digit `next` (the digit of
@@ -102,10 +105,10 @@ int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const Exp
 // formed in registers as (ka_i + kb_j, fl(ca_i * cb_j)); atomic ranking only.
 struct ExpandSrc {
     const void* ka;
-    const double* ca;
+    CoefIn ca;
     int64_t na;
     const void* kb;
-    const double* cb;
+    CoefIn cb;
     int64_t nb;
 };
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
@@ -125,13 +128,13 @@ struct ReduceScratch {
     double* tile_frag;
     uint8_t* tile_cont;
 };
-int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coefs, void* ukeys, double* usums,
+int launch_reduce(int key_bytes, int64_t n, const void* keys, CoefIn coefs, void* ukeys, double* usums,
                   const ReduceScratch& sc, Control* ctl, cudaStream_t stream);
 
 // S4+S5: keep |s| > tol, order-preserving compaction, unpack into out_coef/out_exps (row-major, exp_bytes);
 // ctl->survivors = U'.  max_units bounds U (grid sizing); tile_state: ceil(max_units/kPruneTile) words, zeroed.
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
-                        double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
+                        CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
                         Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys = nullptr);
 // (out_keys != nullptr: packed output -- the survivors' KEYS go to out_keys[U'] instead of unpacked rows to out_exps)
 
@@ -144,7 +147,7 @@ int launch_async_status(const Control* ctl, int32_t* status_device, int64_t* out
 // between the finish kernel and the scan/emit kernels, for the stage timing.  Sets ctl->overflow (nothing emitted) when a bucket is too long,
 // ctl->unsorted when the prefix order or the local order check fails, ctl->distinct, ctl->survivors.
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
-                  double tol, void* ukeys, double* usums, double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
+                  double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
                   uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
                   int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream);
 
@@ -154,7 +157,7 @@ int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, 
 // n_device (optional, DEVICE): the pair count is read on the device (clamped) instead of `n`.
 constexpr int kSmallCap = 8192;          // 64-bit keys; 4096 for 128-bit keys, 2048 for 256-bit keys
 inline int small_cap(int key_bytes) { return kSmallCap * 8 / key_bytes; }
-int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
+int launch_block_sort_reduce(const Plan& plan, const void* keys, CoefIn coefs, const uint32_t* n_device, uint32_t n,
                              void* ukeys, double* usums, Control* ctl, cudaStream_t stream);
 
 // Batched simplify (batch.cu): the records of all entries, keyed (entry, monomial).
@@ -164,8 +167,8 @@ struct BatchSeg {
     uint32_t b0, nb;        // terms [b0, b0 + nb) of B: the segment holds the na * nb products; nb == 0: the na raw terms
     uint32_t entry;         // the polynomial (matrix entry) the segment's records belong to
 };
-int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, const double* ca,
-                          const void* kb, const double* cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
+int launch_batched_expand(const Plan& plan, const BatchSeg* segs, uint32_t nseg, int64_t n, const void* ka, CoefIn ca,
+                          const void* kb, CoefIn cb, int entry_shift, void* keys, double* coefs, Control* ctl, cudaStream_t stream);
 int launch_entry_count(int key_bytes, int key_bits, int64_t max_units, const void* ukeys, const double* usums, const Control* ctl, double tol,
                        int entry_shift, uint32_t* counts, cudaStream_t stream);
 
@@ -177,11 +180,11 @@ struct __align__(16) TableSlot {
 };
 struct TableSrc {           // the N records: packed keys + coefficients, or (keys == nullptr) the products of packed operands
     const uint64_t* keys;
-    const double* coef;
+    CoefIn coef;
     const void* ka;
-    const double* ca;
+    CoefIn ca;
     const void* kb;
-    const double* cb;
+    CoefIn cb;
     uint32_t nb;
     uint32_t n;
 };
@@ -205,7 +208,7 @@ inline uint32_t table_dense_tile() { return 256u * 8u; }
 int launch_table_insert(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
 int launch_table_accum(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
 int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cudaStream_t stream);
-int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, double* out_coef, void* out_exps, int exp_bytes,
+int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, CoefOut out_coef, void* out_exps, int exp_bytes,
                             int64_t out_capacity, uint32_t* tile_state, int64_t* out_count_device, cudaStream_t stream);
 
 }  // namespace polylab

@@ -493,12 +493,26 @@ int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hd,
     return 1;
 }
 
+__global__ void __launch_bounds__(256) widen_kernel(const float* __restrict__ in, double* __restrict__ out, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) out[i] = (double)in[i];
+}
+
+int launch_widen(const void* in_f32, double* out, int64_t n, cudaStream_t stream)
+{
+    if (n <= 0) return 0;
+    int64_t blocks = (n + 1023) / 1024;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+    widen_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const float*)in_f32, out, n);
+    return 1;
+}
+
 // ----------------------------------------------------------------------------------------------- X1
 
 template <typename K>
-__global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict__ ka, const double* __restrict__ ca,
+__global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict__ ka, CoefIn ca,
                                                             uint32_t na, const K* __restrict__ kb,
-                                                            const double* __restrict__ cb, uint32_t nb,
+                                                            CoefIn cb, uint32_t nb,
                                                             K* __restrict__ keys, double* __restrict__ coefs, int dpos,
                                                             uint32_t dmask, uint32_t* hist)
 {
@@ -524,7 +538,7 @@ __global__ void __launch_bounds__(256) expand_packed_kernel(const K* __restrict_
     bh.flush(hist);
 }
 
-int launch_expand_packed(const void* ka, const double* ca, int64_t na, const void* kb, const double* cb, int64_t nb,
+int launch_expand_packed(const void* ka, CoefIn ca, int64_t na, const void* kb, CoefIn cb, int64_t nb,
                          const Plan& plan, void* keys, double* coefs, Control* ctl, int hd, cudaStream_t stream)
 {
     const int64_t n = na * nb;
@@ -584,9 +598,9 @@ int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hd, Control* c
 }
 
 // Raw product in (coef, exps) form, no keys: polylab_expand (reading A10).
-__global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, const double* __restrict__ ca, uint32_t na,
-                                                         ExpView eb, const double* __restrict__ cb, uint32_t nb,
-                                                         int nvars, double* __restrict__ out_coef, void* out_exps,
+__global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, CoefIn ca, uint32_t na,
+                                                         ExpView eb, CoefIn cb, uint32_t nb,
+                                                         int nvars, CoefOut out_coef, void* out_exps,
                                                          int32_t* status)
 {
     const uint32_t n = na * nb;
@@ -594,7 +608,7 @@ __global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, const doubl
     bool bad = false;
     for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += gridDim.x * blockDim.x) {
         const uint32_t i = q / nb, j = q - i * nb;
-        out_coef[q] = __dmul_rn(ca[i], cb[j]);
+        out_coef.store(q, __dmul_rn(ca[i], cb[j]));
         for (int v = 0; v < nvars; ++v) {
             const uint32_t x = load_exp(ea.base, ea.exp_bytes, (int64_t)i * ea.term_stride + (int64_t)v * ea.var_stride);
             const uint32_t y = load_exp(eb.base, eb.exp_bytes, (int64_t)j * eb.term_stride + (int64_t)v * eb.var_stride);
@@ -606,8 +620,8 @@ __global__ void __launch_bounds__(256) expand_raw_kernel(ExpView ea, const doubl
     if (bad) atomicMax(status, (int)POLYLAB_ERR_EXPONENT_RANGE);
 }
 
-int launch_expand_raw(const ExpView& ea, const double* ca, int64_t na, const ExpView& eb, const double* cb, int64_t nb,
-                      int nvars, double* out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream)
+int launch_expand_raw(const ExpView& ea, CoefIn ca, int64_t na, const ExpView& eb, CoefIn cb, int64_t nb,
+                      int nvars, CoefOut out_coef, void* out_exps, Control* ctl_status, cudaStream_t stream)
 {
     const int64_t n = na * nb;
     if (n <= 0) return 0;

@@ -16,7 +16,7 @@ namespace polylab {
 
 template <typename K, int THREADS, int ITEMS>
 __global__ void __launch_bounds__(THREADS)
-reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs, uint32_t n, K* __restrict__ ukeys,
+reduce_kernel(const K* __restrict__ keys, CoefIn coefs, uint32_t n, K* __restrict__ ukeys,
               double* __restrict__ usums, ReduceScratch sc, Control* ctl)
 {
     constexpr int TILE = THREADS * ITEMS, NW = THREADS / 32;
@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(256) reduce_fixup_kernel(uint32_t ntiles, doub
 }
 
 template <typename K>
-static int launch_reduce_t(int64_t n, const void* keys, const double* coefs, void* ukeys, double* usums,
+static int launch_reduce_t(int64_t n, const void* keys, CoefIn coefs, void* ukeys, double* usums,
                            const ReduceScratch& sc, Control* ctl, cudaStream_t stream)
 {
     constexpr int TILE = kReduceTile;
@@ -215,7 +215,7 @@ static int launch_reduce_t(int64_t n, const void* keys, const double* coefs, voi
     return 1;
 }
 
-int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coefs, void* ukeys, double* usums,
+int launch_reduce(int key_bytes, int64_t n, const void* keys, CoefIn coefs, void* ukeys, double* usums,
                   const ReduceScratch& sc, Control* ctl, cudaStream_t stream)
 {
     if (n <= 0) return 0;
@@ -229,7 +229,7 @@ int launch_reduce(int key_bytes, int64_t n, const void* keys, const double* coef
 template <typename K, int THREADS, int ITEMS>
 __global__ void __launch_bounds__(THREADS)
 prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usums, double tol,
-                    const __grid_constant__ Plan plan, double* __restrict__ out_coef, void* out_exps, int exp_bytes,
+                    const __grid_constant__ Plan plan, CoefOut out_coef, void* out_exps, int exp_bytes,
                     int wpr, int64_t out_capacity, uint32_t* tile_state, Control* ctl, int64_t* out_count_device,
                     K* __restrict__ out_keys)
 {
@@ -282,7 +282,7 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
         __syncthreads();
         const uint64_t obase = sm_base;
         for (uint32_t i = tid; i < total; i += THREADS)
-            if ((int64_t)(obase + i) < out_capacity) out_coef[obase + i] = usums[tile_base + sel[i]];
+            if ((int64_t)(obase + i) < out_capacity) out_coef.store(obase + i, usums[tile_base + sel[i]]);
         if (out_keys) {
             // packed output (the intermediate powers of polylab_pow_simplify): the survivors' keys stay keys
             for (uint32_t i = tid; i < total; i += THREADS)
@@ -326,7 +326,7 @@ int launch_async_status(const Control* ctl, int32_t* status_device, int64_t* out
 }
 
 int launch_prune_unpack(const Plan& plan, int64_t max_units, const void* ukeys, const double* usums, double tol,
-                        double* out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
+                        CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity, uint32_t* tile_state,
                         Control* ctl, int64_t* out_count_device, cudaStream_t stream, void* out_keys)
 {
     if (max_units <= 0) return 0;

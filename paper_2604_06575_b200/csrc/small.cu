@@ -34,7 +34,7 @@ struct SmallSmem {
 };
 
 template <typename K>
-__global__ void __launch_bounds__(kSmallThreads, 1) block_sort_reduce_kernel(const K* __restrict__ keys, const double* __restrict__ coefs,
+__global__ void __launch_bounds__(kSmallThreads, 1) block_sort_reduce_kernel(const K* __restrict__ keys, CoefIn coefs,
                                                                            const uint32_t* n_device, uint32_t n_host,
                                                                            const __grid_constant__ Plan plan, K* __restrict__ ukeys,
                                                                            double* __restrict__ usums, Control* ctl)
@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) block_sort_reduce_kernel(con
 }
 
 template <typename K>
-static int launch_block_sort_reduce_t(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
+static int launch_block_sort_reduce_t(const Plan& plan, const void* keys, CoefIn coefs, const uint32_t* n_device, uint32_t n,
                                       void* ukeys, double* usums, Control* ctl, cudaStream_t stream)
 {
     auto kern = block_sort_reduce_kernel<K>;
@@ -213,7 +213,7 @@ static int launch_block_sort_reduce_t(const Plan& plan, const void* keys, const 
     return 1;
 }
 
-int launch_block_sort_reduce(const Plan& plan, const void* keys, const double* coefs, const uint32_t* n_device, uint32_t n,
+int launch_block_sort_reduce(const Plan& plan, const void* keys, CoefIn coefs, const uint32_t* n_device, uint32_t n,
                              void* ukeys, double* usums, Control* ctl, cudaStream_t stream)
 {
     if (plan.key_bytes == 8) return launch_block_sort_reduce_t<uint64_t>(plan, keys, coefs, n_device, n, ukeys, usums, ctl, stream);

@@ -345,7 +345,7 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     a.rows = nullptr; a.exp_bytes = 0; a.status = &ctl->status;
     a.xa_keys = nullptr; a.xb_keys = nullptr; a.xa_coef = nullptr; a.xb_coef = nullptr; a.xnb = 1;
     if (xs) {
-        a.xa_keys = xs->ka; a.xb_keys = xs->kb; a.xa_coef = xs->ca; a.xb_coef = xs->cb; a.xnb = (uint32_t)xs->nb;
+        a.xa_keys = xs->ka; a.xb_keys = xs->kb; a.xa_coef = (const double*)xs->ca.p; a.xb_coef = (const double*)xs->cb.p; a.xnb = (uint32_t)xs->nb;   // fp64 here: api.cu widens fp32 operands
         auto go = [&](auto kern) {
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
             kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);

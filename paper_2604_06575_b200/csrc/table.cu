@@ -252,7 +252,7 @@ constexpr int kDenseItems = 8;
 constexpr int kDenseTile = kDenseThreads * kDenseItems;
 
 __global__ void __launch_bounds__(kDenseThreads) table_dense_emit_kernel(const __grid_constant__ TableArgs t, const __grid_constant__ Plan plan,
-                                                                         double tol, double* __restrict__ out_coef, void* out_exps,
+                                                                         double tol, CoefOut out_coef, void* out_exps,
                                                                          int exp_bytes, int wpr, int64_t out_capacity, uint32_t* tile_state,
                                                                          int64_t* out_count_device)
 {
@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(kDenseThreads) table_dense_emit_kernel(const _
         for (int j = 0; j < kDenseItems; ++j) {
             if (keep & (1u << j)) {
                 if ((int64_t)o < out_capacity) {
-                    out_coef[o] = s[j];
+                    out_coef.store(o, s[j]);
                     const uint64_t kk = first + j;
                     if (wpr > 0) {
                         uint32_t* row = (uint32_t*)out_exps + o * (uint64_t)wpr;
@@ -365,7 +365,7 @@ int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cu
     return 1;
 }
 
-int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, double* out_coef, void* out_exps, int exp_bytes,
+int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, CoefOut out_coef, void* out_exps, int exp_bytes,
                             int64_t out_capacity, uint32_t* tile_state, int64_t* out_count_device, cudaStream_t stream)
 {
     int64_t blocks = ((int64_t)t.nord + kDenseTile - 1) / kDenseTile;
