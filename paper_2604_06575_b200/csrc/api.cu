@@ -8,7 +8,26 @@
 
 #include "kernels.h"
 
+#include <mutex>
+
 namespace polylab {
+
+// (kernel address -> devices on which its dynamic shared-memory limit has been raised); see ensure_dynamic_smem
+bool smem_attr_done(const void* kern, int dev, bool mark)
+{
+    static std::mutex mu;
+    static const void* keys[256];
+    static unsigned long long masks[256];
+    static int used = 0;
+    std::lock_guard<std::mutex> lock(mu);
+    for (int i = 0; i < used; ++i)
+        if (keys[i] == kern) {
+            if (mark) masks[i] |= 1ull << dev;
+            return (masks[i] >> dev) & 1ull;
+        }
+    if (mark && used < 256) { keys[used] = kern; masks[used] = 1ull << dev; ++used; return true; }
+    return false;
+}
 
 static thread_local char g_cuda_error[256] = "";
 

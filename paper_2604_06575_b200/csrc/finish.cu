@@ -684,7 +684,7 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
                                                                        ntiles, tile_start, worklist, ctl);
     auto kern = finish_kernel<K>;
     constexpr size_t smem = FinishSmem::bytes;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device: set on every launch
+    ensure_dynamic_smem(kern, (size_t)smem);
     FinishArgs a;
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state; a.worklist = worklist;

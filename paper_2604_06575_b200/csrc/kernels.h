@@ -44,6 +44,19 @@ inline int sm_count()
     return cached[dev];
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE property of a kernel: set once per (kernel, device) -- a
+// small table keyed by the kernel's address (many kernels share one function-pointer TYPE) -- instead of on every launch.
+bool smem_attr_done(const void* kern, int dev, bool mark);
+template <typename F>
+inline void ensure_dynamic_smem(F kern, size_t bytes)
+{
+    int dev = 0;
+    const bool known = cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64;
+    if (known && smem_attr_done((const void*)kern, dev, false)) return;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess && known)
+        smem_attr_done((const void*)kern, dev, true);
+}
+
 inline int sort_tile(int key_bytes)
 {
     return key_bytes == 8 ? kSortThreads64 * kSortItems64 : key_bytes == 16 ? kSortThreads128 * kSortItems128 : kSortThreads256 * kSortItems256;

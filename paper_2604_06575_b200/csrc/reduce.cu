@@ -205,7 +205,7 @@ static int launch_reduce_t(int64_t n, const void* keys, CoefIn coefs, void* ukey
     constexpr int TILE = kReduceTile;
     const size_t smem = (size_t)TILE * (sizeof(K) + sizeof(double));
     auto kern = reduce_kernel<K, kReduceThreads, kReduceItems>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device: set on every launch
+    ensure_dynamic_smem(kern, (size_t)smem);
     const unsigned tiles = (unsigned)((n + TILE - 1) / TILE);
     kern<<<tiles, kReduceThreads, smem, stream>>>((const K*)keys, coefs, (uint32_t)n, (K*)ukeys, usums, sc, ctl);
     if (tiles > 1) {

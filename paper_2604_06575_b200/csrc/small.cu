@@ -210,7 +210,7 @@ static int launch_block_sort_reduce_t(const Plan& plan, const void* keys, CoefIn
                                       void* ukeys, double* usums, Control* ctl, cudaStream_t stream)
 {
     auto kern = block_sort_reduce_kernel<K>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallSmem<K>::bytes);
+    ensure_dynamic_smem(kern, (size_t)SmallSmem<K>::bytes);
     kern<<<1, kSmallThreads, SmallSmem<K>::bytes, stream>>>((const K*)keys, coefs, n_device, n, plan, (K*)ukeys, usums, ctl);
     return 1;
 }

@@ -318,7 +318,7 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 {
     using S = SortSmem<K, THREADS, ITEMS>;
     auto kern = sort_pass_kernel<K, THREADS, ITEMS, MINB, NEXT, RANK_ATOMIC>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());   // per device: set on every launch
+    ensure_dynamic_smem(kern, (size_t)S::bytes());
     kern<<<tiles, THREADS, S::bytes(), stream>>>(a);
 }
 
@@ -347,7 +347,7 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     if (xs) {
         a.xa_keys = xs->ka; a.xb_keys = xs->kb; a.xa_coef = (const double*)xs->ca.p; a.xb_coef = (const double*)xs->cb.p; a.xnb = (uint32_t)xs->nb;   // fp64 here: api.cu widens fp32 operands
         auto go = [&](auto kern) {
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
+            ensure_dynamic_smem(kern, (size_t)S::bytes());
             kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);
         };
         if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, kLoadProducts, false>);
@@ -360,7 +360,7 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
         for (int v = 0; v < plan.nvars && fast; ++v) fast = plan.width[v] == 8 && plan.bound[v] >= 255u;
         const int rb = plan.nvars * rows->exp_bytes;
         auto go = [&](auto kern) {
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes());
+            ensure_dynamic_smem(kern, (size_t)S::bytes());
             kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);
         };
         constexpr int KB = (int)sizeof(K);          // the byte-reversal path needs rows as long as the key

@@ -349,7 +349,7 @@ int launch_table_accum(const TableSrc& src, const TableArgs& t_in, bool dense, c
     const size_t smem = (size_t)t.nsm * 16;
     const bool prod = src.keys == nullptr;
     auto go = [&](auto kern) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)kAccSlots * 16));
+        ensure_dynamic_smem(kern, (size_t)((size_t)kAccSlots * 16));
         kern<<<(unsigned)blocks, threads, smem, stream>>>(src, t);
     };
     if (prod) { if (dense) go(table_accum_kernel<true, true>); else go(table_accum_kernel<true, false>); }
