@@ -511,9 +511,13 @@ static bool table_eligible(const Plan& plan, int64_t n, const Opts& o, const Att
 
 // Merges the N records of `src` in a table and emits the simplified polynomial.  *done = false: the table was abandoned
 // (too many distinct monomials) and nothing was emitted -- the caller continues on the sort path.
+// S1 fused into the table's insert pass (simplify, contiguous rows): the rows to pack and the digit whose histogram the sort
+// path would need if the table is abandoned
+struct FusedRows { const ExpView* ev; int hd; };
+
 static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layout& L, TableSrc src, double tol, const Opts& o,
                       CoefOut out_coef, void* out_exps, int64_t out_capacity, int64_t* out_nterms, int* launches, Timing& tm,
-                      cudaStream_t stream, bool* done, void* packed_keys = nullptr)
+                      cudaStream_t stream, bool* done, void* packed_keys = nullptr, const FusedRows* fr = nullptr)
 {
     *done = false;
     Control* ctl = (Control*)(ws + L.control);
@@ -544,7 +548,8 @@ static int table_path(const Plan& plan, int64_t n, unsigned char* ws, const Layo
         t.acc_lo = t.acc_hi + t.limit;
         PL_CUDA(cudaMemsetAsync(base, 0, (size_t)cap * sizeof(TableSlot) + (size_t)t.limit * 16, stream));
     }
-    *launches += launch_table_insert(src, t, dense, stream);
+    if (fr) *launches += launch_table_insert_rows(*fr->ev, n, plan, (uint64_t*)(ws + L.keys[0]), src.coef, t, dense, fr->hd, stream);
+    else *launches += launch_table_insert(src, t, dense, stream);
     struct Tail { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish, fin_count, tab_count, tab_overflow; } res;
     if (!dense) {
         PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
@@ -688,14 +693,20 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     int k = choose_prefix_passes(plan, nterms, o, at);
     const bool try_table = table_eligible(plan, nterms, o, at);
     const bool fuse = !try_table && k > 0 && rows_fusable(ev, nvars) && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
-    if (fuse) launches += launch_row_hist(ev, nterms, plan, plan.npasses - k, ctl, stream);      // S1 itself runs inside the first pass
+    // table path over contiguous rows: S1 runs inside the table's insert pass
+    const bool fuse_table = try_table && ev.row_major_contiguous && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
+    const int pack_hd = plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1;
+    if (fuse_table) { /* nothing here */ }
+    else if (fuse) launches += launch_row_hist(ev, nterms, plan, plan.npasses - k, ctl, stream);      // S1 itself runs inside the first pass
     else launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
     if (try_table) {
         tm.mark(POLYLAB_STAGE_PACK);
         TableSrc src = TableSrc();
         src.keys = (const uint64_t*)(ws + L.keys[0]); src.coef = CoefIn(coef, o.coef_f32);
         bool done = false;
-        rc = table_path(plan, nterms, ws, L, src, tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm, stream, &done);
+        const FusedRows fr = {&ev, pack_hd};
+        rc = table_path(plan, nterms, ws, L, src, tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm, stream, &done,
+                        nullptr, fuse_table ? &fr : nullptr);
         if (done || rc != POLYLAB_OK) return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
     }
     rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);

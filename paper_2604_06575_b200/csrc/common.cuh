@@ -263,6 +263,20 @@ __host__ inline int row_words(int nvars, int exp_bytes, const void* out_exps)
     return (rb % 4 == 0 && ((uintptr_t)out_exps & 3) == 0) ? rb / 4 : 0;      // 0: rows cannot be written as words
 }
 
+// S1 for one variable: range check against the plan's bound, field into the key (pack.cu, table.cu)
+template <typename K>
+__device__ __forceinline__ void pack_field(K& key, uint32_t e, int v, const Plan& plan, bool& bad)
+{
+    bad |= e > plan.bound[v];
+    key_or_field(key, e, plan.shift[v]);     // width 0 => bound 0 => e must be 0: nothing is OR-ed
+}
+
+// 16-byte asynchronous copy global -> shared (both 16-byte aligned); completion through cp.async.commit_group / wait_group
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+
 // --------------------------------------------------------------------------- control block
 
 // Small device-side state at the head of the workspace, zeroed at the start of every call.

@@ -219,6 +219,10 @@ constexpr int kTableDenseMaxBits = 22;
 constexpr uint32_t kTableMaxDistinct = 1u << 20;
 inline uint32_t table_dense_tile() { return 256u * 8u; }
 int launch_table_insert(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
+// S1 fused into the insert pass: contiguous row-major rows (ev.row_major_contiguous) -> keys[nterms] written, every record
+// inserted, the range check into ctl->status and (hd >= 0) the histogram of plan digit hd into ctl->hist[hd] as launch_pack does.
+int launch_table_insert_rows(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* keys, CoefIn coef, const TableArgs& t,
+                             bool dense, int hd, cudaStream_t stream);
 int launch_table_accum(const TableSrc& src, const TableArgs& t, bool dense, cudaStream_t stream);
 int launch_table_finalize(const TableArgs& t, uint64_t* ukeys, double* usums, cudaStream_t stream);
 int launch_table_dense_emit(const TableArgs& t, const Plan& plan, double tol, CoefOut out_coef, void* out_exps, int exp_bytes,

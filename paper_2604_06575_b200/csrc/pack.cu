@@ -175,12 +175,6 @@ struct BlockHist {
     }
 };
 
-template <typename K>
-__device__ __forceinline__ void pack_field(K& key, uint32_t e, int v, const Plan& plan, bool& bad)
-{
-    bad |= e > plan.bound[v];
-    key_or_field(key, e, plan.shift[v]);     // width 0 => bound 0 => e must be 0: nothing is OR-ed
-}
 
 // Rows contiguous in memory (row-major, 16-byte aligned base): each thread reads its row with the widest
 // word WB (bytes) that divides the row size; ES = bytes per exponent.
@@ -229,10 +223,6 @@ __global__ void __launch_bounds__(256) pack_rows_kernel(const uint8_t* __restric
 // its own row would issue narrow, misaligned loads (five 2-byte loads for a 10-byte row).  Instead the block brings a tile
 // of `tile_rows` consecutive rows into shared memory with aligned 16-byte asynchronous copies (cp.async), double-buffered:
 // the next tile is in flight while every thread picks its rows of the current one out of shared memory.
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
-}
 
 template <typename K, int ES>
 __global__ void __launch_bounds__(256) pack_rows_staged_kernel(const uint8_t* __restrict__ base, int64_t nterms, int tile_rows,

@@ -92,6 +92,31 @@ constexpr int kTabThreads = 256;
 constexpr int kTabItems = 8;
 constexpr int kTabTile = kTabThreads * kTabItems;
 
+// One record of the insert pass; called by all 32 lanes of a warp together (`valid` masks the tail).
+template <bool DENSE>
+__device__ __forceinline__ void insert_record(const TableArgs& t, bool valid, uint64_t key, double c, unsigned lane)
+{
+    uint32_t slot = 0, ord_unused, meta = 0;
+    bool ins = false, ok = true;
+    if (valid) ok = find_slot<DENSE, true>(t, key, slot, ins, ord_unused, meta);
+    if (!DENSE) {
+        // dense ordinals for the new keys: one atomicAdd per warp instruction
+        const unsigned m = __ballot_sync(kFullMask, ins);
+        if (m) {
+            uint32_t b = 0;
+            if (lane == (unsigned)(__ffs(m) - 1)) b = atomicAdd(&t.ctl->tab_count, (uint32_t)__popc(m));
+            b = __shfl_sync(kFullMask, b, __ffs(m) - 1);
+            if (ins) t.slots[slot].ord = b + __popc(m & lanemask_lt());
+            if (b + __popc(m) > t.limit) t.ctl->tab_overflow = 1u;
+        }
+        if (!ok) t.ctl->tab_overflow = 1u;
+    }
+    if (valid && ok) {
+        const uint32_t e = coef_meta(c);
+        if (meta < e) atomicMax(DENSE ? &t.meta[slot] : &t.slots[slot].meta, e);
+    }
+}
+
 template <bool PRODUCTS, bool DENSE>
 __global__ void __launch_bounds__(kTabThreads) table_insert_kernel(const __grid_constant__ TableSrc src, const __grid_constant__ TableArgs t)
 {
@@ -110,26 +135,81 @@ __global__ void __launch_bounds__(kTabThreads) table_insert_kernel(const __grid_
             uint64_t key = 0;
             double c = 0.0;
             if (valid) load_record<PRODUCTS>(src, q, key, c);
-            uint32_t slot = 0, ord_unused, meta = 0;
-            bool ins = false, ok = true;
-            if (valid) ok = find_slot<DENSE, true>(t, key, slot, ins, ord_unused, meta);
-            if (!DENSE) {
-                // dense ordinals for the new keys: one atomicAdd per warp instruction
-                const unsigned m = __ballot_sync(kFullMask, ins);
-                if (m) {
-                    uint32_t b = 0;
-                    if (lane == (unsigned)(__ffs(m) - 1)) b = atomicAdd(&t.ctl->tab_count, (uint32_t)__popc(m));
-                    b = __shfl_sync(kFullMask, b, __ffs(m) - 1);
-                    if (ins) t.slots[slot].ord = b + __popc(m & lanemask_lt());
-                    if (b + __popc(m) > t.limit) t.ctl->tab_overflow = 1u;
-                }
-                if (!ok) t.ctl->tab_overflow = 1u;
-            }
-            if (valid && ok) {
-                const uint32_t e = coef_meta(c);
-                if (meta < e) atomicMax(DENSE ? &t.meta[slot] : &t.slots[slot].meta, e);
+            insert_record<DENSE>(t, valid, key, c, lane);
+        }
+    }
+}
+
+// S1 fused into the insert pass (simplify with contiguous row-major exponent rows): a tile of rows comes into shared memory
+// by double-buffered 16-byte cp.async copies exactly as in pack_rows_staged_kernel (pack.cu); each thread packs its row,
+// stores the key -- the accumulate pass and, should the table be abandoned, the sort path read it -- and inserts it.  Saves
+// the pack kernel's launch and one read of the keys.  Blocks never stop early here (every key must be written); once the
+// table is abandoned they stop inserting.
+template <int ES, bool DENSE>
+__global__ void __launch_bounds__(kTabThreads) table_insert_rows_kernel(const uint8_t* __restrict__ base, int64_t nterms, int tile_rows,
+                                                                        const __grid_constant__ Plan plan, uint64_t* __restrict__ keys,
+                                                                        CoefIn coef, const __grid_constant__ TableArgs t, int hd)
+{
+    extern __shared__ __align__(16) unsigned char stage[];          // two buffers of tile_rows * row bytes + 16
+    __shared__ uint32_t sh[kRadix];
+    const unsigned lane = lane_id();
+    for (int b = threadIdx.x; b < kRadix; b += kTabThreads) sh[b] = 0u;
+    const int rb = plan.nvars * ES;
+    const int dpos = plan.digit_pos[hd >= 0 ? hd : 0];
+    const uint32_t dmask = (1u << plan.digit_bits[hd >= 0 ? hd : 0]) - 1u;
+    const int64_t nbytes = nterms * rb;
+    const int bufsz = (tile_rows * rb + 16 + 15) & ~15;
+    const int64_t step = (int64_t)gridDim.x * tile_rows;
+    auto issue = [&](int buf, int64_t t0) {
+        if (t0 < nterms) {
+            const int nr = (int)min((int64_t)tile_rows, nterms - t0);
+            const int64_t b0 = t0 * rb, b1 = b0 + (int64_t)nr * rb, a0 = b0 & ~(int64_t)15;
+            unsigned char* dst = stage + (size_t)buf * bufsz;
+            for (int64_t off = a0 + 16 * (int64_t)threadIdx.x; off < b1; off += 16 * kTabThreads) {
+                if (off + 16 <= nbytes) cp_async16(dst + (off - a0), base + off);
+                else for (int64_t b = off; b < nbytes; ++b) dst[b - a0] = base[b];
             }
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    bool bad = false;
+    int64_t t0 = (int64_t)blockIdx.x * tile_rows;
+    issue(0, t0);
+    for (int it = 0; t0 < nterms; ++it, t0 += step) {
+        const int cur = it & 1;
+        issue(cur ^ 1, t0 + step);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncthreads();
+        const int nr = (int)min((int64_t)tile_rows, nterms - t0);
+        const int64_t b0 = t0 * rb, a0 = b0 & ~(int64_t)15;
+        const unsigned char* src = stage + (size_t)cur * bufsz + (b0 - a0);
+        // once the table is abandoned the block only packs (a full table would cost 256 probes per record); warp-uniform
+        const bool live = DENSE || __shfl_sync(kFullMask, lane == 0 ? *(volatile uint32_t*)&t.ctl->tab_overflow : 0u, 0) == 0u;
+        for (int r0 = 0; r0 < nr; r0 += kTabThreads) {               // every lane of a warp takes part in insert_record
+            const int r = r0 + (int)threadIdx.x;
+            const bool valid = r < nr;
+            uint64_t key = 0;
+            double c = 0.0;
+            if (valid) {
+                const unsigned char* row = src + (int64_t)r * rb;
+                for (int v = 0; v < plan.nvars; ++v) {
+                    const uint32_t e = ES == 1 ? row[v] : ES == 2 ? ((const uint16_t*)row)[v] : ((const uint32_t*)row)[v];
+                    pack_field(key, e, v, plan, bad);
+                }
+                keys[t0 + r] = key;
+                c = coef[(size_t)(t0 + r)];
+                if (hd >= 0) atomicAdd(&sh[key_digit(key, dpos, dmask)], 1u);
+            }
+            if (live) insert_record<DENSE>(t, valid, key, c, lane);
+        }
+        __syncthreads();
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (bad) atomicMax(&t.ctl->status, (int)POLYLAB_ERR_EXPONENT_RANGE);
+    if (hd >= 0) {
+        __syncthreads();
+        for (int b = threadIdx.x; b < kRadix; b += kTabThreads)
+            if (sh[b]) atomicAdd(&t.ctl->hist[hd][b], sh[b]);
     }
 }
 
@@ -329,6 +409,25 @@ int launch_table_insert(const TableSrc& src, const TableArgs& t, bool dense, cud
     const bool prod = src.keys == nullptr;
     if (prod) { if (dense) table_insert_kernel<true, true><<<(unsigned)blocks, kTabThreads, 0, stream>>>(src, t); else table_insert_kernel<true, false><<<(unsigned)blocks, kTabThreads, 0, stream>>>(src, t); }
     else { if (dense) table_insert_kernel<false, true><<<(unsigned)blocks, kTabThreads, 0, stream>>>(src, t); else table_insert_kernel<false, false><<<(unsigned)blocks, kTabThreads, 0, stream>>>(src, t); }
+    return 1;
+}
+
+int launch_table_insert_rows(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* keys, CoefIn coef, const TableArgs& t,
+                             bool dense, int hd, cudaStream_t stream)
+{
+    if (nterms <= 0) return 0;
+    const int rb = plan.nvars * ev.exp_bytes;
+    int tile_rows = 16384 / rb;                              // at most 16 KB of rows per tile, two tiles in shared memory
+    tile_rows = tile_rows > 1024 ? 1024 : tile_rows < 32 ? 32 : tile_rows / 32 * 32;
+    int64_t blocks = (nterms + tile_rows - 1) / tile_rows;
+    if (blocks > sm_count() * 6) blocks = sm_count() * 6;
+    const size_t smem = 2 * (((size_t)tile_rows * rb + 16 + 15) & ~(size_t)15);
+    const uint8_t* base = (const uint8_t*)ev.base;
+#define POLYLAB_TIR(ES, D) table_insert_rows_kernel<ES, D><<<(unsigned)blocks, kTabThreads, smem, stream>>>(base, nterms, tile_rows, plan, keys, coef, t, hd)
+    if (ev.exp_bytes == 1) { if (dense) POLYLAB_TIR(1, true); else POLYLAB_TIR(1, false); }
+    else if (ev.exp_bytes == 2) { if (dense) POLYLAB_TIR(2, true); else POLYLAB_TIR(2, false); }
+    else { if (dense) POLYLAB_TIR(4, true); else POLYLAB_TIR(4, false); }
+#undef POLYLAB_TIR
     return 1;
 }
 
