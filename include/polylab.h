@@ -108,6 +108,12 @@ enum {
                                         no max_exp_host takes the maxima of a sample of the rows, sizes the key fields by
                                         their bit lengths, and lets S1's range check verify every row; a violation
                                         re-runs the call with full bounds (stats->bounds_retry = 1).  Same result. */
+    POLYLAB_FLAG_EXACT_HIST = 256u,   /* the bucket path always sweeps the rows for the exact histogram of its first prefix digit.  By
+                                        default a fused call with >= 2^22 terms and two or more prefix passes estimates that
+                                        histogram from a 1-2 % sample of the rows, lays the first pass's bins out with slack (7
+                                        sigma above the estimate) and lets the pass itself verify that none overran
+                                        (stats->hist_sampled = 1); an overrun re-runs the call with the sweep
+                                        (stats->hist_retry = 1).  Same result, bit for bit. */
     POLYLAB_FLAG_NO_TABLE = 64u,      /* never take the table path.  By default a call with 2^15 <= N <= 2^26 terms whose key fits 63 bits
                                         first merges like terms in a table (the packed key itself as the index when 2^B slots
                                         are affordable, else a hash table) with order-independent fixed-point accumulators,
@@ -161,6 +167,8 @@ typedef struct polylab_stats {
                                 distinct monomials were sorted (see POLYLAB_FLAG_NO_TABLE); 0: sort path */
     int32_t table_fallback;  /* 1 if the table path was tried and abandoned (too many distinct monomials) */
     int32_t small_path;      /* 1 if one thread block did the sort and the segmented sum (see POLYLAB_FLAG_NO_SMALL) */
+    int32_t hist_sampled;    /* 1 if the first prefix pass took slack bins from a sampled histogram (POLYLAB_FLAG_EXACT_HIST) */
+    int32_t hist_retry;      /* 1 if such a bin overran and the call re-ran with the exact histogram */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

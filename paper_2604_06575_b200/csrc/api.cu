@@ -36,12 +36,14 @@ static thread_local char g_cuda_error[256] = "";
 constexpr int kRetrySafeRank = -1000;
 constexpr int kRetryNoBucket = -1001;
 constexpr int kRetryExactBounds = -1002;       // an exponent exceeded the field sized from the sampled maxima
+constexpr int kRetryExactHist = -1003;         // a slack bin sized from the sampled histogram was too small
 
 struct Attempt {
     bool safe_rank;        // ballot-matching radix passes, LSD path only
     bool allow_bucket;     // may take the bucket path (finish.cu)
     bool exact_bounds;     // S0 reads every row (otherwise large inputs are sampled and S1's range check verifies)
     bool allow_table;      // may take the table path (table.cu); only the first attempt does
+    bool exact_hist;       // the first prefix pass gets an exact histogram (otherwise large fused inputs use slack bins)
 };
 
 static bool cuda_failed(cudaError_t e, const char* what)
@@ -184,6 +186,10 @@ static size_t table_region_bytes(int64_t n)
     return dense > hash ? dense : hash;
 }
 
+// Slack bins (sort.cu): from kSampleBoundsMinTerms terms on, the first prefix pass of a fused bucket-path call may take its
+// bin capacities from a sampled histogram; its output then needs room for the sum of the capacities.
+static int64_t slack_capacity(int64_t n) { return n >= kSampleBoundsMinTerms ? n + n / 8 + ((int64_t)1 << 21) : n; }
+
 static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
 {
     Layout L;
@@ -209,8 +215,9 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.red_hb = take(red_tiles * sizeof(uint32_t));
     L.red_frag = take(red_tiles * sizeof(double));
     L.red_cont = take(red_tiles);
-    for (int i = 0; i < 2; ++i) L.keys[i] = take((size_t)n * key_bytes);
-    for (int i = 0; i < 2; ++i) L.coefs[i] = take((size_t)n * sizeof(double));
+    // (the second buffers receive the first prefix pass, which may lay its bins out with slack: see slack_capacity)
+    for (int i = 0; i < 2; ++i) L.keys[i] = take((size_t)(i ? slack_capacity(n) : n) * key_bytes);
+    for (int i = 0; i < 2; ++i) L.coefs[i] = take((size_t)(i ? slack_capacity(n) : n) * sizeof(double));
     L.ka = take((size_t)na * key_bytes);
     L.kb = take((size_t)nb * key_bytes);
     L.ca = take((size_t)na * sizeof(double));
@@ -242,9 +249,10 @@ static void fill_stats(polylab_stats* st, const Plan& plan, int64_t n)
 {
     if (!st) return;
     const int32_t launches = st->kernel_launches, fallback = st->rank_fallback, bfall = st->bucket_fallback, bretry = st->bounds_retry;
-    const int32_t tfall = st->table_fallback;
+    const int32_t tfall = st->table_fallback, hretry = st->hist_retry;
     memset(st, 0, sizeof *st);
     st->table_fallback = tfall;
+    st->hist_retry = hretry;
     st->kernel_launches = launches;
     st->rank_fallback = fallback;
     st->bucket_fallback = bfall;
@@ -354,14 +362,14 @@ static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* w
 // ----------------------------------------------------------------------- shared tail of both paths
 
 // keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
-struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish; };
+struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish, fin_count, tab_count, tab_overflow, slack_overflow; };
 
 // Bucket path: k stable passes over the top k digits, then finish.cu.  The pairs are in (L.keys[0], coef0) and the
 // histogram of digit P-k is in ctl->hist[P-k].
 static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* ws, const Layout& L, CoefIn coef0,
                             double tol, const Opts& o, CoefOut out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, cudaStream_t stream, const ExpView* rows,
-                            const ExpandSrc* xs)
+                            const ExpandSrc* xs, bool slack)
 {
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
@@ -373,10 +381,11 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     }
     for (int s = 0; s < k; ++s) {
         const double* cin = (s == 0) ? (const double*)coef0.p : cbuf[s & 1];
+        const SlackIO sio = {slack && s == 0, slack && s == 1, ctl->slack_cap};
         *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
                                       cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr,
-                                      s == 0 ? xs : nullptr);
+                                      s == 0 ? xs : nullptr, (slack && s < 2) ? &sio : nullptr);
     }
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
@@ -396,12 +405,14 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     PL_CUDA(cudaMemcpyAsync(&res, &ctl->status, sizeof res, cudaMemcpyDeviceToHost, stream));
     PL_CUDA(cudaStreamSynchronize(stream));
     if (res.status == POLYLAB_ERR_EXPONENT_RANGE) return res.status;   // keys built from out-of-range exponents prove nothing below
+    if (slack && res.slack_overflow) return kRetryExactHist;           // a sampled bin capacity was too small: nothing valid below
     if (res.overflow) return kRetryNoBucket;
     if (res.unsorted) return kRetrySafeRank;
     tm.finish(o.stats);
     if (o.stats) {
         o.stats->distinct = res.distinct; o.stats->survivors = res.survivors;
         o.stats->prefix_passes = k; o.stats->sort_passes = k; o.stats->refinish_tiles = (int32_t)res.refinish;
+        o.stats->hist_sampled = slack ? 1 : 0;
     }
     if (res.status != POLYLAB_OK) return res.status;
     *out_nterms = (int64_t)res.survivors;
@@ -422,11 +433,11 @@ static int sort_reduce_emit(const Plan& plan, int k_bucket, int64_t n, unsigned 
                             double tol, const Opts& o, CoefOut out_coef, void* out_exps, int64_t out_capacity,
                             int64_t* out_nterms, int* launches, Timing& tm, bool safe_rank, cudaStream_t stream,
                             const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr, const BatchOut* batch = nullptr,
-                            void* packed_keys = nullptr)
+                            void* packed_keys = nullptr, bool slack = false)
 {
     if (k_bucket > 0)
         return bucket_sort_emit(plan, k_bucket, n, ws, L, coef0, tol, o, out_coef, out_exps, out_capacity, out_nterms, launches,
-                                tm, stream, rows, xs);
+                                tm, stream, rows, xs, slack);
     Control* ctl = (Control*)(ws + L.control);
     void* kbuf[2] = {ws + L.keys[0], ws + L.keys[1]};
     double* cbuf[2] = {(double*)(ws + L.coefs[0]), (double*)(ws + L.coefs[1])};
@@ -696,7 +707,40 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     // table path over contiguous rows: S1 runs inside the table's insert pass
     const bool fuse_table = try_table && ev.row_major_contiguous && !(o.flags & POLYLAB_FLAG_NO_FUSED_PACK);
     const int pack_hd = plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1;
-    if (fuse_table) { /* nothing here */ }
+    // Slack bins: a large fused bucket-path call does not sweep the rows for the first prefix digit's exact histogram (0.5 ms
+    // on 2e8 terms); it estimates the bins from a 1-2 % sample, gives each a capacity 7 sigma above its estimate, and the pass
+    // itself verifies that no bin overran (else the call re-runs with the exact sweep: stats->hist_retry).
+    bool slack = false;
+    if (fuse && k >= 2 && nterms >= kSampleBoundsMinTerms && !at.exact_hist &&
+        !(o.flags & (POLYLAB_FLAG_EXACT_HIST | POLYLAB_FLAG_DEVICE_COUNT | POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE))) {
+        const int d = plan.npasses - k;
+        const int nsegs = sm_count() * 8;
+        launches += launch_row_hist_sample(ev, nterms, plan, d, ctl->est, nsegs, 2048, stream);
+        uint32_t est[kRadix], cap[kRadix];
+        PL_CUDA(cudaMemcpyAsync(est, ctl->est, sizeof est, cudaMemcpyDeviceToHost, stream));
+        PL_CUDA(cudaStreamSynchronize(stream));
+        uint64_t ssum = 0, cmax = 0;
+        for (int b = 0; b < kRadix; ++b) { ssum += est[b]; cmax = est[b] > cmax ? est[b] : cmax; }
+        if (ssum > 0) {
+            const double f = (double)nterms / (double)ssum;
+            double total = 0.0;
+            for (int b = 0; b < kRadix; ++b) {
+                const double c = (double)est[b];
+                const double cb = ceil(f * (c + 7.0 * sqrt(c + 1.0) + 8.0));
+                cap[b] = cb > 4.0e9 ? 0xffffffffu : (uint32_t)cb;
+                total += cb;
+            }
+            // the skew pre-check of bucket_precheck, on the estimate; and the capacities must fit the buffer
+            const int rest = plan.key_bits - plan.digit_pos[d] - plan.digit_bits[d];
+            const bool even = ((uint64_t)((double)cmax * f) >> rest) <= (uint64_t)bucket_room(plan, k, nterms) * 7 / 8;
+            if (even && total <= (double)slack_capacity(nterms)) {
+                PL_CUDA(cudaMemcpyAsync(ctl->hist[d], cap, sizeof cap, cudaMemcpyHostToDevice, stream));
+                PL_CUDA(cudaMemcpyAsync(ctl->slack_cap, cap, sizeof cap, cudaMemcpyHostToDevice, stream));
+                slack = true;
+            }
+        }
+    }
+    if (fuse_table || slack) { /* S1 runs inside the table's insert pass / the histogram is an estimate */ }
     else if (fuse) launches += launch_row_hist(ev, nterms, plan, plan.npasses - k, ctl, stream);      // S1 itself runs inside the first pass
     else launches += launch_pack(ev, nterms, plan, ws + L.keys[0], ctl, plan.npasses > 0 ? (k ? plan.npasses - k : 0) : -1, stream);
     if (try_table) {
@@ -709,11 +753,13 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
                         nullptr, fuse_table ? &fr : nullptr);
         if (done || rc != POLYLAB_OK) return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
     }
-    rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
-    if (rc != POLYLAB_OK) return rc;
+    if (!slack) {
+        rc = bucket_precheck(plan, &k, nterms, ws, L, o, &launches, stream, fuse ? &ev : nullptr);
+        if (rc != POLYLAB_OK) return rc;
+    }
     tm.mark(POLYLAB_STAGE_PACK);
     rc = sort_reduce_emit(plan, k, nterms, ws, L, CoefIn(coef, o.coef_f32), tol, o, CoefOut(out_coef, o.coef_f32), out_exps, out_capacity, out_nterms, &launches, tm,
-                          at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr);
+                          at.safe_rank, stream, (fuse && k > 0) ? &ev : nullptr, nullptr, nullptr, nullptr, slack);
     return (rc == POLYLAB_ERR_EXPONENT_RANGE && sampled) ? kRetryExactBounds : rc;
 }
 
@@ -728,13 +774,16 @@ extern "C++" {
 template <typename F>
 static int run_attempts(const polylab_opts* opts, F once)
 {
-    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; opts->stats->bounds_retry = 0; opts->stats->table_fallback = 0; }
-    Attempt at = {wants_safe_rank(opts), true, false, true};
+    if (opts && opts->stats) { opts->stats->kernel_launches = 0; opts->stats->rank_fallback = 0; opts->stats->bucket_fallback = 0; opts->stats->bounds_retry = 0; opts->stats->table_fallback = 0; opts->stats->hist_retry = 0; }
+    Attempt at = {wants_safe_rank(opts), true, false, true, false};
     int rc = once(at);
-    for (int tries = 0; tries < 3 && (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank); ++tries) {
+    for (int tries = 0; tries < 4 && (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank || rc == kRetryExactHist); ++tries) {
         polylab_stats* st = opts ? opts->stats : nullptr;
-        if (rc != kRetryExactBounds) at.allow_table = false;
-        if (rc == kRetryExactBounds) {             // each retry only ever tightens the attempt, so three suffice
+        if (rc != kRetryExactBounds && rc != kRetryExactHist) at.allow_table = false;
+        if (rc == kRetryExactHist) {
+            if (st) st->hist_retry = 1;
+            at.exact_hist = true;
+        } else if (rc == kRetryExactBounds) {             // each retry only ever tightens the attempt, so three suffice
             if (st) st->bounds_retry = 1;
             at.exact_bounds = true;
         } else if (rc == kRetryNoBucket) {
@@ -747,7 +796,7 @@ static int run_attempts(const polylab_opts* opts, F once)
         }
         rc = once(at);
     }
-    if (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank) rc = POLYLAB_ERR_INTERNAL;
+    if (rc == kRetryExactBounds || rc == kRetryNoBucket || rc == kRetrySafeRank || rc == kRetryExactHist) rc = POLYLAB_ERR_INTERNAL;
     return rc;
 }
 }  // extern "C++"

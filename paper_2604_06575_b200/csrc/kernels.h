@@ -93,6 +93,10 @@ bool rows_fusable(const ExpView& ev, int nvars);
 // Histogram of plan digit `hist_digit` straight from such rows into ctl->hist[hist_digit] (no keys are written).
 int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hist_digit, Control* ctl, cudaStream_t stream);
 
+// The same histogram over a sample: `nsegs` evenly spaced segments of `seg_rows` rows, into est[256] (zero before).
+int launch_row_hist_sample(const ExpView& ev, int64_t nterms, const Plan& plan, int hist_digit, uint32_t* est, int nsegs, int seg_rows,
+                           cudaStream_t stream);
+
 // S1 for the test entry point: always writes (hi, lo) pairs.
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,
                      cudaStream_t stream);
@@ -116,6 +120,13 @@ int launch_expand_raw(const ExpView& ea, CoefIn ca, int64_t na, const ExpView& e
 // debug_unstable: test hook, reverses the lane order of the atomic kernel.
 // `xs` (packed operands of a product): X1 fused into the pass -- keys_in / coef_in are ignored, record q = i*nb + j is
 // formed in registers as (ka_i + kb_j, fl(ca_i * cb_j)); atomic ranking only.
+// Slack bins: a pass given per-bin CAPACITIES instead of an exact histogram (`write`: ctl->hist[pass] holds them) lays its
+// output out with holes and records the exact counts; the pass after it (`read`, `cap` = the same capacities) maps compact
+// record numbers onto that layout.  ctl->slack_overflow != 0 afterwards: a bin was too small, nothing valid was produced.
+struct SlackIO {
+    bool write, read;
+    const uint32_t* cap;        // DEVICE [256]
+};
 struct ExpandSrc {
     const void* ka;
     CoefIn ca;
@@ -126,7 +137,8 @@ struct ExpandSrc {
 };
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream, const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr);
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows = nullptr, const ExpandSrc* xs = nullptr,
+                     const struct SlackIO* slack = nullptr);
 
 // Histogram of plan digit `hist_digit` over the na*nb products of packed operands, without storing them.
 int launch_expand_hist(const ExpandSrc& xs, const Plan& plan, int hist_digit, Control* ctl, cudaStream_t stream);

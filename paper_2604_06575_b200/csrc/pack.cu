@@ -450,10 +450,86 @@ __global__ void __launch_bounds__(256) row_hist_kernel(const uint8_t* __restrict
     bh.flush(hist);
 }
 
+// The same histogram over a SAMPLE of the rows: block b reads rows [b * seg_stride, b * seg_stride + seg_rows).  The first
+// prefix pass of the bucket path then lays its bins out with slack sized from this estimate (api.cu, sort.cu: slack bins)
+// instead of waiting for a sweep over every row.
+template <int RB, int ES>
+__global__ void __launch_bounds__(256) row_hist_sample_kernel(const uint8_t* __restrict__ base, int64_t nterms, int64_t seg_stride,
+                                                              int seg_rows, DigitParts dp, uint32_t* hist)
+{
+    __shared__ uint32_t sh[kRadix];
+    BlockHist bh;
+    bh.init(sh);
+    __syncthreads();
+    const int64_t t0 = (int64_t)blockIdx.x * seg_stride, t1 = min(nterms, t0 + seg_rows);
+    for (int64_t t = t0 + threadIdx.x; t < t1; t += blockDim.x) {
+        uint32_t w[RB / 4];
+        if (RB == 16) {
+            const uint4 q = __ldg((const uint4*)(base + t * RB));
+            w[0] = q.x; w[RB / 4 > 1 ? 1 : 0] = q.y; w[RB / 4 > 2 ? 2 : 0] = q.z; w[RB / 4 > 3 ? 3 : 0] = q.w;
+        } else {
+            const uint2 q = __ldg((const uint2*)(base + t * RB));
+            w[0] = q.x; w[RB / 4 > 1 ? 1 : 0] = q.y;
+        }
+        uint32_t d = 0;
+        for (int i = 0; i < dp.n; ++i) {
+            const int v = dp.var[i];
+            const int wi = ES == 4 ? v : ES == 2 ? (v >> 1) : (v >> 2);
+            uint32_t x = w[0];
+            if (RB / 4 > 1 && wi == 1) x = w[RB / 4 > 1 ? 1 : 0];
+            if (RB / 4 > 2 && wi == 2) x = w[RB / 4 > 2 ? 2 : 0];
+            if (RB / 4 > 3 && wi == 3) x = w[RB / 4 > 3 ? 3 : 0];
+            uint32_t e;
+            if (ES == 4) e = x;
+            else if (ES == 2) e = (x >> (16 * (v & 1))) & 0xffffu;
+            else e = (x >> (8 * (v & 3))) & 0xffu;
+            e = min(e, dp.emax[i]);
+            const int ls = dp.lshift[i];
+            d |= ls >= 0 ? (e << ls) : (e >> -ls);
+        }
+        bh.add(d & dp.mask);
+    }
+    __syncthreads();
+    bh.flush(hist);
+}
+
 bool rows_fusable(const ExpView& ev, int nvars)
 {
     const int rb = nvars * ev.exp_bytes;
     return ev.row_major_contiguous && (rb == 8 || rb == 16);
+}
+
+static DigitParts digit_parts(const Plan& plan, int hd);
+
+int launch_row_hist_sample(const ExpView& ev, int64_t nterms, const Plan& plan, int hd, uint32_t* est, int nsegs, int seg_rows, cudaStream_t stream)
+{
+    if (nterms <= 0 || !rows_fusable(ev, plan.nvars) || hd < 0 || hd >= plan.npasses || nsegs < 1) return 0;
+    const DigitParts dp = digit_parts(plan, hd);
+    const int rb = plan.nvars * ev.exp_bytes;
+    const uint8_t* base = (const uint8_t*)ev.base;
+    const int64_t seg_stride = nterms / nsegs > 0 ? nterms / nsegs : 1;
+#define POLYLAB_RHS(RB, ES) row_hist_sample_kernel<RB, ES><<<(unsigned)nsegs, 256, 0, stream>>>(base, nterms, seg_stride, seg_rows, dp, est)
+    if (rb == 16) { if (ev.exp_bytes == 1) POLYLAB_RHS(16, 1); else if (ev.exp_bytes == 2) POLYLAB_RHS(16, 2); else POLYLAB_RHS(16, 4); }
+    else { if (ev.exp_bytes == 1) POLYLAB_RHS(8, 1); else if (ev.exp_bytes == 2) POLYLAB_RHS(8, 2); else POLYLAB_RHS(8, 4); }
+#undef POLYLAB_RHS
+    return 1;
+}
+
+static DigitParts digit_parts(const Plan& plan, int hd)
+{
+    DigitParts dp;
+    dp.n = 0;
+    const int dpos = plan.digit_pos[hd], dbits = plan.digit_bits[hd];
+    dp.mask = (1u << dbits) - 1u;
+    for (int v = 0; v < plan.nvars; ++v) {
+        const int lo = plan.shift[v], hi = lo + plan.width[v];
+        if (plan.width[v] == 0 || hi <= dpos || lo >= dpos + dbits) continue;
+        dp.var[dp.n] = (uint8_t)v;
+        dp.lshift[dp.n] = (int8_t)(lo - dpos);
+        dp.emax[dp.n] = plan.bound[v];
+        ++dp.n;
+    }
+    return dp;
 }
 
 int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int hd, Control* ctl, cudaStream_t stream)

@@ -21,8 +21,12 @@ struct SortSmem {
     static constexpr int NW = THREADS / 32;
     static constexpr size_t stage_bytes = (size_t)TILE * sizeof(K);
     // per-warp histograms of this digit, the block's histogram of the next digit, bin starts, deltas, scan scratch
-    static constexpr size_t bytes() { return stage_bytes + (size_t)(NW * kRadix + 3 * kRadix + NW + 4) * sizeof(uint32_t); }
+    static constexpr size_t total_bytes = stage_bytes + (size_t)(NW * kRadix + 3 * kRadix + NW + 4) * sizeof(uint32_t);
+    static constexpr size_t bytes() { return total_bytes; }
 };
+
+constexpr int kHoleyStride = kRadix + 4;                              // the holey reader's two prefix arrays in shared memory
+constexpr size_t kHoleyBytes = 2 * kHoleyStride * sizeof(uint32_t);
 
 struct PassArgs {
     const void* keys_in;
@@ -40,6 +44,16 @@ struct PassArgs {
     uint32_t* hist_next;
     uint32_t* ticket;
     int reverse_lanes;          // POLYLAB_FLAG_DEBUG_UNSTABLE: the atomic kernel maps lane l to record 31 - l
+    // Slack bins (first prefix pass without an exact histogram, api.cu): hist_this holds per-bin CAPACITIES, so the bins
+    // of the output are laid out with holes.  The pass refuses to write a tile that would overrun a bin (slack_overflow)
+    // and its last tile leaves the exact bin counts in slack_count.
+    uint32_t* slack_count;      // [256] or nullptr
+    uint32_t* slack_overflow;
+    uint32_t last_tile;
+    // ... and the pass that READS such an output (HOLEY): record number pos of the compact order lives at
+    // slack_pstart[b] + (pos - slack_cstart[b]) for the bin b with slack_cstart[b] <= pos < slack_cstart[b + 1]
+    const uint32_t* slack_cstart;   // [257] exclusive prefix of the exact counts
+    const uint32_t* slack_pstart;   // [257] exclusive prefix of the capacities
     // S1 fused into the pass (ROWS > 0): keys are packed in registers from contiguous exponent rows of ROWS bytes
     const uint8_t* rows;
     int exp_bytes;
@@ -99,7 +113,7 @@ __device__ __forceinline__ K pack_row_inline(const PassArgs& a, const Plan& plan
 // values in ascending lane order on sm_100a (measured, profiles/r1b_shared_atomics.md; not documented), which
 // is what makes the pass stable; the reduce step verifies the sorted order and the call falls back to the
 // ballot-matching kernel (RANK_ATOMIC = false) if it ever does not hold.
-template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC, int ROWS, bool BYTES = false>
+template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC, int ROWS, bool BYTES = false, bool HOLEY = false, bool SLACK = false>
 __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* plan, unsigned char* smem_raw, uint32_t tile,
                                                uint32_t tile_base, uint32_t tile_n)
 {
@@ -123,6 +137,30 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
     const uint32_t chunk = warp * 32u * ITEMS + ((RANK_ATOMIC && a.reverse_lanes) ? 31u - lane : lane);
     K key[ITEMS];
     bool bad = false;
+    // HOLEY input: the bin of the tile's first record = the number of compact bin starts at or below it, minus one.  A tile nearly always lies inside one or two bins: then a record's address is its number plus one of two
+    // shifts; only a tile that spans more walks the bin starts per record.
+    uint32_t hb0 = 0, hbnd = 0xffffffffu, hshift0 = 0, hshift1 = 0;
+    bool two_bins = true;
+    const uint32_t* hs_c = (const uint32_t*)(smem_raw + S::total_bytes);     // [257] compact bin starts, [257] physical bin starts
+    const uint32_t* hs_p = hs_c + kHoleyStride;
+    if (HOLEY) {
+        // (the kernel copied both prefix arrays into shared memory while the tile ticket was in flight; a block-wide count
+        // instead of a binary search: dependent global loads at the head of every tile cost the pass 5-10 %)
+        const bool below = tid < (unsigned)kRadix && hs_c[tid] <= tile_base;
+        hb0 = (uint32_t)__syncthreads_count(below ? 1 : 0) - 1u;
+        hshift0 = hs_p[hb0] - hs_c[hb0];
+        hbnd = hs_c[hb0 + 1];
+        if (hb0 + 1 < (uint32_t)kRadix) {
+            hshift1 = hs_p[hb0 + 1] - hbnd;
+            two_bins = tile_base + tile_n <= hs_c[hb0 + 2];
+        }
+    }
+    auto holey_index = [&](uint32_t pos) -> uint32_t {
+        if (two_bins) return pos + (pos < hbnd ? hshift0 : hshift1);
+        uint32_t bb = hb0;
+        while (pos >= hs_c[bb + 1]) ++bb;
+        return hs_p[bb] + (pos - hs_c[bb]);
+    };
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
@@ -132,7 +170,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
                 // step X1 in registers: key = ka_i + kb_j (fields never carry into each other), the product is never stored
                 const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
                 key[j] = key_add(((const K*)a.xa_keys)[i], ((const K*)a.xb_keys)[jj]);
-            } else key[j] = keys_in[tile_base + li];
+            } else key[j] = keys_in[HOLEY ? holey_index(tile_base + li) : tile_base + li];
         } else key[j] = key_max<K>();
     }
     if (ROWS > 0 && bad) atomicMax(a.status, (int)POLYLAB_ERR_EXPONENT_RANGE);
@@ -216,7 +254,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         if (ROWS == kLoadProducts) {
             const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
             c[j] = (FULL || li < tile_n) ? __dmul_rn(a.xa_coef[i], a.xb_coef[jj]) : 0.0;     // one IEEE multiplication, never contracted
-        } else c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
+        } else c[j] = (FULL || li < tile_n) ? coef_in[HOLEY ? holey_index(tile_base + li) : tile_base + li] : 0.0;   // (the mapping is recomputed: 20 indices kept live through the ranking would spill)
     }
 
     // ---- decoupled look-back: number of records with digit b in all earlier tiles.  The walk over the predecessors
@@ -246,14 +284,25 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         st_volatile_u32(my_state, ((excl + count) << 2) | a.flag_inclusive);
     }
     if (bt) sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
-    __syncthreads();
+    bool skip = false;
+    if (SLACK) {
+        // slack bins: hist_this are capacities.  A tile that would overrun one writes nothing and raises the flag (the call
+        // re-runs with an exact histogram); the last tile's inclusive totals are the exact bin counts.
+        bool ovf = false;
+        if (bt) {
+            ovf = excl + count > a.hist_this[b];
+            if (tile == a.last_tile) a.slack_count[b] = excl + count;
+        }
+        skip = __syncthreads_or(ovf ? 1 : 0) != 0;
+        if (skip && tid == 0) *a.slack_overflow = 1u;
+    } else __syncthreads();
 
     // ---- write keys: slot s of the sorted tile, contiguous per bin
     uint32_t dst[ITEMS];
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if (FULL || s < tile_n) {
+        if ((FULL || s < tile_n) && !skip) {
             const K kk = stage[s];
             dst[k] = s + sm_delta[(key_word(kk, a.dword) >> a.dshift) & a.dmask];
             keys_out[dst[k]] = kk;
@@ -267,7 +316,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if (FULL || s < tile_n) coef_out[dst[k]] = stage_c[s];
+        if ((FULL || s < tile_n) && !skip) coef_out[dst[k]] = stage_c[s];
     }
 }
 
@@ -292,8 +341,50 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_c
     else sort_tile_body<K, THREADS, ITEMS, NEXT, false, RANK_ATOMIC, 0>(a, nullptr, smem_raw, tile, tile_base, tile_n);
 }
 
+// The same pass over an input whose bins were laid out with slack by the previous pass (see PassArgs::slack_cstart).
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT>
+__global__ void __launch_bounds__(THREADS, MINB) sort_pass_holey_kernel(const __grid_constant__ PassArgs a)
+{
+    using S = SortSmem<K, THREADS, ITEMS>;
+    constexpr int TILE = S::TILE, NW = S::NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* whist = (uint32_t*)(smem_raw + S::stage_bytes);
+    uint32_t* scratch = whist + NW * kRadix + 3 * kRadix;
+
+    const unsigned tid = threadIdx.x;
+    if (tid == 0) scratch[NW + 2] = atomicAdd(a.ticket, 1u);
+    uint32_t* hs = (uint32_t*)(smem_raw + S::total_bytes);
+    for (int i = tid; i <= kRadix; i += THREADS) {
+        hs[i] = __ldg(a.slack_cstart + i);
+        hs[kHoleyStride + i] = __ldg(a.slack_pstart + i);
+    }
+    for (int i = tid; i < (NW + 1) * kRadix; i += THREADS) whist[i] = 0u;
+    __syncthreads();
+    const uint32_t tile = scratch[NW + 2];
+    const uint32_t tile_base = tile * (uint32_t)TILE;
+    const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, 0, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, 0, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+}
+
+// exclusive prefixes of the exact bin counts and of the bin capacities (257 entries each), for the holey reader
+__global__ void slack_prefix_kernel(const uint32_t* __restrict__ count, const uint32_t* __restrict__ cap, uint32_t* cstart, uint32_t* pstart)
+{
+    __shared__ uint32_t scratch[kRadix / 32 + 2];
+    const unsigned b = threadIdx.x;
+    uint32_t total;
+    const uint32_t c = count[b], p = cap[b];
+    const uint32_t ce = block_exclusive_scan<kRadix>(c, scratch, &total);
+    cstart[b] = ce;
+    if (b == kRadix - 1) cstart[kRadix] = total;
+    __syncthreads();
+    const uint32_t pe = block_exclusive_scan<kRadix>(p, scratch, &total);
+    pstart[b] = pe;
+    if (b == kRadix - 1) pstart[kRadix] = total;
+}
+
 // The same pass with S1 fused in: reads exponent rows instead of keys (first pass of the bucket path).
-template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, int ROWS, bool BYTES>
+template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, int ROWS, bool BYTES, bool SLACK = false>
 __global__ void __launch_bounds__(THREADS, MINB) sort_pass_rows_kernel(const __grid_constant__ PassArgs a, const __grid_constant__ Plan plan)
 {
     using S = SortSmem<K, THREADS, ITEMS>;
@@ -309,8 +400,8 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_rows_kernel(const __g
     const uint32_t tile = scratch[NW + 2];
     const uint32_t tile_base = tile * (uint32_t)TILE;
     const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
-    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, ROWS, BYTES>(a, &plan, smem_raw, tile, tile_base, tile_n);
-    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES>(a, &plan, smem_raw, tile, tile_base, tile_n);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, ROWS, BYTES, false, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES, false, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
 }
 
 template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
@@ -325,7 +416,8 @@ static void launch_sort_pass_k(const PassArgs& a, unsigned tiles, cudaStream_t s
 template <typename K, int THREADS, int ITEMS, int MINB>
 static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in,
                               const double* coef_in, void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl,
-                              bool safe_rank, bool debug_unstable, const ExpView* rows, const ExpandSrc* xs, cudaStream_t stream)
+                              bool safe_rank, bool debug_unstable, const ExpView* rows, const ExpandSrc* xs, cudaStream_t stream,
+                              const SlackIO* slack)
 {
     using S = SortSmem<K, THREADS, ITEMS>;
     const unsigned tiles = (unsigned)((n + S::TILE - 1) / S::TILE);
@@ -342,6 +434,20 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     a.flag_inclusive = (seq & 1) ? 0u : 2u;
     a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[has_next ? next : kMaxPasses]; a.ticket = &ctl->ticket[seq];
     a.reverse_lanes = debug_unstable ? 1 : 0;
+    a.slack_count = nullptr; a.slack_overflow = nullptr; a.last_tile = tiles - 1u; a.slack_cstart = nullptr; a.slack_pstart = nullptr;
+    if (slack && slack->write) { a.slack_count = ctl->slack_count; a.slack_overflow = &ctl->slack_overflow; }
+    if (slack && slack->read) {
+        // the previous pass left holes: prefixes of its exact counts and of its capacities, then the holey reader
+        slack_prefix_kernel<<<1, kRadix, 0, stream>>>(ctl->slack_count, slack->cap, ctl->slack_cstart, ctl->slack_pstart);
+        a.slack_cstart = ctl->slack_cstart; a.slack_pstart = ctl->slack_pstart;
+        auto go = [&](auto kern) {
+            ensure_dynamic_smem(kern, (size_t)S::bytes() + kHoleyBytes);
+            kern<<<tiles, THREADS, S::bytes() + kHoleyBytes, stream>>>(a);
+        };
+        if (has_next) go(sort_pass_holey_kernel<K, THREADS, ITEMS, MINB, true>);
+        else go(sort_pass_holey_kernel<K, THREADS, ITEMS, MINB, false>);
+        return 2;
+    }
     a.rows = nullptr; a.exp_bytes = 0; a.status = &ctl->status;
     a.xa_keys = nullptr; a.xb_keys = nullptr; a.xa_coef = nullptr; a.xb_coef = nullptr; a.xnb = 1;
     if (xs) {
@@ -364,6 +470,12 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
             kern<<<tiles, THREADS, S::bytes(), stream>>>(a, plan);
         };
         constexpr int KB = (int)sizeof(K);          // the byte-reversal path needs rows as long as the key
+        if (a.slack_count && has_next) {               // slack bins: the first of two or more prefix passes (always has a next digit)
+            if (fast) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, KB, true, true>);
+            else if (rb == 16) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 16, false, true>);
+            else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 8, false, true>);
+            return 1;
+        }
         if (fast) { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, KB, true>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, KB, true>); }
         else if (rb == 16) { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 16, false>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, 16, false>); }
         else { if (has_next) go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, true, 8, false>); else go(sort_pass_rows_kernel<K, THREADS, ITEMS, MINB, false, 8, false>); }
@@ -381,17 +493,17 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
 
 int launch_sort_pass(const Plan& plan, int pass, int next, int seq, int64_t n, const void* keys_in, const double* coef_in,
                      void* keys_out, double* coef_out, uint32_t* tile_state, Control* ctl, bool safe_rank,
-                     bool debug_unstable, cudaStream_t stream, const ExpView* rows, const ExpandSrc* xs)
+                     bool debug_unstable, cudaStream_t stream, const ExpView* rows, const ExpandSrc* xs, const SlackIO* slack)
 {
     if (n <= 0) return 0;
     if (plan.key_bytes == 8)
         return launch_sort_pass_t<uint64_t, kSortThreads64, kSortItems64, 3>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                             tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
+                                                             tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream, slack);
     if (plan.key_bytes == 16)
         return launch_sort_pass_t<Key128, kSortThreads128, kSortItems128, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                            tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream);
+                                                            tile_state, ctl, safe_rank, debug_unstable, rows, xs, stream, slack);
     return launch_sort_pass_t<Key256, kSortThreads256, kSortItems256, 2>(plan, pass, next, seq, n, keys_in, coef_in, keys_out, coef_out,
-                                                        tile_state, ctl, safe_rank, debug_unstable, nullptr, xs, stream);
+                                                        tile_state, ctl, safe_rank, debug_unstable, nullptr, xs, stream, slack);
 }
 
 }  // namespace polylab

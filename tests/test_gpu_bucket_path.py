@@ -312,3 +312,46 @@ def test_async_call_takes_the_bucket_path():
     c, e, status, st = _async(q, 0.0, flags=B.FLAG_SAFE_RANK | B.FLAG_NO_BUCKET)
     assert status == B.OK
     assert_parity(oracle.simplify(q.coef, q.exps, 0.0), c, e)
+
+
+# ------------------------------------------------------------------ slack bins from a sampled histogram
+
+def test_slack_bins_match_the_exact_histogram_bit_for_bit():
+    """>= 2^22 terms, fused pack, two prefix passes: the first pass's bins are laid out with slack from a sampled histogram and
+    the second pass reads through the holes -- same records in the same order as with the exact sweep, so identical bits."""
+    n = (1 << 22) + 16
+    p, tol = W.config5(n)
+    c, e, st = run(p, tol)
+    assert st.hist_sampled == 1 and st.hist_retry == 0 and st.prefix_passes == 2
+    c1, e1, st1 = run(p, tol, flags=B.FLAG_EXACT_HIST)
+    assert st1.hist_sampled == 0 and st1.prefix_passes == 2
+    assert (e == e1).all() and (c.view(np.uint64) == c1.view(np.uint64)).all()
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+    # 64-bit keys (rows of 8 bytes), non-uniform but smooth first digit
+    r = np.random.default_rng(5)
+    m = 6_000_000
+    pool = r.integers(0, 256, size=(m // 6, 8)).astype(np.uint8)
+    pool[:, 1] = (r.integers(0, 256, size=m // 6) * r.integers(0, 256, size=m // 6) // 256).astype(np.uint8)   # triangular-ish
+    q = W.Poly(r.standard_normal(m), np.ascontiguousarray(pool[r.integers(0, m // 6, size=m)]))
+    c, e, st = run(q, 0.0, flags=B.FLAG_NO_TABLE)
+    assert st.key_bytes == 8
+    assert_parity(oracle.simplify(q.coef, q.exps, 0.0), c, e)
+    if st.hist_sampled:
+        c1, e1, _ = run(q, 0.0, flags=B.FLAG_NO_TABLE | B.FLAG_EXACT_HIST)
+        assert (e == e1).all() and (c.view(np.uint64) == c1.view(np.uint64)).all()
+
+
+def test_slack_bin_overrun_is_detected_and_the_call_reruns():
+    """An input whose sampled segments are NOT representative: the rows the sample never reads (segments of 2048 rows every
+    16,891) all share one value of the first prefix digit, so that bin overruns its capacity -> the pass raises slack_overflow,
+    the call re-runs with the exact sweep (stats->hist_retry) and still agrees with the oracle."""
+    n = 20_000_020
+    p, tol = W.config5(n)
+    exps = p.exps.copy()
+    stride = n // (148 * 8)
+    pos = np.arange(n) % stride
+    exps[pos >= 2048, 1] = 7                                   # the second variable is the first prefix digit (T = 16: digits of variables 0, 1)
+    q = W.Poly(p.coef, exps)
+    c, e, st = run(q, tol)
+    assert st.hist_retry == 1 and st.hist_sampled == 0
+    assert_parity(oracle.simplify(q.coef, q.exps, tol), c, e)

@@ -52,6 +52,7 @@ def test_config5_recipe_in_the_bench_configuration(n):
     res = oracle.simplify(p.coef, p.exps, tol)
     c, e, st = run(p, tol)
     assert st.bounds_sampled == 1 and st.bounds_retry == 0
+    assert st.hist_sampled == 1 and st.hist_retry == 0             # slack bins from a sampled histogram, no exact sweep
     assert st.prefix_passes == 2 and st.sort_passes == 2 and st.key_bytes == 16 and st.key_bits == 128
     assert st.bucket_fallback == 0 and st.rank_fallback == 0
     assert st.distinct == n // 10 and st.survivors == n // 20 == len(c)
