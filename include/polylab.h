@@ -60,7 +60,7 @@ typedef enum {
     POLYLAB_ERR_CUDA = 6,               /* a CUDA runtime call failed (see polylab_last_cuda_error) */
     POLYLAB_ERR_INTERNAL = 7,           /* the sorted-order self-check failed even with the ballot-ranking kernel */
     POLYLAB_ERR_RETRY = 8               /* only ever written to opts->status_device by a POLYLAB_FLAG_DEVICE_COUNT call: a
-                                           self-check of the fast path failed (ranking order, bucket length), nothing valid
+                                           self-check of the fast path failed (ranking order, bucket length, slack-bin size), nothing valid
                                            was emitted and the device count is 0 -- call again with POLYLAB_FLAG_SAFE_RANK |
                                            POLYLAB_FLAG_NO_BUCKET (or without POLYLAB_FLAG_DEVICE_COUNT, which retries itself) */
 } polylab_status;
@@ -113,7 +113,8 @@ enum {
                                         histogram from a 1-2 % sample of the rows, lays the first pass's bins out with slack (7
                                         sigma above the estimate) and lets the pass itself verify that none overran
                                         (stats->hist_sampled = 1); an overrun re-runs the call with the sweep
-                                        (stats->hist_retry = 1).  Same result, bit for bit. */
+                                        (stats->hist_retry = 1).  Same result, bit for bit.  A POLYLAB_FLAG_DEVICE_COUNT call
+                                        with a status word sizes the bins on the device; an overrun is POLYLAB_ERR_RETRY there. */
     POLYLAB_FLAG_NO_TABLE = 64u,      /* never take the table path.  By default a call with 2^15 <= N <= 2^26 terms whose key fits 63 bits
                                         first merges like terms in a table (the packed key itself as the index when 2^B slots
                                         are affordable, else a hash table) with order-independent fixed-point accumulators,

@@ -397,7 +397,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     PL_CUDA(cudaGetLastError());
     if (o.flags & POLYLAB_FLAG_DEVICE_COUNT) {             // no read-back: the self-checks report through status_device
         *launches += launch_async_status(ctl, o.status_device, out_nterms, stream);
-        if (o.stats) { o.stats->kernel_launches += *launches; o.stats->prefix_passes = k; o.stats->sort_passes = k; }
+        if (o.stats) { o.stats->kernel_launches += *launches; o.stats->prefix_passes = k; o.stats->sort_passes = k; o.stats->hist_sampled = slack ? 1 : 0; }
         return POLYLAB_OK;
     }
     if (o.stats) o.stats->kernel_launches += *launches;
@@ -711,11 +711,21 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
     // on 2e8 terms); it estimates the bins from a 1-2 % sample, gives each a capacity 7 sigma above its estimate, and the pass
     // itself verifies that no bin overran (else the call re-runs with the exact sweep: stats->hist_retry).
     bool slack = false;
-    if (fuse && k >= 2 && nterms >= kSampleBoundsMinTerms && !at.exact_hist &&
-        !(o.flags & (POLYLAB_FLAG_EXACT_HIST | POLYLAB_FLAG_DEVICE_COUNT | POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE))) {
+    const bool slack_wanted = fuse && k >= 2 && nterms >= kSampleBoundsMinTerms && !at.exact_hist &&
+                              !(o.flags & (POLYLAB_FLAG_EXACT_HIST | POLYLAB_FLAG_DEBUG_FORCE_BUCKET | POLYLAB_FLAG_DEBUG_UNSTABLE));
+    if (slack_wanted) {
         const int d = plan.npasses - k;
         const int nsegs = sm_count() * 8;
         launches += launch_row_hist_sample(ev, nterms, plan, d, ctl->est, nsegs, 2048, stream);
+        if (o.flags & POLYLAB_FLAG_DEVICE_COUNT) {
+            // no read-back: capacities computed on the device; a bin that overruns (or a sample that does not fit the buffer)
+            // surfaces as POLYLAB_ERR_RETRY in status_device.  (Without a status word the call took safe ranking: k == 0.)
+            launches += launch_slack_caps(ctl->est, nterms, slack_capacity(nterms), ctl->hist[d], ctl->slack_cap, stream);
+            slack = true;
+        }
+    }
+    if (slack_wanted && !slack) {
+        const int d = plan.npasses - k;
         uint32_t est[kRadix], cap[kRadix];
         PL_CUDA(cudaMemcpyAsync(est, ctl->est, sizeof est, cudaMemcpyDeviceToHost, stream));
         PL_CUDA(cudaStreamSynchronize(stream));

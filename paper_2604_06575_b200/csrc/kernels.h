@@ -96,6 +96,7 @@ int launch_row_hist(const ExpView& ev, int64_t nterms, const Plan& plan, int his
 // The same histogram over a sample: `nsegs` evenly spaced segments of `seg_rows` rows, into est[256] (zero before).
 int launch_row_hist_sample(const ExpView& ev, int64_t nterms, const Plan& plan, int hist_digit, uint32_t* est, int nsegs, int seg_rows,
                            cudaStream_t stream);
+int launch_slack_caps(const uint32_t* est, int64_t n, int64_t capacity, uint32_t* hist, uint32_t* cap, cudaStream_t stream);
 
 // S1 for the test entry point: always writes (hi, lo) pairs.
 int launch_pack_hilo(const ExpView& ev, int64_t nterms, const Plan& plan, uint64_t* out_hilo, Control* ctl,

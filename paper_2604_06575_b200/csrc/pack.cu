@@ -493,6 +493,42 @@ __global__ void __launch_bounds__(256) row_hist_sample_kernel(const uint8_t* __r
     bh.flush(hist);
 }
 
+// Slack-bin capacities on the device, for calls that must not synchronise (POLYLAB_FLAG_DEVICE_COUNT): the same rule as the
+// host applies in api.cu -- estimate scaled to N, plus 7 sigma of the sample count, plus 8 -- written as the first prefix
+// digit's "histogram" and as the capacities the second pass reads.  If the sample is empty or the capacities do not fit the
+// buffer, every capacity is 0: the pass then writes nothing and raises slack_overflow (-> POLYLAB_ERR_RETRY).
+__global__ void __launch_bounds__(kRadix) slack_caps_kernel(const uint32_t* __restrict__ est, uint32_t n, uint64_t capacity,
+                                                            uint32_t* __restrict__ hist, uint32_t* __restrict__ cap)
+{
+    __shared__ double part[kRadix / 32];
+    __shared__ double bcast;
+    const unsigned b = threadIdx.x, lane = b & 31u, warp = b >> 5;
+    auto block_sum = [&](double x) -> double {
+        for (int o = 16; o; o >>= 1) x += __shfl_xor_sync(kFullMask, x, o);
+        __syncthreads();
+        if (lane == 0) part[warp] = x;
+        __syncthreads();
+        if (b == 0) { double t = 0.0; for (int w = 0; w < kRadix / 32; ++w) t += part[w]; bcast = t; }
+        __syncthreads();
+        return bcast;
+    };
+    const double c = (double)est[b];
+    const double ssum = block_sum(c);
+    double cb = 0.0;
+    if (ssum > 0.0) cb = ceil((double)n / ssum * (c + 7.0 * sqrt(c + 1.0) + 8.0));
+    const double total = block_sum(cb);
+    const uint32_t out = (ssum > 0.0 && total <= (double)capacity && cb < 4.0e9) ? (uint32_t)cb : 0u;
+    const bool any_zero = __syncthreads_or(out == 0u ? 1 : 0) != 0;       // one unusable capacity voids all of them
+    hist[b] = any_zero ? 0u : out;
+    cap[b] = any_zero ? 0u : out;
+}
+
+int launch_slack_caps(const uint32_t* est, int64_t n, int64_t capacity, uint32_t* hist, uint32_t* cap, cudaStream_t stream)
+{
+    slack_caps_kernel<<<1, kRadix, 0, stream>>>(est, (uint32_t)n, (uint64_t)capacity, hist, cap);
+    return 1;
+}
+
 bool rows_fusable(const ExpView& ev, int nvars)
 {
     const int rb = nvars * ev.exp_bytes;

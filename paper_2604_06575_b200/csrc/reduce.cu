@@ -311,10 +311,11 @@ prune_unpack_kernel(const K* __restrict__ ukeys, const double* __restrict__ usum
 }
 
 // Asynchronous calls (POLYLAB_FLAG_DEVICE_COUNT): the status the host would have read back, on the device.  A failed
-// self-check (unstable ranking, a bucket too long for a tile) is POLYLAB_ERR_RETRY: nothing valid was emitted.
+// self-check (unstable ranking, a bucket too long for a tile, a slack bin too small) is POLYLAB_ERR_RETRY: nothing valid was
+// emitted.
 __global__ void async_status_kernel(const Control* ctl, int32_t* status_device, int64_t* out_count_device)
 {
-    const int32_t st = ctl->status != POLYLAB_OK ? ctl->status : (ctl->unsorted || ctl->overflow) ? (int32_t)POLYLAB_ERR_RETRY : (int32_t)POLYLAB_OK;
+    const int32_t st = ctl->status != POLYLAB_OK ? ctl->status : (ctl->unsorted || ctl->overflow || ctl->slack_overflow) ? (int32_t)POLYLAB_ERR_RETRY : (int32_t)POLYLAB_OK;
     if (status_device) *status_device = st;
     if (st == POLYLAB_ERR_RETRY && out_count_device) *out_count_device = 0;
 }

@@ -355,3 +355,25 @@ def test_slack_bin_overrun_is_detected_and_the_call_reruns():
     c, e, st = run(q, tol)
     assert st.hist_retry == 1 and st.hist_sampled == 0
     assert_parity(oracle.simplify(q.coef, q.exps, tol), c, e)
+
+
+def test_async_call_uses_slack_bins_with_capacities_computed_on_the_device():
+    """POLYLAB_FLAG_DEVICE_COUNT at >= 2^22 terms: the sampled histogram never reaches the host (slack_caps_kernel sizes the
+    bins); same bits as the synchronous call.  An unrepresentative sample (the input of the test above) cannot re-run
+    without a read-back: status POLYLAB_ERR_RETRY, count 0, and the prescribed retry gives the oracle's result."""
+    n = (1 << 22) + 16
+    p, tol = W.config5(n)
+    c, e, status, st = _async(p, tol)
+    assert status == B.OK and st.prefix_passes == 2 and st.hist_sampled == 1 and len(c) == n // 20
+    c0, e0, st0 = run(p, tol)
+    assert st0.hist_sampled == 1
+    assert (e0 == e).all() and (c0.view(np.uint64) == c.view(np.uint64)).all()
+    exps = p.exps.copy()
+    stride = n // (148 * 8)
+    exps[(np.arange(n) % stride) >= 2048, 1] = 7
+    q = W.Poly(p.coef, exps)
+    c, e, status, st = _async(q, tol)
+    assert status == B.ERR_RETRY and len(c) == 0
+    c, e, status, st = _async(q, tol, flags=B.FLAG_SAFE_RANK | B.FLAG_NO_BUCKET)
+    assert status == B.OK
+    assert_parity(oracle.simplify(q.coef, q.exps, tol), c, e)
