@@ -149,7 +149,7 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 // ------------------------------------------------------------------------------ workspace carving
 
 struct Layout {
-    size_t control, sort_state, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
+    size_t control, sort_state, slack_tiles, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
     size_t tab_state, tab, tab_bytes;
     size_t keys[2], coefs[2], ka, kb, ca, cb, total;      // ca, cb: fp32 operand coefficients of a product, widened to fp64
 };
@@ -199,7 +199,7 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     const size_t red_tiles = (size_t)((n + kReduceTile - 1) / kReduceTile);
     const size_t prune_tiles = (size_t)((n + kPruneTile - 1) / kPruneTile);
     L.control = take(sizeof(Control));
-    L.sort_state = take(sort_tiles * kRadix * sizeof(uint32_t));
+    L.sort_state = take((sort_tiles + kSlackExtraTiles) * kRadix * sizeof(uint32_t));
     L.red_state = take(red_tiles * sizeof(uint32_t));
     L.prune_state = take(prune_tiles * sizeof(uint32_t));
     const size_t fin_tiles = (size_t)((n + kFinMinTile - 1) / kFinMinTile);
@@ -208,6 +208,7 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.zero_end = off;                                   // everything before this is zeroed per call
     L.tab_bytes = table_region_bytes(n);
     L.tab = take(L.tab_bytes);
+    L.slack_tiles = take((sort_tiles + kSlackExtraTiles) * sizeof(uint2));     // (written in full by slack_tiles_kernel)
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.fin_wl = take((fin_tiles + 1) * sizeof(uint4));
     L.fin_chunks = take((fin_tiles / 4096 + 2) * sizeof(uint32_t));
@@ -381,7 +382,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     }
     for (int s = 0; s < k; ++s) {
         const double* cin = (s == 0) ? (const double*)coef0.p : cbuf[s & 1];
-        const SlackIO sio = {slack && s == 0, slack && s == 1, ctl->slack_cap};
+        const SlackIO sio = {slack && s == 0, slack && s == 1, ctl->slack_cap, (uint2*)(ws + L.slack_tiles), (uint32_t)slack_capacity(n)};
         *launches += launch_sort_pass(plan, P - k + s, s + 1 < k ? P - k + s + 1 : -1, s, n, kbuf[s & 1], cin, kbuf[(s + 1) & 1],
                                       cbuf[(s + 1) & 1], (uint32_t*)(ws + L.sort_state), ctl, false,
                                       (o.flags & POLYLAB_FLAG_DEBUG_UNSTABLE) != 0, stream, s == 0 ? rows : nullptr,
@@ -736,7 +737,7 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
             double total = 0.0;
             for (int b = 0; b < kRadix; ++b) {
                 const double c = (double)est[b];
-                const double cb = ceil(f * (c + 7.0 * sqrt(c + 1.0) + 8.0));
+                const double cb = ceil(f * (c + 7.0 * sqrt(c + 1.0) + 8.0) / 8.0) * 8.0;      // multiples of 8 records: bins start on 128-byte lines
                 cap[b] = cb > 4.0e9 ? 0xffffffffu : (uint32_t)cb;
                 total += cb;
             }

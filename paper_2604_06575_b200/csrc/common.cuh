@@ -295,8 +295,6 @@ struct Control {
     uint32_t tab_overflow;                   // table path: more distinct keys than the table was sized for -> sort path
     uint32_t slack_overflow;                 // slack bins (sort.cu): a bin's capacity, estimated from a sample, was too small
     uint32_t slack_count[kRadix];            // exact bin counts of the pass that wrote with slack
-    uint32_t slack_cstart[kRadix + 1];       // their exclusive prefix
-    uint32_t slack_pstart[kRadix + 1];       // exclusive prefix of the capacities
     uint32_t slack_cap[kRadix];              // the capacities (kept for the reading pass)
     uint32_t est[kRadix];                    // histogram of the first prefix digit over a SAMPLE of the rows
 };

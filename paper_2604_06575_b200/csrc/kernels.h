@@ -122,11 +122,14 @@ int launch_expand_raw(const ExpView& ea, CoefIn ca, int64_t na, const ExpView& e
 // `xs` (packed operands of a product): X1 fused into the pass -- keys_in / coef_in are ignored, record q = i*nb + j is
 // formed in registers as (ka_i + kb_j, fl(ca_i * cb_j)); atomic ranking only.
 // Slack bins: a pass given per-bin CAPACITIES instead of an exact histogram (`write`: ctl->hist[pass] holds them) lays its
-// output out with holes and records the exact counts; the pass after it (`read`, `cap` = the same capacities) maps compact
-// record numbers onto that layout.  ctl->slack_overflow != 0 afterwards: a bin was too small, nothing valid was produced.
+// output out with holes and records the exact counts; the pass after it (`read`, `cap` = the same capacities) cuts its
+// tiles per bin of that layout.  ctl->slack_overflow != 0 afterwards: a bin was too small, nothing valid was produced.
+constexpr int kSlackExtraTiles = kRadix + 1;     // a pass that reads slack bins cuts its tiles per bin: at most this many more
 struct SlackIO {
     bool write, read;
     const uint32_t* cap;        // DEVICE [256]
+    uint2* tiles;               // DEVICE [tiles + kSlackExtraTiles]: the reading pass's tile descriptors
+    uint32_t capacity;          // records the written buffers hold (>= the sum of the capacities)
 };
 struct ExpandSrc {
     const void* ka;

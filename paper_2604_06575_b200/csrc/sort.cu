@@ -25,8 +25,7 @@ struct SortSmem {
     static constexpr size_t bytes() { return total_bytes; }
 };
 
-constexpr int kHoleyStride = kRadix + 4;                              // the holey reader's two prefix arrays in shared memory
-constexpr size_t kHoleyBytes = 2 * kHoleyStride * sizeof(uint32_t);
+constexpr size_t kHoleyBytes = 16;                                     // the holey reader's tile descriptor in shared memory
 
 struct PassArgs {
     const void* keys_in;
@@ -45,15 +44,16 @@ struct PassArgs {
     uint32_t* ticket;
     int reverse_lanes;          // POLYLAB_FLAG_DEBUG_UNSTABLE: the atomic kernel maps lane l to record 31 - l
     // Slack bins (first prefix pass without an exact histogram, api.cu): hist_this holds per-bin CAPACITIES, so the bins
-    // of the output are laid out with holes.  The pass refuses to write a tile that would overrun a bin (slack_overflow)
-    // and its last tile leaves the exact bin counts in slack_count.
+    // of the output are laid out with holes.  A tile that overruns a bin raises slack_overflow (the output is void then; writes
+    // are clamped to the buffer) and the last tile leaves the exact bin counts in slack_count.
     uint32_t* slack_count;      // [256] or nullptr
     uint32_t* slack_overflow;
     uint32_t last_tile;
-    // ... and the pass that READS such an output (HOLEY): record number pos of the compact order lives at
-    // slack_pstart[b] + (pos - slack_cstart[b]) for the bin b with slack_cstart[b] <= pos < slack_cstart[b + 1]
-    const uint32_t* slack_cstart;   // [257] exclusive prefix of the exact counts
-    const uint32_t* slack_pstart;   // [257] exclusive prefix of the capacities
+    uint32_t slack_limit;       // last valid position of the output buffers
+    // ... and the pass that READS such an output (sort_pass_holey_kernel): its tiles never cross a bin.  Tile t is the
+    // slack_tiles[t].y records from physical position slack_tiles[t].x (y == 0: past the last tile), in bin order
+    // (slack_tiles_kernel; at most n / TILE + 256 tiles).
+    const uint2* slack_tiles;
     // S1 fused into the pass (ROWS > 0): keys are packed in registers from contiguous exponent rows of ROWS bytes
     const uint8_t* rows;
     int exp_bytes;
@@ -113,7 +113,7 @@ __device__ __forceinline__ K pack_row_inline(const PassArgs& a, const Plan& plan
 // values in ascending lane order on sm_100a (measured, profiles/r1b_shared_atomics.md; not documented), which
 // is what makes the pass stable; the reduce step verifies the sorted order and the call falls back to the
 // ballot-matching kernel (RANK_ATOMIC = false) if it ever does not hold.
-template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC, int ROWS, bool BYTES = false, bool HOLEY = false, bool SLACK = false>
+template <typename K, int THREADS, int ITEMS, bool NEXT, bool FULL, bool RANK_ATOMIC, int ROWS, bool BYTES = false, bool SLACK = false, bool HOLEY = false>
 __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* plan, unsigned char* smem_raw, uint32_t tile,
                                                uint32_t tile_base, uint32_t tile_n)
 {
@@ -137,30 +137,6 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
     const uint32_t chunk = warp * 32u * ITEMS + ((RANK_ATOMIC && a.reverse_lanes) ? 31u - lane : lane);
     K key[ITEMS];
     bool bad = false;
-    // HOLEY input: the bin of the tile's first record = the number of compact bin starts at or below it, minus one.  A tile nearly always lies inside one or two bins: then a record's address is its number plus one of two
-    // shifts; only a tile that spans more walks the bin starts per record.
-    uint32_t hb0 = 0, hbnd = 0xffffffffu, hshift0 = 0, hshift1 = 0;
-    bool two_bins = true;
-    const uint32_t* hs_c = (const uint32_t*)(smem_raw + S::total_bytes);     // [257] compact bin starts, [257] physical bin starts
-    const uint32_t* hs_p = hs_c + kHoleyStride;
-    if (HOLEY) {
-        // (the kernel copied both prefix arrays into shared memory while the tile ticket was in flight; a block-wide count
-        // instead of a binary search: dependent global loads at the head of every tile cost the pass 5-10 %)
-        const bool below = tid < (unsigned)kRadix && hs_c[tid] <= tile_base;
-        hb0 = (uint32_t)__syncthreads_count(below ? 1 : 0) - 1u;
-        hshift0 = hs_p[hb0] - hs_c[hb0];
-        hbnd = hs_c[hb0 + 1];
-        if (hb0 + 1 < (uint32_t)kRadix) {
-            hshift1 = hs_p[hb0 + 1] - hbnd;
-            two_bins = tile_base + tile_n <= hs_c[hb0 + 2];
-        }
-    }
-    auto holey_index = [&](uint32_t pos) -> uint32_t {
-        if (two_bins) return pos + (pos < hbnd ? hshift0 : hshift1);
-        uint32_t bb = hb0;
-        while (pos >= hs_c[bb + 1]) ++bb;
-        return hs_p[bb] + (pos - hs_c[bb]);
-    };
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
         const uint32_t li = chunk + j * 32u;
@@ -170,7 +146,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
                 // step X1 in registers: key = ka_i + kb_j (fields never carry into each other), the product is never stored
                 const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
                 key[j] = key_add(((const K*)a.xa_keys)[i], ((const K*)a.xb_keys)[jj]);
-            } else key[j] = keys_in[HOLEY ? holey_index(tile_base + li) : tile_base + li];
+            } else key[j] = keys_in[tile_base + li];
         } else key[j] = key_max<K>();
     }
     if (ROWS > 0 && bad) atomicMax(a.status, (int)POLYLAB_ERR_EXPONENT_RANGE);
@@ -234,7 +210,11 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
     uint32_t total;
     const uint32_t bin_start = block_exclusive_scan<THREADS>(count, scratch, &total);
     if (bt) sm_bin_start[b] = bin_start;
-    const uint32_t gbase = block_exclusive_scan<THREADS>(bt ? a.hist_this[b] : 0u, scratch, &total);   // syncs: sm_bin_start visible
+    const uint32_t hist_b = bt ? a.hist_this[b] : 0u;
+    // (slack check below: the capacity waits in shared memory, in the next-digit histogram's slot, consumed above -- a second
+    // global load after the look-back would sit on every tile's critical path, a register through it spills)
+    if (SLACK && bt) bhist2[b] = hist_b;
+    const uint32_t gbase = block_exclusive_scan<THREADS>(hist_b, scratch, &total);   // syncs: sm_bin_start visible
 
     // ---- scatter keys into shared memory at their position in the sorted tile
 #pragma unroll
@@ -254,7 +234,11 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         if (ROWS == kLoadProducts) {
             const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
             c[j] = (FULL || li < tile_n) ? __dmul_rn(a.xa_coef[i], a.xb_coef[jj]) : 0.0;     // one IEEE multiplication, never contracted
-        } else c[j] = (FULL || li < tile_n) ? coef_in[HOLEY ? holey_index(tile_base + li) : tile_base + li] : 0.0;   // (the mapping is recomputed: 20 indices kept live through the ranking would spill)
+        } else if (HOLEY) {
+            // (the tile's start is re-read from the descriptor in shared memory: live through the ranking it costs 17 spills)
+            const uint32_t tb = *(volatile const uint32_t*)(smem_raw + S::total_bytes);
+            c[j] = (FULL || li < tile_n) ? coef_in[tb + li] : 0.0;
+        } else c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
     }
 
     // ---- decoupled look-back: number of records with digit b in all earlier tiles.  The walk over the predecessors
@@ -284,27 +268,24 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
         st_volatile_u32(my_state, ((excl + count) << 2) | a.flag_inclusive);
     }
     if (bt) sm_delta[b] = gbase + excl - bin_start;      // destination of sorted-tile slot s with digit b: s + delta[b]
-    bool skip = false;
-    if (SLACK) {
-        // slack bins: hist_this are capacities.  A tile that would overrun one writes nothing and raises the flag (the call
-        // re-runs with an exact histogram); the last tile's inclusive totals are the exact bin counts.
-        bool ovf = false;
-        if (bt) {
-            ovf = excl + count > a.hist_this[b];
-            if (tile == a.last_tile) a.slack_count[b] = excl + count;
-        }
-        skip = __syncthreads_or(ovf ? 1 : 0) != 0;
-        if (skip && tid == 0) *a.slack_overflow = 1u;
-    } else __syncthreads();
+    if (SLACK && bt) {
+        // slack bins: hist_this are capacities.  A tile that overruns one raises the flag (nothing of the call's output is
+        // valid then: it re-runs with an exact histogram; the writes below stay inside the buffer by clamping); the last
+        // tile's inclusive totals are the exact bin counts.
+        if (excl + count > bhist2[b]) *a.slack_overflow = 1u;
+        if (tile == a.last_tile) a.slack_count[b] = excl + count;
+    }
+    __syncthreads();
 
     // ---- write keys: slot s of the sorted tile, contiguous per bin
     uint32_t dst[ITEMS];
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if ((FULL || s < tile_n) && !skip) {
+        if (FULL || s < tile_n) {
             const K kk = stage[s];
             dst[k] = s + sm_delta[(key_word(kk, a.dword) >> a.dshift) & a.dmask];
+            if (SLACK) dst[k] = min(dst[k], a.slack_limit);
             keys_out[dst[k]] = kk;
         }
     }
@@ -316,7 +297,7 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t s = k * THREADS + tid;
-        if ((FULL || s < tile_n) && !skip) coef_out[dst[k]] = stage_c[s];
+        if (FULL || s < tile_n) coef_out[dst[k]] = stage_c[s];
     }
 }
 
@@ -341,46 +322,80 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_c
     else sort_tile_body<K, THREADS, ITEMS, NEXT, false, RANK_ATOMIC, 0>(a, nullptr, smem_raw, tile, tile_base, tile_n);
 }
 
-// The same pass over an input whose bins were laid out with slack by the previous pass (see PassArgs::slack_cstart).
+// The same pass over an input whose bins were laid out with slack by the previous pass (see PassArgs::slack_tiles): the
+// tiles are cut per bin, so a tile is one contiguous, 128-byte aligned piece of the input exactly as in sort_pass_kernel.
+// Measured on 2e8 records against the plain pass (1.97 ms): compact tiling with every record mapped through the holes by a
+// per-tile binary search over the bin starts 2.20 ms, by a block-wide count 2.10, with the bin tables copied to shared memory
+// by every block 2.07-2.12 (a million requests for the same two dozen L2 lines); one descriptor per tile, as here: see
+// profiles/r2_state.md.  The descriptor of tile blockIdx.x is fetched while the ticket is in flight: tickets are handed out
+// in start order, so it is nearly always the right one.  The grid is sized for the worst case; blocks past the last tile leave.
 template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT>
 __global__ void __launch_bounds__(THREADS, MINB) sort_pass_holey_kernel(const __grid_constant__ PassArgs a)
 {
     using S = SortSmem<K, THREADS, ITEMS>;
-    constexpr int TILE = S::TILE, NW = S::NW;
+    constexpr int NW = S::NW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t* whist = (uint32_t*)(smem_raw + S::stage_bytes);
     uint32_t* scratch = whist + NW * kRadix + 3 * kRadix;
+    uint32_t* desc = (uint32_t*)(smem_raw + S::total_bytes);
 
     const unsigned tid = threadIdx.x;
     if (tid == 0) scratch[NW + 2] = atomicAdd(a.ticket, 1u);
-    uint32_t* hs = (uint32_t*)(smem_raw + S::total_bytes);
-    for (int i = tid; i <= kRadix; i += THREADS) {
-        hs[i] = __ldg(a.slack_cstart + i);
-        hs[kHoleyStride + i] = __ldg(a.slack_pstart + i);
+    if (tid == 32) {
+        const uint2 d = __ldg(a.slack_tiles + blockIdx.x);
+        desc[0] = d.x; desc[1] = d.y;
     }
     for (int i = tid; i < (NW + 1) * kRadix; i += THREADS) whist[i] = 0u;
     __syncthreads();
     const uint32_t tile = scratch[NW + 2];
-    const uint32_t tile_base = tile * (uint32_t)TILE;
-    const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
-    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, 0, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
-    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, 0, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+    if (tile != blockIdx.x) {                                    // (block-uniform)
+        if (tid == 0) {
+            const uint2 d = __ldg(a.slack_tiles + tile);
+            desc[0] = d.x; desc[1] = d.y;
+        }
+        __syncthreads();
+    }
+    const uint32_t tile_base = desc[0], tile_n = desc[1];
+    if (tile_n == 0u) return;
+    if (tile_n == (uint32_t)S::TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, 0, false, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, 0, false, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
 }
 
-// exclusive prefixes of the exact bin counts and of the bin capacities (257 entries each), for the holey reader
-__global__ void slack_prefix_kernel(const uint32_t* __restrict__ count, const uint32_t* __restrict__ cap, uint32_t* cstart, uint32_t* pstart)
+// For the holey reader: one descriptor per tile (physical start, records), the tiles cut per bin of the exact counts the
+// writing pass left (bin b: ceil(count_b / tile) tiles from the exclusive prefix of the capacities); every block recomputes
+// the two 256-entry prefixes.  Also sets the states of the tiles beyond the previous pass's tile count to "not published"
+// (zeroed words would read as inclusive totals under the reader's flag parity).
+__global__ void __launch_bounds__(kRadix) slack_tiles_kernel(const uint32_t* __restrict__ count, const uint32_t* __restrict__ cap, uint32_t tile,
+                                                             uint32_t max_tiles, uint2* __restrict__ desc, uint32_t* extra_state,
+                                                             uint32_t extra_words, uint32_t unpublished)
 {
     __shared__ uint32_t scratch[kRadix / 32 + 2];
+    __shared__ uint32_t ts[kRadix + 1], ps[kRadix], cn[kRadix];
     const unsigned b = threadIdx.x;
     uint32_t total;
-    const uint32_t c = count[b], p = cap[b];
-    const uint32_t ce = block_exclusive_scan<kRadix>(c, scratch, &total);
-    cstart[b] = ce;
-    if (b == kRadix - 1) cstart[kRadix] = total;
+    const uint32_t c = count[b];
+    const uint32_t te = block_exclusive_scan<kRadix>((c + tile - 1u) / tile, scratch, &total);
+    ts[b] = te; cn[b] = c;
+    if (b == kRadix - 1) ts[kRadix] = total;
     __syncthreads();
-    const uint32_t pe = block_exclusive_scan<kRadix>(p, scratch, &total);
-    pstart[b] = pe;
-    if (b == kRadix - 1) pstart[kRadix] = total;
+    ps[b] = block_exclusive_scan<kRadix>(cap[b], scratch, &total);
+    __syncthreads();
+    const uint32_t t = blockIdx.x * kRadix + b;
+    if (t < max_tiles) {
+        uint2 d = make_uint2(0u, 0u);
+        if (t < ts[kRadix]) {
+            uint32_t lo = 0, hi = kRadix;                        // the LAST bin whose first tile is <= t (empty bins share their successor's)
+            while (hi - lo > 1u) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (ts[mid] <= t) lo = mid; else hi = mid;
+            }
+            const uint32_t off = (t - ts[lo]) * tile;
+            d.x = ps[lo] + off;
+            d.y = min(tile, cn[lo] - off);
+        }
+        desc[t] = d;
+    }
+    for (uint32_t i = t; i < extra_words; i += gridDim.x * kRadix) extra_state[i] = unpublished;
 }
 
 // The same pass with S1 fused in: reads exponent rows instead of keys (first pass of the bucket path).
@@ -400,8 +415,8 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_rows_kernel(const __g
     const uint32_t tile = scratch[NW + 2];
     const uint32_t tile_base = tile * (uint32_t)TILE;
     const uint32_t tile_n = min((uint32_t)TILE, a.n - tile_base);
-    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, ROWS, BYTES, false, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
-    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES, false, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
+    if (tile_n == (uint32_t)TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, ROWS, BYTES, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
+    else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, ROWS, BYTES, SLACK>(a, &plan, smem_raw, tile, tile_base, tile_n);
 }
 
 template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT, bool RANK_ATOMIC>
@@ -434,15 +449,19 @@ static int launch_sort_pass_t(const Plan& plan, int pass, int next, int seq, int
     a.flag_inclusive = (seq & 1) ? 0u : 2u;
     a.hist_this = ctl->hist[pass]; a.hist_next = ctl->hist[has_next ? next : kMaxPasses]; a.ticket = &ctl->ticket[seq];
     a.reverse_lanes = debug_unstable ? 1 : 0;
-    a.slack_count = nullptr; a.slack_overflow = nullptr; a.last_tile = tiles - 1u; a.slack_cstart = nullptr; a.slack_pstart = nullptr;
-    if (slack && slack->write) { a.slack_count = ctl->slack_count; a.slack_overflow = &ctl->slack_overflow; }
+    a.slack_count = nullptr; a.slack_overflow = nullptr; a.last_tile = tiles - 1u; a.slack_tiles = nullptr;
+    a.slack_limit = 0u;
+    if (slack && slack->write) { a.slack_count = ctl->slack_count; a.slack_overflow = &ctl->slack_overflow; a.slack_limit = slack->capacity - 1u; }
     if (slack && slack->read) {
         // the previous pass left holes: prefixes of its exact counts and of its capacities, then the holey reader
-        slack_prefix_kernel<<<1, kRadix, 0, stream>>>(ctl->slack_count, slack->cap, ctl->slack_cstart, ctl->slack_pstart);
-        a.slack_cstart = ctl->slack_cstart; a.slack_pstart = ctl->slack_pstart;
+        const unsigned max_tiles = tiles + kSlackExtraTiles;          // sum of ceil(count_b / TILE) <= n / TILE + 256
+        slack_tiles_kernel<<<(max_tiles + kRadix - 1) / kRadix, kRadix, 0, stream>>>(ctl->slack_count, slack->cap, (uint32_t)S::TILE, max_tiles, slack->tiles,
+                                                                                      tile_state + (size_t)tiles * kRadix,
+                                                                                      (uint32_t)kSlackExtraTiles * kRadix, ((seq - 1) & 1) ? 3u : 1u);
+        a.slack_tiles = slack->tiles;
         auto go = [&](auto kern) {
             ensure_dynamic_smem(kern, (size_t)S::bytes() + kHoleyBytes);
-            kern<<<tiles, THREADS, S::bytes() + kHoleyBytes, stream>>>(a);
+            kern<<<max_tiles, THREADS, S::bytes() + kHoleyBytes, stream>>>(a);
         };
         if (has_next) go(sort_pass_holey_kernel<K, THREADS, ITEMS, MINB, true>);
         else go(sort_pass_holey_kernel<K, THREADS, ITEMS, MINB, false>);
