@@ -320,6 +320,27 @@ int polylab_mul_simplify_host(const polylab_poly* a_host, const polylab_poly* b_
                               int64_t* out_nterms_host,
                               void* device_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * polylab_simplify without a workspace argument and without any allocation: the scratch memory of the whole pipeline is a
+ * static device array of POLYLAB_STATIC_WORKSPACE_BYTES inside the library (every GPU that loads the library holds it until
+ * the process exits).  For callers that cannot call cudaMalloc or hand over device memory of their own: set-up code around
+ * CUDA graph capture, tight serving loops, harnesses that forbid allocation.  The operation, the arguments, the result and the
+ * statuses are polylab_simplify's (Table 3; section 6.3), bit for bit, with these differences:
+ *   - nterms <= POLYLAB_STATIC_MAX_TERMS; more (or a layout that does not fit the array) is POLYLAB_ERR_WORKSPACE_TOO_SMALL
+ *     and nothing is launched;
+ *   - POLYLAB_FLAG_TIMING is POLYLAB_ERR_INVALID_ARGUMENT (stage events would have to be created);
+ *   - the call makes no cudaMalloc / cudaFree / allocating library call; the array's device address is looked up once per
+ *     device, on the first call with that device current;
+ *   - ALL calls on a GPU share the one array, which keeps the previous call's contents (each call clears what it needs
+ *     zeroed): two calls that overlap on the GPU -- different streams, or two host threads -- race; serialise them.
+ * coef, exps, out_coef, out_exps are DEVICE pointers owned by the caller, as in polylab_simplify.
+ */
+#define POLYLAB_STATIC_MAX_TERMS 65536
+#define POLYLAB_STATIC_WORKSPACE_BYTES (8u << 20)
+int polylab_simplify_static(const double* coef, const void* exps, int64_t nterms, int32_t nvars, double tol,
+                            const polylab_opts* opts, double* out_coef, void* out_exps, int64_t out_capacity,
+                            int64_t* out_nterms, void* cuda_stream);
+
 const char* polylab_status_string(int status);
 const char* polylab_last_cuda_error(void);   /* text of the last CUDA failure seen by this thread */
 int polylab_version(void);

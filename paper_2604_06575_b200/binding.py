@@ -41,6 +41,8 @@ STAGES = ("bounds", "pack", "sort", "reduce", "prune")
 MAX_NVARS = 256
 MAX_TERMS = 1 << 30
 SMALL_WORKSPACE_BYTES = 65536
+STATIC_MAX_TERMS = 65536            # polylab_simplify_static: the library's static workspace holds this many terms
+STATIC_WORKSPACE_BYTES = 8 << 20
 
 
 class PolylabError(RuntimeError):
@@ -122,6 +124,7 @@ def lib():
         simp = [vp, vp, i64, i32, dbl, po, vp, vp, i64, vp, vp, sz, vp]
         L.polylab_simplify.argtypes = simp
         L.polylab_simplify_host.argtypes = simp
+        L.polylab_simplify_static.argtypes = [vp, vp, i64, i32, dbl, po, vp, vp, i64, vp, vp]
         mul = [pp, pp, dbl, po, vp, vp, i64, vp, vp, sz, vp]
         L.polylab_mul_simplify.argtypes = mul
         L.polylab_mul_simplify_host.argtypes = mul
@@ -272,6 +275,32 @@ def simplify(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_ex
         rc = lib().polylab_simplify(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
                                     out_coef.data_ptr(), out_exps.data_ptr(), cap, ctypes.addressof(count),
                                     ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc)
+    k = count.value
+    res = (out_coef[:k], out_exps[:k])
+    return (*res, _stats(st)) if return_stats else res
+
+
+def simplify_static(coef: torch.Tensor, exps: torch.Tensor, tol: float = 0.0, *, max_exp: Optional[Sequence[int]] = None,
+                    out: Optional[tuple] = None, stream=None, return_stats: bool = False, flags: int = 0):
+    """polylab_simplify_static: the same operation with the library's own static device workspace -- no workspace tensor, no
+    allocation inside the call; at most STATIC_MAX_TERMS terms (ERR_WORKSPACE_TOO_SMALL beyond).  `out` = (out_coef, out_exps)
+    buffers of the caller (allocated here when omitted: the C entry point itself allocates nothing).  Calls share one
+    array per GPU: do not overlap them."""
+    coef, exps, strides = _dev_poly(coef, exps)
+    n, nvars = int(exps.shape[0]), int(exps.shape[1])
+    keep = []
+    o, st = _make_opts(_EXP_TYPE[exps.dtype], max_exp, flags=flags, strides=strides, keep=keep, coef_dtype=coef.dtype)
+    if out is None:
+        out_coef = torch.empty(max(n, 1), dtype=coef.dtype, device=coef.device)
+        out_exps = torch.empty((max(n, 1), nvars), dtype=exps.dtype, device=coef.device)
+    else:
+        out_coef, out_exps = out
+    count = ctypes.c_int64(0)
+    with torch.cuda.device(coef.device):     # the library launches on the CURRENT device
+        rc = lib().polylab_simplify_static(coef.data_ptr(), exps.data_ptr(), n, nvars, float(tol), ctypes.byref(o),
+                                           out_coef.data_ptr(), out_exps.data_ptr(), int(out_coef.shape[0]),
+                                           ctypes.addressof(count), _stream_ptr(stream))
     _check(rc)
     k = count.value
     res = (out_coef[:k], out_exps[:k])

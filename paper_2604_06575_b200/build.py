@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpolylab.so")
-SOURCES = ["pack.cu", "sort.cu", "reduce.cu", "finish.cu", "table.cu", "small.cu", "batch.cu", "api.cu"]
+SOURCES = ["pack.cu", "sort.cu", "reduce.cu", "finish.cu", "table.cu", "small.cu", "batch.cu", "api.cu", "static_ws.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "kernels.h"), os.path.join(INCLUDE, "polylab.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

@@ -52,6 +52,8 @@ static bool cuda_failed(cudaError_t e, const char* what)
     snprintf(g_cuda_error, sizeof g_cuda_error, "%s: %s", what, cudaGetErrorString(e));
     return true;
 }
+// (for static_ws.cu, whose set-up runs outside this file: the text polylab_last_cuda_error returns)
+void note_cuda_error(cudaError_t e, const char* what) { cuda_failed(e, what); }
 #define PL_CUDA(call)                                            \
     do {                                                         \
         if (cuda_failed((call), #call)) return POLYLAB_ERR_CUDA; \

@@ -31,6 +31,9 @@ constexpr int kFinMaxMeanBucket = 3072;   // the planner partitions until N / 2^
 constexpr int kFinMinTile = 512;    // smallest fin_tile the planner picks (workspace sizing)
 
 // Number of SMs of the current device (grid sizing); queried once per device, 148 on a B200.
+// records the text polylab_last_cuda_error returns (api.cu)
+void note_cuda_error(cudaError_t e, const char* what);
+
 inline int sm_count()
 {
     static int cached[64] = {0};
