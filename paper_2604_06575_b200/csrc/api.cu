@@ -739,7 +739,7 @@ static int simplify_once(const double* coef, const void* exps, int64_t nterms, i
             double total = 0.0;
             for (int b = 0; b < kRadix; ++b) {
                 const double c = (double)est[b];
-                const double cb = ceil(f * (c + 7.0 * sqrt(c + 1.0) + 8.0) / 8.0) * 8.0;      // multiples of 8 records: bins start on 128-byte lines
+                const double cb = ceil(f * (c + 7.0 * sqrt(c + 1.0) + 8.0) / 16.0) * 16.0;      // multiples of 16 records: keys and coefficients of a bin start on 128-byte lines
                 cap[b] = cb > 4.0e9 ? 0xffffffffu : (uint32_t)cb;
                 total += cb;
             }

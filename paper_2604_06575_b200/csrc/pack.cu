@@ -515,7 +515,7 @@ __global__ void __launch_bounds__(kRadix) slack_caps_kernel(const uint32_t* __re
     const double c = (double)est[b];
     const double ssum = block_sum(c);
     double cb = 0.0;
-    if (ssum > 0.0) cb = ceil((double)n / ssum * (c + 7.0 * sqrt(c + 1.0) + 8.0) / 8.0) * 8.0;   // multiples of 8 records
+    if (ssum > 0.0) cb = ceil((double)n / ssum * (c + 7.0 * sqrt(c + 1.0) + 8.0) / 16.0) * 16.0;   // multiples of 16 records
     const double total = block_sum(cb);
     const uint32_t out = (ssum > 0.0 && total <= (double)capacity && cb < 4.0e9) ? (uint32_t)cb : 0u;
     const bool any_zero = __syncthreads_or(out == 0u ? 1 : 0) != 0;       // one unusable capacity voids all of them

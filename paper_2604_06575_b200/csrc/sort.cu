@@ -25,7 +25,8 @@ struct SortSmem {
     static constexpr size_t bytes() { return total_bytes; }
 };
 
-constexpr size_t kHoleyBytes = 16;                                     // the holey reader's tile descriptor in shared memory
+constexpr int kHoleyWindow = 64, kHoleyBack = 24;                      // the holey reader prefetches the descriptors of tiles blockIdx.x - 24 .. + 39
+constexpr size_t kHoleyBytes = 16 + kHoleyWindow * sizeof(uint2);     // its tile descriptor + that window, in shared memory
 
 struct PassArgs {
     const void* keys_in;
@@ -228,17 +229,25 @@ __device__ __forceinline__ void sort_tile_body(const PassArgs& a, const Plan* pl
 #undef POLYLAB_DIGIT
     // coefficients: issue the loads now, they land while the look-back runs
     double c[ITEMS];
+    if constexpr (HOLEY || SLACK) {
+        static_assert(ROWS != kLoadProducts, "slack bins are written by the fused-rows pass and read by the plain one");
+        // HOLEY: the tile's start is re-read from the descriptor in shared memory (live through the ranking it costs 17
+        // spills); the SLACK instantiation goes through the same copy because ptxas then spills 20 bytes instead of 36
+        const uint32_t tb = HOLEY ? *(volatile const uint32_t*)(smem_raw + S::total_bytes) : tile_base;
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-        const uint32_t li = chunk + j * 32u;
-        if (ROWS == kLoadProducts) {
-            const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
-            c[j] = (FULL || li < tile_n) ? __dmul_rn(a.xa_coef[i], a.xb_coef[jj]) : 0.0;     // one IEEE multiplication, never contracted
-        } else if (HOLEY) {
-            // (the tile's start is re-read from the descriptor in shared memory: live through the ranking it costs 17 spills)
-            const uint32_t tb = *(volatile const uint32_t*)(smem_raw + S::total_bytes);
+        for (int j = 0; j < ITEMS; ++j) {
+            const uint32_t li = chunk + j * 32u;
             c[j] = (FULL || li < tile_n) ? coef_in[tb + li] : 0.0;
-        } else c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < ITEMS; ++j) {
+            const uint32_t li = chunk + j * 32u;
+            if (ROWS == kLoadProducts) {
+                const uint32_t q = tile_base + li, i = q / a.xnb, jj = q - i * a.xnb;
+                c[j] = (FULL || li < tile_n) ? __dmul_rn(a.xa_coef[i], a.xb_coef[jj]) : 0.0;     // one IEEE multiplication, never contracted
+            } else c[j] = (FULL || li < tile_n) ? coef_in[tile_base + li] : 0.0;
+        }
     }
 
     // ---- decoupled look-back: number of records with digit b in all earlier tiles.  The walk over the predecessors
@@ -327,8 +336,8 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_kernel(const __grid_c
 // Measured on 2e8 records against the plain pass (1.97 ms): compact tiling with every record mapped through the holes by a
 // per-tile binary search over the bin starts 2.20 ms, by a block-wide count 2.10, with the bin tables copied to shared memory
 // by every block 2.07-2.12 (a million requests for the same two dozen L2 lines); one descriptor per tile, as here: see
-// profiles/r2_state.md.  The descriptor of tile blockIdx.x is fetched while the ticket is in flight: tickets are handed out
-// in start order, so it is nearly always the right one.  The grid is sized for the worst case; blocks past the last tile leave.
+// profiles/r2_state.md.  The descriptors of the tiles around blockIdx.x are fetched while the ticket is in flight: tickets are
+// handed out in start order, so the block's tile is nearly always among them.  The grid is sized for the worst case; blocks past the last tile leave.
 template <typename K, int THREADS, int ITEMS, int MINB, bool NEXT>
 __global__ void __launch_bounds__(THREADS, MINB) sort_pass_holey_kernel(const __grid_constant__ PassArgs a)
 {
@@ -341,21 +350,28 @@ __global__ void __launch_bounds__(THREADS, MINB) sort_pass_holey_kernel(const __
 
     const unsigned tid = threadIdx.x;
     if (tid == 0) scratch[NW + 2] = atomicAdd(a.ticket, 1u);
-    if (tid == 32) {
-        const uint2 d = __ldg(a.slack_tiles + blockIdx.x);
-        desc[0] = d.x; desc[1] = d.y;
+    uint2* win = (uint2*)(desc + 4);
+    const uint32_t w0 = max(blockIdx.x, (unsigned)kHoleyBack) - kHoleyBack;
+    if (tid >= 32 && tid < 32 + kHoleyWindow) {
+        const uint32_t t = w0 + (tid - 32);
+        win[tid - 32] = t < gridDim.x ? __ldg(a.slack_tiles + t) : make_uint2(0u, 0u);
     }
     for (int i = tid; i < (NW + 1) * kRadix; i += THREADS) whist[i] = 0u;
     __syncthreads();
     const uint32_t tile = scratch[NW + 2];
-    if (tile != blockIdx.x) {                                    // (block-uniform)
+    uint2 d;
+    if (tile - w0 < (uint32_t)kHoleyWindow) {                    // (block-uniform)
+        d = win[tile - w0];
+        if (tid == 0) desc[0] = d.x;                             // (the body re-reads the tile's start after its first barrier)
+    } else {
         if (tid == 0) {
-            const uint2 d = __ldg(a.slack_tiles + tile);
+            d = __ldg(a.slack_tiles + tile);
             desc[0] = d.x; desc[1] = d.y;
         }
         __syncthreads();
+        d = make_uint2(desc[0], desc[1]);
     }
-    const uint32_t tile_base = desc[0], tile_n = desc[1];
+    const uint32_t tile_base = d.x, tile_n = d.y;
     if (tile_n == 0u) return;
     if (tile_n == (uint32_t)S::TILE) sort_tile_body<K, THREADS, ITEMS, NEXT, true, true, 0, false, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
     else sort_tile_body<K, THREADS, ITEMS, NEXT, false, true, 0, false, false, true>(a, nullptr, smem_raw, tile, tile_base, tile_n);
