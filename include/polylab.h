@@ -115,6 +115,12 @@ enum {
                                         (stats->hist_sampled = 1); an overrun re-runs the call with the sweep
                                         (stats->hist_retry = 1).  Same result, bit for bit.  A POLYLAB_FLAG_DEVICE_COUNT call
                                         with a status word sizes the bins on the device; an overrun is POLYLAB_ERR_RETRY there. */
+    POLYLAB_FLAG_NO_GROUP_FINISH = 512u, /* bucket path: finish every tile with the sorting kernel.  By default a tile first tries to GROUP
+                                        its records: like terms are found through a shared-memory hash table (full keys compared), only
+                                        the tile's distinct monomials are sorted, and one stable counting pass puts the records in
+                                        order (stats->grouped_tiles); a tile with more than 768 distinct monomials, a fingerprint
+                                        collision or an overlong probe sequence goes through the sorting kernel instead, and once most
+                                        tiles do, the rest no longer try.  Same result, bit for bit. */
     POLYLAB_FLAG_NO_TABLE = 64u,      /* never take the table path.  By default a call with 2^15 <= N <= 2^26 terms whose key fits 63 bits
                                         first merges like terms in a table (the packed key itself as the index when 2^B slots
                                         are affordable, else a hash table) with order-independent fixed-point accumulators,
@@ -131,12 +137,14 @@ enum {
     POLYLAB_FLAG_DEBUG_FORCE_HASH = 0x08000000u,   /* test hook: use the hash table even where the dense table applies */
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
                                         skew pre-check), so that small tests reach it and its overflow fallback */
+    POLYLAB_FLAG_DEBUG_GROUP_HANDS_ON = 0x04000000u, /* test hook: the bucket path's group kernel runs and hands every tile on to the
+                                        sorting kernel (the second work list in full) */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
                                         (reversed lane order) so that tests can exercise detection and fallback */
 };
-/* test hook: bits 8..11 of flags, when non-zero, override how many low digits the bucket path's first local sort
+/* test hook: bits 16..19 of flags, when non-zero, override how many low digits the bucket path's first local sort
    attempt uses (default 3); 1 makes most tiles fail the order check and re-sort on every digit */
-#define POLYLAB_FLAG_DEBUG_NFAST_SHIFT 8
+#define POLYLAB_FLAG_DEBUG_NFAST_SHIFT 16
 
 /* indices into polylab_stats.stage_ms */
 enum { POLYLAB_STAGE_BOUNDS = 0, POLYLAB_STAGE_PACK = 1, POLYLAB_STAGE_SORT = 2, POLYLAB_STAGE_REDUCE = 3,
@@ -170,6 +178,7 @@ typedef struct polylab_stats {
     int32_t small_path;      /* 1 if one thread block did the sort and the segmented sum (see POLYLAB_FLAG_NO_SMALL) */
     int32_t hist_sampled;    /* 1 if the first prefix pass took slack bins from a sampled histogram (POLYLAB_FLAG_EXACT_HIST) */
     int32_t hist_retry;      /* 1 if such a bin overran and the call re-ran with the exact histogram */
+    int32_t grouped_tiles;   /* bucket path: tiles finished by grouping like terms in a hash table (POLYLAB_FLAG_NO_GROUP_FINISH) */
 } polylab_stats;
 
 /* Options; a zero-initialised struct (or a NULL pointer) means the defaults. */

@@ -32,11 +32,13 @@ FLAG_EXACT_BOUNDS = 32
 FLAG_NO_TABLE = 64
 FLAG_NO_SMALL = 128
 FLAG_EXACT_HIST = 256
+FLAG_NO_GROUP_FINISH = 512
+FLAG_DEBUG_GROUP_HANDS_ON = 0x04000000
 FLAG_DEBUG_FORCE_TABLE = 0x10000000
 FLAG_DEBUG_FORCE_HASH = 0x08000000
 FLAG_DEBUG_FORCE_BUCKET = 0x20000000
 FLAG_DEBUG_UNSTABLE = 0x40000000
-FLAG_DEBUG_NFAST_SHIFT = 8
+FLAG_DEBUG_NFAST_SHIFT = 16
 STAGES = ("bounds", "pack", "sort", "reduce", "prune")
 MAX_NVARS = 256
 MAX_TERMS = 1 << 30
@@ -58,7 +60,7 @@ class _Stats(ctypes.Structure):
                 ("stage_ms", ctypes.c_float * 8), ("prefix_passes", ctypes.c_int32), ("bucket_fallback", ctypes.c_int32),
                 ("refinish_tiles", ctypes.c_int32), ("plan_digits", ctypes.c_int32), ("bounds_sampled", ctypes.c_int32),
                 ("bounds_retry", ctypes.c_int32), ("table_path", ctypes.c_int32), ("table_fallback", ctypes.c_int32),
-                ("small_path", ctypes.c_int32), ("hist_sampled", ctypes.c_int32), ("hist_retry", ctypes.c_int32)]
+                ("small_path", ctypes.c_int32), ("hist_sampled", ctypes.c_int32), ("hist_retry", ctypes.c_int32), ("grouped_tiles", ctypes.c_int32)]
 
 
 class _Opts(ctypes.Structure):
@@ -98,6 +100,7 @@ class Stats:
     small_path: int = 0
     hist_sampled: int = 0
     hist_retry: int = 0
+    grouped_tiles: int = 0
 
 
 _lib = None
@@ -224,7 +227,7 @@ def _stats(st: _Stats) -> Stats:
                  st.distinct, st.survivors, st.kernel_launches, {k: float(st.stage_ms[i]) for i, k in enumerate(STAGES)},
                  rank_fallback=st.rank_fallback, prefix_passes=st.prefix_passes, bucket_fallback=st.bucket_fallback,
                  refinish_tiles=st.refinish_tiles, bounds_sampled=st.bounds_sampled, bounds_retry=st.bounds_retry,
-                 table_path=st.table_path, table_fallback=st.table_fallback, small_path=st.small_path, hist_sampled=st.hist_sampled, hist_retry=st.hist_retry)
+                 table_path=st.table_path, table_fallback=st.table_fallback, small_path=st.small_path, hist_sampled=st.hist_sampled, hist_retry=st.hist_retry, grouped_tiles=st.grouped_tiles)
 
 
 def _dev_poly(coef: torch.Tensor, exps: torch.Tensor, strides=None):

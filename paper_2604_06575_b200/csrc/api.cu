@@ -151,7 +151,7 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 // ------------------------------------------------------------------------------ workspace carving
 
 struct Layout {
-    size_t control, sort_state, slack_tiles, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
+    size_t control, sort_state, slack_tiles, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_wl2, fin_chunks, zero_end;
     size_t tab_state, tab, tab_bytes;
     size_t keys[2], coefs[2], ka, kb, ca, cb, total;      // ca, cb: fp32 operand coefficients of a product, widened to fp64
 };
@@ -213,6 +213,7 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.slack_tiles = take((sort_tiles + kSlackExtraTiles) * sizeof(uint2));     // (written in full by slack_tiles_kernel)
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.fin_wl = take((fin_tiles + 1) * sizeof(uint4));
+    L.fin_wl2 = take((fin_tiles + 1) * sizeof(uint4));
     L.fin_chunks = take((fin_tiles / 4096 + 2) * sizeof(uint32_t));
     L.red_heads = take(red_tiles * sizeof(uint32_t));
     L.red_hb = take(red_tiles * sizeof(uint32_t));
@@ -336,6 +337,15 @@ static int fast_digits(const Opts& o)
     return dbg;                    // 0 = no limit: as many bits below the prefix as fit the 27-bit composite sort word
 }
 
+// 1: tiles go through the group kernel first (finish.cu); 0: the sorting finish kernel only; 2: test hook, the group kernel
+// runs and hands every tile on
+static int finish_group_mode(const Opts& o)
+{
+    if (o.flags & POLYLAB_FLAG_NO_GROUP_FINISH) return 0;
+    // (the fast-digits hook is about the sorting kernel's local sort: every tile must reach it)
+    return ((o.flags & POLYLAB_FLAG_DEBUG_GROUP_HANDS_ON) || fast_digits(o) != 0) ? 2 : 1;
+}
+
 // After S1/X1 accumulated the histogram of the first prefix digit: do its bins predict buckets that fit a tile?
 // (A necessary test only; tile_bounds_kernel has the last word.)  On rejection the LSD path needs digit 0's histogram.
 static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* ws, const Layout& L, const Opts& o,
@@ -365,7 +375,7 @@ static int bucket_precheck(const Plan& plan, int* k, int64_t n, unsigned char* w
 // ----------------------------------------------------------------------- shared tail of both paths
 
 // keys/coefs of the N unsorted pairs are in (L.keys[0], coef0); digit-0 histogram is in ctl->hist[0].
-struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish, fin_count, tab_count, tab_overflow, slack_overflow; };
+struct Readback { int32_t status; uint32_t distinct, survivors, unsorted, overflow, refinish, fin_count, tab_count, tab_overflow, slack_overflow, fin2_count; };
 
 // Bucket path: k stable passes over the top k digits, then finish.cu.  The pairs are in (L.keys[0], coef0) and the
 // histogram of digit P-k is in ctl->hist[P-k].
@@ -393,7 +403,8 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
                                kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes, out_capacity,
-                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint32_t*)(ws + L.fin_chunks), ctl,
+                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint4*)(ws + L.fin_wl2),
+                               finish_group_mode(o), (uint32_t*)(ws + L.fin_chunks), ctl,
                                (o.flags & POLYLAB_FLAG_DEVICE_COUNT) ? out_nterms : nullptr,
                                tm.on ? tm.ev[POLYLAB_STAGE_REDUCE + 1] : nullptr, stream);      // REDUCE = tiles, PRUNE = scan + emit
     tm.mark(POLYLAB_STAGE_PRUNE);
@@ -415,6 +426,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     if (o.stats) {
         o.stats->distinct = res.distinct; o.stats->survivors = res.survivors;
         o.stats->prefix_passes = k; o.stats->sort_passes = k; o.stats->refinish_tiles = (int32_t)res.refinish;
+        o.stats->grouped_tiles = finish_group_mode(o) ? (int32_t)(res.fin_count - res.fin2_count) : 0;
         o.stats->hist_sampled = slack ? 1 : 0;
     }
     if (res.status != POLYLAB_OK) return res.status;

@@ -294,6 +294,7 @@ struct Control {
     uint32_t tab_count;                      // table path: distinct keys inserted so far (= U after the insert pass)
     uint32_t tab_overflow;                   // table path: more distinct keys than the table was sized for -> sort path
     uint32_t slack_overflow;                 // slack bins (sort.cu): a bin's capacity, estimated from a sample, was too small
+    uint32_t fin2_count;                     // bucket path: tiles the group kernel handed on to the sorting finish kernel (second work list)
     uint32_t slack_count[kRadix];            // exact bin counts of the pass that wrote with slack
     uint32_t slack_cap[kRadix];              // the capacities (kept for the reading pass)
     uint32_t est[kRadix];                    // histogram of the first prefix digit over a SAMPLE of the rows

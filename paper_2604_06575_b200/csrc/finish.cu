@@ -243,7 +243,11 @@ struct FinishArgs {
     uint32_t n, ntiles;
     uint32_t fin_tile;              // positions per tile; a tile owns at most kFinCap records
     const uint32_t* tile_start;     // [ntiles + 1]
-    const uint4* worklist;          // the ctl->fin_count tiles that own records: (tile, first record, end, -)
+    const uint4* worklist;          // the *list_count tiles that own records: (tile, first record, end, first and last share the prefix)
+    const uint32_t* list_count;     // DEVICE: length of the work list (ctl->fin_count, or ctl->fin2_count behind the group kernel)
+    int strided;                    // the grid is smaller than the list may be: blocks walk it with stride gridDim.x
+    uint4* worklist2;               // group kernel: the tiles it hands on to finish_kernel (ctl->fin2_count of them)
+    int no_group;                   // group kernel, test hook: hand every tile on
     uint32_t* tile_state;           // [ntiles + 1] survivors per tile, zero before the kernel
     int pfx_pos;                    // the prefix is the key bits at positions >= pfx_pos
     int fast_bits;                  // most key bits below the prefix the first attempt sorts on (test hook; 32 = no limit)
@@ -282,30 +286,140 @@ __device__ __forceinline__ void emit_term(const EmitArgs& a, const Plan& plan, u
         store_exp(a.out_exps, a.exp_bytes, (int64_t)o * plan.nvars + v, key_get_field(kk, plan.shift[v], plan.width[v]));
 }
 
+// ------------------------------------------------------------------- S3 + S4 of a tile (shared tail)
+
+// A thread walks `itn` consecutive sorted positions [first, first + itn) of its tile: heads of runs of equal keys, the sum
+// since the last head, and S4 for the runs that END inside its stretch.
+struct RunState {
+    uint32_t hm = 0, nh = 0;            // head mask of the thread's positions, number of heads
+    uint32_t keep = 0, nkeep = 0;       // bit k: the k-th run that ends in this thread survives the prune
+    uint32_t nclosed = 0;               // runs that end in this thread
+    double acc = 0.0, part0 = 0.0;      // sum since the last head; this thread's part of the first run that ends here
+};
+
+__device__ __forceinline__ void run_step(RunState& r, bool head, double c, uint32_t j, uint32_t pos, double tol, double* scs)
+{
+    if (head) {
+        // S4 for the run that ENDS here (a run ends where the next head is met): a run that also began in this thread has
+        // its whole sum in acc; the first one needs the other threads' part (finish_tail)
+        if (pos > 0) {
+            if (r.nclosed == 0) r.part0 = r.acc;
+            else if (fabs(r.acc) > tol) {                  // NaN compares false: dropped (A12)
+                r.keep |= 1u << r.nclosed;
+                ++r.nkeep;
+                scs[pos - 1] = r.acc;                      // the run's sum, parked on its last record (own position)
+            }
+            ++r.nclosed;
+        }
+        r.hm |= 1u << j; ++r.nh; r.acc = c;
+    } else r.acc = __dadd_rn(r.acc, c);
+}
+
+// Segmented scan across the block, prune, and the tile's survivors compacted in order at the tile's own place.
+// key_of(pos, q): the key of the run that ends at sorted position pos, q = the run's ordinal in the tile.
+template <typename K, typename KeyOf>
+__device__ __forceinline__ void finish_tail(const FinishArgs& a, const RunState& r, double* scs, uint32_t* scratch, uint32_t first,
+                                            uint32_t n_loc, uint32_t lo, uint32_t tile, KeyOf key_of)
+{
+    constexpr int THREADS = kFinThreads, NW = THREADS / 32;
+    __shared__ uint32_t wagg_f[NW];
+    __shared__ double wagg_v[NW];
+    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    uint32_t keep = r.keep, nkeep = r.nkeep;
+
+    // ---- S3: segmented scan of (has head, sum since last head) across the block; no run crosses a tile
+    SegPair incl;
+    incl.f = r.nh > 0;
+    incl.v = r.acc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        SegPair l;
+        l.f = __shfl_up_sync(kFullMask, incl.f, o);
+        l.v = __shfl_up_sync(kFullMask, incl.v, o);
+        if (lane >= (unsigned)o) incl = seg_combine(l, incl);
+    }
+    if (lane == 31) { wagg_f[warp] = incl.f; wagg_v[warp] = incl.v; }
+    SegPair carry;                                 // exclusive within the warp
+    carry.f = __shfl_up_sync(kFullMask, incl.f, 1);
+    carry.v = __shfl_up_sync(kFullMask, incl.v, 1);
+    if (lane == 0) { carry.f = 0; carry.v = 0.0; }
+    __syncthreads();
+    {
+        SegPair wp;
+        wp.f = 0;
+        wp.v = 0.0;
+        for (unsigned w = 0; w < warp; ++w) {
+            SegPair x;
+            x.f = wagg_f[w];
+            x.v = wagg_v[w];
+            wp = seg_combine(wp, x);
+        }
+        carry = seg_combine(wp, carry);
+        incl = seg_combine(wp, incl);
+    }
+
+    // ---- S4 for the first run that ends in this thread (its head lies in an earlier thread); the run still open at the
+    // end of the tile is closed by the last thread, whose inclusive scan value is its sum
+    const uint32_t chm = (first == 0) ? (r.hm & ~1u) : r.hm;    // the heads that close a run (every head but the tile's first record)
+    if (r.nclosed > 0) {
+        const double total0 = __dadd_rn(carry.v, r.part0);
+        if (fabs(total0) > a.tol) {
+            keep |= 1u;
+            ++nkeep;
+            scs[first + (__ffs(chm) - 1) - 1] = total0;             // its last record is the one before that head (maybe the previous thread's: nobody else touches it)
+        }
+    }
+    const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
+    // one scan for two counts (each at most CAP < 2^16): survivors in the low half, heads (distinct monomials) in the high half
+    uint32_t tile_keep, tot_heads;
+    uint32_t kexcl = block_exclusive_scan<THREADS>((nkeep + (last_keep ? 1u : 0u)) | (r.nh << 16), scratch, &tile_keep);
+    const uint32_t hexcl = kexcl >> 16;            // heads in the threads before this one
+    kexcl &= 0xffffu;
+    tot_heads = tile_keep >> 16;
+    tile_keep &= 0xffffu;
+
+    // ---- the tile's survivors, compacted in order at the tile's own place; S5 (emit_kernel) puts the tiles together
+    {
+        K* __restrict__ uk = (K*)a.ukeys + lo;
+        double* __restrict__ us = a.usums + lo;
+        uint32_t o = kexcl;
+        uint32_t k = 0;
+        // head number hexcl + k (+ 1 in the thread that holds the tile's first record, whose own head closes nothing)
+        // closes run number hexcl + k (- 1 elsewhere)
+        uint32_t q = hexcl - (first == 0 ? 0u : 1u);
+        for (uint32_t m = chm; m != 0u; m &= m - 1u, ++k, ++q) {    // the runs that end in this thread, in order
+            if (keep & (1u << k)) {
+                const uint32_t pos = first + (__ffs(m) - 1) - 1;    // the run's last record, where its sum was parked
+                us[o] = scs[pos];
+                uk[o] = key_of(pos, q);
+                ++o;
+            }
+        }
+        if (last_keep) { us[o] = incl.v; uk[o] = key_of(n_loc - 1, tot_heads - 1u); }
+    }
+    if (tid == 0) {
+        if (tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);      // distinct monomials, for the statistics
+        a.tile_state[tile] = tile_keep;
+    }
+}
+
 // ------------------------------------------------------------------------------------ finish kernel
 
+// One work-list tile through the sorting finish: local sort, S3, S4 (the body of finish_kernel).
 template <typename K>
-__global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(const __grid_constant__ FinishArgs a, const __grid_constant__ Plan plan)
+__device__ __forceinline__ void finish_tile(const FinishArgs& a, unsigned char* smem_raw, const uint4 wl)
 {
-    constexpr int THREADS = kFinThreads, CAP = kFinCap, NW = THREADS / 32;
+    constexpr int THREADS = kFinThreads, CAP = kFinCap;
     static_assert(CAP <= 8192 && CAP / THREADS <= 32, "13-bit record indices in the sort elements, 32-bit head masks");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t* bx = (uint32_t*)(smem_raw + FinishSmem::off_x);
     uint32_t* by = (uint32_t*)(smem_raw + FinishSmem::off_y);
     uint16_t* py = (uint16_t*)(smem_raw + FinishSmem::off_p);              // head flags -> ordinals -> final permutation
     uint32_t* whist = (uint32_t*)(smem_raw + FinishSmem::off_whist);
-    uint32_t* scratch = (uint32_t*)(smem_raw + FinishSmem::off_scratch);   // [0..NW+1] scans, [40] tile, [41] base
+    uint32_t* scratch = (uint32_t*)(smem_raw + FinishSmem::off_scratch);   // [0..NW+1] scans
     double* scs = (double*)smem_raw;               // coefficients in sorted order, over X / Y once the sort is done
     static_assert(FinishSmem::whist_bytes >= (size_t)kFinCap * 2, "the inverse permutation borrows the histogram rows");
-    __shared__ uint32_t wagg_f[NW];
-    __shared__ double wagg_v[NW];
 
-    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    if (a.ctl->overflow) return;                   // set by tile_bounds_kernel: the call will re-run on the LSD path
-    const uint32_t fin_count = a.ctl->fin_count;
-    if (blockIdx.x == 0 && tid == 0 && fin_count > gridDim.x) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
-    if (blockIdx.x >= fin_count) return;           // the grid is sized for the most tiles that can own records
-    const uint4 wl = a.worklist[blockIdx.x];       // one load instead of three dependent ones
+    const unsigned tid = threadIdx.x;
     const uint32_t tile = wl.x, lo = wl.y, hi = wl.z;
     const uint32_t n_loc = hi > lo ? min(hi - lo, (uint32_t)CAP) : 0u;
     const K* __restrict__ gkeys = (const K*)a.keys + lo;
@@ -324,8 +438,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
     // raw sort bits of the fast attempt: the (up to 32) key bits just below the prefix
     const int rbits = min(32, a.pfx_pos);
     bool full = (rbits == 0);                      // nothing below the prefix: only the ordinal is sorted on
-    uint32_t hm = 0, nh = 0, keep = 0, nkeep = 0, nclosed = 0;
-    double acc = 0.0, part0 = 0.0;
+    RunState r;
     bool try_single = wl.w != 0u && !full;        // first and last record share the prefix: probably one bucket
     while (true) {
         // ---- stream the keys once: bucket heads and the raw sort bits
@@ -474,8 +587,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         }
 
         // ---- gather through the permutation: heads of runs of equal keys, sums since the last head, order check
-        hm = 0; nh = 0; acc = 0.0;
-        keep = 0; nkeep = 0; nclosed = 0; part0 = 0.0;
+        r = RunState();
         bool viol = false;
         {
             K kp;
@@ -485,25 +597,11 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
 #pragma unroll 2
             for (uint32_t j = 0; j < itn; ++j) {
                 if (first + j < n_loc) {
-                    const uint32_t r = py[first + j];
-                    const K kk = gkeys[r];
+                    const K kk = gkeys[py[first + j]];
                     const double c = scs[first + j];
                     const bool head = !hp || !key_eq(kk, kp);
                     viol |= hp && key_lt(kk, kp);
-                    if (head) {
-                        // S4 for the runs that END here (a run ends where the next head is met): a run that also began
-                        // in this thread has its whole sum in acc; the first one needs the other threads' part (below)
-                        if (first + j > 0) {
-                            if (nclosed == 0) part0 = acc;
-                            else if (fabs(acc) > a.tol) {                  // NaN compares false: dropped (A12)
-                                keep |= 1u << nclosed;
-                                ++nkeep;
-                                scs[first + j - 1] = acc;                  // the run's sum, parked on its last record (own position)
-                            }
-                            ++nclosed;
-                        }
-                        hm |= 1u << j; ++nh; acc = c;
-                    } else acc = __dadd_rn(acc, c);
+                    run_step(r, head, c, j, first + j, a.tol, scs);
                     kp = kk;
                     hp = true;
                 }
@@ -519,76 +617,386 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
         if (tid == 0) atomicAdd(&a.ctl->refinish, 1u);
     }
 
-    // ---- S3: segmented scan of (has head, sum since last head) across the block; no run crosses a tile
-    SegPair incl;
-    incl.f = nh > 0;
-    incl.v = acc;
+    finish_tail<K>(a, r, scs, scratch, first, n_loc, lo, tile, [&](uint32_t pos, uint32_t) { return gkeys[py[pos]]; });
+}
+
+template <typename K>
+__global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(const __grid_constant__ FinishArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (a.ctl->overflow) return;                   // set by tile_bounds_kernel: the call will re-run on the LSD path
+    const uint32_t count = *a.list_count;
+    // one block per tile, the grid sized for the most tiles that can own records (at most one per bucket): more of them
+    // than that and the array is not sorted by prefix.  Behind the group kernel the list is usually short and the blocks stride.
+    if (!a.strided && blockIdx.x == 0 && threadIdx.x == 0 && count > gridDim.x) a.ctl->unsorted = 1u;
+    for (uint32_t b = blockIdx.x; b < count; b += gridDim.x) {
+        finish_tile<K>(a, smem_raw, a.worklist[b]);            // one load instead of three dependent ones
+        if (!a.strided) break;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------- group kernel
+
+// The sorting finish moves every RECORD through three counting-sort passes and then gathers every record's key again to
+// find the runs.  When a tile holds few distinct keys (the paper's regime: like terms by the dozen; config 5:
+// ten records per monomial) that is the wrong amount of work.  finish_group_kernel, tried first on every work-list tile:
+//   G1  streams the keys once and looks each up in a shared-memory hash table (256 buckets of four slots, a 31-bit
+//       fingerprint per slot: one 16-byte load shows a bucket; atomicCAS on the bucket's first empty slot, the winner parks
+//       the full key and its record number); after a barrier every record compares its FULL key with the slot's -- a
+//       fingerprint collision, an overlong probe sequence or more than 768 distinct keys hand the tile on to finish_kernel
+//       through a second work list;
+//   G2  puts the U distinct keys (not the records) in order: a 10-bit leading digit (prefix difference above the top key
+//       bits below the prefix) bins them, and inside a bin -- one or two keys as a rule, more than 16 hand the tile on -- a
+//       key's place is the number of smaller keys, full keys compared: exact, no order check needed;
+//   G3  ONE stable counting pass of the records on their slot (per-warp rows of 1024 packed 16-bit counters, rank = old
+//       value of the atomic), the bin scan walking the slots in KEY order: every record now knows its final sorted position;
+//   G4  coefficients go to their sorted position (coalesced read, as before) and run heads into a bit mask -- no key gather;
+//   then the shared tail (S3, S4).  Equal keys keep their input order exactly as through the stable sort, so the sums are
+//   bit-identical to finish_kernel's (tests/test_gpu_bucket_path.py compares the two).
+constexpr int kGrpSlots = 1024;
+constexpr int kGrpMaxDistinct = 768;
+constexpr int kGrpMaxProbe = 48;
+constexpr int kGrpBPT = kGrpMaxDistinct / kFinThreads;      // slots per thread in the bin scan
+constexpr int kGrpDigit = 10;           // bits of the distinct keys' leading digit
+constexpr int kGrpMaxBin = 16;          // most distinct keys that may share a leading digit
+
+struct GroupSmem {
+    static constexpr int NW = kFinThreads / 32;
+    // region A, kFinCap * 8 bytes: [tags u32][keys 16 B][bins u32][order u16][perm u16] while the table lives, then the
+    // counting rows [NW][kGrpSlots] u16 over the keys (perm still alive), then the sorted coefficients over all of it
+    static constexpr size_t off_tags = 0;
+    static constexpr size_t off_keys = off_tags + (size_t)kGrpSlots * 4;
+    static constexpr size_t off_bins = off_keys + (size_t)kGrpSlots * 16;
+    static constexpr size_t off_order = off_bins + (size_t)kGrpSlots * 4;
+    static constexpr size_t off_perm = off_order + (size_t)kGrpSlots * 2;
+    static constexpr size_t region_a = off_perm + (size_t)kGrpSlots * 2;
+    static constexpr size_t off_rows = off_keys;
+    static constexpr size_t off_ids = (size_t)kFinCap * 8;           // u16 per record: its slot; later the head bit mask
+    static constexpr size_t off_rk = off_ids + (size_t)kFinCap * 2;  // u16 per record: rank, then sorted position; before that
+                                                                     // [record that claimed the slot]
+    static constexpr size_t off_rep = off_rk + (size_t)kFinCap * 2;  // u16 per distinct key, in key order: a record that holds it
+    static constexpr size_t off_scratch = off_rep + (size_t)kGrpMaxDistinct * 2;
+    static constexpr size_t bytes = off_scratch + 64 * 4;
+};
+static_assert(GroupSmem::region_a <= (size_t)kFinCap * 8, "the table lives where the sorted coefficients go");
+static_assert((size_t)GroupSmem::NW * kGrpSlots * 2 <= (size_t)kGrpSlots * 16, "the counting rows take the place of the table's keys");
+static_assert(kGrpSlots <= kFinCap && kGrpBPT * kFinThreads == kGrpMaxDistinct && kGrpMaxDistinct <= kGrpSlots, "group path sizes");
+static_assert((1 << kGrpDigit) == kGrpSlots && kGrpSlots % kFinThreads == 0, "one bin per slot index, whole slots per thread");
+static_assert((GroupSmem::bytes + 96 + 1024) * kFinBlocksPerSM <= 228 * 1024, "four blocks per SM");
+
+// bucket and fingerprint of a key: x = a multiply-add mix of the key's 32-bit words; the bucket is x's top byte and the
+// fingerprint a bijection of x (two keys of one bucket share a fingerprint only if they share x, or differ in the forced bit)
+__device__ __forceinline__ uint32_t key_mix(uint64_t k) { return (uint32_t)k * 0x9E3779B1u + (uint32_t)(k >> 32) * 0x85EBCA77u; }
+__device__ __forceinline__ uint32_t key_mix(const Key128& k)
+{
+    return (uint32_t)k.lo * 0x9E3779B1u + (uint32_t)(k.lo >> 32) * 0x85EBCA77u + (uint32_t)k.hi * 0xC2B2AE3Du + (uint32_t)(k.hi >> 32) * 0x27D4EB2Fu;
+}
+template <typename K>
+__device__ __forceinline__ void key_hash(const K& k, uint32_t* bucket, uint32_t* fp)
+{
+    uint32_t x = key_mix(k);
+    x ^= x >> 15;
+    *bucket = (x * 0x2C1B3C6Du) >> (32 - 8);                  // kGrpSlots / 4 = 256 buckets of four slots
+    *fp = ((x ^ (x >> 13)) * 0x297A2D39u) | 0x80000000u;      // never 0 = empty
+}
+static_assert(kGrpSlots / 4 == 256, "key_hash takes the bucket from eight bits");
+// the key bits at positions >= pos as a number (the prefix has at most 48 bits)
+__device__ __forceinline__ uint64_t key_prefix64(uint64_t k, int pos) { return k >> pos; }
+__device__ __forceinline__ uint64_t key_prefix64(const Key128& k, int pos)
+{
+    if (pos >= 64) return k.hi >> (pos - 64);
+    return pos == 0 ? k.lo : ((k.lo >> pos) | (k.hi << (64 - pos)));
+}
+
+template <typename K>
+__global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_kernel(const __grid_constant__ FinishArgs a)
+{
+    constexpr int THREADS = kFinThreads, CAP = kFinCap, NW = THREADS / 32, SPT = kGrpSlots / THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* tags = (uint32_t*)(smem_raw + GroupSmem::off_tags);
+    const uint4* tags4 = (const uint4*)tags;
+    K* tkeys = (K*)(smem_raw + GroupSmem::off_keys);
+    uint32_t* bins = (uint32_t*)(smem_raw + GroupSmem::off_bins);            // count of the distinct keys per leading digit, then (start | count << 16)
+    uint16_t* order = (uint16_t*)(smem_raw + GroupSmem::off_order);          // slots grouped by leading digit
+    uint16_t* perm = (uint16_t*)(smem_raw + GroupSmem::off_perm);            // slots in key order
+    uint32_t* rows32 = (uint32_t*)(smem_raw + GroupSmem::off_rows);
+    uint16_t* rows16 = (uint16_t*)(smem_raw + GroupSmem::off_rows);
+    uint16_t* ids = (uint16_t*)(smem_raw + GroupSmem::off_ids);
+    uint32_t* hb = (uint32_t*)(smem_raw + GroupSmem::off_ids);              // head bits by sorted position, once the slots are dead
+    uint16_t* rk = (uint16_t*)(smem_raw + GroupSmem::off_rk);
+    uint16_t* own = rk;                                                      // [kGrpSlots] record that claimed the slot
+    uint16_t* rep = (uint16_t*)(smem_raw + GroupSmem::off_rep);
+    uint32_t* scratch = (uint32_t*)(smem_raw + GroupSmem::off_scratch);      // [0..NW+1] scans, [48] largest prefix difference
+    double* scs = (double*)smem_raw;
+
+    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    // (persistent blocks that take tiles by ticket and pull the NEXT tile's descriptor and records into L2 while one is worked
+    // on were measured: 3.00 against 2.95 ms on config 5 -- the hardware's block scheduler already overlaps the start-up loads)
+    const uint32_t overflow = a.ctl->overflow, fin_count = a.ctl->fin_count;
+    if (overflow) return;                          // set by tile_bounds_kernel: the call will re-run on the LSD path
+    if (blockIdx.x == 0 && tid == 0 && fin_count > gridDim.x) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
+    if (blockIdx.x >= fin_count) return;
+    const uint4 wl = a.worklist[blockIdx.x];
+    const uint32_t tile = wl.x, lo = wl.y, hi = wl.z;
+    const uint32_t n_loc = hi > lo ? min(hi - lo, (uint32_t)CAP) : 0u;
+    const K* __restrict__ gkeys = (const K*)a.keys + lo;
+    const double* __restrict__ gcoef = a.coefs + lo;
+    const uint32_t itn = ((n_loc + THREADS - 1) / THREADS) | 1u;
+    const uint32_t first = tid * itn;
+
+    // Is grouping worth trying?  Not when most tiles so far were handed on (an input without duplicates): blocks start in
+    // order, so blockIdx.x is about the number of tiles begun.
+    bool hand_on = a.no_group != 0 || n_loc < 64u;
+    if (tid == 0 && !hand_on) {
+        const uint32_t f = *(volatile const uint32_t*)&a.ctl->fin2_count;
+        hand_on = f >= 64u && 2u * f > blockIdx.x;
+    }
+    hand_on = __syncthreads_or(hand_on ? 1 : 0) != 0;
+    bool bad = false;
+    uint32_t U = 0;
+    if (!hand_on) {
+        for (uint32_t i = tid * 8u; i < n_loc; i += THREADS * 8u) asm volatile("prefetch.global.L2 [%0];" ::"l"(gkeys + i));
+        for (uint32_t i = tid * 16u; i < n_loc; i += THREADS * 16u) asm volatile("prefetch.global.L2 [%0];" ::"l"(gcoef + i));
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        SegPair l;
-        l.f = __shfl_up_sync(kFullMask, incl.f, o);
-        l.v = __shfl_up_sync(kFullMask, incl.v, o);
-        if (lane >= (unsigned)o) incl = seg_combine(l, incl);
-    }
-    if (lane == 31) { wagg_f[warp] = incl.f; wagg_v[warp] = incl.v; }
-    SegPair carry;                                 // exclusive within the warp
-    carry.f = __shfl_up_sync(kFullMask, incl.f, 1);
-    carry.v = __shfl_up_sync(kFullMask, incl.v, 1);
-    if (lane == 0) { carry.f = 0; carry.v = 0.0; }
-    __syncthreads();
-    {
-        SegPair wp;
-        wp.f = 0;
-        wp.v = 0.0;
-        for (unsigned w = 0; w < warp; ++w) {
-            SegPair x;
-            x.f = wagg_f[w];
-            x.v = wagg_v[w];
-            wp = seg_combine(wp, x);
-        }
-        carry = seg_combine(wp, carry);
-        incl = seg_combine(wp, incl);
-    }
+        for (int j = 0; j < SPT; ++j) { tags[tid + j * THREADS] = 0u; bins[tid + j * THREADS] = 0u; }
+        if (tid == 0) scratch[48] = 0u;
+        __syncthreads();
 
-    // ---- S4 for the first run that ends in this thread (its head lies in an earlier thread); the run still open at the
-    // end of the tile is closed by the last thread, whose inclusive scan value is its sum
-    const uint32_t chm = (first == 0) ? (hm & ~1u) : hm;        // the heads that close a run (every head but the tile's first record)
-    if (nclosed > 0) {
-        const double total0 = __dadd_rn(carry.v, part0);
-        if (fabs(total0) > a.tol) {
-            keep |= 1u;
-            ++nkeep;
-            scs[first + (__ffs(chm) - 1) - 1] = total0;             // its last record is the one before that head (maybe the previous thread's: nobody else touches it)
-        }
-    }
-    const bool last_keep = (tid == THREADS - 1) && n_loc > 0 && fabs(incl.v) > a.tol;
-    // one scan for two counts (each at most CAP < 2^16): survivors in the low half, heads (distinct monomials) in the high half
-    uint32_t tile_keep, tot_heads;
-    uint32_t kexcl = block_exclusive_scan<THREADS>((nkeep + (last_keep ? 1u : 0u)) | (nh << 16), scratch, &tile_keep);
-    kexcl &= 0xffffu;
-    tot_heads = tile_keep >> 16;
-    tile_keep &= 0xffffu;
-
-    // ---- the tile's survivors, compacted in order at the tile's own place; S5 (emit_kernel) puts the tiles together
-    {
-        K* __restrict__ uk = (K*)a.ukeys + lo;
-        double* __restrict__ us = a.usums + lo;
-        uint32_t o = kexcl;
-        uint32_t k = 0;
-        for (uint32_t m = chm; m != 0u; m &= m - 1u, ++k) {         // the runs that end in this thread, in order
-            if (keep & (1u << k)) {
-                const uint32_t pos = first + (__ffs(m) - 1) - 1;    // the run's last record, where its sum was parked
-                us[o] = scs[pos];
-                uk[o] = gkeys[py[pos]];
-                ++o;
+        // ---- G1: every record finds or claims the slot of its key.  The table is 256 buckets of four tags: one 16-byte
+        // load shows a bucket, a key takes the bucket's first empty slot (slots fill in order and never empty again, so two
+        // records of one key cannot claim two slots).
+        const K k0 = gkeys[0];
+        const bool single = wl.w != 0u;            // first and last record share the prefix: one bucket if the array is sorted
+        bool descending = false;
+        for (uint32_t base = 0; base < n_loc; base += 4 * THREADS) {
+            K k[4];
+            uint32_t sl[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = base + u * THREADS + tid;
+                k[u] = k0;
+                if (i < n_loc) k[u] = gkeys[i];
+            }
+            if (!single) {                         // prefix-order self-check (a one-bucket tile is checked on its distinct keys, G2)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = base + u * THREADS + tid;
+                    if (i > 0 && i < n_loc) {
+                        const K kp = gkeys[i - 1];
+                        descending |= key_prefix64(k[u], a.pfx_pos) < key_prefix64(kp, a.pfx_pos);
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = base + u * THREADS + tid;
+                sl[u] = 0u;
+                if (i < n_loc) {
+                    uint32_t b, fp, s = 0u;
+                    key_hash(k[u], &b, &fp);
+                    for (int tries = 0;; ++tries) {
+                        const uint4 t = tags4[b];
+                        int j = t.x == fp ? 0 : t.y == fp ? 1 : t.z == fp ? 2 : t.w == fp ? 3 : -1;
+                        if (j >= 0) { s = 4u * b + (uint32_t)j; break; }
+                        j = t.x == 0u ? 0 : t.y == 0u ? 1 : t.z == 0u ? 2 : t.w == 0u ? 3 : -1;
+                        if (j >= 0) {
+                            s = 4u * b + (uint32_t)j;
+                            const uint32_t old = atomicCAS(&tags[s], 0u, fp);
+                            if (old == 0u) { tkeys[s] = k[u]; own[s] = (uint16_t)i; break; }
+                            if (old == fp) break;
+                        } else b = (b + 1u) & (uint32_t)(kGrpSlots / 4 - 1);       // (a lost race looks at the same bucket again)
+                        if (tries >= kGrpMaxProbe) { bad = true; break; }
+                    }
+                    sl[u] = s;
+                    ids[i] = (uint16_t)s;
+                }
+            }
+            __syncthreads();                       // the keys of every slot claimed so far are in place
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = base + u * THREADS + tid;
+                if (i < n_loc) bad |= !key_eq(tkeys[sl[u]], k[u]);
             }
         }
-        if (last_keep) { us[o] = incl.v; uk[o] = gkeys[py[n_loc - 1]]; }
+        if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
+
+        // ---- G2: the distinct keys in order.  Leading digit = prefix difference above the top key bits below the prefix,
+        // ten bits in all: a key's place is the start of its digit's bin plus the number of smaller keys in that bin (full
+        // keys compared, so the order is exact; a bin of more than kGrpMaxBin keys hands the tile on)
+        const uint64_t p0 = key_prefix64(k0, a.pfx_pos);
+        K kk[SPT];
+        uint32_t occ = 0, dmax = 0;
+#pragma unroll
+        for (int j = 0; j < SPT; ++j) {
+            const uint32_t s = tid + j * THREADS;
+            kk[j] = k0;
+            if (tags[s] != 0u) {
+                occ |= 1u << j;
+                kk[j] = tkeys[s];
+                const uint64_t d = key_prefix64(kk[j], a.pfx_pos) - p0;
+                if (d >> kGrpDigit) bad = true;                       // prefixes too far apart for the digit (or not sorted)
+                dmax = max(dmax, (uint32_t)d & (uint32_t)((1 << kGrpDigit) - 1));
+            }
+        }
+        if (dmax) atomicMax(&scratch[48], dmax);
+        if (single && dmax) bad = true;            // a second prefix inside a tile whose ends share theirs: not sorted by prefix
+        bad = __syncthreads_or(bad ? 1 : 0) != 0;
+        if (!bad) {
+            dmax = scratch[48];
+            int ob = 0;
+            while ((dmax >> ob) != 0u) ++ob;
+            const int fb = min(kGrpDigit - ob, a.pfx_pos);
+            uint32_t dig[SPT], rnk[SPT];
+#pragma unroll
+            for (int j = 0; j < SPT; ++j) {
+                dig[j] = 0u; rnk[j] = 0u;
+                if (occ & (1u << j)) {
+                    const uint32_t d = (uint32_t)(key_prefix64(kk[j], a.pfx_pos) - p0);
+                    dig[j] = (d << fb) | (fb ? key_get_field(kk[j], a.pfx_pos - fb, fb) : 0u);
+                    rnk[j] = atomicAdd(&bins[dig[j]], 1u);
+                    bad |= rnk[j] >= (uint32_t)kGrpMaxBin;
+                }
+            }
+            __syncthreads();
+            {
+                uint32_t c[SPT], sum = 0;
+#pragma unroll
+                for (int j = 0; j < SPT; ++j) { c[j] = bins[tid * SPT + j]; sum += c[j]; }
+                uint32_t start = block_exclusive_scan<THREADS>(sum, scratch, &U);
+#pragma unroll
+                for (int j = 0; j < SPT; ++j) { bins[tid * SPT + j] = start | (c[j] << 16); start += c[j]; }
+            }
+            bad = __syncthreads_or(bad ? 1 : 0) != 0 || U > (uint32_t)kGrpMaxDistinct;
+            if (!bad) {
+#pragma unroll
+                for (int j = 0; j < SPT; ++j)
+                    if (occ & (1u << j)) order[(bins[dig[j]] & 0xffffu) + rnk[j]] = (uint16_t)(tid + j * THREADS);
+                __syncthreads();
+#pragma unroll
+                for (int j = 0; j < SPT; ++j) {
+                    if (occ & (1u << j)) {
+                        const uint32_t s = tid + j * THREADS, bs = bins[dig[j]], start = bs & 0xffffu, cnt = bs >> 16;
+                        uint32_t below = 0;
+                        if (cnt > 1u)
+                            for (uint32_t m = 0; m < cnt; ++m) {
+                                const uint32_t s2 = order[start + m];
+                                if (s2 != s) below += key_lt(tkeys[s2], kk[j]) ? 1u : 0u;
+                            }
+                        perm[start + below] = (uint16_t)s;
+                        rep[start + below] = own[s];
+                    }
+                }
+                __syncthreads();
+            }
+        }
     }
-    if (tid == 0) {
-        if (tot_heads) atomicAdd(&a.ctl->distinct, tot_heads);      // distinct monomials, for the statistics
-        a.tile_state[tile] = tile_keep;
+    if (hand_on || bad) {
+        if (tid == 0) a.worklist2[atomicAdd(&a.ctl->fin2_count, 1u)] = wl;
+        return;
     }
+
+    // ---- G3: one stable counting pass of the records on their slot; warp w owns the contiguous chunk [w*per, (w+1)*per)
+    // and row w (see local_pass); the bins are scanned in KEY order
+    const uint32_t per = (((n_loc + NW - 1) / NW) + 31u) & ~31u;
+    const uint32_t wbeg = min(warp * per, n_loc), wend = min(wbeg + per, n_loc);
+    {
+        uint4* z = (uint4*)rows32;
+#pragma unroll
+        for (int j = 0; j < NW * kGrpSlots * 2 / 16 / THREADS; ++j) z[tid + j * THREADS] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    __syncthreads();
+    {
+        uint32_t* my_row = rows32 + warp * (kGrpSlots / 2);
+        for (uint32_t base = wbeg; base < wend; base += 64u) {
+            const uint32_t i0 = base + lane, i1 = i0 + 32u;
+            const uint32_t d0 = (i0 < wend) ? ids[i0] : 0u, d1 = (i1 < wend) ? ids[i1] : 0u;
+            if (i0 < wend) {
+                const uint32_t sh = (d0 & 1u) * 16u;
+                rk[i0] = (uint16_t)(atomicAdd(&my_row[d0 >> 1], 1u << sh) >> sh);
+            }
+            __syncwarp();
+            if (i1 < wend) {
+                const uint32_t sh = (d1 & 1u) * 16u;
+                rk[i1] = (uint16_t)(atomicAdd(&my_row[d1 >> 1], 1u << sh) >> sh);
+            }
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    {
+        uint32_t c[kGrpBPT][NW], sl[kGrpBPT];
+        uint32_t count = 0;
+#pragma unroll
+        for (int j = 0; j < kGrpBPT; ++j) {
+            const uint32_t q = tid * kGrpBPT + j;
+            sl[j] = q < U ? perm[q] : 0u;
+#pragma unroll
+            for (int w = 0; w < NW; ++w) c[j][w] = q < U ? rows16[w * kGrpSlots + sl[j]] : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < kGrpBPT; ++j)
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { const uint32_t x = c[j][w]; c[j][w] = count; count += x; }
+        uint32_t total;
+        const uint32_t bin_start = block_exclusive_scan<THREADS>(count, scratch, &total);
+#pragma unroll
+        for (int j = 0; j < kGrpBPT; ++j) {
+            const uint32_t q = tid * kGrpBPT + j;
+            if (q < U) {
+                // bit 15: this warp holds the key's first record (its rank-0 record is the head of the run)
+                const uint32_t end = (j + 1 < kGrpBPT) ? c[j + 1][0] : count;
+                bool seen = false;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    const uint32_t nxt = (w + 1 < NW) ? c[j][w + 1] : end;
+                    const bool has = nxt != c[j][w];
+                    rows16[w * kGrpSlots + sl[j]] = (uint16_t)((bin_start + c[j][w]) | ((has && !seen) ? 0x8000u : 0u));
+                    seen |= has;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // sorted position of every record (over its rank), bit 15 = head of its run
+#pragma unroll 4
+    for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
+        const uint32_t h = rows16[warp * kGrpSlots + ids[i]], r = rk[i];
+        rk[i] = (uint16_t)(((h & 0x1fffu) + r) | ((r == 0u) ? (h & 0x8000u) : 0u));
+    }
+    // the head bits take the place of the first 320 slot ids: when those all belong to warp 0's chunk, warp 0 clears them as
+    // soon as it has read them
+    if (per >= 320u) {
+        if (warp == 0) {
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 5; ++j) hb[lane + 32 * j] = 0u;
+        }
+    } else {
+        __syncthreads();
+        if (tid < 160u) hb[tid] = 0u;               // CAP / 32 words and the two a thread past the end may load
+    }
+    __syncthreads();
+
+    // ---- G4: coefficients to their sorted position (coalesced global read), heads into the bit mask
+#pragma unroll 4
+    for (uint32_t i = tid; i < n_loc; i += THREADS) {
+        const uint32_t p = rk[i], pos = p & 0x1fffu;
+        scs[pos] = gcoef[i];
+        if (p & 0x8000u) atomicOr(&hb[pos >> 5], 1u << (pos & 31u));
+    }
+    __syncthreads();
+
+    // ---- runs, sums since the last head, S4 for the runs that end inside the thread's stretch
+    RunState r;
+    {
+        const uint32_t w0 = hb[first >> 5], w1 = hb[(first >> 5) + 1u];
+        const uint32_t bits = __funnelshift_r(w0, w1, first & 31u);      // bit j: position first + j is a head
+#pragma unroll 2
+        for (uint32_t j = 0; j < itn; ++j)
+            if (first + j < n_loc) run_step(r, ((bits >> j) & 1u) != 0u, scs[first + j], j, first + j, a.tol, scs);
+    }
+    finish_tail<K>(a, r, scs, scratch, first, n_loc, lo, tile, [&](uint32_t, uint32_t q) { return gkeys[rep[q]]; });
 }
 
 // ------------------------------------------------------------------------------- S4/S5 across tiles
@@ -675,7 +1083,8 @@ template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
                            const double* coefs, double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps,
                            int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint4* worklist,
-                           uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
+                           uint4* worklist2, int group, uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device,
+                           cudaEvent_t after_tiles, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
     const int nlow = plan.npasses - prefix_passes;
@@ -689,10 +1098,23 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state; a.worklist = worklist;
     a.pfx_pos = pfx_pos; a.fast_bits = nfast > 0 ? nfast * 8 : 32; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
+    a.list_count = &ctl->fin_count; a.strided = 0; a.worklist2 = worklist2; a.no_group = group == 2 ? 1 : 0;
     // a tile owns records only if a bucket starts in it: at most one tile per bucket, at most 2^T buckets
     const int T = plan.key_bits - pfx_pos;
     const uint32_t fin_blocks = (T < 31 && (1u << T) < ntiles) ? (1u << T) : ntiles;
-    kern<<<fin_blocks, kFinThreads, smem, stream>>>(a, plan);
+    int launches = 5;
+    if (group) {
+        // every tile first through the group kernel; the tiles it hands on (few, or nearly all of them when the input has
+        // no duplicates to group) through the sorting kernel, whose blocks then stride over the second work list
+        auto gkern = finish_group_kernel<K>;
+        ensure_dynamic_smem(gkern, GroupSmem::bytes);
+        gkern<<<fin_blocks, kFinThreads, GroupSmem::bytes, stream>>>(a);
+        FinishArgs b = a;
+        b.worklist = worklist2; b.list_count = &ctl->fin2_count; b.strided = 1;
+        const uint32_t resident = (uint32_t)(sm_count() * kFinBlocksPerSM);
+        kern<<<fin_blocks < resident ? fin_blocks : resident, kFinThreads, smem, stream>>>(b);
+        ++launches;
+    } else kern<<<fin_blocks, kFinThreads, smem, stream>>>(a);
     if (after_tiles) cudaEventRecord(after_tiles, stream);
     const uint32_t nchunks = (ntiles + kScanChunk - 1) / kScanChunk;
     tile_sum_kernel<<<nchunks, 1024, 0, stream>>>(tile_state, ntiles, chunk_sum);
@@ -707,20 +1129,20 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     if (blocks > sm_count() * 64) blocks = sm_count() * 64;
     if (blocks < 1) blocks = 1;
     emit_kernel<K><<<(unsigned)blocks, 256, 0, stream>>>(e, plan);
-    return 5;
+    return launches;
 }
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint32_t* chunk_sum, Control* ctl,
-                  int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
+                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint4* worklist2, int group, uint32_t* chunk_sum,
+                  Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;
     if (plan.key_bytes == 8)
         return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                         exp_bytes, out_capacity, tile_start, tile_state, worklist, chunk_sum, ctl, out_count_device, after_tiles, stream);
+                                         exp_bytes, out_capacity, tile_start, tile_state, worklist, worklist2, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
     return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                   exp_bytes, out_capacity, tile_start, tile_state, worklist, chunk_sum, ctl, out_count_device, after_tiles, stream);
+                                   exp_bytes, out_capacity, tile_start, tile_state, worklist, worklist2, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
 }
 
 }  // namespace polylab

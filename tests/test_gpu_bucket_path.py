@@ -377,3 +377,72 @@ def test_async_call_uses_slack_bins_with_capacities_computed_on_the_device():
     c, e, status, st = _async(q, tol, flags=B.FLAG_SAFE_RANK | B.FLAG_NO_BUCKET)
     assert status == B.OK
     assert_parity(oracle.simplify(q.coef, q.exps, tol), c, e)
+
+
+# ---------------------------------------------------------------------------------- group kernel (finish.cu, round 2)
+
+def _bits(c, e):
+    return c.view(np.uint64).copy(), e.copy()
+
+
+def test_group_finish_is_taken_and_matches_the_sorting_finish_bit_for_bit():
+    """Config 5's structure (ten records per monomial): the tiles are finished by grouping like terms in the shared-memory hash
+    table; the sorting kernel alone (POLYLAB_FLAG_NO_GROUP_FINISH) and the group kernel handing every tile on give the same bits."""
+    p, tol = W.config5(2_000_000)
+    res = oracle.simplify(p.coef, p.exps, tol)
+    c, e, st = run(p, tol)
+    assert st.prefix_passes == 2 and st.bucket_fallback == 0 and st.rank_fallback == 0
+    assert st.grouped_tiles > 0
+    assert_parity(res, c, e)
+    c0, e0, st0 = run(p, tol, flags=B.FLAG_NO_GROUP_FINISH)
+    assert st0.grouped_tiles == 0 and st0.prefix_passes == 2
+    c1, e1, st1 = run(p, tol, flags=B.FLAG_DEBUG_GROUP_HANDS_ON)
+    assert st1.grouped_tiles == 0 and st1.prefix_passes == 2
+    assert st.distinct == st0.distinct == st1.distinct and st.survivors == st0.survivors == st1.survivors
+    for cc, ee in ((c0, e0), (c1, e1)):
+        assert (e == ee).all() and (c.view(np.uint64) == cc.view(np.uint64)).all()
+    c2, e2, st2 = run(p, tol)                               # bit-reproducible run to run
+    assert (c.view(np.uint64) == c2.view(np.uint64)).all() and (e == e2).all()
+
+
+@pytest.mark.parametrize("n,nvars,dup,seed", [(300_000, 9, 10, 1), (300_000, 16, 3, 2), (1_200_000, 8, 4, 3), (1_200_000, 12, 40, 4),
+                                              (150_003, 5, 7, 5), (2_500_000, 16, 1, 6), (600_000, 10, 40, 7)])
+def test_group_finish_shapes(n, nvars, dup, seed):
+    """One- and two-word keys, one bucket per tile and dozens of buckets per tile (the composite word's prefix difference),
+    heavy and no duplication (tiles with more than 768 distinct keys are handed on): oracle parity and the same bits as the
+    sorting kernel."""
+    p = pooled(n, nvars, dup, seed)
+    res = oracle.simplify(p.coef, p.exps, 0.0)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.prefix_passes >= 1 and st.bucket_fallback == 0
+    assert_parity(res, c, e)
+    c0, e0, st0 = run(p, 0.0, flags=FORCE | B.FLAG_NO_GROUP_FINISH)
+    assert st0.grouped_tiles == 0 and st0.prefix_passes == st.prefix_passes
+    assert (e == e0).all() and (c.view(np.uint64) == c0.view(np.uint64)).all()
+    if dup >= 3 and n // dup < 100_000:
+        assert st.grouped_tiles > 0
+
+
+def test_group_finish_cancelling_terms_and_tolerance():
+    """p - p through the group kernel: every run sums to exactly zero and is pruned at tol = 0; with a tolerance the parity rule's
+    exemption band applies as everywhere."""
+    r = np.random.default_rng(21)
+    base = pooled(400_000, 16, 8, seed=22)
+    p = W.Poly(np.concatenate([base.coef, -base.coef]), np.concatenate([base.exps, base.exps]))
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.grouped_tiles > 0
+    res = oracle.simplify(p.coef, p.exps, 0.0)
+    assert_parity(res, c, e)
+    q = W.Poly(r.standard_normal(len(p.coef)), p.exps)
+    c, e, st = run(q, 1e-3, flags=FORCE)
+    assert st.grouped_tiles > 0
+    assert_parity(oracle.simplify(q.coef, q.exps, 1e-3), c, e)
+
+
+def test_group_finish_short_fast_digit_list_hands_tiles_on():
+    """With 8 sort bits below the prefix the group kernel's sort of the distinct keys fails its order check: such tiles go
+    through the sorting kernel, which re-sorts them on every digit."""
+    p, tol = W.config5(300_000)
+    c, e, st = run(p, tol, flags=FORCE | (1 << B.FLAG_DEBUG_NFAST_SHIFT))
+    assert st.refinish_tiles > 0
+    assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
