@@ -556,13 +556,18 @@ def main():
         fin_ms = stage_ms["reduce"]
         fin_bytes = float(N * S + U1 * S)
         achieved = fin_bytes / (fin_ms * 1e-3) / 1e9
-        fin_roof = {"bound": "hbm", "kernel": "finish_kernel (bucket path: shared-memory sort of each bucket + segmented sum + prune)",
+        grouped = getattr(st, "grouped_tiles", 0) > 0
+        fin_name = ("finish_group_kernel (bucket path: like terms of a tile grouped in a shared-memory hash table, distinct keys ordered, "
+                    "one counting pass, segmented sum + prune; %d tiles, the rest through finish_kernel)" % st.grouped_tiles) if grouped else \
+                   "finish_kernel (bucket path: shared-memory sort of each bucket + segmented sum + prune)"
+        fin_roof = {"bound": "hbm", "kernel": fin_name,
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                    "traffic": tinfo.get("finish_dram_bytes_per_launch"), "peak_source": peak_src,
+                    "traffic": tinfo.get("finish_group_dram_bytes_per_launch" if grouped else "finish_dram_bytes_per_launch"), "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": fin_bytes, "launch_ms": fin_ms, "launches_per_step": 1,
                     "share_of_step": fin_ms / ms_per_step,
-                    "limiter": "shared-memory / LSU pipe, not DRAM (ncu, profiles/): the kernel trades HBM passes for on-chip work",
-                    "lsu_pipe": lsu_pipe(tinfo.get("finish_lsu_wavefronts_per_launch"), fin_ms,
+                    "limiter": "on-chip work, not DRAM (ncu, profiles/): the kernel trades HBM passes for shared-memory traffic (LSU data pipe) "
+                               "and barrier-separated phases at 32 warps per SM",
+                    "lsu_pipe": lsu_pipe(tinfo.get("finish_group_lsu_wavefronts_per_launch" if grouped else "finish_lsu_wavefronts_per_launch"), fin_ms,
                                          torch.cuda.get_device_properties(local_rank).multi_processor_count, clocks.get("sm_mhz")),
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
         # the dominant kernel is the one with the larger share of the step: the radix pass (all its launches) or the finish
@@ -679,7 +684,7 @@ def main():
             "config": {"workload": desc, "sort_terms_per_step": n_sort, "distinct": st.distinct, "survivors": int(n_out),
                        "key_bits": st.key_bits, "key_bytes": Wb, "sort_passes": P, "prefix_passes": st.prefix_passes,
                        "bucket_fallback": st.bucket_fallback, "rank_fallback": st.rank_fallback, "bounds_retry": st.bounds_retry,
-                       "refinish_tiles": st.refinish_tiles, "digit_bits": st.digit_bits, "path": path_name(st),
+                       "refinish_tiles": st.refinish_tiles, "grouped_tiles": st.grouped_tiles, "digit_bits": st.digit_bits, "path": path_name(st),
                        "bounds": ("S0 on a 0.3 % sample of the rows, every row verified by S1's range check (DESIGN.md reading B4; "
                                   "reading every row adds 0.47 ms on config 5)") if st.bounds_sampled else "S0 reads every row",
                        "parallelism": f"replicas x{world} (no collective on the path)",

@@ -721,7 +721,6 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
     uint16_t* order = (uint16_t*)(smem_raw + GroupSmem::off_order);          // slots grouped by leading digit
     uint16_t* perm = (uint16_t*)(smem_raw + GroupSmem::off_perm);            // slots in key order
     uint32_t* rows32 = (uint32_t*)(smem_raw + GroupSmem::off_rows);
-    uint16_t* rows16 = (uint16_t*)(smem_raw + GroupSmem::off_rows);
     uint16_t* ids = (uint16_t*)(smem_raw + GroupSmem::off_ids);
     uint32_t* hb = (uint32_t*)(smem_raw + GroupSmem::off_ids);              // head bits by sorted position, once the slots are dead
     uint16_t* rk = (uint16_t*)(smem_raw + GroupSmem::off_rk);
@@ -906,20 +905,18 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
         for (int j = 0; j < NW * kGrpSlots * 2 / 16 / THREADS; ++j) z[tid + j * THREADS] = make_uint4(0u, 0u, 0u, 0u);
     }
     __syncthreads();
+    // Counter of (slot, warp): 16 bits, the eight warps of a slot side by side in one 16-byte group (the bin scan reads a
+    // slot with one load), warps 2p and 2p + 1 sharing word (p + slot / 8) mod 4 of the group -- the rotation spreads one
+    // warp's atomics over all 32 banks.
+    static_assert(NW == 8, "eight 16-bit counters per 16-byte group");
+    const uint32_t wpair = warp >> 1, wsh = (warp & 1u) * 16u;
     {
-        uint32_t* my_row = rows32 + warp * (kGrpSlots / 2);
         for (uint32_t base = wbeg; base < wend; base += 64u) {
             const uint32_t i0 = base + lane, i1 = i0 + 32u;
             const uint32_t d0 = (i0 < wend) ? ids[i0] : 0u, d1 = (i1 < wend) ? ids[i1] : 0u;
-            if (i0 < wend) {
-                const uint32_t sh = (d0 & 1u) * 16u;
-                rk[i0] = (uint16_t)(atomicAdd(&my_row[d0 >> 1], 1u << sh) >> sh);
-            }
+            if (i0 < wend) rk[i0] = (uint16_t)(atomicAdd(&rows32[d0 * 4u + ((wpair + (d0 >> 3)) & 3u)], 1u << wsh) >> wsh);
             __syncwarp();
-            if (i1 < wend) {
-                const uint32_t sh = (d1 & 1u) * 16u;
-                rk[i1] = (uint16_t)(atomicAdd(&my_row[d1 >> 1], 1u << sh) >> sh);
-            }
+            if (i1 < wend) rk[i1] = (uint16_t)(atomicAdd(&rows32[d1 * 4u + ((wpair + (d1 >> 3)) & 3u)], 1u << wsh) >> wsh);
             __syncwarp();
         }
     }
@@ -931,8 +928,13 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
         for (int j = 0; j < kGrpBPT; ++j) {
             const uint32_t q = tid * kGrpBPT + j;
             sl[j] = q < U ? perm[q] : 0u;
-#pragma unroll
-            for (int w = 0; w < NW; ++w) c[j][w] = q < U ? rows16[w * kGrpSlots + sl[j]] : 0u;
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (q < U) v = ((const uint4*)rows32)[sl[j]];
+            const uint32_t rot = (sl[j] >> 3) & 3u;                 // word (p + rot) mod 4 holds pair p
+            if (rot & 1u) v = make_uint4(v.y, v.z, v.w, v.x);
+            if (rot & 2u) v = make_uint4(v.z, v.w, v.x, v.y);
+            c[j][0] = v.x & 0xffffu; c[j][1] = v.x >> 16; c[j][2] = v.y & 0xffffu; c[j][3] = v.y >> 16;
+            c[j][4] = v.z & 0xffffu; c[j][5] = v.z >> 16; c[j][6] = v.w & 0xffffu; c[j][7] = v.w >> 16;
         }
 #pragma unroll
         for (int j = 0; j < kGrpBPT; ++j)
@@ -947,13 +949,19 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
                 // bit 15: this warp holds the key's first record (its rank-0 record is the head of the run)
                 const uint32_t end = (j + 1 < kGrpBPT) ? c[j + 1][0] : count;
                 bool seen = false;
+                uint32_t h[NW];
 #pragma unroll
                 for (int w = 0; w < NW; ++w) {
                     const uint32_t nxt = (w + 1 < NW) ? c[j][w + 1] : end;
                     const bool has = nxt != c[j][w];
-                    rows16[w * kGrpSlots + sl[j]] = (uint16_t)((bin_start + c[j][w]) | ((has && !seen) ? 0x8000u : 0u));
+                    h[w] = (bin_start + c[j][w]) | ((has && !seen) ? 0x8000u : 0u);
                     seen |= has;
                 }
+                uint4 v = make_uint4(h[0] | (h[1] << 16), h[2] | (h[3] << 16), h[4] | (h[5] << 16), h[6] | (h[7] << 16));
+                const uint32_t rot = (sl[j] >> 3) & 3u;             // back into the rotated order
+                if (rot & 1u) v = make_uint4(v.w, v.x, v.y, v.z);
+                if (rot & 2u) v = make_uint4(v.z, v.w, v.x, v.y);
+                ((uint4*)rows32)[sl[j]] = v;
             }
         }
     }
@@ -961,7 +969,8 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
     // sorted position of every record (over its rank), bit 15 = head of its run
 #pragma unroll 4
     for (uint32_t i = wbeg + lane; i < wend; i += 32u) {
-        const uint32_t h = rows16[warp * kGrpSlots + ids[i]], r = rk[i];
+        const uint32_t d = ids[i], r = rk[i];
+        const uint32_t h = (rows32[d * 4u + ((wpair + (d >> 3)) & 3u)] >> wsh) & 0xffffu;
         rk[i] = (uint16_t)(((h & 0x1fffu) + r) | ((r == 0u) ? (h & 0x8000u) : 0u));
     }
     // the head bits take the place of the first 320 slot ids: when those all belong to warp 0's chunk, warp 0 clears them as
