@@ -446,3 +446,53 @@ def test_group_finish_short_fast_digit_list_hands_tiles_on():
     c, e, st = run(p, tol, flags=FORCE | (1 << B.FLAG_DEBUG_NFAST_SHIFT))
     assert st.refinish_tiles > 0
     assert_parity(oracle.simplify(p.coef, p.exps, tol), c, e)
+
+
+def test_group_finish_crowded_leading_digit_hands_tiles_on():
+    """Variables 1..3 take one value each, so every key of a bucket shares the ten bits below the prefix and all of a tile's
+    distinct keys fall into one leading-digit bin: more than 16 of them, the group kernel hands the tile on and the sorting
+    kernel finishes it.  Same answer, no grouped tile."""
+    r = np.random.default_rng(31)
+    n, dup = 400_000, 8
+    pool = r.integers(0, 256, size=(n // dup, 9)).astype(np.uint8)
+    pool[:, 1] = 255                                          # full-width fields (the layout is sized from the maxima) ...
+    pool[:, 2] = 255
+    pool[:, 3] = 255                                          # ... that never vary: 24 constant bits right below the first digit
+    exps = np.ascontiguousarray(pool[r.permutation(n) // dup])
+    p = W.Poly(r.standard_normal(n), exps)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.prefix_passes == 1 and st.bucket_fallback == 0 and st.grouped_tiles == 0
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
+    c0, e0, _ = run(p, 0.0, flags=FORCE | B.FLAG_NO_GROUP_FINISH)
+    assert (e == e0).all() and (c.view(np.uint64) == c0.view(np.uint64)).all()
+
+
+def test_group_finish_mixed_tiles():
+    """Half of the buckets hold few distinct monomials (grouped), the other half only distinct ones (more than 768 per tile:
+    handed on, but never so many that the give-up rule fires): both kernels contribute to one output."""
+    r = np.random.default_rng(32)
+    nd, nu = 600_000, 600_000
+    pd = r.integers(0, 256, size=(nd // 20, 8)).astype(np.uint8)
+    pd[:, 0] &= 0x7f                                          # duplicated monomials under the low half of the first digit
+    ed = pd[r.permutation(nd) // 20]
+    eu = r.integers(0, 256, size=(nu, 8)).astype(np.uint8)
+    eu[:, 0] |= 0x80                                          # distinct ones under the high half
+    exps = np.ascontiguousarray(np.concatenate([ed, eu])[r.permutation(nd + nu)])
+    p = W.Poly(r.standard_normal(nd + nu), exps)
+    c, e, st = run(p, 0.0, flags=FORCE)
+    assert st.prefix_passes >= 1 and st.bucket_fallback == 0
+    assert 0 < st.grouped_tiles
+    res = oracle.simplify(p.coef, p.exps, 0.0)
+    assert_parity(res, c, e)
+    c0, e0, st0 = run(p, 0.0, flags=FORCE | B.FLAG_NO_GROUP_FINISH)
+    assert st0.grouped_tiles == 0 and (e == e0).all() and (c.view(np.uint64) == c0.view(np.uint64)).all()
+
+
+def test_group_finish_without_like_terms_gives_up_and_matches():
+    """2.4e6 distinct monomials: every tile holds more than 768 distinct keys; after the first tiles the group kernel stops
+    trying (the give-up rule), the sorting kernel finishes everything."""
+    p = pooled(2_400_000, 8, 1, seed=33)
+    c, e, st = run(p, 0.0)
+    assert st.prefix_passes == 2 and st.bucket_fallback == 0 and st.grouped_tiles == 0
+    assert len(c) == st.distinct
+    assert_parity(oracle.simplify(p.coef, p.exps, 0.0), c, e)
