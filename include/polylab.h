@@ -115,12 +115,13 @@ enum {
                                         (stats->hist_sampled = 1); an overrun re-runs the call with the sweep
                                         (stats->hist_retry = 1).  Same result, bit for bit.  A POLYLAB_FLAG_DEVICE_COUNT call
                                         with a status word sizes the bins on the device; an overrun is POLYLAB_ERR_RETRY there. */
-    POLYLAB_FLAG_NO_GROUP_FINISH = 512u, /* bucket path: finish every tile with the sorting kernel.  By default a tile first tries to GROUP
-                                        its records: like terms are found through a shared-memory hash table (full keys compared), only
-                                        the tile's distinct monomials are sorted, and one stable counting pass puts the records in
-                                        order (stats->grouped_tiles); a tile with more than 768 distinct monomials, a fingerprint
-                                        collision or an overlong probe sequence goes through the sorting kernel instead, and once most
-                                        tiles do, the rest no longer try.  Same result, bit for bit. */
+    POLYLAB_FLAG_NO_GROUP_FINISH = 512u, /* bucket path: finish every tile with the sorting kernel.  By default a tile with enough records first
+                                        tries to GROUP them: like terms are found through a shared-memory hash table (full keys
+                                        compared), only the tile's distinct monomials are put in order, and one stable counting pass
+                                        puts the records in order (stats->grouped_tiles).  A tile whose records-per-monomial ratio
+                                        is too low for that to pay (about 6 at 3000 records), or with more than 768 distinct
+                                        monomials, a fingerprint collision or an overlong probe sequence, is finished by the sorting
+                                        kernel instead, and once most tiles are, the rest no longer try.  Same result, bit for bit. */
     POLYLAB_FLAG_NO_TABLE = 64u,      /* never take the table path.  By default a call with 2^15 <= N <= 2^26 terms whose key fits 63 bits
                                         first merges like terms in a table (the packed key itself as the index when 2^B slots
                                         are affordable, else a hash table) with order-independent fixed-point accumulators,
@@ -138,7 +139,7 @@ enum {
     POLYLAB_FLAG_DEBUG_FORCE_BUCKET = 0x20000000u, /* test hook: take the bucket path whenever it is defined (any size, no
                                         skew pre-check), so that small tests reach it and its overflow fallback */
     POLYLAB_FLAG_DEBUG_GROUP_HANDS_ON = 0x04000000u, /* test hook: the bucket path's group kernel runs and hands every tile on to the
-                                        sorting kernel (the second work list in full) */
+                                        sorting kernel */
     POLYLAB_FLAG_DEBUG_UNSTABLE = 0x40000000u  /* test hook: makes the atomic-ranking kernel unstable on purpose
                                         (reversed lane order) so that tests can exercise detection and fallback */
 };

@@ -151,7 +151,7 @@ static int make_plan(int nvars, const uint64_t* m, const uint32_t* bound, Plan* 
 // ------------------------------------------------------------------------------ workspace carving
 
 struct Layout {
-    size_t control, sort_state, slack_tiles, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_wl2, fin_chunks, zero_end;
+    size_t control, sort_state, slack_tiles, red_state, red_heads, red_hb, red_frag, red_cont, prune_state, fin_state, fin_start, fin_wl, fin_chunks, zero_end;
     size_t tab_state, tab, tab_bytes;
     size_t keys[2], coefs[2], ka, kb, ca, cb, total;      // ca, cb: fp32 operand coefficients of a product, widened to fp64
 };
@@ -213,7 +213,6 @@ static Layout make_layout(int64_t n, int key_bytes, int64_t na, int64_t nb)
     L.slack_tiles = take((sort_tiles + kSlackExtraTiles) * sizeof(uint2));     // (written in full by slack_tiles_kernel)
     L.fin_start = take((fin_tiles + 1) * sizeof(uint32_t));
     L.fin_wl = take((fin_tiles + 1) * sizeof(uint4));
-    L.fin_wl2 = take((fin_tiles + 1) * sizeof(uint4));
     L.fin_chunks = take((fin_tiles / 4096 + 2) * sizeof(uint32_t));
     L.red_heads = take(red_tiles * sizeof(uint32_t));
     L.red_hb = take(red_tiles * sizeof(uint32_t));
@@ -403,7 +402,7 @@ static int bucket_sort_emit(const Plan& plan, int k, int64_t n, unsigned char* w
     tm.mark(POLYLAB_STAGE_SORT);
     *launches += launch_finish(plan, k, fast_digits(o), kFinCap - bucket_room(plan, k, n), n, kbuf[k & 1], cbuf[k & 1], tol,
                                kbuf[(k + 1) & 1], cbuf[(k + 1) & 1], out_coef, out_exps, o.exp_bytes, out_capacity,
-                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl), (uint4*)(ws + L.fin_wl2),
+                               (uint32_t*)(ws + L.fin_start), (uint32_t*)(ws + L.fin_state), (uint4*)(ws + L.fin_wl),
                                finish_group_mode(o), (uint32_t*)(ws + L.fin_chunks), ctl,
                                (o.flags & POLYLAB_FLAG_DEVICE_COUNT) ? out_nterms : nullptr,
                                tm.on ? tm.ev[POLYLAB_STAGE_REDUCE + 1] : nullptr, stream);      // REDUCE = tiles, PRUNE = scan + emit

@@ -294,7 +294,11 @@ struct Control {
     uint32_t tab_count;                      // table path: distinct keys inserted so far (= U after the insert pass)
     uint32_t tab_overflow;                   // table path: more distinct keys than the table was sized for -> sort path
     uint32_t slack_overflow;                 // slack bins (sort.cu): a bin's capacity, estimated from a sample, was too small
-    uint32_t fin2_count;                     // bucket path: tiles the group kernel handed on to the sorting finish kernel (second work list)
+    uint32_t fin2_count;                     // bucket path: tiles the sorting finish kernel did behind the group kernel (one add per block)
+    uint32_t grp_fail;                       // bucket path: tiles the group kernel tried and gave back
+    uint32_t grp_off;                        // bucket path: sticky, set once most tiles were given back: the group kernel stops trying
+    uint32_t grp_left;                       // bucket path: tiles the group kernel did not finish (one add per block)
+    uint32_t fin_ticket;                     // bucket path: next work-list entry the sorting kernel behind the group kernel hands out
     uint32_t slack_count[kRadix];            // exact bin counts of the pass that wrote with slack
     uint32_t slack_cap[kRadix];              // the capacities (kept for the reading pass)
     uint32_t est[kRadix];                    // histogram of the first prefix digit over a SAMPLE of the rows

@@ -243,10 +243,10 @@ struct FinishArgs {
     uint32_t n, ntiles;
     uint32_t fin_tile;              // positions per tile; a tile owns at most kFinCap records
     const uint32_t* tile_start;     // [ntiles + 1]
-    const uint4* worklist;          // the *list_count tiles that own records: (tile, first record, end, first and last share the prefix)
-    const uint32_t* list_count;     // DEVICE: length of the work list (ctl->fin_count, or ctl->fin2_count behind the group kernel)
-    int strided;                    // the grid is smaller than the list may be: blocks walk it with stride gridDim.x
-    uint4* worklist2;               // group kernel: the tiles it hands on to finish_kernel (ctl->fin2_count of them)
+    uint4* worklist;                // the ctl->fin_count tiles that own records: (tile, first record, end, flags); flag bit 0: first and
+                                    // last record share the prefix; bit 1: set by the group kernel when it has finished the tile
+    uint32_t max_list;              // group kernel: most tiles that can own records (one per bucket)
+    int behind_group;               // finish_kernel: the group kernel ran first -- a smaller grid walks the list in chunks and skips the done tiles
     int no_group;                   // group kernel, test hook: hand every tile on
     uint32_t* tile_state;           // [ntiles + 1] survivors per tile, zero before the kernel
     int pfx_pos;                    // the prefix is the key bits at positions >= pfx_pos
@@ -624,16 +624,49 @@ template <typename K>
 __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(const __grid_constant__ FinishArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t todo[kFinThreads], ntodo;
     if (a.ctl->overflow) return;                   // set by tile_bounds_kernel: the call will re-run on the LSD path
-    const uint32_t count = *a.list_count;
-    // one block per tile, the grid sized for the most tiles that can own records (at most one per bucket): more of them
-    // than that and the array is not sorted by prefix.  Behind the group kernel the list is usually short and the blocks stride.
-    if (!a.strided && blockIdx.x == 0 && threadIdx.x == 0 && count > gridDim.x) a.ctl->unsorted = 1u;
-    for (uint32_t b = blockIdx.x; b < count; b += gridDim.x) {
-        finish_tile<K>(a, smem_raw, a.worklist[b]);            // one load instead of three dependent ones
-        if (!a.strided) break;
-        __syncthreads();
+    const uint32_t count = a.ctl->fin_count;
+    if (!a.behind_group) {
+        // one block per tile, the grid sized for the most tiles that can own records (at most one per bucket): more of them
+        // than that and the array is not sorted by prefix
+        if (blockIdx.x == 0 && threadIdx.x == 0 && count > gridDim.x) a.ctl->unsorted = 1u;
+        if (blockIdx.x < count) finish_tile<K>(a, smem_raw, a.worklist[blockIdx.x]);       // one load instead of three dependent ones
+        return;
     }
+    // Behind the group kernel: the blocks take runs of list entries by ticket, long runs first and shorter ones as the list
+    // runs out (a run is 1/(2 gridDim.x) of what is left: a few thousand tickets in all, and the blocks finish together --
+    // equal shares per block measured 8 % slower on a list that is all work, the sum of 111 tile times varies that much),
+    // look at a run's descriptors with one load and finish the tiles the group kernel left: none at all on an input full of
+    // like terms, all of them on one without.  No list of its own and no atomic per tile: 65,536 adds to one address cost
+    // the group kernel 0.4-0.7 ms when they were tried.
+    if (a.ctl->grp_left == 0u) return;             // the group kernel finished every tile
+    uint32_t done = 0;
+    __shared__ uint32_t run_lo, run_hi;
+    while (true) {
+        if (threadIdx.x == 0) {
+            const uint32_t seen = *(volatile const uint32_t*)&a.ctl->fin_ticket;
+            const uint32_t left = seen < count ? count - seen : 0u;
+            const uint32_t len = min(max(left / (2u * gridDim.x), 1u), (uint32_t)kFinThreads);
+            run_lo = atomicAdd(&a.ctl->fin_ticket, len);
+            run_hi = run_lo + len;
+            ntodo = 0u;
+        }
+        __syncthreads();
+        const uint32_t r0 = run_lo, r1 = min(run_hi, count);
+        if (r0 >= count) break;
+        const uint32_t q = r0 + threadIdx.x;
+        if (q < r1 && !(a.worklist[q].w & 2u)) todo[atomicAdd(&ntodo, 1u)] = q;     // (any order: tiles are independent)
+        __syncthreads();
+        const uint32_t n = ntodo;
+        for (uint32_t j = 0; j < n; ++j) {
+            finish_tile<K>(a, smem_raw, a.worklist[todo[j]]);
+            __syncthreads();
+        }
+        done += n;
+        __syncthreads();                           // (everybody has read the run and the count before thread 0 takes the next)
+    }
+    if (threadIdx.x == 0 && done) atomicAdd(&a.ctl->fin2_count, done);
 }
 
 // ------------------------------------------------------------------------------------- group kernel
@@ -644,8 +677,8 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_kernel(co
 //   G1  streams the keys once and looks each up in a shared-memory hash table (256 buckets of four slots, a 31-bit
 //       fingerprint per slot: one 16-byte load shows a bucket; atomicCAS on the bucket's first empty slot, the winner parks
 //       the full key and its record number); after a barrier every record compares its FULL key with the slot's -- a
-//       fingerprint collision, an overlong probe sequence or more than 768 distinct keys hand the tile on to finish_kernel
-//       through a second work list;
+//       fingerprint collision, an overlong probe sequence, more than 768 distinct keys, or more keys than grouping pays for
+//       (group_pays) give the tile back: it stays unmarked in the work list and finish_kernel behind finishes it;
 //   G2  puts the U distinct keys (not the records) in order: a 10-bit leading digit (prefix difference above the top key
 //       bits below the prefix) bins them, and inside a bin -- one or two keys as a rule, more than 16 hand the tile on -- a
 //       key's place is the number of smaller keys, full keys compared: exact, no order check needed;
@@ -660,6 +693,7 @@ constexpr int kGrpMaxProbe = 48;
 constexpr int kGrpBPT = kGrpMaxDistinct / kFinThreads;      // slots per thread in the bin scan
 constexpr int kGrpDigit = 10;           // bits of the distinct keys' leading digit
 constexpr int kGrpMaxBin = 16;          // most distinct keys that may share a leading digit
+constexpr int kGrpTilesPerBlock = 1;    // consecutive work-list entries a block finishes, one after the other
 
 struct GroupSmem {
     static constexpr int NW = kFinThreads / 32;
@@ -684,6 +718,9 @@ static_assert((size_t)GroupSmem::NW * kGrpSlots * 2 <= (size_t)kGrpSlots * 16, "
 static_assert(kGrpSlots <= kFinCap && kGrpBPT * kFinThreads == kGrpMaxDistinct && kGrpMaxDistinct <= kGrpSlots, "group path sizes");
 static_assert((1 << kGrpDigit) == kGrpSlots && kGrpSlots % kFinThreads == 0, "one bin per slot index, whole slots per thread");
 static_assert((GroupSmem::bytes + 96 + 1024) * kFinBlocksPerSM <= 228 * 1024, "four blocks per SM");
+
+// does grouping a tile of n records with (at least) u distinct keys cost less than sorting it?  (finish_group_kernel, set-up)
+__device__ __forceinline__ bool group_pays(uint32_t n, uint32_t u) { return 10u * n > 8400u + 52u * u; }
 
 // bucket and fingerprint of a key: x = a multiply-add mix of the key's 32-bit words; the bucket is x's top byte and the
 // fingerprint a bijection of x (two keys of one bucket share a fingerprint only if they share x, or differ in the forced bit)
@@ -730,13 +767,22 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
     double* scs = (double*)smem_raw;
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    // (persistent blocks that take tiles by ticket and pull the NEXT tile's descriptor and records into L2 while one is worked
-    // on were measured: 3.00 against 2.95 ms on config 5 -- the hardware's block scheduler already overlaps the start-up loads)
+    // A block takes kGrpTilesPerBlock consecutive entries of the work list, one after the other: still thousands of blocks for
+    // the block scheduler to balance, but a call whose tiles are not worth grouping (grp_off, below) pays an eighth of the
+    // block starts -- 65,536 blocks that only look at a flag and leave cost 0.2 ms.  (Persistent blocks that take tiles by ticket
+    // and pull the NEXT tile's descriptor and records into L2 were measured too: 3.00 against 2.95 ms on config 5.)
     const uint32_t overflow = a.ctl->overflow, fin_count = a.ctl->fin_count;
+    uint32_t off = a.ctl->grp_off;
+    const uint32_t b0 = blockIdx.x * (uint32_t)kGrpTilesPerBlock;
+    uint4* wls = (uint4*)(scratch + 16);           // the block's descriptors, one coalesced load
+    if (tid < (unsigned)kGrpTilesPerBlock && b0 + tid < fin_count) wls[tid] = a.worklist[b0 + tid];
     if (overflow) return;                          // set by tile_bounds_kernel: the call will re-run on the LSD path
-    if (blockIdx.x == 0 && tid == 0 && fin_count > gridDim.x) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
-    if (blockIdx.x >= fin_count) return;
-    const uint4 wl = a.worklist[blockIdx.x];
+    if (blockIdx.x == 0 && tid == 0 && fin_count > a.max_list) a.ctl->unsorted = 1u;   // more bucket starts than buckets: not sorted by prefix
+    __syncthreads();
+    const uint32_t b_end = min(b0 + (uint32_t)kGrpTilesPerBlock, fin_count);
+    uint32_t left_here = 0;                        // tiles this block leaves to the sorting kernel (thread 0 reports them)
+    for (uint32_t b = b0; b < b_end; ++b) {
+    const uint4 wl = wls[b - b0];
     const uint32_t tile = wl.x, lo = wl.y, hi = wl.z;
     const uint32_t n_loc = hi > lo ? min(hi - lo, (uint32_t)CAP) : 0u;
     const K* __restrict__ gkeys = (const K*)a.keys + lo;
@@ -744,22 +790,26 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
     const uint32_t itn = ((n_loc + THREADS - 1) / THREADS) | 1u;
     const uint32_t first = tid * itn;
 
-    // Is grouping worth trying?  Not when most tiles so far were handed on (an input without duplicates): blocks start in
-    // order, so blockIdx.x is about the number of tiles begun.
-    bool hand_on = a.no_group != 0 || n_loc < 64u;
-    if (tid == 0 && !hand_on) {
-        const uint32_t f = *(volatile const uint32_t*)&a.ctl->fin2_count;
-        hand_on = f >= 64u && 2u * f > blockIdx.x;
-    }
-    hand_on = __syncthreads_or(hand_on ? 1 : 0) != 0;
+    // Is grouping worth trying?  Measured on B200 (profiles/r2b_state.md; pooled 128-bit keys, tiles of 1526 and 3052 records,
+    // 2 to 20 records per key; ms per 65,536 tiles): this kernel costs about 1.07 + 0.26 n/1000 + 3.3 U/1000 for a tile of n
+    // records with U distinct keys, the sorting kernel about 0.65 + 0.81 n/1000 + 0.72 U/1000, so grouping pays when
+    // n > 764 + 4.7 U (group_pays asks for 10 % more): never below about 840 records, and as U is known only from the look-ups,
+    // every batch of 1024 records checks the keys met so far.  And not once most tiles so far were given back (an input
+    // with few like terms): grp_off is sticky, the sorting kernel behind finds the tiles unmarked.
+    // (the barrier: a block must not split over a flag that flips between its warps' loads)
+    if (b > b0 && tid == 0) off = *(volatile const uint32_t*)&a.ctl->grp_off;
+    const int leave = __syncthreads_or((a.no_group != 0 || off != 0u) ? 1 : 0);
+    if (leave) { left_here += b_end - b; break; }
+    if (!group_pays(n_loc, 0u)) ++left_here;
+    else {
     bool bad = false;
     uint32_t U = 0;
-    if (!hand_on) {
+    {
         for (uint32_t i = tid * 8u; i < n_loc; i += THREADS * 8u) asm volatile("prefetch.global.L2 [%0];" ::"l"(gkeys + i));
         for (uint32_t i = tid * 16u; i < n_loc; i += THREADS * 16u) asm volatile("prefetch.global.L2 [%0];" ::"l"(gcoef + i));
 #pragma unroll
         for (int j = 0; j < SPT; ++j) { tags[tid + j * THREADS] = 0u; bins[tid + j * THREADS] = 0u; }
-        if (tid == 0) scratch[48] = 0u;
+        if (tid < 8u) scratch[48 + tid] = 0u;      // [48] largest prefix difference, [51..55] keys met per batch
         __syncthreads();
 
         // ---- G1: every record finds or claims the slot of its key.  The table is 256 buckets of four tags: one 16-byte
@@ -767,10 +817,11 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
         // records of one key cannot claim two slots).
         const K k0 = gkeys[0];
         const bool single = wl.w != 0u;            // first and last record share the prefix: one bucket if the array is sorted
-        bool descending = false;
+        bool descending = false, early = false;
+        uint32_t met = 0;
         for (uint32_t base = 0; base < n_loc; base += 4 * THREADS) {
             K k[4];
-            uint32_t sl[4];
+            uint32_t sl[4], nwon = 0;
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const uint32_t i = base + u * THREADS + tid;
@@ -802,7 +853,7 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
                         if (j >= 0) {
                             s = 4u * b + (uint32_t)j;
                             const uint32_t old = atomicCAS(&tags[s], 0u, fp);
-                            if (old == 0u) { tkeys[s] = k[u]; own[s] = (uint16_t)i; break; }
+                            if (old == 0u) { tkeys[s] = k[u]; own[s] = (uint16_t)i; ++nwon; break; }
                             if (old == fp) break;
                         } else b = (b + 1u) & (uint32_t)(kGrpSlots / 4 - 1);       // (a lost race looks at the same bucket again)
                         if (tries >= kGrpMaxProbe) { bad = true; break; }
@@ -811,14 +862,19 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
                     ids[i] = (uint16_t)s;
                 }
             }
+            if (nwon) atomicAdd(&scratch[51 + base / (4 * THREADS)], nwon);      // (a word per batch: final once the barrier is passed)
             __syncthreads();                       // the keys of every slot claimed so far are in place
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const uint32_t i = base + u * THREADS + tid;
                 if (i < n_loc) bad |= !key_eq(tkeys[sl[u]], k[u]);
             }
+            // distinct keys met so far: too many for grouping to pay?  (the same answer in every thread)
+            met += scratch[51 + base / (4 * THREADS)];
+            if (!group_pays(n_loc, met)) { early = true; break; }
         }
         if (descending) a.ctl->unsorted = 1u;      // the prefix passes were not stable (see sort.cu)
+        bad |= early;
 
         // ---- G2: the distinct keys in order.  Leading digit = prefix difference above the top key bits below the prefix,
         // ten bits in all: a key's place is the start of its digit's bin plus the number of smaller keys in that bin (full
@@ -890,10 +946,15 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
             }
         }
     }
-    if (hand_on || bad) {
-        if (tid == 0) a.worklist2[atomicAdd(&a.ctl->fin2_count, 1u)] = wl;
-        return;
-    }
+    if (bad) {
+        // given back: the sorting kernel behind takes the tile.  Once at least 64 tiles and more than half of the tiles begun
+        // (blocks start in order) came back -- an input with few like terms -- the rest no longer try.
+        ++left_here;
+        if (tid == 0) {
+            const uint32_t f = atomicAdd(&a.ctl->grp_fail, 1u) + 1u;
+            if (f >= 64u && 2u * f > b) a.ctl->grp_off = 1u;
+        }
+    } else {
 
     // ---- G3: one stable counting pass of the records on their slot; warp w owns the contiguous chunk [w*per, (w+1)*per)
     // and row w (see local_pass); the bins are scanned in KEY order
@@ -1006,6 +1067,12 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
             if (first + j < n_loc) run_step(r, ((bits >> j) & 1u) != 0u, scs[first + j], j, first + j, a.tol, scs);
     }
     finish_tail<K>(a, r, scs, scratch, first, n_loc, lo, tile, [&](uint32_t, uint32_t q) { return gkeys[rep[q]]; });
+    if (tid == 0) a.worklist[b].w = wl.w | 2u;                 // done: the sorting kernel behind skips the tile
+    }
+    }
+    __syncthreads();                               // the tail read what the next tile overwrites
+    }
+    if (tid == 0 && left_here) atomicAdd(&a.ctl->grp_left, left_here);
 }
 
 // ------------------------------------------------------------------------------- S4/S5 across tiles
@@ -1092,7 +1159,7 @@ template <typename K>
 static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys,
                            const double* coefs, double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps,
                            int exp_bytes, int64_t out_capacity, uint32_t* tile_start, uint32_t* tile_state, uint4* worklist,
-                           uint4* worklist2, int group, uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device,
+                           int group, uint32_t* chunk_sum, Control* ctl, int64_t* out_count_device,
                            cudaEvent_t after_tiles, cudaStream_t stream)
 {
     const uint32_t ntiles = (uint32_t)((n + fin_tile - 1) / fin_tile);
@@ -1107,19 +1174,20 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
     a.keys = keys; a.coefs = coefs; a.n = (uint32_t)n; a.ntiles = ntiles; a.fin_tile = (uint32_t)fin_tile;
     a.tile_start = tile_start; a.tile_state = tile_state; a.worklist = worklist;
     a.pfx_pos = pfx_pos; a.fast_bits = nfast > 0 ? nfast * 8 : 32; a.tol = tol; a.ukeys = ukeys; a.usums = usums; a.ctl = ctl;
-    a.list_count = &ctl->fin_count; a.strided = 0; a.worklist2 = worklist2; a.no_group = group == 2 ? 1 : 0;
+    a.behind_group = 0; a.max_list = 0; a.no_group = group == 2 ? 1 : 0;
     // a tile owns records only if a bucket starts in it: at most one tile per bucket, at most 2^T buckets
     const int T = plan.key_bits - pfx_pos;
     const uint32_t fin_blocks = (T < 31 && (1u << T) < ntiles) ? (1u << T) : ntiles;
     int launches = 5;
     if (group) {
-        // every tile first through the group kernel; the tiles it hands on (few, or nearly all of them when the input has
-        // no duplicates to group) through the sorting kernel, whose blocks then stride over the second work list
+        // every tile first through the group kernel; the tiles it leaves unmarked (few, or nearly all of them when the input
+        // has too few like terms) through the sorting kernel, whose blocks then take runs of the list by ticket
         auto gkern = finish_group_kernel<K>;
         ensure_dynamic_smem(gkern, GroupSmem::bytes);
-        gkern<<<fin_blocks, kFinThreads, GroupSmem::bytes, stream>>>(a);
+        a.max_list = fin_blocks;
+        gkern<<<(fin_blocks + kGrpTilesPerBlock - 1) / kGrpTilesPerBlock, kFinThreads, GroupSmem::bytes, stream>>>(a);
         FinishArgs b = a;
-        b.worklist = worklist2; b.list_count = &ctl->fin2_count; b.strided = 1;
+        b.behind_group = 1;
         const uint32_t resident = (uint32_t)(sm_count() * kFinBlocksPerSM);
         kern<<<fin_blocks < resident ? fin_blocks : resident, kFinThreads, smem, stream>>>(b);
         ++launches;
@@ -1143,15 +1211,15 @@ static int launch_finish_t(const Plan& plan, int prefix_passes, int nfast, int f
 
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint4* worklist2, int group, uint32_t* chunk_sum,
+                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, int group, uint32_t* chunk_sum,
                   Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream)
 {
     if (n <= 0 || prefix_passes < 1 || prefix_passes > plan.npasses || fin_tile < kFinMinTile || fin_tile >= kFinCap) return 0;
     if (plan.key_bytes == 8)
         return launch_finish_t<uint64_t>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                         exp_bytes, out_capacity, tile_start, tile_state, worklist, worklist2, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
+                                         exp_bytes, out_capacity, tile_start, tile_state, worklist, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
     return launch_finish_t<Key128>(plan, prefix_passes, nfast, fin_tile, n, keys, coefs, tol, ukeys, usums, out_coef, out_exps,
-                                   exp_bytes, out_capacity, tile_start, tile_state, worklist, worklist2, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
+                                   exp_bytes, out_capacity, tile_start, tile_state, worklist, group, chunk_sum, ctl, out_count_device, after_tiles, stream);
 }
 
 }  // namespace polylab

@@ -179,11 +179,11 @@ int launch_async_status(const Control* ctl, int32_t* status_device, int64_t* out
 // between the finish kernel and the scan/emit kernels, for the stage timing.  Sets ctl->overflow (nothing emitted) when a bucket is too long,
 // ctl->unsorted when the prefix order or the local order check fails, ctl->distinct, ctl->survivors.
 // group: 1 = every tile goes through finish_group_kernel first (like terms grouped in a shared-memory hash table, only the
-// distinct keys sorted) and the tiles it hands on -- ctl->fin2_count of them, listed in worklist2 (as long as worklist) --
-// through the sorting finish_kernel; 2 = test hook, the group kernel hands every tile on; 0 = sorting kernel only.
+// distinct keys sorted), which marks the tiles it finished in the work list; the sorting finish_kernel behind it does the
+// rest (ctl->fin2_count of them); 2 = test hook, the group kernel leaves every tile; 0 = sorting kernel only.
 int launch_finish(const Plan& plan, int prefix_passes, int nfast, int fin_tile, int64_t n, const void* keys, const double* coefs,
                   double tol, void* ukeys, double* usums, CoefOut out_coef, void* out_exps, int exp_bytes, int64_t out_capacity,
-                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, uint4* worklist2, int group, uint32_t* chunk_sum,
+                  uint32_t* tile_start, uint32_t* tile_state, uint4* worklist, int group, uint32_t* chunk_sum,
                   Control* ctl, int64_t* out_count_device, cudaEvent_t after_tiles, cudaStream_t stream);
 
 // Small inputs (small.cu): S2 + S3 of at most small_cap() (key, coef) pairs in ONE thread block -- radix sort of a permutation
