@@ -58,6 +58,27 @@ def test_struct_layouts_match(L, tmp_path):
     assert sizes == [ctypes.sizeof(binding._Opts), ctypes.sizeof(binding._Stats), ctypes.sizeof(binding._Poly)]
 
 
+def test_flag_values_match_the_header(tmp_path):
+    """binding.py's FLAG_* constants are the header's POLYLAB_FLAG_* (the fast-digits test hook once shared bit 8 with
+    POLYLAB_FLAG_EXACT_HIST: every flag owns its bits)."""
+    from paper_2604_06575_b200 import binding
+    names = ["DEVICE_COUNT", "TIMING", "SAFE_RANK", "NO_BUCKET", "NO_FUSED_PACK", "EXACT_BOUNDS", "NO_TABLE", "NO_SMALL", "EXACT_HIST",
+             "NO_GROUP_FINISH", "DEBUG_FORCE_TABLE", "DEBUG_FORCE_HASH", "DEBUG_FORCE_BUCKET", "DEBUG_UNSTABLE", "DEBUG_GROUP_HANDS_ON"]
+    src = tmp_path / "f.c"
+    body = "".join('printf("%%u\\n", (unsigned)POLYLAB_FLAG_%s);' % n for n in names)
+    src.write_text('#include <stdio.h>\n#include "polylab.h"\nint main(void){%s printf("%%d\\n", POLYLAB_FLAG_DEBUG_NFAST_SHIFT); return 0;}\n' % body)
+    import subprocess
+    exe = tmp_path / "f"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    vals = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
+    assert vals[:-1] == [getattr(binding, "FLAG_" + n) for n in names]
+    assert vals[-1] == binding.FLAG_DEBUG_NFAST_SHIFT
+    used = 0
+    for v in vals[:-1] + [0xf << vals[-1]]:
+        assert used & v == 0, "two flags share a bit"
+        used |= v
+
+
 def test_version_and_status_strings(L):
     assert L.polylab_version() == 110
     seen = {L.polylab_status_string(i).decode() for i in range(9)}
