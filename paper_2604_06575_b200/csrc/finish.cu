@@ -1146,9 +1146,25 @@ __global__ void __launch_bounds__(256) emit_kernel(const __grid_constant__ EmitA
         const uint32_t t = wl.x;
         const uint32_t off = a.tile_off[t], cnt = a.tile_off[t + 1] - off;
         const uint64_t src = wl.y;
-        for (uint32_t i = lane; i < cnt; i += 32u) {
-            const uint64_t o = (uint64_t)off + i;
-            if ((int64_t)o < a.out_capacity) emit_term<K>(a, plan, o, a.usums[src + i], ((const K*)a.ukeys)[src + i]);
+        // four terms per lane in flight (all loads of a round first; a tile seldom holds more than a few hundred survivors):
+        // 0.191 -> 0.163 ms on config 5, 1.67 -> 1.39 ms on 1e8 unpruned terms.  Eight tiles per block with all their
+        // survivors spread evenly over the block's threads measured 0.173 / 1.42.
+        for (uint32_t i0 = lane; i0 < cnt; i0 += 128u) {
+            double sv[4];
+            K kv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + 32u * u;
+                sv[u] = 0.0;
+                key_zero(kv[u]);
+                if (i < cnt) { sv[u] = a.usums[src + i]; kv[u] = ((const K*)a.ukeys)[src + i]; }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + 32u * u;
+                const uint64_t o = (uint64_t)off + i;
+                if (i < cnt && (int64_t)o < a.out_capacity) emit_term<K>(a, plan, o, sv[u], kv[u]);
+            }
         }
     }
 }
