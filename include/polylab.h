@@ -42,7 +42,7 @@ extern "C" {
 #pragma GCC visibility push(default)
 #endif
 
-#define POLYLAB_VERSION 110          /* 0.1.1 */
+#define POLYLAB_VERSION 120          /* 0.1.2: polylab_stats.grouped_tiles, POLYLAB_FLAG_NO_GROUP_FINISH, the fast-digits test hook in flag bits 16..19 */
 #define POLYLAB_MAX_NVARS 256        /* packed keys hold at most 256 bits (reading A9) */
 #define POLYLAB_MAX_TERMS ((int64_t)1 << 30)   /* exclusive bound on nterms and on na*nb */
 #define POLYLAB_SMALL_WORKSPACE_BYTES 65536    /* workspace of polylab_expand and polylab_pack_keys */

@@ -80,7 +80,7 @@ def test_flag_values_match_the_header(tmp_path):
 
 
 def test_version_and_status_strings(L):
-    assert L.polylab_version() == 110
+    assert L.polylab_version() == 120
     seen = {L.polylab_status_string(i).decode() for i in range(9)}
     assert len(seen) == 9 and "ok" in seen
     assert L.polylab_status_string(99).decode() == "unknown status"
