@@ -12,6 +12,10 @@
 //                        ctl->overflow and the call falls back to the plain LSD path.  TILE is chosen per call
 //                        (api.cu): CAP minus room for the longest bucket expected from N / 2^T.  Tiles that own
 //                        records go on a work list; every tile start is checked to be a strict prefix increase.
+//   finish_group_kernel  (round 2) tried first on every work-list tile: like terms are grouped through a shared-memory hash
+//                        table, only the tile's distinct keys are put in order, one stable counting pass places the
+//                        records; the tiles it finishes are marked in the work list, finish_kernel does the rest (see the
+//                        comment above the kernel; bit-identical results).
 //   finish_kernel        one block per work-list tile (<= CAP = 4608 records, 256 threads, four blocks per SM).
 //                        Shared memory holds 10 bytes per record, not the record: two 32-bit ping-pong buffers of sort
 //                        elements (record index in the low 13 bits, the not yet consumed sort bits above) and one
