@@ -1052,8 +1052,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinBlocksPerSM) finish_group_ker
     }
     __syncthreads();
 
-    // ---- G4: coefficients to their sorted position (coalesced global read), heads into the bit mask
-#pragma unroll 4
+    // ---- G4: coefficients to their sorted position (coalesced global read), heads into the bit mask; eight loads in flight
+    // per thread (four: +0.03 ms on config 5)
+#pragma unroll 8
     for (uint32_t i = tid; i < n_loc; i += THREADS) {
         const uint32_t p = rk[i], pos = p & 0x1fffu;
         scs[pos] = gcoef[i];
